@@ -1,0 +1,258 @@
+#!/usr/bin/env python
+"""bench.py -- strain-seconds/s of the gwi hot path on B200 (BASELINE.json metric), one JSON line on stdout.
+
+Workload at N=1 (BASELINE.json configs[1]): one paper-scale model (2 branches x 20 gated dilated blocks, 64 residual /
+128 skip channels, k=2) in FP16 mode on a batch of 1024 windows x 4096 samples x 2 detectors of seeded N(0,1) noise
+with 10 % of windows carrying a chirp.  One "step" = one pass of the whole hot path over one batch:
+gwi_infer (lift, 40 block-layers, head) -> gwi_ensemble_triggers (mean, threshold 0.5, runs >= 2048) -> trigger count.
+1 window = 1 s of two-detector strain, so value = windows / s.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--windows B] [--impl reference]
+
+Multi-GPU: weak scaling, every rank runs the same per-GPU batch (the path shards over windows; no collective on the
+data path); value = all ranks' windows / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import gwsynth as gs  # noqa: E402
+
+METRIC = "strain-seconds/s (2 detectors, ensemble) on 1 B200; % FP16 tensor peak"
+UNIT = "strain-seconds/s"
+T = 4096
+THETA, LMIN = 0.5, 2048
+NROT = 8  # rotating input/output buffers: 8 x (16.8 MB in + 16.8 MB out) > 126 MB L2
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i",
+                                      str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows for n, v in zip(names, r[2:6]) if v.lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def oracle_sample(model_path, x16, n_windows):
+    """Times the oracle as it stands on the host cores over `n_windows` windows of the workload."""
+    from oracle import gwo
+    om = gwo.Model(model_path, round_fp16=True)
+    xs = x16[:n_windows].astype(np.float64)
+    t0 = time.perf_counter()
+    p = om.infer_windows(xs)
+    pb = gwo.ensemble_mean([p.reshape(-1)])
+    gwo.triggers(pb, THETA, LMIN)
+    dt = time.perf_counter() - t0
+    return n_windows / dt, dt, gwo.num_threads()
+
+
+def run_reference(args, model_path, x16):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import gwo
+    nthreads = gwo.num_threads()
+    nwin = max(1, min(nthreads, 16))
+    times = []
+    for i in range(args.warmup + args.steps):
+        rate, dt, _ = oracle_sample(model_path, x16[(i * nwin) % 64:], nwin)
+        if i >= args.warmup:
+            times.append(dt)
+    dt = float(np.mean(times))
+    val = nwin / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[1] paper-scale single model, bounded sample", "windows_per_step": nwin, "T": T},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": nthreads, "kind": "oracle",
+                             "sample": f"{nwin} windows x {T} samples per step (of the 1024-window batch)"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--windows", type=int, default=1024)
+    ap.add_argument("--impl", default="gwi")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+
+    work = os.path.join(ROOT, "gpurun_out") if os.access(ROOT, os.W_OK) else "/tmp"
+    os.makedirs(work, exist_ok=True)
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    model_path = os.path.join(work, f"bench_paper_seed0_r{rank}.gwim")
+    gs.make_model_file(model_path, gs.PAPER_ARCH, seed=0)
+    B = args.windows
+
+    if args.impl == "reference":
+        x16, _ = gs.cfg2_windows(seed=1, B=64, T=T)
+        run_reference(args, model_path, x16)
+        return
+
+    import torch
+    import paper_2201_11133_b200 as gwi
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the gwi library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    # ---- inputs: NROT different seeded batches so that the rotating working set exceeds L2 -------------------
+    x_host = []
+    for r in range(NROT):
+        x, _ = gs.cfg2_windows(seed=1 + r + 100 * rank, B=B, T=T)
+        x_host.append(torch.from_numpy(x).pin_memory())
+    x_dev = [x.to(dev) for x in x_host]
+    p_dev = [torch.empty((B, T), dtype=torch.float32, device=dev) for _ in range(NROT)]
+    model = gwi.load_model(model_path, gwi.FP16, local_rank)
+    flops_per_step = gs.PAPER_ARCH.flops_per_timestep() * B * T
+
+    def step(i, timing=None):
+        x, p = x_dev[i % NROT], p_dev[i % NROT]
+        if timing is not None:
+            timing[0].record()
+        model.infer(x, out=p)
+        if timing is not None:
+            timing[1].record()
+        cnt, trig, _ = gwi.ensemble_triggers([p.view(-1)], THETA, LMIN, capacity=4096, sync=False)
+        return cnt
+
+    def e2e_step(i, xd, pd, cnt_host):
+        xd.copy_(x_host[i % NROT], non_blocking=True)       # H2D of this step's strain from pinned memory
+        model.infer(xd, out=pd)
+        cnt, trig, _ = gwi.ensemble_triggers([pd.view(-1)], THETA, LMIN, capacity=4096, sync=False)
+        cnt_host.copy_(cnt, non_blocking=True)              # D2H of the result
+        trig_host.copy_(trig, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        return int(cnt_host.item())
+
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = gwi.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t_start.record()
+    for i in range(args.steps):
+        step(i, ev[i])
+    t_end.record()
+    torch.cuda.synchronize()
+    launches = gwi.launch_count() - l0
+    total_ms = t_start.elapsed_time(t_end)
+    infer_ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    if world > 1:
+        tt = torch.tensor([total_ms], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+
+    # ---- end to end through the public API with host buffers ------------------------------------------------
+    xd = torch.empty_like(x_dev[0])
+    pd = torch.empty_like(p_dev[0])
+    cnt_host = torch.zeros(1, dtype=torch.int32).pin_memory()
+    trig_host = torch.zeros(4096 * 32, dtype=torch.uint8).pin_memory()
+    for i in range(2):
+        e2e_step(i, xd, pd, cnt_host)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        e2e_step(i, xd, pd, cnt_host)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([e2e_s], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    sampler.stop_flag = True
+    sampler.join(timeout=3)
+
+    if rank != 0:
+        return
+    pk, pk_kind = peaks()
+    ms_per_step = total_ms / args.steps
+    value = world * B * args.steps / (total_ms * 1e-3)
+    tflops = flops_per_step / (infer_ms * 1e-3) / 1e12
+    peak_tf = pk.get("bf16_tflops_sustained", pk["bf16_tflops"])
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
+        "data": "synthetic",
+        "config": {"workload": "configs[1]: paper-scale single model (2x20 blocks, R64/S128, k2), FP16 operands / FP32 "
+                               "accumulate, batch of windows x 4096 x 2, then mean/threshold/cluster",
+                   "windows_per_gpu": B, "T": T, "threshold": THETA, "min_len": LMIN,
+                   "l2": f"rotating {NROT} input+output buffer pairs ({NROT * B * T * 8 / 1e6:.0f} MB) > 126 MB L2",
+                   "tensor_core_kernel": bool(model.uses_tensor_cores), "parallelism": f"replicas x{world} (weak)"},
+        "clocks": sampler.summary(),
+        "e2e": {"value": world * B * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": B * T * 2 * 2,
+                "d2h_bytes_per_step": 4 + 4096 * 32},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "tensor", "achieved": tflops, "peak": peak_tf, "unit": "TFLOP/s", "frac": tflops / peak_tf,
+                     "traffic": None, "peak_kind": f"bf16 cuBLAS sustained, {pk_kind}; fp16 = same tensor rate",
+                     "kernel": "gwi_infer (all launches of one call)", "flops_per_launch": flops_per_step,
+                     "infer_ms": infer_ms, "frac_of_nominal_2250": tflops / 2250.0},
+    }
+    if not args.no_cpu_baseline and world == 1:
+        nthreads = os.cpu_count() or 1
+        nwin = max(1, min(3 * nthreads, 48))
+        rate, dt, cores = oracle_sample(model_path, x_host[0].numpy(), nwin)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"{nwin} windows x {T} samples of the same batch, {dt:.1f} s"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

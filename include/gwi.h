@@ -1,0 +1,131 @@
+/* gwi.h -- C-ABI of the B200-native hot path of arXiv 2201.11133
+ * ("Inference-optimized AI and high performance computing for gravitational wave detection at scale").
+ *
+ * What the library computes (citations are PAPER.md lines; readings A1..A31 are listed in DESIGN.md):
+ *   - batched inference of one detection model over 1 s windows of two-detector whitened strain,
+ *     tensor contract (B,4096,2) -> (B,4096,1), one probability per time step
+ *   - the same model run as ONE causal pass over a long stream (overlap reuse, reading A15)
+ *   - ensemble averaging of the models' probabilities, strict threshold, clustering of supra-threshold
+ *     runs of >= min_len samples into triggers
+ *   - time slides of L1 against H1 for background estimation
+ *
+ * Conventions
+ *   - Every entry point returns gwi_status; nothing throws or aborts across the ABI.  gwi_last_error()
+ *     returns a thread-local message for the last non-OK status on the calling thread.
+ *   - Pointers named d_* are DEVICE pointers on the model's device, everything else is a HOST pointer.
+ *   - The caller owns every buffer it passes in (inputs, outputs, workspace, carry).  The library owns only
+ *     what it returns through an opaque handle (gwi_model, gwi_stream) until the matching free/destroy.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
+ *     enqueued asynchronously on it; results are valid after the caller synchronises that stream.
+ *   - There is no CPU fallback: without a usable CUDA device the calls fail with GWI_ERR_CUDA.
+ */
+#ifndef GWI_H
+#define GWI_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gwi_model gwi_model;   /* opaque; owns the packed device weights of ONE network */
+typedef struct gwi_stream gwi_stream; /* opaque; streaming ensemble + slides + triggers state  */
+
+typedef enum {
+    GWI_OK = 0,
+    GWI_ERR_ARG = 1,         /* null / misaligned / out-of-range argument                         */
+    GWI_ERR_IO = 2,          /* model file cannot be opened or is truncated                       */
+    GWI_ERR_FORMAT = 3,      /* model file is not GWIM v1 or has inconsistent fields               */
+    GWI_ERR_UNSUPPORTED = 4, /* architecture outside what the kernels cover                       */
+    GWI_ERR_CUDA = 5,        /* a CUDA runtime call failed (message in gwi_last_error())          */
+    GWI_ERR_NOMEM = 6,       /* workspace / carry / capacity buffer too small                     */
+    GWI_ERR_CAPACITY = 7     /* more triggers than `capacity`; the first `capacity` are valid     */
+} gwi_status;
+
+/* GWI_FP32: fp32 weights, inputs and arithmetic (CUDA-core FMA; parity bar 1e-5 on probabilities).
+ * GWI_FP16: weights rounded to binary16 (RNE) at load, inputs binary16, fp32 accumulation (reading A14);
+ *           paper-scale models (R=64,S=128,k=2) run on the tcgen05 tensor-core kernel (parity bar 2e-3). */
+typedef enum { GWI_FP32 = 0, GWI_FP16 = 1 } gwi_precision;
+
+/* One trigger (readings A19-A22): a maximal run [start,end) of samples with mean probability > threshold
+ * and end-start >= min_len.  start/end are global sample indices (t0 added).  `end` is the merger-time
+ * estimate.  model_mask bit j: model j alone exceeded the threshold somewhere in the run.
+ * Exactly compared with the oracle: slide, start, end.  peak_p / mean_p are fp32 statistics of the mean
+ * probability over the run. */
+typedef struct {
+    int32_t slide;
+    int32_t model_mask;
+    int64_t start;
+    int64_t end;
+    float peak_p;
+    float mean_p;
+} gwi_trigger;
+
+/* ---- model ------------------------------------------------------------------------------------------- */
+
+/* Load a GWIM v1 model file (layout: DESIGN.md "Model file"; network: DESIGN.md C.1 = PAPER.md:45, 49) and
+ * upload its weights to CUDA device `device`, packed for the kernels of precision `prec`.
+ * path: host C string.  out: receives the handle (owned by the caller until gwi_free_model).
+ * Errors: GWI_ERR_ARG (null), GWI_ERR_IO, GWI_ERR_FORMAT, GWI_ERR_UNSUPPORTED (k > 8, R or S > 256,
+ * Hh > 512), GWI_ERR_CUDA. */
+gwi_status gwi_load_model(const char* path, gwi_precision prec, int device, gwi_model** out);
+
+/* Free the handle and its device memory.  NULL is a no-op. */
+void gwi_free_model(gwi_model* m);
+
+/* Architecture of a loaded model.  Any out pointer may be NULL.  receptive_field = 1 + (k-1) * sum(d_i). */
+gwi_status gwi_model_info(const gwi_model* m, int32_t* n_branch, int32_t* c_in, int32_t* R, int32_t* S,
+                          int32_t* k, int32_t* n_blocks, int32_t* Hh, int32_t* receptive_field);
+
+/* 1 if FP16-mode gwi_infer on this model runs the tcgen05 tensor-core kernel, 0 if it runs the generic
+ * CUDA-core kernel on fp16-rounded operands. */
+int gwi_model_uses_tensor_cores(const gwi_model* m);
+
+/* ---- window inference (the paper's tensor contract) --------------------------------------- */
+
+/* Bytes of device workspace gwi_infer needs for B windows of T samples (0 on bad arguments). */
+size_t gwi_infer_workspace_bytes(const gwi_model* m, int64_t B, int32_t T);
+
+/* p[b][t] for B independent windows, each evaluated with zero history at t < 0 of every layer (reading A4).
+ * d_strain: [B][T][C] channels-last, C = n_branch*c_in (H1 first); float in FP32 mode, __half in FP16 mode;
+ *           16-byte aligned.   d_prob: [B][T] float.   d_workspace: >= gwi_infer_workspace_bytes, 256 B aligned.
+ * T: any length >= 1 (not only 4096).  B >= 0 (B == 0 is a no-op).
+ * Errors: GWI_ERR_ARG, GWI_ERR_NOMEM (workspace too small), GWI_ERR_CUDA. */
+gwi_status gwi_infer(const gwi_model* m, const void* d_strain, int64_t B, int32_t T, float* d_prob,
+                     void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- ensemble mean + threshold + trigger clustering (readings A18-A22) ------------------- */
+
+/* Bytes of the opaque device carry block / of the device scratch needed for N samples. */
+size_t gwi_carry_bytes(void);
+size_t gwi_triggers_workspace_bytes(int64_t N);
+
+/* Post-processing on materialised probabilities.
+ * d_prob: HOST array of n_models DEVICE pointers; d_prob[j] is model j's [N] float stream chunk.
+ * The mean is the fixed fp32 expression (((p0+p1)+p2)+...)/(float)n_models, IEEE round-to-nearest adds and one
+ * correctly rounded division; a sample is supra-threshold iff mean > threshold (strict).
+ * t0: global sample index of element 0.  slide_id: copied into every record.
+ * d_carry: NULL (the chunk is a whole stream) or a device block of gwi_carry_bytes() that the caller zeroes
+ *          before the first chunk; it carries the open run across calls on consecutive chunks.
+ * last_chunk != 0: a run still open at the end of this chunk is closed there (reading A21).
+ * d_triggers / d_count: device; records sorted by start; *d_count = number of qualifying runs closed by this
+ *          call (may exceed capacity; then only the first `capacity` are written and the status, reported by
+ *          gwi_triggers_status after synchronising, is GWI_ERR_CAPACITY).
+ * d_pbar: optional device [N] float, receives the mean probability (NULL: not written).
+ * 1 <= n_models <= 16, N >= 1.  Errors: GWI_ERR_ARG, GWI_ERR_NOMEM, GWI_ERR_CUDA. */
+gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0,
+                                 float threshold, int64_t min_len, int32_t slide_id, int last_chunk,
+                                 void* d_carry, gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count,
+                                 float* d_pbar, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- misc ---------------------------------------------------------------------------------------------- */
+const char* gwi_last_error(void);
+int gwi_version(void);
+/* number of kernels this library has launched since load (all threads); bench.py reports it */
+int64_t gwi_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GWI_H */

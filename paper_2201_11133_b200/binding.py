@@ -1,0 +1,179 @@
+"""ctypes binding of libgwi.so.  Same names as include/gwi.h; marshalling only."""
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+FP32, FP16 = 0, 1
+STATUS_NAMES = {0: "GWI_OK", 1: "GWI_ERR_ARG", 2: "GWI_ERR_IO", 3: "GWI_ERR_FORMAT", 4: "GWI_ERR_UNSUPPORTED",
+                5: "GWI_ERR_CUDA", 6: "GWI_ERR_NOMEM", 7: "GWI_ERR_CAPACITY"}
+EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_model_uses_tensor_cores",
+                    "gwi_infer_workspace_bytes", "gwi_infer", "gwi_carry_bytes", "gwi_triggers_workspace_bytes",
+                    "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count"]
+
+
+class GwiError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {msg}")
+        self.status = status
+
+
+class Trigger(C.Structure):
+    _fields_ = [("slide", C.c_int32), ("model_mask", C.c_int32), ("start", C.c_int64), ("end", C.c_int64),
+                ("peak_p", C.c_float), ("mean_p", C.c_float)]
+
+
+_lib = None
+
+
+def lib():
+    """Load (building if stale and nvcc is present) the shared library.  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    try:
+        path = _build.build()
+    except Exception:
+        if not os.path.exists(path):
+            raise
+    L = C.CDLL(path)
+    vp, i32p = C.c_void_p, C.POINTER(C.c_int32)
+    L.gwi_load_model.restype = C.c_int
+    L.gwi_load_model.argtypes = [C.c_char_p, C.c_int, C.c_int, C.POINTER(vp)]
+    L.gwi_free_model.restype = None
+    L.gwi_free_model.argtypes = [vp]
+    L.gwi_model_info.restype = C.c_int
+    L.gwi_model_info.argtypes = [vp] + [i32p] * 8
+    L.gwi_model_uses_tensor_cores.restype = C.c_int
+    L.gwi_model_uses_tensor_cores.argtypes = [vp]
+    L.gwi_infer_workspace_bytes.restype = C.c_size_t
+    L.gwi_infer_workspace_bytes.argtypes = [vp, C.c_int64, C.c_int32]
+    L.gwi_infer.restype = C.c_int
+    L.gwi_infer.argtypes = [vp, vp, C.c_int64, C.c_int32, vp, vp, C.c_size_t, vp]
+    L.gwi_carry_bytes.restype = C.c_size_t
+    L.gwi_triggers_workspace_bytes.restype = C.c_size_t
+    L.gwi_triggers_workspace_bytes.argtypes = [C.c_int64]
+    L.gwi_ensemble_triggers.restype = C.c_int
+    L.gwi_ensemble_triggers.argtypes = [C.POINTER(vp), C.c_int32, C.c_int64, C.c_int64, C.c_float, C.c_int64, C.c_int32,
+                                        C.c_int, vp, vp, C.c_int32, vp, vp, vp, C.c_size_t, vp]
+    L.gwi_last_error.restype = C.c_char_p
+    L.gwi_version.restype = C.c_int
+    L.gwi_launch_count.restype = C.c_int64
+    _lib = L
+    return L
+
+
+def last_error():
+    return lib().gwi_last_error().decode()
+
+
+def version():
+    return lib().gwi_version()
+
+
+def launch_count():
+    return lib().gwi_launch_count()
+
+
+def _check(st):
+    if st != 0:
+        raise GwiError(st, last_error())
+
+
+def _stream_ptr(device):
+    return C.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+class Model:
+    """Handle on a gwi_model (gwi_load_model / gwi_free_model)."""
+
+    def __init__(self, path, precision=FP32, device=0):
+        self._h = C.c_void_p()
+        self.device = int(device)
+        self.precision = precision
+        _check(lib().gwi_load_model(os.fsencode(path), int(precision), self.device, C.byref(self._h)))
+        v = [C.c_int32() for _ in range(8)]
+        _check(lib().gwi_model_info(self._h, *[C.byref(x) for x in v]))
+        (self.n_branch, self.c_in, self.R, self.S, self.k, self.L, self.Hh, self.receptive_field) = [x.value for x in v]
+        self.uses_tensor_cores = bool(lib().gwi_model_uses_tensor_cores(self._h))
+        self._ws = None
+
+    def close(self):
+        if self._h:
+            lib().gwi_free_model(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def workspace_bytes(self, B, T):
+        return lib().gwi_infer_workspace_bytes(self._h, int(B), int(T))
+
+    def infer(self, strain, out=None):
+        """gwi_infer: strain [B][T][C] device tensor (float32 in FP32 mode, float16 in FP16 mode) -> prob [B][T]."""
+        return infer(self, strain, out)
+
+
+def load_model(path, precision=FP32, device=0):
+    return Model(path, precision, device)
+
+
+def infer(model, strain, out=None):
+    if not strain.is_cuda:
+        raise GwiError(1, "strain must be a CUDA tensor (no CPU fallback)")
+    want = torch.float16 if model.precision == FP16 else torch.float32
+    if strain.dtype != want or strain.dim() != 3 or strain.shape[2] != model.n_branch * model.c_in:
+        raise GwiError(1, f"strain must be [B][T][{model.n_branch * model.c_in}] {want}")
+    strain = strain.contiguous()
+    B, T, _ = strain.shape
+    if out is None:
+        out = torch.empty((B, T), dtype=torch.float32, device=strain.device)
+    need = model.workspace_bytes(B, T)
+    if model._ws is None or model._ws.numel() < need:
+        model._ws = torch.empty(max(need, 256), dtype=torch.uint8, device=strain.device)
+    _check(lib().gwi_infer(model._h, C.c_void_p(strain.data_ptr()), B, T, C.c_void_p(out.data_ptr()),
+                           C.c_void_p(model._ws.data_ptr()), model._ws.numel(), _stream_ptr(strain.device)))
+    return out
+
+
+def ensemble_triggers(probs, threshold, min_len, t0=0, slide_id=0, last_chunk=True, carry=None, capacity=4096,
+                      want_pbar=False, sync=True):
+    """gwi_ensemble_triggers on a list of [N] float32 device tensors.
+    Returns (count, [Trigger...], pbar or None); raises GwiError(GWI_ERR_CAPACITY) when count > capacity
+    (the exception carries .count and .records with the valid prefix)."""
+    dev = probs[0].device
+    if not probs[0].is_cuda:
+        raise GwiError(1, "probabilities must be CUDA tensors (no CPU fallback)")
+    probs = [p.contiguous() for p in probs]
+    N = probs[0].numel()
+    ptrs = (C.c_void_p * len(probs))(*[p.data_ptr() for p in probs])
+    trig = torch.zeros(max(capacity, 1) * C.sizeof(Trigger), dtype=torch.uint8, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int32, device=dev)
+    pbar = torch.empty(N, dtype=torch.float32, device=dev) if want_pbar else None
+    wsb = lib().gwi_triggers_workspace_bytes(N)
+    ws = torch.empty(max(wsb, 256), dtype=torch.uint8, device=dev)
+    _check(lib().gwi_ensemble_triggers(ptrs, len(probs), N, int(t0), float(threshold), int(min_len), int(slide_id),
+                                       int(bool(last_chunk)), C.c_void_p(carry.data_ptr()) if carry is not None else None,
+                                       C.c_void_p(trig.data_ptr()), int(capacity), C.c_void_p(cnt.data_ptr()),
+                                       C.c_void_p(pbar.data_ptr()) if pbar is not None else None,
+                                       C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(dev)))
+    if not sync:
+        return cnt, trig, pbar
+    n = int(cnt.item())
+    raw = trig.cpu().numpy().tobytes()
+    recs = [Trigger.from_buffer_copy(raw, i * C.sizeof(Trigger)) for i in range(min(n, capacity))]
+    if n > capacity:
+        e = GwiError(7, f"{n} triggers > capacity {capacity}")
+        e.count, e.records = n, recs
+        raise e
+    return n, recs, pbar
+
+
+def new_carry(device=0):
+    return torch.zeros(lib().gwi_carry_bytes(), dtype=torch.uint8, device=f"cuda:{device}" if isinstance(device, int) else device)

@@ -1,0 +1,79 @@
+// gwi_internal.h -- shared declarations of the library's translation units (NOT part of the C-ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/gwi.h"
+
+#define GWI_MAX_LAYERS 64
+#define GWI_MAX_MODELS 16
+
+// ---- error plumbing ---------------------------------------------------------------------------------------
+void gwi_set_error(const char* fmt, ...);
+#define GWI_CUDA_CHECK(expr)                                                                     \
+    do {                                                                                         \
+        cudaError_t e__ = (expr);                                                                \
+        if (e__ != cudaSuccess) {                                                                \
+            gwi_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #expr, cudaGetErrorString(e__)); \
+            return GWI_ERR_CUDA;                                                                 \
+        }                                                                                        \
+    } while (0)
+void gwi_count_launch(int n = 1);
+
+// ---- architecture (GWIM v1 header) -------------------------------------------------
+struct GwiArch {
+    int n_branch, c_in, R, S, k, L, Hh;
+    int dil[GWI_MAX_LAYERS];
+    int receptive_field() const {
+        long s = 0;
+        for (int i = 0; i < L; i++) s += dil[i];
+        return (int)(1 + (long)(k - 1) * s);
+    }
+};
+
+// Offsets (in floats) of every tensor inside the fp32 weight blob, which is the file's tensor section verbatim
+// (FP16 mode: every value rounded to binary16 and widened again).
+struct GwiLayerOff {
+    int64_t Wf, bf, Wg, bg, Wr, br, Ws, bs;
+};
+struct GwiOffsets {
+    int64_t W_in[4], b_in[4];             // per branch (n_branch <= 4)
+    GwiLayerOff layer[4][GWI_MAX_LAYERS]; // [branch][block]
+    int64_t W1, b1, W2, b2;
+};
+
+// Device-side view used by the generic fp32 kernels (passed by value to kernels: small).
+struct GwiDevModel {
+    const float* blob;
+    int n_branch, c_in, R, S, k, L, Hh;
+};
+
+// Packed fp16 weights of the tcgen05 kernel (gwi_tc.cu); null when the architecture is not covered.
+struct GwiTcPack;
+
+struct gwi_model {
+    GwiArch arch;
+    gwi_precision prec;
+    int device;
+    std::vector<float> host_blob; // weights as the kernels see them (rounded to fp16 and widened in FP16 mode)
+    GwiOffsets off;
+    float* d_blob = nullptr;
+    GwiOffsets* d_off = nullptr; // copy of `off` in device memory
+    GwiTcPack* tc = nullptr;
+};
+
+// ---- generic CUDA-core path (gwi_generic.cu) ---------------------------------------------------------------
+size_t gwi_generic_workspace_bytes(const gwi_model* m, int64_t B, int32_t T);
+gwi_status gwi_generic_infer(const gwi_model* m, const void* d_strain, bool strain_is_half, int64_t B, int32_t T,
+                             float* d_prob, void* d_ws, size_t ws_bytes, cudaStream_t st);
+
+// ---- tcgen05 path (gwi_tc.cu) -------------------------------------------------------------------------------
+bool gwi_tc_supported(const GwiArch& a);
+gwi_status gwi_tc_pack(gwi_model* m);
+void gwi_tc_free(gwi_model* m);
+size_t gwi_tc_workspace_bytes(const gwi_model* m, int64_t B, int32_t T);
+gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, int32_t T, float* d_prob, void* d_ws,
+                        size_t ws_bytes, cudaStream_t st);

@@ -1,0 +1,393 @@
+// gwi_post.cu -- ensemble mean + strict threshold + run-length trigger clustering (gwi_ensemble_triggers).
+//
+// Definition (DESIGN.md C.1 "Triggers", readings A18-A22; "height" and "width >= 0.5 s"):
+//   pbar[t] = (((p0[t]+p1[t])+p2[t])+...)/(float)M   fixed fp32 expression (tier T1: bit-reproducible)
+//   a[t]    = pbar[t] > theta                        strict
+//   every maximal run [s,e) of a = 1 with e - s >= L_min is a trigger, sorted by s; runs are carried across
+//   consecutive chunks through the caller's carry block and closed at the stream end when last_chunk != 0.
+//
+// Kernels:
+//   k_mask      HBM-bound pass: reads M x N floats once, writes N/8 bytes of bit mask (+ optional pbar).  This is
+//               the roofline kernel of the post-processing: 4*M (+4) algorithmic bytes per sample.
+//   k_blkflags  per 256-word block "all ones" flag so that long runs are walked 8192 samples per step
+//   k_head_run  closes / continues the run carried in from the previous chunk
+//   k_runs<0>   one thread per 32-sample word: finds run starts, walks to the run end, counts qualifying runs
+//   k_scan      exclusive scan of the per-CTA counts -> output offsets, total -> *d_count
+//   k_runs<1>   same walk, writes {slide,start,end} at its slot (records come out sorted by start)
+//   k_stats     one CTA per record: peak / mean / model_mask over the run; last CTA updates the carry block
+#include "gwi_internal.h"
+
+namespace {
+
+constexpr int WB = 256;    // words per all-ones block
+constexpr int RT = 1024;   // threads (= words) per CTA in k_runs
+
+struct Ptrs {
+    const float* p[GWI_MAX_MODELS];
+};
+
+struct Carry {             // the caller's opaque carry block (gwi_carry_bytes())
+    int32_t open;
+    int32_t mask;
+    int64_t start;         // global start of the open run
+    double sum;
+    float peak;
+    int32_t pad;
+};
+
+struct Header {            // per-call scratch header at the start of the workspace
+    Carry in;              // copy of the incoming carry (zero if none)
+    int32_t head_emit;     // the carried run closes in this chunk and qualifies -> record 0
+    int32_t head_closed;   // the carried run closes in this chunk
+    int64_t head_end;      // local index where it closes
+    int32_t out_open;      // a run is open at the end of this chunk
+    int32_t pad;
+    int64_t out_start;     // its global start
+    int32_t total;         // number of records of this call
+    int32_t pad2;
+};
+
+__device__ __forceinline__ float ens_mean(const Ptrs& P, int M, int64_t i)
+{
+    float s = P.p[0][i];
+    for (int j = 1; j < M; j++) s = __fadd_rn(s, P.p[j][i]);
+    return __fdiv_rn(s, (float)M);
+}
+
+template <bool VEC>
+__global__ void k_mask(Ptrs P, int M, int64_t N, float theta, uint32_t* __restrict__ bits, int64_t NW,
+                       float* __restrict__ pbar)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    const float fM = (float)M;
+    for (int64_t base = warp * 128; base < NW * 32; base += nwarps * 128) {
+        int64_t i = base + 4 * lane;
+        float m4[4] = {0.f, 0.f, 0.f, 0.f};
+        uint32_t nib = 0;
+        if (VEC && i + 3 < N) {
+            float4 s = *reinterpret_cast<const float4*>(P.p[0] + i);
+            for (int j = 1; j < M; j++) {
+                float4 v = *reinterpret_cast<const float4*>(P.p[j] + i);
+                s.x = __fadd_rn(s.x, v.x), s.y = __fadd_rn(s.y, v.y), s.z = __fadd_rn(s.z, v.z), s.w = __fadd_rn(s.w, v.w);
+            }
+            m4[0] = __fdiv_rn(s.x, fM), m4[1] = __fdiv_rn(s.y, fM), m4[2] = __fdiv_rn(s.z, fM), m4[3] = __fdiv_rn(s.w, fM);
+            nib = (m4[0] > theta) | ((m4[1] > theta) << 1) | ((m4[2] > theta) << 2) | ((m4[3] > theta) << 3);
+            if (pbar) *reinterpret_cast<float4*>(pbar + i) = make_float4(m4[0], m4[1], m4[2], m4[3]);
+        } else {
+            for (int e = 0; e < 4; e++)
+                if (i + e < N) {
+                    float v = ens_mean(P, M, i + e);
+                    nib |= (uint32_t)(v > theta) << e;
+                    if (pbar) pbar[i + e] = v;
+                }
+        }
+        uint32_t w = nib << (4 * (lane & 7));
+        w |= __shfl_xor_sync(0xffffffffu, w, 1);
+        w |= __shfl_xor_sync(0xffffffffu, w, 2);
+        w |= __shfl_xor_sync(0xffffffffu, w, 4);
+        int64_t wi = (base >> 5) + (lane >> 3);
+        if ((lane & 7) == 0 && wi < NW) bits[wi] = w;
+    }
+}
+
+__global__ void k_blkflags(const uint32_t* __restrict__ bits, int64_t NW, uint8_t* __restrict__ flags)
+{
+    int64_t i = (int64_t)blockIdx.x * WB + threadIdx.x;
+    int ok = (i < NW) ? (bits[i] == 0xffffffffu) : 0;
+    int all = __syncthreads_and(ok);
+    if (threadIdx.x == 0) flags[blockIdx.x] = (uint8_t)all;
+}
+
+// first index >= pos whose bit is 0 (bits past N are 0), capped at N
+__device__ int64_t find_end(const uint32_t* __restrict__ bits, const uint8_t* __restrict__ flags, int64_t NW,
+                            int64_t N, int64_t pos)
+{
+    int64_t i = pos >> 5;
+    uint32_t w = ~bits[i] & (0xffffffffu << (pos & 31));
+    if (w) return min((int64_t)(i * 32 + __ffs(w) - 1), N);
+    for (i++; i < NW; i++) {
+        if ((i % WB) == 0)
+            while (i + WB <= NW && flags[i / WB]) i += WB;
+        if (i >= NW) break;
+        w = ~bits[i];
+        if (w) return min((int64_t)(i * 32 + __ffs(w) - 1), N);
+    }
+    return N;
+}
+
+__global__ void k_head_run(const uint32_t* __restrict__ bits, const uint8_t* __restrict__ flags, int64_t NW, int64_t N,
+                           int64_t t0, int64_t Lmin, int last_chunk, const Carry* __restrict__ carry, Header* hd)
+{
+    if (threadIdx.x != 0) return;
+    Carry c;
+    if (carry) c = *carry;
+    else { c.open = 0, c.mask = 0, c.start = 0, c.sum = 0.0, c.peak = 0.f, c.pad = 0; }
+    hd->in = c;
+    hd->head_emit = 0, hd->head_closed = 0, hd->head_end = 0, hd->out_open = 0, hd->out_start = 0, hd->total = 0;
+    if (c.open) {
+        int64_t e0 = (bits[0] & 1u) ? find_end(bits, flags, NW, N, 0) : 0;
+        if (e0 < N || last_chunk) {
+            hd->head_closed = 1;
+            hd->head_end = e0;
+            hd->head_emit = (t0 + e0 - c.start >= Lmin) ? 1 : 0;
+        } else {
+            hd->out_open = 1;
+            hd->out_start = c.start;
+        }
+    }
+}
+
+// MODE 0: count qualifying closed runs per CTA.  MODE 1: write the records.
+template <int MODE>
+__global__ void k_runs(const uint32_t* __restrict__ bits, const uint8_t* __restrict__ flags, int64_t NW, int64_t N,
+                       int64_t t0, int64_t Lmin, int last_chunk, int slide, Header* hd, uint32_t* __restrict__ blkcnt,
+                       const uint32_t* __restrict__ blkoff, gwi_trigger* __restrict__ out, int capacity)
+{
+    __shared__ uint32_t wsum[RT / 32];
+    const int64_t i = (int64_t)blockIdx.x * RT + threadIdx.x;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t cnt = 0;
+    int64_t rs[32 / 2], re[32 / 2];   // a word holds at most 16 run starts
+    if (i < NW) {
+        uint32_t w = bits[i];
+        uint32_t prev = (i > 0) ? (bits[i - 1] >> 31) : (uint32_t)(hd->in.open != 0);
+        uint32_t starts = w & ~((w << 1) | prev);
+        while (starts) {
+            int s = __ffs(starts) - 1;
+            starts &= starts - 1;
+            int64_t g = i * 32 + s;
+            int64_t e = find_end(bits, flags, NW, N, g);
+            if (e < N || last_chunk) {
+                if (e - g >= Lmin) {
+                    if (MODE == 1) rs[cnt] = g, re[cnt] = e;
+                    cnt++;
+                }
+            } else if (MODE == 0) {   // touches the chunk end and the stream continues: becomes the carry
+                hd->out_open = 1;
+                hd->out_start = t0 + g;
+            }
+        }
+    }
+    // CTA-wide exclusive scan of cnt
+    uint32_t incl = cnt;
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) wsum[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+        uint32_t v = wsum[lane];
+        uint32_t inc2 = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t u = __shfl_up_sync(0xffffffffu, inc2, o);
+            if (lane >= o) inc2 += u;
+        }
+        wsum[lane] = inc2 - v;   // exclusive warp offsets
+        if (MODE == 0 && lane == 31) blkcnt[blockIdx.x] = inc2;
+    }
+    __syncthreads();
+    if (MODE == 1 && cnt) {
+        int64_t slot = (int64_t)blkoff[blockIdx.x] + wsum[wid] + (incl - cnt);
+        for (uint32_t q = 0; q < cnt; q++, slot++)
+            if (slot < capacity) {
+                gwi_trigger r;
+                r.slide = slide, r.model_mask = 0, r.start = t0 + rs[q], r.end = t0 + re[q], r.peak_p = 0.f, r.mean_p = 0.f;
+                out[slot] = r;
+            }
+    }
+}
+
+__global__ void k_scan(const uint32_t* __restrict__ blkcnt, uint32_t* __restrict__ blkoff, int64_t nblk, int64_t t0,
+                       int slide, Header* hd, gwi_trigger* __restrict__ out, int capacity, int32_t* __restrict__ d_count)
+{
+    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t running;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) running = (uint32_t)hd->head_emit;   // the carried run, if emitted, is record 0
+    __syncthreads();
+    for (int64_t base = 0; base < nblk; base += blockDim.x) {
+        int64_t i = base + threadIdx.x;
+        uint32_t v = (i < nblk) ? blkcnt[i] : 0, incl = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += u;
+        }
+        if (lane == 31) wsum[wid] = incl;
+        __syncthreads();
+        if (wid == 0) {
+            uint32_t x = wsum[lane], inc2 = x;
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t u = __shfl_up_sync(0xffffffffu, inc2, o);
+                if (lane >= o) inc2 += u;
+            }
+            wsum[lane] = inc2 - x;
+        }
+        __syncthreads();
+        uint32_t excl = running + wsum[wid] + incl - v;
+        if (i < nblk) blkoff[i] = excl;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) running = excl + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        hd->total = (int32_t)running;
+        *d_count = (int32_t)running;
+        if (hd->head_emit && capacity > 0 && out) {
+            gwi_trigger r;
+            r.slide = slide, r.model_mask = 0, r.start = hd->in.start, r.end = t0 + hd->head_end, r.peak_p = 0.f, r.mean_p = 0.f;
+            out[0] = r;
+        }
+    }
+}
+
+// statistics of pbar over local [a,b): peak, sum (double), per-model mask.  256 threads cooperate.
+__device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t b, float& peak, double& sum, int& mask)
+{
+    __shared__ float s_peak[256];
+    __shared__ double s_sum[256];
+    __shared__ int s_mask[256];
+    float pk = -1.f;
+    double sm = 0.0;
+    int mk = 0;
+    for (int64_t i = a + threadIdx.x; i < b; i += blockDim.x) {
+        float v = ens_mean(P, M, i);
+        pk = fmaxf(pk, v);
+        sm += (double)v;
+        for (int j = 0; j < M; j++) mk |= (P.p[j][i] > theta) << j;
+    }
+    s_peak[threadIdx.x] = pk, s_sum[threadIdx.x] = sm, s_mask[threadIdx.x] = mk;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            s_peak[threadIdx.x] = fmaxf(s_peak[threadIdx.x], s_peak[threadIdx.x + o]);
+            s_sum[threadIdx.x] += s_sum[threadIdx.x + o];
+            s_mask[threadIdx.x] |= s_mask[threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    peak = s_peak[0], sum = s_sum[0], mask = s_mask[0];
+    __syncthreads();
+}
+
+__global__ void k_stats(Ptrs P, int M, float theta, int64_t N, int64_t t0, const Header* __restrict__ hd,
+                        gwi_trigger* __restrict__ out, int capacity, Carry* carry)
+{
+    const int nrec = min(hd->total, capacity);
+    if ((int)blockIdx.x == (int)gridDim.x - 1) {   // last CTA: write the outgoing carry
+        if (!carry) return;
+        Carry c;
+        c.open = hd->out_open, c.mask = 0, c.start = hd->out_start, c.sum = 0.0, c.peak = 0.f, c.pad = 0;
+        if (c.open) {
+            int64_t a = c.start > t0 ? c.start - t0 : 0;
+            float pk; double sm; int mk;
+            run_stats(P, M, theta, a, N, pk, sm, mk);
+            if (c.start < t0) pk = fmaxf(pk, hd->in.peak), sm += hd->in.sum, mk |= hd->in.mask;
+            c.peak = pk, c.sum = sm, c.mask = mk;
+        }
+        if (threadIdx.x == 0) *carry = c;
+        return;
+    }
+    if (!out) return;
+    for (int r = blockIdx.x; r < nrec; r += gridDim.x - 1) {
+        int64_t s = out[r].start, e = out[r].end;
+        int64_t a = s > t0 ? s - t0 : 0;
+        float pk; double sm; int mk;
+        run_stats(P, M, theta, a, e - t0, pk, sm, mk);
+        if (s < t0) pk = fmaxf(pk, hd->in.peak), sm += hd->in.sum, mk |= hd->in.mask;
+        if (threadIdx.x == 0) {
+            out[r].peak_p = pk;
+            out[r].mean_p = (float)(sm / (double)(e - s));
+            out[r].model_mask = mk;
+        }
+    }
+}
+
+struct Layout {
+    size_t hdr, bits, flags, cnt, off, total;
+    int64_t NW, NB, NR;
+};
+Layout layout(int64_t N)
+{
+    Layout L;
+    L.NW = (N + 31) / 32;
+    L.NB = (L.NW + WB - 1) / WB;
+    L.NR = (L.NW + RT - 1) / RT;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 255) & ~(size_t)255; return at; };
+    L.hdr = take(sizeof(Header));
+    L.bits = take((size_t)(L.NW + 4) * 4);
+    L.flags = take((size_t)L.NB);
+    L.cnt = take((size_t)L.NR * 4);
+    L.off = take((size_t)L.NR * 4);
+    L.total = o;
+    return L;
+}
+
+} // namespace
+
+extern "C" size_t gwi_carry_bytes(void) { return sizeof(Carry); }
+extern "C" size_t gwi_triggers_workspace_bytes(int64_t N) { return N < 1 ? 0 : layout(N).total; }
+
+extern "C" gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0,
+                                            float threshold, int64_t min_len, int32_t slide_id, int last_chunk,
+                                            void* d_carry, gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count,
+                                            float* d_pbar, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!d_prob || n_models < 1 || n_models > GWI_MAX_MODELS || N < 1 || capacity < 0 || !d_count || !d_workspace ||
+        (capacity > 0 && !d_triggers) || ((uintptr_t)d_workspace & 255)) {
+        gwi_set_error("gwi_ensemble_triggers: bad argument");
+        return GWI_ERR_ARG;
+    }
+    Ptrs P;
+    bool vec = ((uintptr_t)d_pbar & 15) == 0;
+    for (int j = 0; j < n_models; j++) {
+        if (!d_prob[j] || ((uintptr_t)d_prob[j] & 3)) {
+            gwi_set_error("gwi_ensemble_triggers: d_prob[%d] null or misaligned", j);
+            return GWI_ERR_ARG;
+        }
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, d_prob[j]) != cudaSuccess || pa.type != cudaMemoryTypeDevice) {
+            cudaGetLastError();
+            gwi_set_error("gwi_ensemble_triggers: d_prob[%d] is not a device pointer", j);
+            return GWI_ERR_ARG;
+        }
+        P.p[j] = d_prob[j];
+        vec = vec && (((uintptr_t)d_prob[j] & 15) == 0);
+    }
+    for (int j = n_models; j < GWI_MAX_MODELS; j++) P.p[j] = nullptr;
+    Layout L = layout(N);
+    if (workspace_bytes < L.total) {
+        gwi_set_error("gwi_ensemble_triggers: workspace %zu < %zu bytes", workspace_bytes, L.total);
+        return GWI_ERR_NOMEM;
+    }
+    if (!d_carry) last_chunk = 1;   // a chunk without carry is a whole stream
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char* ws = (char*)d_workspace;
+    Header* hd = (Header*)(ws + L.hdr);
+    uint32_t* bits = (uint32_t*)(ws + L.bits);
+    uint8_t* flags = (uint8_t*)(ws + L.flags);
+    uint32_t* cnt = (uint32_t*)(ws + L.cnt);
+    uint32_t* off = (uint32_t*)(ws + L.off);
+    // one warp handles 128 samples per iteration; 148 SMs x 8 CTAs of 256 threads
+    int64_t warps_needed = (L.NW * 32 + 127) / 128;
+    int grid = (int)((warps_needed + 7) / 8);
+    if (grid > 148 * 8) grid = 148 * 8;
+    if (grid < 1) grid = 1;
+    if (vec) k_mask<true><<<grid, 256, 0, st>>>(P, n_models, N, threshold, bits, L.NW, d_pbar);
+    else k_mask<false><<<grid, 256, 0, st>>>(P, n_models, N, threshold, bits, L.NW, d_pbar);
+    k_blkflags<<<(unsigned)L.NB, WB, 0, st>>>(bits, L.NW, flags);
+    k_head_run<<<1, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd);
+    k_runs<0><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
+                                             d_triggers, capacity);
+    k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count);
+    k_runs<1><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
+                                             d_triggers, capacity);
+    int sgrid = capacity < 1024 ? capacity + 1 : 1025;
+    k_stats<<<sgrid, 256, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry);
+    gwi_count_launch(7);
+    GWI_CUDA_CHECK(cudaGetLastError());
+    return GWI_OK;
+}
