@@ -119,6 +119,50 @@ gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t n_models, i
                                  void* d_carry, gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count,
                                  float* d_pbar, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- streaming ensemble: one causal pass over a long two-detector stream ---
+ *
+ * What it computes (DESIGN.md C.1 "Stream", "Ensemble", "Slide k", "Triggers"):
+ *   p_m[t], t in [0, n_total): model m evaluated ONCE over the whole stream with zero history only at t = 0 (by
+ *   reading A15 / pin P8 this equals stitching 1 s windows taken every 0.5 s); for slide j with lag_j samples
+ *   p_{m,j}[t] = head_m(u_{m,H1}[t], u_{m,L1}[(t - lag_j) mod n_total]) (reading A24; slide 0 is the zero lag);
+ *   pbar_j = fp32 mean over models; triggers = maximal runs of pbar_j > threshold with length >= min_len, runs
+ *   carried across chunk boundaries; records sorted by (slide, start).  Pushing the stream in chunks of any sizes
+ *   gives bit-identical results to pushing it whole (reading A17).
+ *
+ * gwi_stream_create   models: HOST array of n_models loaded models sharing device, precision and architecture
+ *                     (1..16).  lags: HOST array of n_lags lags in SAMPLES, each in [1, n_total) (n_lags = 0: zero lag
+ *                     only; slides need a two-branch model).  max_chunk: largest n a push will carry.  capacity:
+ *                     records the stream can hold.  d_pbar: NULL, or a DEVICE array [1 + n_lags][n_total] float that
+ *                     receives pbar_j (for parity tests; ~4 B x n_total per slide).  The handle owns all its device
+ *                     memory (staging, per-layer histories, L1 feature ring, probabilities, records).
+ *                     Errors: GWI_ERR_ARG, GWI_ERR_UNSUPPORTED (slides on a one-branch model), GWI_ERR_NOMEM, GWI_ERR_CUDA.
+ * gwi_stream_tail_samples / gwi_stream_prime   (only when n_lags > 0, before the first push) the circular wrap of the
+ *                     slides needs the L1 features of the last max-lag samples at the START: the caller passes the last
+ *                     gwi_stream_tail_samples() samples of the L1 strain (HOST or DEVICE pointer; __half in FP16 mode,
+ *                     float in FP32 mode; for c_in > 1 planar [c_in][n_tail]).  The tail is max-lag + R_f - 1 samples
+ *                     (or the whole stream if shorter), which makes its features exact.
+ * gwi_stream_push     d_h1, d_l1: DEVICE pointers to the next n samples of each detector (planar; d_l1 ignored for a
+ *                     one-branch model).  Enqueued on cuda_stream; the buffers may be reused once that work is done.
+ * gwi_stream_push_host  same from HOST buffers (pinned for real overlap): the H2D copy runs on the handle's side
+ *                     stream into a double-buffered staging area while the previous chunk computes on cuda_stream.
+ *                     The host buffers must stay valid until the copy has completed (synchronise cuda_stream).
+ * gwi_stream_finish   after exactly n_total samples: waits for cuda_stream, copies the records to the HOST array
+ *                     h_triggers (up to `capacity`, sorted by (slide, start)) and the total to *h_count.
+ *                     GWI_ERR_CAPACITY if the total exceeds either capacity (the returned prefix is then not guaranteed
+ *                     to be the globally first records).
+ * gwi_stream_destroy  frees the handle (NULL is a no-op).  The models must outlive the stream. */
+gwi_status gwi_stream_create(const gwi_model* const* models, int32_t n_models, const int64_t* lags, int32_t n_lags,
+                             int64_t n_total, int64_t max_chunk, float threshold, int64_t min_len, int32_t capacity,
+                             float* d_pbar, gwi_stream** out);
+int64_t gwi_stream_tail_samples(const gwi_stream* s);
+gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64_t n_tail, void* cuda_stream);
+gwi_status gwi_stream_push(gwi_stream* s, const void* d_h1, const void* d_l1, int64_t n, void* cuda_stream);
+gwi_status gwi_stream_push_host(gwi_stream* s, const void* h_h1, const void* h_l1, int64_t n, void* cuda_stream);
+gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, int32_t capacity, int32_t* h_count,
+                             void* cuda_stream);
+int64_t gwi_stream_samples_done(const gwi_stream* s);
+void gwi_stream_destroy(gwi_stream* s);
+
 /* ---- misc ---------------------------------------------------------------------------------------------- */
 const char* gwi_last_error(void);
 int gwi_version(void);

@@ -11,7 +11,9 @@ STATUS_NAMES = {0: "GWI_OK", 1: "GWI_ERR_ARG", 2: "GWI_ERR_IO", 3: "GWI_ERR_FORM
                 5: "GWI_ERR_CUDA", 6: "GWI_ERR_NOMEM", 7: "GWI_ERR_CAPACITY"}
 EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_model_uses_tensor_cores",
                     "gwi_infer_workspace_bytes", "gwi_infer", "gwi_carry_bytes", "gwi_triggers_workspace_bytes",
-                    "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count"]
+                    "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
+                    "gwi_stream_tail_samples", "gwi_stream_prime", "gwi_stream_push", "gwi_stream_push_host",
+                    "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_destroy"]
 
 
 class GwiError(RuntimeError):
@@ -59,6 +61,23 @@ def lib():
     L.gwi_ensemble_triggers.restype = C.c_int
     L.gwi_ensemble_triggers.argtypes = [C.POINTER(vp), C.c_int32, C.c_int64, C.c_int64, C.c_float, C.c_int64, C.c_int32,
                                         C.c_int, vp, vp, C.c_int32, vp, vp, vp, C.c_size_t, vp]
+    L.gwi_stream_create.restype = C.c_int
+    L.gwi_stream_create.argtypes = [C.POINTER(vp), C.c_int32, C.POINTER(C.c_int64), C.c_int32, C.c_int64, C.c_int64,
+                                    C.c_float, C.c_int64, C.c_int32, vp, C.POINTER(vp)]
+    L.gwi_stream_tail_samples.restype = C.c_int64
+    L.gwi_stream_tail_samples.argtypes = [vp]
+    L.gwi_stream_prime.restype = C.c_int
+    L.gwi_stream_prime.argtypes = [vp, vp, C.c_int64, vp]
+    L.gwi_stream_push.restype = C.c_int
+    L.gwi_stream_push.argtypes = [vp, vp, vp, C.c_int64, vp]
+    L.gwi_stream_push_host.restype = C.c_int
+    L.gwi_stream_push_host.argtypes = [vp, vp, vp, C.c_int64, vp]
+    L.gwi_stream_finish.restype = C.c_int
+    L.gwi_stream_finish.argtypes = [vp, vp, C.c_int32, i32p, vp]
+    L.gwi_stream_samples_done.restype = C.c_int64
+    L.gwi_stream_samples_done.argtypes = [vp]
+    L.gwi_stream_destroy.restype = None
+    L.gwi_stream_destroy.argtypes = [vp]
     L.gwi_last_error.restype = C.c_char_p
     L.gwi_version.restype = C.c_int
     L.gwi_launch_count.restype = C.c_int64
@@ -177,3 +196,70 @@ def ensemble_triggers(probs, threshold, min_len, t0=0, slide_id=0, last_chunk=Tr
 
 def new_carry(device=0):
     return torch.zeros(lib().gwi_carry_bytes(), dtype=torch.uint8, device=f"cuda:{device}" if isinstance(device, int) else device)
+
+
+class Stream:
+    """Handle on a gwi_stream (gwi_stream_create ... gwi_stream_destroy).  Marshalling only.
+
+    models: list of Model (same architecture / precision); lags: lags in samples; n_total: stream length;
+    max_chunk: largest push; want_pbar: keep the mean probability of every slide ([1+n_lags][n_total] float32 device
+    tensor in .pbar) for parity tests."""
+
+    def __init__(self, models, n_total, max_chunk, threshold=0.5, min_len=2048, lags=(), capacity=4096, want_pbar=False):
+        self.models = list(models)
+        self.device = torch.device("cuda", self.models[0].device)
+        self.dtype = torch.float16 if self.models[0].precision == FP16 else torch.float32
+        self.capacity = int(capacity)
+        self.pbar = (torch.zeros((1 + len(lags), int(n_total)), dtype=torch.float32, device=self.device)
+                     if want_pbar else None)
+        mp = (C.c_void_p * len(self.models))(*[m._h for m in self.models])
+        lg = (C.c_int64 * max(len(lags), 1))(*[int(v) for v in lags])
+        self._h = C.c_void_p()
+        _check(lib().gwi_stream_create(mp, len(self.models), lg, len(lags), int(n_total), int(max_chunk), float(threshold),
+                                       int(min_len), self.capacity,
+                                       C.c_void_p(self.pbar.data_ptr()) if want_pbar else None, C.byref(self._h)))
+
+    @property
+    def tail_samples(self):
+        return lib().gwi_stream_tail_samples(self._h)
+
+    def prime(self, l1_tail):
+        """l1_tail: the last .tail_samples samples of L1 (torch tensor on the host or the device)."""
+        assert l1_tail.dtype == self.dtype and l1_tail.is_contiguous()
+        _check(lib().gwi_stream_prime(self._h, C.c_void_p(l1_tail.data_ptr()), l1_tail.shape[-1], _stream_ptr(self.device)))
+        torch.cuda.current_stream(self.device).synchronize()   # the caller may free a host tail right away
+
+    def push(self, h1, l1):
+        """h1, l1: [n] tensors of the stream dtype; device tensors -> gwi_stream_push, host tensors (pin them) ->
+        gwi_stream_push_host."""
+        assert h1.dtype == self.dtype and l1.dtype == self.dtype and h1.is_contiguous() and l1.is_contiguous()
+        f = lib().gwi_stream_push if h1.is_cuda else lib().gwi_stream_push_host
+        _check(f(self._h, C.c_void_p(h1.data_ptr()), C.c_void_p(l1.data_ptr()), h1.shape[-1], _stream_ptr(self.device)))
+
+    @property
+    def samples_done(self):
+        return lib().gwi_stream_samples_done(self._h)
+
+    def finish(self):
+        """-> (count, [Trigger...]) sorted by (slide, start)."""
+        buf = (Trigger * max(self.capacity, 1))()
+        n = C.c_int32(0)
+        st = lib().gwi_stream_finish(self._h, buf, self.capacity, C.byref(n), _stream_ptr(self.device))
+        recs = [Trigger.from_buffer_copy(buf[i]) for i in range(min(n.value, self.capacity))]
+        if st == 7:
+            e = GwiError(7, last_error())
+            e.count, e.records = n.value, recs
+            raise e
+        _check(st)
+        return n.value, recs
+
+    def close(self):
+        if self._h:
+            lib().gwi_stream_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

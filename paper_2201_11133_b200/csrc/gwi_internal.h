@@ -70,6 +70,20 @@ size_t gwi_generic_workspace_bytes(const gwi_model* m, int64_t B, int32_t T);
 gwi_status gwi_generic_infer(const gwi_model* m, const void* d_strain, bool strain_is_half, int64_t B, int32_t T,
                              float* d_prob, void* d_ws, size_t ws_bytes, cudaStream_t st);
 
+// stream mode (gwi_stream.cu): branch stacks with per-layer history carried across chunks, head with an L1 lag
+int64_t gwi_generic_hist_floats(const gwi_model* m);
+gwi_status gwi_generic_stream_branches(const gwi_model* m, const void* d_strain, bool strain_is_half, int64_t ldx, int n,
+                                       float* hA, float* hB, int64_t ldh, float* skip, int64_t lds,
+                                       const float* hist_cur, float* hist_next, int br0, int nbr, cudaStream_t st);
+gwi_status gwi_generic_stream_head(const gwi_model* m, const float* skip, int64_t lds, int64_t lag, int n, float* d_prob,
+                                   cudaStream_t st);
+
+// ---- post-processing (gwi_post.cu) ---------------------------------------------------------------------------
+gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0, float threshold,
+                        int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry, gwi_trigger* d_triggers,
+                        int32_t capacity, int32_t* d_count, int append, float* d_pbar, void* d_workspace,
+                        size_t workspace_bytes, cudaStream_t st);
+
 // ---- tcgen05 path (gwi_tc.cu) -------------------------------------------------------------------------------
 bool gwi_tc_supported(const GwiArch& a);
 gwi_status gwi_tc_pack(gwi_model* m);

@@ -43,8 +43,8 @@ struct Header {            // per-call scratch header at the start of the worksp
     int32_t out_open;      // a run is open at the end of this chunk
     int32_t pad;
     int64_t out_start;     // its global start
-    int32_t total;         // number of records of this call
-    int32_t pad2;
+    int32_t total;         // records in the output buffer after this call (base + this call's)
+    int32_t base;          // records already in the buffer before this call (append mode; else 0)
 };
 
 __device__ __forceinline__ float ens_mean(const Ptrs& P, int M, int64_t i)
@@ -201,12 +201,16 @@ __global__ void k_runs(const uint32_t* __restrict__ bits, const uint8_t* __restr
 }
 
 __global__ void k_scan(const uint32_t* __restrict__ blkcnt, uint32_t* __restrict__ blkoff, int64_t nblk, int64_t t0,
-                       int slide, Header* hd, gwi_trigger* __restrict__ out, int capacity, int32_t* __restrict__ d_count)
+                       int slide, Header* hd, gwi_trigger* __restrict__ out, int capacity, int32_t* __restrict__ d_count,
+                       int append)
 {
     __shared__ uint32_t wsum[32];
     __shared__ uint32_t running;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    if (threadIdx.x == 0) running = (uint32_t)hd->head_emit;   // the carried run, if emitted, is record 0
+    if (threadIdx.x == 0) {
+        hd->base = append ? *d_count : 0;
+        running = (uint32_t)hd->base + (uint32_t)hd->head_emit;   // the carried run, if emitted, is the first new record
+    }
     __syncthreads();
     for (int64_t base = 0; base < nblk; base += blockDim.x) {
         int64_t i = base + threadIdx.x;
@@ -235,10 +239,10 @@ __global__ void k_scan(const uint32_t* __restrict__ blkcnt, uint32_t* __restrict
     if (threadIdx.x == 0) {
         hd->total = (int32_t)running;
         *d_count = (int32_t)running;
-        if (hd->head_emit && capacity > 0 && out) {
+        if (hd->head_emit && hd->base < capacity && out) {
             gwi_trigger r;
             r.slide = slide, r.model_mask = 0, r.start = hd->in.start, r.end = t0 + hd->head_end, r.peak_p = 0.f, r.mean_p = 0.f;
-            out[0] = r;
+            out[hd->base] = r;
         }
     }
 }
@@ -291,7 +295,7 @@ __global__ void k_stats(Ptrs P, int M, float theta, int64_t N, int64_t t0, const
         return;
     }
     if (!out) return;
-    for (int r = blockIdx.x; r < nrec; r += gridDim.x - 1) {
+    for (int r = hd->base + blockIdx.x; r < nrec; r += gridDim.x - 1) {
         int64_t s = out[r].start, e = out[r].end;
         int64_t a = s > t0 ? s - t0 : 0;
         float pk; double sm; int mk;
@@ -336,6 +340,16 @@ extern "C" gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t 
                                             void* d_carry, gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count,
                                             float* d_pbar, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
+    return gwi_post_run(d_prob, n_models, N, t0, threshold, min_len, slide_id, last_chunk, d_carry, d_triggers, capacity,
+                        d_count, 0, d_pbar, d_workspace, workspace_bytes, (cudaStream_t)cuda_stream);
+}
+
+// append != 0: *d_count holds the number of records already in d_triggers; the new ones go behind them.
+gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0, float threshold,
+                        int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry, gwi_trigger* d_triggers,
+                        int32_t capacity, int32_t* d_count, int append, float* d_pbar, void* d_workspace,
+                        size_t workspace_bytes, cudaStream_t st)
+{
     if (!d_prob || n_models < 1 || n_models > GWI_MAX_MODELS || N < 1 || capacity < 0 || !d_count || !d_workspace ||
         (capacity > 0 && !d_triggers) || ((uintptr_t)d_workspace & 255)) {
         gwi_set_error("gwi_ensemble_triggers: bad argument");
@@ -364,7 +378,6 @@ extern "C" gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t 
         return GWI_ERR_NOMEM;
     }
     if (!d_carry) last_chunk = 1;   // a chunk without carry is a whole stream
-    cudaStream_t st = (cudaStream_t)cuda_stream;
     char* ws = (char*)d_workspace;
     Header* hd = (Header*)(ws + L.hdr);
     uint32_t* bits = (uint32_t*)(ws + L.bits);
@@ -382,7 +395,7 @@ extern "C" gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t 
     k_head_run<<<1, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd);
     k_runs<0><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
                                              d_triggers, capacity);
-    k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count);
+    k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append);
     k_runs<1><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
                                              d_triggers, capacity);
     int sgrid = capacity < 1024 ? capacity + 1 : 1025;

@@ -1,0 +1,388 @@
+// gwi_stream.cu -- streaming ensemble driver (gwi_stream_*): SURVEY.md section 8 rows a-1, a-2, a-7, a-8..a-11.
+//
+//   a-1  host -> device streaming of strain chunks from (pinned) host buffers on a side stream, double-buffered, so
+//        that the copy of chunk c+1 overlaps the compute of chunk c
+//   a-2  overlap reuse: the stream is evaluated by ONE causal pass (reading A15: stitched 1 s windows with 0.5 s
+//        stride == one pass), every output sample computed once; the (k-1) d_i samples of each layer's input that
+//        precede a chunk are carried in a per-layer history (reading A17: chunked == unchunked, bit for bit)
+//   a-7  time slides on branch features (reading A24): p_k[t] = head(u_H1[t], u_L1[(t - lag_k) mod N]); the L1
+//        features of the last max-lag samples are kept in a ring, primed with the features of the stream's tail so
+//        that the circular wrap needs no second pass
+//   a-8..a-10  per slide: ensemble mean, strict threshold, run clustering with the run carried across chunks
+//   a-11 trigger records copied to the host at finish, sorted by (slide, start)
+//
+// The branch stacks run on the generic CUDA-core kernels (gwi_generic.cu) for every architecture: each output sample
+// is an independent, fixed-order fp32 accumulation, which is what makes chunked == unchunked exact.
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "gwi_internal.h"
+
+struct gwi_stream {
+    std::vector<const gwi_model*> models;
+    int M = 0, device = 0;
+    bool half_in = false;
+    std::vector<int64_t> lags;     // lags[0] = 0 (zero lag), then the caller's lags in samples
+    int64_t maxlag = 0, N_total = 0, min_len = 0, t_done = 0;
+    float theta = 0.5f;
+    int cap = 0, sub = 0;          // record capacity; internal sub-chunk length (samples)
+    int R = 0, S = 0, nb = 0, Rf = 0;
+    int64_t lds = 0;               // row stride of the skip buffers = maxlag + sub
+    bool primed = false, finished = false;
+    // device memory
+    void* d_x[2] = {nullptr, nullptr};   // staging: planar [nb*c_in][xcap] strain, double-buffered
+    int64_t xcap = 0;
+    float *d_hA = nullptr, *d_hB = nullptr;
+    std::vector<float*> d_skip;          // per model [nb][S][lds]; column maxlag = first sample of the sub-chunk
+    float* d_tmp = nullptr;              // [S][maxlag] scratch for the ring shift
+    std::vector<float*> d_hist[2];       // per model, ping-pong
+    int hist_cur = 0;
+    float* d_prob = nullptr;             // [n_slides][M][sub]
+    void* d_carry = nullptr;             // [n_slides] carry blocks
+    void* d_post_ws = nullptr;
+    size_t post_ws_bytes = 0;
+    gwi_trigger* d_trig = nullptr;
+    int32_t* d_count = nullptr;
+    float* d_pbar = nullptr;             // optional caller sink [n_slides][N_total]
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
+    int stage = 0;
+    int64_t launches = 0;
+};
+
+namespace {
+
+size_t elt(const gwi_stream* s) { return s->half_in ? 2 : 4; }
+
+// one sub-chunk of n <= sub samples, already in staging buffer `xb` at column `x0`
+gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStream_t st)
+{
+    const int nslides = (int)s->lags.size();
+    const char* x = (const char*)s->d_x[xb] + (size_t)x0 * elt(s);
+    for (int m = 0; m < s->M; m++) {
+        const gwi_model* gm = s->models[m];
+        float* skip0 = s->d_skip[m] + s->maxlag;
+        gwi_status rc = gwi_generic_stream_branches(gm, x, s->half_in, s->xcap, n, s->d_hA, s->d_hB, s->sub, skip0, s->lds,
+                                                    s->d_hist[s->hist_cur][m], s->d_hist[s->hist_cur ^ 1][m], 0, s->nb, st);
+        if (rc != GWI_OK) return rc;
+        for (int k = 0; k < nslides; k++) {
+            rc = gwi_generic_stream_head(gm, skip0, s->lds, s->lags[k], n, s->d_prob + ((size_t)k * s->M + m) * s->sub, st);
+            if (rc != GWI_OK) return rc;
+        }
+        if (s->maxlag > 0 && s->nb > 1) {
+            // ring shift: the last maxlag columns of the L1 (and later) branches move to the front
+            float* base = s->d_skip[m] + (size_t)s->S * s->lds;   // branch 1 onwards
+            size_t rows = (size_t)(s->nb - 1) * s->S;
+            GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_tmp, s->maxlag * 4, base + n, s->lds * 4, s->maxlag * 4, rows,
+                                             cudaMemcpyDeviceToDevice, st));
+            GWI_CUDA_CHECK(cudaMemcpy2DAsync(base, s->lds * 4, s->d_tmp, s->maxlag * 4, s->maxlag * 4, rows,
+                                             cudaMemcpyDeviceToDevice, st));
+        }
+    }
+    s->hist_cur ^= 1;
+    for (int k = 0; k < nslides; k++) {
+        const float* ptrs[GWI_MAX_MODELS];
+        for (int m = 0; m < s->M; m++) ptrs[m] = s->d_prob + ((size_t)k * s->M + m) * s->sub;
+        float* pb = s->d_pbar ? s->d_pbar + (size_t)k * s->N_total + s->t_done : nullptr;
+        gwi_status rc = gwi_post_run(ptrs, s->M, n, s->t_done, s->theta, s->min_len, k, last ? 1 : 0,
+                                     (char*)s->d_carry + (size_t)k * gwi_carry_bytes(), s->d_trig, s->cap, s->d_count, 1, pb,
+                                     s->d_post_ws, s->post_ws_bytes, st);
+        if (rc != GWI_OK) return rc;
+    }
+    s->t_done += n;
+    return GWI_OK;
+}
+
+gwi_status run_chunk(gwi_stream* s, int xb, int64_t n, cudaStream_t st)
+{
+    for (int64_t o = 0; o < n; o += s->sub) {
+        int nn = (int)std::min<int64_t>(s->sub, n - o);
+        bool last = (s->t_done + nn == s->N_total);
+        gwi_status rc = run_sub(s, xb, o, nn, last, st);
+        if (rc != GWI_OK) return rc;
+    }
+    return GWI_OK;
+}
+
+gwi_status check_push(gwi_stream* s, const void* a, const void* b, int64_t n, const char* who)
+{
+    if (!s || !a || (s->nb > 1 && !b) || n < 1) {
+        gwi_set_error("%s: bad argument", who);
+        return GWI_ERR_ARG;
+    }
+    if (s->finished || s->t_done + n > s->N_total) {
+        gwi_set_error("%s: %lld samples pushed + %lld > stream length %lld (or stream finished)", who, (long long)s->t_done,
+                      (long long)n, (long long)s->N_total);
+        return GWI_ERR_ARG;
+    }
+    if (n > s->xcap) {
+        gwi_set_error("%s: chunk of %lld samples > max_chunk %lld", who, (long long)n, (long long)s->xcap);
+        return GWI_ERR_ARG;
+    }
+    if (s->maxlag > 0 && !s->primed) {
+        gwi_set_error("%s: a stream with time slides must be primed with gwi_stream_prime first", who);
+        return GWI_ERR_ARG;
+    }
+    return GWI_OK;
+}
+
+} // namespace
+
+extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t n_models, const int64_t* lags,
+                                        int32_t n_lags, int64_t n_total, int64_t max_chunk, float threshold,
+                                        int64_t min_len, int32_t capacity, float* d_pbar, gwi_stream** out)
+{
+    if (!models || n_models < 1 || n_models > GWI_MAX_MODELS || n_lags < 0 || (n_lags > 0 && !lags) || n_total < 1 ||
+        max_chunk < 1 || min_len < 1 || capacity < 1 || !out) {
+        gwi_set_error("gwi_stream_create: bad argument");
+        return GWI_ERR_ARG;
+    }
+    *out = nullptr;
+    const gwi_model* m0 = models[0];
+    for (int i = 0; i < n_models; i++) {
+        const gwi_model* m = models[i];
+        if (!m || m->device != m0->device || m->prec != m0->prec || m->arch.n_branch != m0->arch.n_branch ||
+            m->arch.c_in != m0->arch.c_in || m->arch.R != m0->arch.R || m->arch.S != m0->arch.S || m->arch.k != m0->arch.k ||
+            m->arch.L != m0->arch.L) {
+            gwi_set_error("gwi_stream_create: the models of an ensemble must share device, precision and architecture");
+            return GWI_ERR_ARG;
+        }
+        for (int l = 0; l < m->arch.L; l++)
+            if (m->arch.dil[l] != m0->arch.dil[l]) {
+                gwi_set_error("gwi_stream_create: the models of an ensemble must share the dilation schedule");
+                return GWI_ERR_ARG;
+            }
+    }
+    gwi_stream* s = new (std::nothrow) gwi_stream();
+    if (!s) return GWI_ERR_NOMEM;
+    s->models.assign(models, models + n_models);
+    s->M = n_models, s->device = m0->device, s->half_in = (m0->prec == GWI_FP16);
+    s->lags.push_back(0);
+    for (int i = 0; i < n_lags; i++) {
+        if (lags[i] < 1 || lags[i] >= n_total) {
+            gwi_set_error("gwi_stream_create: lag %lld outside [1, n_total)", (long long)lags[i]);
+            delete s;
+            return GWI_ERR_ARG;
+        }
+        if (m0->arch.n_branch < 2) {
+            gwi_set_error("gwi_stream_create: time slides need a two-branch model (reading A24)");
+            delete s;
+            return GWI_ERR_UNSUPPORTED;
+        }
+        s->lags.push_back(lags[i]);
+        s->maxlag = std::max(s->maxlag, lags[i]);
+    }
+    s->N_total = n_total, s->min_len = min_len, s->theta = threshold, s->cap = capacity, s->d_pbar = d_pbar;
+    s->R = m0->arch.R, s->S = m0->arch.S, s->nb = m0->arch.n_branch, s->Rf = m0->arch.receptive_field();
+    s->xcap = std::max<int64_t>(std::min(max_chunk, n_total), std::min<int64_t>(n_total, s->maxlag + s->Rf - 1));
+    // sub-chunk: bounds the activation workspace (2R floats per branch-sample) to ~2 GiB
+    int64_t per = (int64_t)s->nb * 2 * s->R * 4;
+    int64_t sub = std::max<int64_t>(4096, (2LL << 30) / per);
+    sub = std::min<int64_t>(sub, 1 << 24);
+    sub = std::min<int64_t>(sub, s->xcap);
+    s->sub = (int)sub;
+    s->lds = s->maxlag + s->sub;
+    const int nslides = (int)s->lags.size();
+    const int C = s->nb * m0->arch.c_in;
+    auto fail = [&](cudaError_t e) {
+        gwi_set_error("gwi_stream_create: %s", cudaGetErrorString(e));
+        gwi_stream_destroy(s);
+        return e == cudaErrorMemoryAllocation ? GWI_ERR_NOMEM : GWI_ERR_CUDA;
+    };
+    cudaError_t e;
+    if ((e = cudaSetDevice(s->device)) != cudaSuccess) return fail(e);
+    for (int b = 0; b < 2; b++)
+        if ((e = cudaMalloc(&s->d_x[b], (size_t)C * s->xcap * elt(s))) != cudaSuccess) return fail(e);
+    size_t hbytes = (size_t)s->nb * s->R * s->sub * 4;
+    if ((e = cudaMalloc(&s->d_hA, hbytes)) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&s->d_hB, hbytes)) != cudaSuccess) return fail(e);
+    size_t histb = (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(m0)) * 4;
+    s->d_skip.assign(s->M, nullptr);
+    s->d_hist[0].assign(s->M, nullptr), s->d_hist[1].assign(s->M, nullptr);
+    for (int m = 0; m < s->M; m++) {
+        size_t sb = (size_t)s->nb * s->S * s->lds * 4;
+        if ((e = cudaMalloc(&s->d_skip[m], sb)) != cudaSuccess) return fail(e);
+        if ((e = cudaMemset(s->d_skip[m], 0, sb)) != cudaSuccess) return fail(e);
+        for (int b = 0; b < 2; b++) {
+            if ((e = cudaMalloc(&s->d_hist[b][m], histb)) != cudaSuccess) return fail(e);
+            if ((e = cudaMemset(s->d_hist[b][m], 0, histb)) != cudaSuccess) return fail(e);   // zero history == A4 padding
+        }
+    }
+    if (s->maxlag > 0 && (e = cudaMalloc(&s->d_tmp, (size_t)(s->nb - 1) * s->S * s->maxlag * 4)) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&s->d_prob, (size_t)nslides * s->M * s->sub * 4)) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&s->d_carry, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
+    if ((e = cudaMemset(s->d_carry, 0, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
+    s->post_ws_bytes = gwi_triggers_workspace_bytes(s->sub);
+    if ((e = cudaMalloc(&s->d_post_ws, s->post_ws_bytes)) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&s->d_trig, (size_t)capacity * sizeof(gwi_trigger))) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&s->d_count, 4)) != cudaSuccess) return fail(e);
+    if ((e = cudaMemset(s->d_count, 0, 4)) != cudaSuccess) return fail(e);
+    if ((e = cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) return fail(e);
+    for (int b = 0; b < 2; b++) {
+        if ((e = cudaEventCreateWithFlags(&s->ev_copied[b], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
+        if ((e = cudaEventCreateWithFlags(&s->ev_consumed[b], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
+    }
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(e);
+    *out = s;
+    return GWI_OK;
+}
+
+extern "C" void gwi_stream_destroy(gwi_stream* s)
+{
+    if (!s) return;
+    cudaSetDevice(s->device);
+    cudaDeviceSynchronize();
+    for (int b = 0; b < 2; b++) {
+        if (s->d_x[b]) cudaFree(s->d_x[b]);
+        for (float* p : s->d_hist[b])
+            if (p) cudaFree(p);
+        if (s->ev_copied[b]) cudaEventDestroy(s->ev_copied[b]);
+        if (s->ev_consumed[b]) cudaEventDestroy(s->ev_consumed[b]);
+    }
+    for (float* p : s->d_skip)
+        if (p) cudaFree(p);
+    if (s->d_hA) cudaFree(s->d_hA);
+    if (s->d_hB) cudaFree(s->d_hB);
+    if (s->d_tmp) cudaFree(s->d_tmp);
+    if (s->d_prob) cudaFree(s->d_prob);
+    if (s->d_carry) cudaFree(s->d_carry);
+    if (s->d_post_ws) cudaFree(s->d_post_ws);
+    if (s->d_trig) cudaFree(s->d_trig);
+    if (s->d_count) cudaFree(s->d_count);
+    if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
+    delete s;
+}
+
+extern "C" int64_t gwi_stream_tail_samples(const gwi_stream* s)
+{
+    if (!s || s->maxlag == 0) return 0;
+    return std::min<int64_t>(s->N_total, s->maxlag + s->Rf - 1);
+}
+
+extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64_t n_tail, void* cuda_stream)
+{
+    if (!s || !l1_tail || s->maxlag == 0 || n_tail != gwi_stream_tail_samples(s) || s->t_done != 0) {
+        gwi_set_error("gwi_stream_prime: bad argument (n_tail must equal gwi_stream_tail_samples(), before the first push)");
+        return GWI_ERR_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    GWI_CUDA_CHECK(cudaSetDevice(s->device));
+    const int c_in = s->models[0]->arch.c_in;
+    // the tail goes to the branch-1 rows of staging buffer 0 (cudaMemcpyDefault: host or device source)
+    GWI_CUDA_CHECK(cudaMemcpy2DAsync((char*)s->d_x[0] + (size_t)c_in * s->xcap * elt(s), s->xcap * elt(s), l1_tail,
+                                     n_tail * elt(s), n_tail * elt(s), (size_t)c_in * (s->nb - 1), cudaMemcpyDefault, st));
+    // features of the tail: zero history is exact for the last maxlag samples because either the tail starts at t = 0
+    // or it starts R_f - 1 samples before them
+    for (int m = 0; m < s->M; m++) {
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
+        for (int64_t o = 0; o < n_tail; o += s->sub) {
+            int nn = (int)std::min<int64_t>(s->sub, n_tail - o);
+            gwi_status rc = gwi_generic_stream_branches(s->models[m], (const char*)s->d_x[0] + (size_t)o * elt(s), s->half_in,
+                                                        s->xcap, nn, s->d_hA, s->d_hB, s->sub, s->d_skip[m] + s->maxlag,
+                                                        s->lds, s->d_hist[0][m], s->d_hist[1][m], 1, s->nb - 1, st);
+            if (rc != GWI_OK) return rc;
+            // keep the last maxlag columns seen so far at the front of the ring, exactly as run_sub does
+            float* base = s->d_skip[m] + (size_t)s->S * s->lds;
+            size_t rows = (size_t)(s->nb - 1) * s->S;
+            GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_tmp, s->maxlag * 4, base + nn, s->lds * 4, s->maxlag * 4, rows,
+                                             cudaMemcpyDeviceToDevice, st));
+            GWI_CUDA_CHECK(cudaMemcpy2DAsync(base, s->lds * 4, s->d_tmp, s->maxlag * 4, s->maxlag * 4, rows,
+                                             cudaMemcpyDeviceToDevice, st));
+            // history ping-pong inside the tail pass
+            std::swap(s->d_hist[0][m], s->d_hist[1][m]);
+        }
+        // the real pass starts from zero history again
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[1][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
+    }
+    s->hist_cur = 0;
+    s->primed = true;
+    return GWI_OK;
+}
+
+extern "C" gwi_status gwi_stream_push(gwi_stream* s, const void* d_h1, const void* d_l1, int64_t n, void* cuda_stream)
+{
+    gwi_status rc = check_push(s, d_h1, d_l1, n, "gwi_stream_push");
+    if (rc != GWI_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    GWI_CUDA_CHECK(cudaSetDevice(s->device));
+    const int c_in = s->models[0]->arch.c_in;
+    const int b = s->stage;
+    // staging buffer b may still be read by work enqueued on another caller stream
+    GWI_CUDA_CHECK(cudaStreamWaitEvent(st, s->ev_consumed[b], 0));
+    size_t rowb = (size_t)s->xcap * elt(s);
+    GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_x[b], rowb, d_h1, n * elt(s), n * elt(s), c_in, cudaMemcpyDeviceToDevice, st));
+    if (s->nb > 1)
+        GWI_CUDA_CHECK(cudaMemcpy2DAsync((char*)s->d_x[b] + c_in * rowb, rowb, d_l1, n * elt(s), n * elt(s),
+                                         (size_t)c_in * (s->nb - 1), cudaMemcpyDeviceToDevice, st));
+    rc = run_chunk(s, b, n, st);
+    if (rc != GWI_OK) return rc;
+    GWI_CUDA_CHECK(cudaEventRecord(s->ev_consumed[b], st));
+    s->stage ^= 1;
+    return GWI_OK;
+}
+
+extern "C" gwi_status gwi_stream_push_host(gwi_stream* s, const void* h_h1, const void* h_l1, int64_t n, void* cuda_stream)
+{
+    gwi_status rc = check_push(s, h_h1, h_l1, n, "gwi_stream_push_host");
+    if (rc != GWI_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    GWI_CUDA_CHECK(cudaSetDevice(s->device));
+    const int c_in = s->models[0]->arch.c_in;
+    const int b = s->stage;
+    size_t rowb = (size_t)s->xcap * elt(s);
+    // H2D on the side stream, as soon as the compute that last read staging buffer b has finished; the compute of
+    // the previous chunk (other buffer) keeps running meanwhile
+    GWI_CUDA_CHECK(cudaStreamWaitEvent(s->copy_stream, s->ev_consumed[b], 0));
+    GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_x[b], rowb, h_h1, n * elt(s), n * elt(s), c_in, cudaMemcpyHostToDevice, s->copy_stream));
+    if (s->nb > 1)
+        GWI_CUDA_CHECK(cudaMemcpy2DAsync((char*)s->d_x[b] + c_in * rowb, rowb, h_l1, n * elt(s), n * elt(s),
+                                         (size_t)c_in * (s->nb - 1), cudaMemcpyHostToDevice, s->copy_stream));
+    GWI_CUDA_CHECK(cudaEventRecord(s->ev_copied[b], s->copy_stream));
+    GWI_CUDA_CHECK(cudaStreamWaitEvent(st, s->ev_copied[b], 0));
+    rc = run_chunk(s, b, n, st);
+    if (rc != GWI_OK) return rc;
+    GWI_CUDA_CHECK(cudaEventRecord(s->ev_consumed[b], st));
+    s->stage ^= 1;
+    return GWI_OK;
+}
+
+extern "C" gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, int32_t capacity, int32_t* h_count,
+                                        void* cuda_stream)
+{
+    if (!s || !h_count || capacity < 0 || (capacity > 0 && !h_triggers)) {
+        gwi_set_error("gwi_stream_finish: bad argument");
+        return GWI_ERR_ARG;
+    }
+    if (s->t_done != s->N_total) {
+        gwi_set_error("gwi_stream_finish: %lld of %lld samples pushed", (long long)s->t_done, (long long)s->N_total);
+        return GWI_ERR_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    GWI_CUDA_CHECK(cudaSetDevice(s->device));
+    int32_t n = 0;
+    GWI_CUDA_CHECK(cudaMemcpyAsync(&n, s->d_count, 4, cudaMemcpyDeviceToHost, st));
+    GWI_CUDA_CHECK(cudaStreamSynchronize(st));
+    int have = std::min(n, s->cap);
+    std::vector<gwi_trigger> recs((size_t)have);
+    if (have > 0) {
+        GWI_CUDA_CHECK(cudaMemcpyAsync(recs.data(), s->d_trig, (size_t)have * sizeof(gwi_trigger), cudaMemcpyDeviceToHost, st));
+        GWI_CUDA_CHECK(cudaStreamSynchronize(st));
+    }
+    // records arrive grouped by sub-chunk; the list is sorted by (slide, start)
+    std::stable_sort(recs.begin(), recs.end(), [](const gwi_trigger& a, const gwi_trigger& b) {
+        return a.slide != b.slide ? a.slide < b.slide : a.start < b.start;
+    });
+    int give = std::min(have, capacity);
+    for (int i = 0; i < give; i++) h_triggers[i] = recs[i];
+    *h_count = n;
+    s->finished = true;
+    if (n > s->cap || n > capacity) {
+        gwi_set_error("gwi_stream_finish: %d triggers, stream capacity %d, caller capacity %d", n, s->cap, capacity);
+        return GWI_ERR_CAPACITY;
+    }
+    return GWI_OK;
+}
+
+extern "C" int64_t gwi_stream_samples_done(const gwi_stream* s) { return s ? s->t_done : -1; }

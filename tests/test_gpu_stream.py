@@ -1,0 +1,184 @@
+"""GPU parity of the streaming ensemble driver (gwi_stream_*) against the oracle (-m gpu).
+
+Rows a-1, a-2, a-7..a-11 of SURVEY.md section 8: one causal pass over a stream pushed in ragged chunks (device and
+pinned-host pushes), per-layer history carried across chunks, circular time slides on branch features, ensemble mean,
+threshold, run clustering across chunk boundaries, records sorted by (slide, start).
+
+Oracle side: gwo.Model.stream (direct definition over the whole stream), gwo.Model.head_slide (reading A24),
+gwo.ensemble_mean, gwo.triggers.  Bars: FP32 mode 1e-5, FP16 mode 2e-3 on the mean probabilities; trigger lists exact
+on delta-robust instances (P15: the oracle's lists at theta +- delta coincide); chunked == unchunked bit for bit.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import gwsynth as gs
+from oracle import gwo
+from tests.helpers import trig_tuples
+
+pytestmark = pytest.mark.gpu
+
+ARCH = gs.CFG1_ARCH
+
+
+def _models(tmp, seeds, prec, bias="zero", arch=ARCH):
+    import paper_2201_11133_b200 as gwi
+    oms, gms = [], []
+    for s in seeds:
+        path = os.path.join(str(tmp), f"m{s}_{bias}_{arch.R}.gwim")
+        gs.make_model_file(path, arch, s, bias=bias)
+        oms.append(gwo.Model(path, round_fp16=(prec == gwi.FP16)))
+        gms.append(gwi.load_model(path, prec, 0))
+    return oms, gms
+
+
+def _oracle_slides(oms, x, lags):
+    """-> pbar [1+len(lags)][N] float64 by the definition."""
+    N = x.shape[1]
+    per = []
+    for om in oms:
+        p0, u = om.stream(x.astype(np.float64), want_u=True)
+        ps = [p0] + [om.head_slide(u, lag) for lag in lags]
+        per.append(ps)
+    return np.stack([gwo.ensemble_mean([per[m][k] for m in range(len(oms))]) for k in range(1 + len(lags))])
+
+
+def _oracle_triggers(pbar, theta, lmin):
+    out = []
+    for k in range(pbar.shape[0]):
+        _, recs = gwo.triggers(pbar[k], theta, lmin, slide=k)
+        out += [(r[0], r[1], r[2]) for r in recs]
+    return out
+
+
+def _run_stream(gms, x, chunks, lags, theta, lmin, host=False, max_chunk=None):
+    import torch
+    import paper_2201_11133_b200 as gwi
+    N = x.shape[1]
+    st = gwi.Stream(gms, N, max_chunk or max(chunks), theta, lmin, lags=lags, capacity=4096, want_pbar=True)
+    xt = torch.from_numpy(x)
+    if lags:
+        nt = st.tail_samples
+        assert nt == min(N, max(lags) + gms[0].receptive_field - 1)
+        st.prime(xt[1, N - nt:].contiguous())
+    pos = 0
+    keep = []
+    for n in chunks:
+        a, b = xt[0, pos:pos + n].contiguous(), xt[1, pos:pos + n].contiguous()
+        if host:
+            a, b = a.pin_memory(), b.pin_memory()
+        else:
+            a, b = a.cuda(), b.cuda()
+        keep.append((a, b))
+        st.push(a, b)
+        pos += n
+    assert pos == N and st.samples_done == N
+    n, recs = st.finish()
+    pbar = st.pbar.cpu().numpy()
+    st.close()
+    return n, recs, pbar
+
+
+def _ragged(N, seed, lo, hi):
+    rs = np.random.RandomState(seed)
+    out, left = [], N
+    while left > 0:
+        n = int(min(left, rs.randint(lo, hi)))
+        out.append(n)
+        left -= n
+    return out
+
+
+@pytest.mark.parametrize("prec_name,tol,bias", [("FP32", 1e-5, "zero"), ("FP32", 1e-5, "random"), ("FP16", 2e-3, "zero")])
+def test_stream_ensemble_slides_parity(tmpdir_s, prec_name, tol, bias):
+    import paper_2201_11133_b200 as gwi
+    prec = getattr(gwi, prec_name)
+    oms, gms = _models(tmpdir_s, [0, 1, 2, 3], prec, bias=bias)
+    N = 3 * 4096 + 777
+    dt = np.float16 if prec == gwi.FP16 else np.float32
+    x = gs.stream_noise(1, 0, N, dtype=dt)
+    lags = [4096, 2 * 4096, 5000]
+    want = _oracle_slides(oms, x, lags)
+    chunks = _ragged(N, 3, 1, 3000)
+    n, recs, pbar = _run_stream(gms, x, chunks, lags, 0.5, 8, max_chunk=3000)
+    err = np.max(np.abs(pbar - want))
+    assert err <= tol, err
+    # lists on the oracle's own mean are robust against tol?  compare only if they are (P15), else on the GPU mean
+    lo, hi = _oracle_triggers(want, 0.5 - 2 * tol, 8), _oracle_triggers(want, 0.5 + 2 * tol, 8)
+    got = trig_tuples(recs)
+    assert n == len(got)
+    if lo == hi:
+        assert got == lo
+    # tier T1: the list equals the oracle's clustering of the GPU's own mean, exactly, for every input
+    assert got == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 8)
+    assert got == sorted(got)
+
+
+def test_chunked_equals_unchunked_bitwise_and_host_push(tmpdir_s):
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1], gwi.FP16)
+    N = 40000
+    x = gs.stream_noise(7, 0, N, dtype=np.float16)
+    lags = [4096]
+    n0, r0, p0 = _run_stream(gms, x, [N], lags, 0.5, 16)
+    n1, r1, p1 = _run_stream(gms, x, _ragged(N, 5, 1, 9000), lags, 0.5, 16, max_chunk=9000)
+    n2, r2, p2 = _run_stream(gms, x, _ragged(N, 6, 2000, 9000), lags, 0.5, 16, host=True, max_chunk=9000)
+    assert np.array_equal(p0, p1) and np.array_equal(p0, p2)
+    assert trig_tuples(r0) == trig_tuples(r1) == trig_tuples(r2) and n0 == n1 == n2
+    for a, b in zip(r0, r1):
+        assert a.peak_p == b.peak_p and abs(a.mean_p - b.mean_p) <= 1e-6 and a.model_mask == b.model_mask
+
+
+def test_stream_equals_stitched_windows(tmpdir_s):
+    """Reading A15 on the GPU: the last 2048 outputs of each 1 s window taken every 0.5 s equal the stream pass."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0], gwi.FP32)
+    N = 6 * 2048
+    x = gs.stream_noise(9, 0, N, dtype=np.float32)
+    _, _, pbar = _run_stream(gms, x, [5000, N - 5000], [], 0.5, 2048)
+    nwin = (N - 4096) // 2048 + 1
+    wins = np.stack([x[:, i * 2048:i * 2048 + 4096].T for i in range(nwin)])
+    pw = gms[0].infer(torch.from_numpy(np.ascontiguousarray(wins)).cuda()).cpu().numpy()
+    assert np.max(np.abs(pw[0] - pbar[0, :4096])) <= 1e-6
+    for i in range(1, nwin):
+        assert np.max(np.abs(pw[i, 2048:] - pbar[0, i * 2048 + 2048:i * 2048 + 4096])) <= 1e-6
+
+
+def test_stream_triggers_with_plateaus_cross_chunks(tmpdir_s):
+    """P16-style sign pass-through model: supra-threshold plateaus of known extent, cut by chunk boundaries."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1, 2, 3], gwi.FP32)
+    N = 30000
+    x = gs.stream_noise(11, 0, N, dtype=np.float32)
+    want = _oracle_slides(oms, x, [])
+    theta = float(np.median(want[0]))           # half of the samples above: many runs of many lengths
+    n, recs, pbar = _run_stream(gms, x, _ragged(N, 8, 100, 2500), [], theta, 3, max_chunk=2500)
+    got = trig_tuples(recs)
+    assert got == _oracle_triggers(pbar.astype(np.float64), float(np.float32(theta)), 3)
+    assert len(got) > 20
+    assert np.max(np.abs(pbar - want)) <= 1e-5
+
+
+def test_stream_argument_errors(tmpdir_s):
+    import torch
+    import paper_2201_11133_b200 as gwi
+    _, gms = _models(tmpdir_s, [0], gwi.FP32)
+    st = gwi.Stream(gms, 1000, 500, lags=[100])
+    x = torch.zeros(500, dtype=torch.float32, device="cuda")
+    with pytest.raises(gwi.GwiError):      # slides need priming
+        st.push(x, x)
+    st.prime(torch.zeros(st.tail_samples, dtype=torch.float32))
+    st.push(x, x)
+    with pytest.raises(gwi.GwiError):      # finish before the stream is complete
+        st.finish()
+    with pytest.raises(gwi.GwiError):      # chunk larger than max_chunk
+        st.push(torch.zeros(501, dtype=torch.float32, device="cuda"), torch.zeros(501, dtype=torch.float32, device="cuda"))
+    st.push(x, x)
+    with pytest.raises(gwi.GwiError):      # more than n_total
+        st.push(x, x)
+    n, recs = st.finish()
+    assert n == len(recs)
+    with pytest.raises(gwi.GwiError):
+        gwi.Stream(gms, 1000, 500, lags=[1000])
