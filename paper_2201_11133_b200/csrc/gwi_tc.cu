@@ -2,7 +2,7 @@
 //
 // Two kernels, both hand-written tcgen05 (sm_100a) with accumulators in TMEM:
 //
-//  k_stack  one persistent CTA per SM walks "jobs" = (pair of windows, branch).  For every 128-timestep tile it runs
+//  k_stack  one persistent CTA per SM walks jobs" = (pair of windows
 //           the lift and all L gated residual blocks depth-first (DESIGN.md C.1 steps 1-3), so that
 //           no activation of a block ever goes to HBM:
 //             GEMM1  [128 x 128] = [h(t-d) | h(t)] [128 x 128] . [Wf|Wg/2]^T      (tcgen05.mma, fp32 accum in TMEM)
@@ -13,7 +13,7 @@
 //           buffer addressed d rows earlier (no-swizzle K-major layout, rows 16 bytes apart), so a dilation costs no
 //           data movement; the d rows that precede a tile come from a per-layer stash in shared memory (d <= 64) or,
 //           for d = 128, 256, 512, from an L2-resident ring in global memory that the bulk-copy engine prefetches.
-//           Two windows ("slots") are in flight per CTA so that the tensor pipe works on one while the epilogue
+//           Two windows (slots") are in flight per CTA so that the tensor pipe works on one while the epilogue"
 //           warps gate the other.  Output: u = ReLU(sum of skips) per branch, fp16, tile-major in the workspace.
 //  k_head   [128 x 128] = [u_H | u_L] . W1^T on tcgen05, then ReLU, dot with W2, sigmoid (C.1 steps 4-5).
 //
@@ -22,8 +22,8 @@
 #include <cstring>
 #include <vector>
 
-#include "gwi_internal.h"
-#include "gwi_tc_ptx.h"
+#include gwi_internal.h""
+#include gwi_tc_ptx.h""
 
 using namespace tc;
 
@@ -33,50 +33,79 @@ constexpr int TM = 128;                 // timesteps per tile = MMA M
 constexpr int TC_MAX_L = 20;
 constexpr int WFG_BYTES = 128 * 128 * 2;            // B operand of GEMM1: N = 128 (f|g) x K = 128 (past|current)
 constexpr int WRS_BYTES = 192 * 64 * 2;             // B operand of GEMM2: N = 192 (skip|res) x K = 64
+constexpr int BIAS_FLOATS = 192;                    // per layer: bf[64], bg/2[64], br[64]; streamed behind Wrs
+constexpr int WRS_STRIDE = WRS_BYTES + BIAS_FLOATS * 4;   // 25344
 constexpr int X_CHUNK = 192 * 16;                   // chunk-column stride of the X buffer (64 pre rows + 128 rows)
 constexpr int X_BYTES = 8 * X_CHUNK;                // 24576
 constexpr int PST_BYTES = 8 * 128 * 16;             // 16384: one past tile, chunk stride 2048
-constexpr int STASH_BYTES = 32768;                  // per slot: sum over layers with d <= 64 of d rows x 128 B
-constexpr int BIAS_FLOATS = 192;                    // per layer: bf[64], bg/2[64], br[64]
+constexpr int PRE_BYTES = 8 * 64 * 16;              // 8192: the 64 rows that precede a tile (d = 64 layers)
+constexpr int STASH_BYTES = 16384;                  // per slot: sum over layers with d <= 32 of d rows x 128 B
 constexpr int U_TILE_BYTES = 16 * 128 * 16;         // 32768: u tile, 16 chunks x 128 rows x 16 B
-constexpr int NTHREADS = 320;
+constexpr int NEPI = 16;                            // epilogue warps: slot = w >> 3, column half = (w >> 2) & 1
+constexpr int NTHREADS = (NEPI + 2) * 32;           // + producer warp + MMA warp
 
 struct TcMeta {
     int L, n_branch;
     int dil[TC_MAX_L];
-    int big[TC_MAX_L];        // 1: d is a multiple of 128 (history through the global ring), 0: d <= 64 (stash)
-    int D[TC_MAX_L];          // d / 128 for big layers
+    int kind[TC_MAX_L];       // 0: d <= 32 (stash in shared memory), 1: d == 64 (pre rows through the global ring64),
+                              // 2: d multiple of 128 (whole past tiles through the global ring)
+    int D[TC_MAX_L];          // d / 128 for kind 2
     int stash_off[TC_MAX_L];  // byte offset of the layer's stash inside the slot's stash area
-    int ring_off[TC_MAX_L];   // first ring entry (in tiles) of the layer
+    int ring_off[TC_MAX_L];   // kind 2: first ring entry (in tiles) of the layer; kind 1: index among the d = 64 layers
     int ring_tiles;           // ring entries per slot
+    int n64;                  // number of d = 64 layers
 };
 
 struct StackArgs {
     const uint8_t* wfg;   // [n_branch][L][WFG_BYTES]
-    const uint8_t* wrs;   // [n_branch][L][WRS_BYTES]
-    const float* bias;    // [n_branch][L][192]
+    const uint8_t* wrs;   // [n_branch][L][WRS_STRIDE]  (Wrs operand followed by the layer's 192 bias floats)
     const float* cst;     // [n_branch][256]: W_in[64], b_in[64], sum_i bs_i[128]
     const __half* strain; // [B][T][C]
     int64_t w0, nwin;     // windows [w0, w0 + nwin) of this launch
     int T, ntiles, C;
     uint8_t* ring;        // [gridDim.x][2][ring_tiles][PST_BYTES]
+    uint8_t* ring64;      // [gridDim.x][2][n64][2][PRE_BYTES]
     uint8_t* u;           // [nwin][n_branch][ntiles][U_TILE_BYTES]
     TcMeta meta;
 };
 
 // ---- shared memory map of k_stack ----------------------------------------------------------------------------------
-constexpr int SM_WFG = 0;
-constexpr int SM_WRS = SM_WFG + WFG_BYTES;
-constexpr int SM_X = SM_WRS + WRS_BYTES;                  // 2 slots
+constexpr int SM_WFG = 0;                                 // 2 stages
+constexpr int SM_WRS = SM_WFG + 2 * WFG_BYTES;            // 2 stages
+constexpr int SM_X = SM_WRS + 2 * WRS_STRIDE;             // 2 slots
 constexpr int SM_PST = SM_X + 2 * X_BYTES;                // 2 slots
 constexpr int SM_STASH = SM_PST + 2 * PST_BYTES;          // 2 slots
-constexpr int SM_BIAS = SM_STASH + 2 * STASH_BYTES;       // L x 192 floats
-constexpr int SM_BAR = SM_BIAS + TC_MAX_L * BIAS_FLOATS * 4;
+constexpr int SM_BAR = SM_STASH + 2 * STASH_BYTES;
 constexpr int SM_TOTAL = SM_BAR + 256;
+static_assert(SM_TOTAL <= 232448, shared memory budget");"
 
-enum { B_WFG_FULL = 0, B_WFG_FREE, B_WRS_FULL, B_WRS_FREE, B_FG_FULL, B_Z_READY = B_FG_FULL + 2, B_RS_FULL = B_Z_READY + 2,
-       B_H_READY = B_RS_FULL + 2, B_PST_FULL = B_H_READY + 2, B_PST_FREE = B_PST_FULL + 2, B_COUNT = B_PST_FREE + 2 };
+enum { B_WFG_FULL = 0, B_WFG_FREE = 2, B_WRS_FULL = 4, B_WRS_FREE = 6, B_FG_FULL = 8, B_Z_READY = 10, B_RS_FULL = 12,
+       B_H_READY = 14, B_PST_FULL = 16, B_PST_FREE = 18, B_PRE_FULL = 20, B_COUNT = 22 };
 
+__device__ __forceinline__ float2 add2(float2 a, float2 b)
+{
+    float2 r;
+    asm({\n\t.reg .b64 ra
+        mov.b64 {%0
+        : =f"(r.x)
+        : f"(a.x)
+    return r;
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
+{
+    float2 r;
+    asm({\n\t.reg .b64 ra
+        fma.rn.f32x2 rd
+        : =f"(r.x)
+        : f"(a.x)
+    return r;
+}
+
+// Schedule (one CTA per SM, persistent over jobs = (pair of windows, branch)).  The two windows of a job are two
+// slots" that run the same (tile
+//     G1(slot 0, n)  G2(slot 1, n-1)  G1(slot 1, n)  G2(slot 0, n)          n = (tile, layer) iteration
+// so that while one slot's 8 epilogue warps gate (MUFU-bound), the tensor pipe and the other slot's warps work on the
+// other slot.  Weights (and the layer's biases) are double-buffered and shared by the two slots.
 __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -89,12 +118,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < B_COUNT; i++) {
-            uint32_t cnt = (i >= B_Z_READY && i < B_Z_READY + 2) || (i >= B_H_READY && i < B_H_READY + 2) ? 128u : 1u;
+            uint32_t cnt = (i >= B_Z_READY && i < B_Z_READY + 2) || (i >= B_H_READY && i < B_H_READY + 2) ? 256u : 1u;
             mbar_init(bar(i), cnt);
         }
         mbar_fence_init();
     }
-    if (warp == 8) tmem_alloc(smem_u32(tmem_slot), 512);
+    if (warp == NEPI) tmem_alloc(smem_u32(tmem_slot), 512);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -103,19 +132,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 
     const int64_t npairs = (a.nwin + 1) / 2;
     const int64_t njobs = npairs * nb;
+    const int NI = a.ntiles * L;
     // phase counters (each role keeps its own copy; the schedules are identical by construction)
     uint32_t n_it = 0;                 // (job, tile, layer) iterations done
     uint32_t n_pst[2] = {0, 0};        // ring-tile loads done per slot
+    uint32_t n_pre[2] = {0, 0};        // pre-row loads done per slot
 
     for (int64_t job = blockIdx.x; job < njobs; job += gridDim.x) {
         const int b = (int)(job % nb);
         const int64_t pair = job / nb;
-        // ---- job prologue (all threads): bias table of this branch, zero the stashes and the X buffers --------------
+        // ---- job prologue (all threads): zero the stashes and the X buffers (causal zero history, reading A4) --------
         __syncthreads();
         {
-            const float* bsrc = a.bias + (size_t)b * L * BIAS_FLOATS;
-            float* bdst = reinterpret_cast<float*>(smem + SM_BIAS);
-            for (int i = threadIdx.x; i < L * BIAS_FLOATS; i += NTHREADS) bdst[i] = bsrc[i];
             uint4 z4 = make_uint4(0, 0, 0, 0);
             uint4* zs = reinterpret_cast<uint4*>(smem + SM_STASH);
             for (int i = threadIdx.x; i < 2 * STASH_BYTES / 16; i += NTHREADS) zs[i] = z4;
@@ -125,93 +153,129 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
         fence_proxy_async_smem();
         __syncthreads();
 
-        if (warp == 8) {
+        if (warp == NEPI) {
             // =========================== producer: weights and ring tiles ===========================================
             if (lane == 0) {
-                for (int j = 0; j < a.ntiles; j++)
-                    for (int i = 0; i < L; i++, n_it++) {
-                        mbar_wait(bar(B_WFG_FREE), (n_it & 1) ^ 1);
-                        mbar_arrive_expect_tx(bar(B_WFG_FULL), WFG_BYTES);
-                        bulk_g2s(sbase + SM_WFG, a.wfg + ((size_t)b * L + i) * WFG_BYTES, WFG_BYTES, bar(B_WFG_FULL));
-                        if (M.big[i] && j >= M.D[i]) {
-                            for (int s = 0; s < 2; s++) {
-                                mbar_wait(bar(B_PST_FREE + s), (n_pst[s] & 1) ^ 1);
-                                mbar_arrive_expect_tx(bar(B_PST_FULL + s), PST_BYTES);
-                                const uint8_t* src = a.ring + (((size_t)blockIdx.x * 2 + s) * M.ring_tiles + M.ring_off[i] +
-                                                               (j - M.D[i]) % (M.D[i] + 1)) * PST_BYTES;
-                                bulk_g2s(sbase + SM_PST + s * PST_BYTES, src, PST_BYTES, bar(B_PST_FULL + s));
-                                n_pst[s]++;
-                            }
+                for (int n = 0; n < NI; n++, n_it++) {
+                    const int i = n % L, j = n / L;
+                    const int st = n_it & 1;
+                    const uint32_t wph = (n_it >> 1) & 1;
+                    mbar_wait(bar(B_WFG_FREE + st), wph ^ 1);
+                    mbar_arrive_expect_tx(bar(B_WFG_FULL + st), WFG_BYTES);
+                    bulk_g2s(sbase + SM_WFG + st * WFG_BYTES, a.wfg + ((size_t)b * L + i) * WFG_BYTES, WFG_BYTES,
+                             bar(B_WFG_FULL + st));
+                    if (M.kind[i] == 2 && j >= M.D[i]) {
+                        for (int s = 0; s < 2; s++) {
+                            // the tile was published (j - D) tiles ago, i.e. before G1 of the previous iteration of
+                            // this slot: waiting for that G1 keeps this thread from running ahead of the writer
+                            mbar_wait(bar(B_FG_FULL + s), (n_it - 1) & 1);
+                            mbar_wait(bar(B_PST_FREE + s), (n_pst[s] & 1) ^ 1);
+                            mbar_arrive_expect_tx(bar(B_PST_FULL + s), PST_BYTES);
+                            const uint8_t* src = a.ring + (((size_t)blockIdx.x * 2 + s) * M.ring_tiles + M.ring_off[i] +
+                                                           (j - M.D[i]) % (M.D[i] + 1)) * PST_BYTES;
+                            bulk_g2s(sbase + SM_PST + s * PST_BYTES, src, PST_BYTES, bar(B_PST_FULL + s));
+                            n_pst[s]++;
                         }
-                        mbar_wait(bar(B_WRS_FREE), (n_it & 1) ^ 1);
-                        mbar_arrive_expect_tx(bar(B_WRS_FULL), WRS_BYTES);
-                        bulk_g2s(sbase + SM_WRS, a.wrs + ((size_t)b * L + i) * WRS_BYTES, WRS_BYTES, bar(B_WRS_FULL));
                     }
+                    mbar_wait(bar(B_WRS_FREE + st), wph ^ 1);
+                    mbar_arrive_expect_tx(bar(B_WRS_FULL + st), WRS_STRIDE);
+                    bulk_g2s(sbase + SM_WRS + st * WRS_STRIDE, a.wrs + ((size_t)b * L + i) * WRS_STRIDE, WRS_STRIDE,
+                             bar(B_WRS_FULL + st));
+                }
             }
             __syncwarp();
-        } else if (warp == 9) {
+        } else if (warp == NEPI + 1) {
             // =========================== MMA issuer ===================================================================
             if (lane == 0) {
                 const uint32_t idesc128 = make_idesc_f16(128, 128), idesc64 = make_idesc_f16(128, 64);
-                for (int j = 0; j < a.ntiles; j++)
-                    for (int i = 0; i < L; i++, n_it++) {
-                        const uint32_t ph = n_it & 1;
-                        const int d = M.dil[i];
-                        // ---- GEMM1: f|g = [h(t-d) | h(t)] . Wfg^T
-                        mbar_wait(bar(B_WFG_FULL), ph);
-                        for (int s = 0; s < 2; s++) {
-                            mbar_wait(bar(B_H_READY + s), ph);
-                            const uint32_t xs = sbase + SM_X + s * X_BYTES;
-                            const uint32_t dt = tmem + 128 * s;
-                            uint32_t acc = 0;
-                            if (!M.big[i]) {
-                                tc_fence_after();
-                                for (int kk = 0; kk < 4; kk++, acc = 1)
-                                    tc_mma_f16(dt, make_sdesc(xs + (64 - d) * 16 + 2 * kk * X_CHUNK, X_CHUNK, 128),
-                                               make_sdesc(sbase + SM_WFG + 2 * kk * 2048, 2048, 128), idesc128, acc);
-                            } else if (j >= M.D[i]) {
-                                mbar_wait(bar(B_PST_FULL + s), n_pst[s] & 1);
-                                n_pst[s]++;
-                                tc_fence_after();
-                                const uint32_t ps = sbase + SM_PST + s * PST_BYTES;
-                                for (int kk = 0; kk < 4; kk++, acc = 1)
-                                    tc_mma_f16(dt, make_sdesc(ps + 2 * kk * 2048, 2048, 128),
-                                               make_sdesc(sbase + SM_WFG + 2 * kk * 2048, 2048, 128), idesc128, acc);
-                            } else {
-                                tc_fence_after();
-                            }
-                            for (int kk = 0; kk < 4; kk++, acc = 1)
-                                tc_mma_f16(dt, make_sdesc(xs + 64 * 16 + 2 * kk * X_CHUNK, X_CHUNK, 128),
-                                           make_sdesc(sbase + SM_WFG + (8 + 2 * kk) * 2048, 2048, 128), idesc128, acc);
-                            tc_commit(bar(B_FG_FULL + s));
-                            if (M.big[i] && j >= M.D[i]) tc_commit(bar(B_PST_FREE + s));
-                        }
-                        tc_commit(bar(B_WFG_FREE));
-                        // ---- GEMM2: skip += z' Ws'^T ; res = z' Wr'^T
-                        mbar_wait(bar(B_WRS_FULL), ph);
-                        for (int s = 0; s < 2; s++) {
-                            mbar_wait(bar(B_Z_READY + s), ph);
-                            tc_fence_after();
-                            const uint32_t zs = sbase + SM_X + s * X_BYTES + 64 * 16;
-                            for (int kk = 0; kk < 4; kk++)
-                                tc_mma_f16(tmem + 256 + 128 * s, make_sdesc(zs + 2 * kk * X_CHUNK, X_CHUNK, 128),
-                                           make_sdesc(sbase + SM_WRS + 2 * kk * 3072, 3072, 128), idesc128,
-                                           (i > 0 || kk > 0) ? 1u : 0u);
-                            if (i < L - 1)   // reading A8: the last block's residual conv has no effect
-                                for (int kk = 0; kk < 4; kk++)
-                                    tc_mma_f16(tmem + 128 * s, make_sdesc(zs + 2 * kk * X_CHUNK, X_CHUNK, 128),
-                                               make_sdesc(sbase + SM_WRS + 128 * 16 + 2 * kk * 3072, 3072, 128), idesc64,
-                                               kk > 0 ? 1u : 0u);
-                            tc_commit(bar(B_RS_FULL + s));
-                        }
-                        tc_commit(bar(B_WRS_FREE));
+                // GEMM1 of slot s, iteration n (global counter nit): f|g = [h(t-d) | h(t)] . Wfg^T
+                auto G1 = [&](int s, int n, uint32_t nit, bool release) {
+                    const int i = n % L, j = n / L;
+                    const int st = nit & 1;
+                    const int d = M.dil[i], kind = M.kind[i];
+                    const uint32_t wfg = sbase + SM_WFG + st * WFG_BYTES;
+                    const uint32_t xs = sbase + SM_X + s * X_BYTES;
+                    const uint32_t dt = tmem + 128 * s;
+                    uint32_t acc = 0;
+                    if (kind < 2) {
+                        if (kind == 1 && j >= 1) n_pre[s]++;
+                        tc_fence_after();
+                        for (int kk = 0; kk < 4; kk++, acc = 1)
+                            tc_mma_f16(dt, make_sdesc(xs + (64 - d) * 16 + 2 * kk * X_CHUNK, X_CHUNK, 128),
+                                       make_sdesc(wfg + 2 * kk * 2048, 2048, 128), idesc128, acc);
+                    } else if (j >= M.D[i]) {
+                        n_pst[s]++;
+                        tc_fence_after();
+                        const uint32_t ps = sbase + SM_PST + s * PST_BYTES;
+                        for (int kk = 0; kk < 4; kk++, acc = 1)
+                            tc_mma_f16(dt, make_sdesc(ps + 2 * kk * 2048, 2048, 128),
+                                       make_sdesc(wfg + 2 * kk * 2048, 2048, 128), idesc128, acc);
+                    } else {
+                        tc_fence_after();
                     }
+                    for (int kk = 0; kk < 4; kk++, acc = 1)
+                        tc_mma_f16(dt, make_sdesc(xs + 64 * 16 + 2 * kk * X_CHUNK, X_CHUNK, 128),
+                                   make_sdesc(wfg + (8 + 2 * kk) * 2048, 2048, 128), idesc128, acc);
+                    tc_commit(bar(B_FG_FULL + s));
+                    if (kind == 2 && j >= M.D[i]) tc_commit(bar(B_PST_FREE + s));
+                    if (release) tc_commit(bar(B_WFG_FREE + st));
+                };
+                // GEMM2 of slot s: skip += z' Ws'^T ; res = z' Wr'^T
+                auto G2 = [&](int s, int n, uint32_t nit, bool release) {
+                    const int i = n % L;
+                    const int st = nit & 1;
+                    const uint32_t wrs = sbase + SM_WRS + st * WRS_STRIDE;
+                    tc_fence_after();
+                    const uint32_t zs = sbase + SM_X + s * X_BYTES + 64 * 16;
+                    for (int kk = 0; kk < 4; kk++)
+                        tc_mma_f16(tmem + 256 + 128 * s, make_sdesc(zs + 2 * kk * X_CHUNK, X_CHUNK, 128),
+                                   make_sdesc(wrs + 2 * kk * 3072, 3072, 128), idesc128, (i > 0 || kk > 0) ? 1u : 0u);
+                    if (i < L - 1)   // reading A8: the last block's residual conv has no effect
+                        for (int kk = 0; kk < 4; kk++)
+                            tc_mma_f16(tmem + 128 * s, make_sdesc(zs + 2 * kk * X_CHUNK, X_CHUNK, 128),
+                                       make_sdesc(wrs + 128 * 16 + 2 * kk * 3072, 3072, 128), idesc64, kk > 0 ? 1u : 0u);
+                    tc_commit(bar(B_RS_FULL + s));
+                    if (release) tc_commit(bar(B_WRS_FREE + st));
+                };
+                // dynamic order: whichever slot's next GEMM has its operands ready is issued next
+                int sn[2] = {0, 0}, sop[2] = {0, 0};     // per slot: iteration inside the job, next op (0: G1, 1: G2)
+                uint32_t idle = 0;
+                while (sn[0] < NI || sn[1] < NI) {
+                    bool any = false;
+#pragma unroll
+                    for (int s = 0; s < 2; s++) {
+                        if (sn[s] >= NI) continue;
+                        const int n = sn[s];
+                        const uint32_t nit = n_it + n;
+                        const int st = nit & 1;
+                        if (sop[s] == 0) {
+                            const int i = n % L, j = n / L, kind = M.kind[i];
+                            bool ok = mbar_test(bar(B_WFG_FULL + st), (nit >> 1) & 1) && mbar_test(bar(B_H_READY + s), nit & 1);
+                            if (ok && kind == 1 && j >= 1) ok = mbar_test(bar(B_PRE_FULL + s), n_pre[s] & 1);
+                            if (ok && kind == 2 && j >= M.D[i]) ok = mbar_test(bar(B_PST_FULL + s), n_pst[s] & 1);
+                            if (!ok) continue;
+                            // the slot that issues G1(n) second releases the weight stage
+                            const int o = s ^ 1;
+                            G1(s, n, nit, sn[o] > n || (sn[o] == n && sop[o] == 1));
+                            sop[s] = 1, any = true;
+                        } else {
+                            if (!(mbar_test(bar(B_WRS_FULL + st), (nit >> 1) & 1) && mbar_test(bar(B_Z_READY + s), nit & 1))) continue;
+                            const int o = s ^ 1;
+                            G2(s, n, nit, sn[o] > n);
+                            sop[s] = 0, sn[s] = n + 1, any = true;
+                        }
+                    }
+                    if (any) idle = 0;
+                    else if (++idle > (1u << 27)) __trap();
+                }
+                n_it += NI;
             }
             __syncwarp();
         } else {
-            // =========================== epilogue warpgroup of slot s ==================================================
-            const int s = warp >> 2;
+            // =========================== epilogue: slot s, column half wg, row r =======================================
+            const int s = warp >> 3, wg = (warp >> 2) & 1;
             const int r = (warp & 3) * 32 + lane;                    // row of the tile = TMEM lane
+            const int ch0 = 32 * wg, c0 = 4 * wg;                     // first channel / first 16-byte chunk of this half
             const int64_t wl = 2 * pair + s;                          // window index inside this launch
             const bool valid = wl < a.nwin;
             const int64_t w = a.w0 + (valid ? wl : a.nwin - 1);
@@ -219,36 +283,49 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
             const uint32_t st0 = sbase + SM_STASH + s * STASH_BYTES;
             const uint32_t lane_t = tmem + ((uint32_t)((warp & 3) * 32) << 16);
             uint8_t* ring_s = a.ring + ((size_t)blockIdx.x * 2 + s) * M.ring_tiles * PST_BYTES;
+            uint8_t* ring64_s = a.ring64 + ((size_t)blockIdx.x * 2 + s) * M.n64 * 2 * PRE_BYTES;
             const float* cst = a.cst + b * 256;
-            const float* biasL = reinterpret_cast<const float*>(smem + SM_BIAS);
-            float h[64];
+            float2 h[16];                                             // fp32 master of the residual stream, 32 channels
 
-            // writes the fp16 copy of h as the operand of layer `inext` for tile j, maintains stash / ring, signals MMA
+            // writes the fp16 copy of h as the operand of layer `inext` for tile j, maintains stash / rings, signals MMA
             auto publish = [&](int inext, int j) {
-                uint32_t pk[32];
+                uint32_t pk[16];
 #pragma unroll
-                for (int c = 0; c < 32; c++) pk[c] = pack_half2(h[2 * c], h[2 * c + 1]);
+                for (int c = 0; c < 16; c++) pk[c] = pack_half2(h[c].x, h[c].y);
 #pragma unroll
-                for (int c = 0; c < 8; c++)
-                    st_shared_v4(xs + (64 + r) * 16 + c * X_CHUNK, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
-                const int d = M.dil[inext];
-                if (!M.big[inext]) {
+                for (int c = 0; c < 4; c++)
+                    st_shared_v4(xs + (64 + r) * 16 + (c0 + c) * X_CHUNK, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+                const int d = M.dil[inext], kind = M.kind[inext];
+                if (kind == 0) {
                     if (r >= 128 - d) {
                         const int rp = r - (128 - d);
                         const uint32_t sb = st0 + M.stash_off[inext] + rp * 16;
 #pragma unroll
-                        for (int c = 0; c < 8; c++) {
-                            uint4 old = ld_shared_v4(sb + c * d * 16);
-                            st_shared_v4(xs + (64 - d + rp) * 16 + c * X_CHUNK, old.x, old.y, old.z, old.w);
-                            st_shared_v4(sb + c * d * 16, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+                        for (int c = 0; c < 4; c++) {
+                            uint4 old = ld_shared_v4(sb + (c0 + c) * d * 16);
+                            st_shared_v4(xs + (64 - d + rp) * 16 + (c0 + c) * X_CHUNK, old.x, old.y, old.z, old.w);
+                            st_shared_v4(sb + (c0 + c) * d * 16, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
                         }
+                    }
+                } else if (kind == 1) {
+                    if (j == 0 && r < 64) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) st_shared_v4(xs + r * 16 + (c0 + c) * X_CHUNK, 0u, 0u, 0u, 0u);
+                    }
+                    if (r >= 64) {
+                        uint8_t* g = ring64_s + (size_t)(M.ring_off[inext] * 2 + (j & 1)) * PRE_BYTES + (r - 64) * 16;
+#pragma unroll
+                        for (int c = 0; c < 4; c++)
+                            *reinterpret_cast<uint4*>(g + (c0 + c) * 1024) = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+                        __threadfence_block();
+                        fence_proxy_async();
                     }
                 } else {
                     uint8_t* g = ring_s + (size_t)(M.ring_off[inext] + j % (M.D[inext] + 1)) * PST_BYTES + r * 16;
 #pragma unroll
-                    for (int c = 0; c < 8; c++)
-                        *reinterpret_cast<uint4*>(g + c * 2048) = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
-                    __threadfence();
+                    for (int c = 0; c < 4; c++)
+                        *reinterpret_cast<uint4*>(g + (c0 + c) * 2048) = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+                    __threadfence_block();
                     fence_proxy_async();
                 }
                 tc_fence_before();
@@ -263,35 +340,57 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     float x = 0.f;
                     if (t < a.T) x = __half2float(a.strain[((size_t)w * a.T + t) * a.C + b]);
 #pragma unroll
-                    for (int c = 0; c < 64; c++) h[c] = fmaf(__ldg(cst + c), x, __ldg(cst + 64 + c));
+                    for (int c = 0; c < 16; c++) {
+                        float2 wi = __ldg(reinterpret_cast<const float2*>(cst + ch0) + c);
+                        float2 bi = __ldg(reinterpret_cast<const float2*>(cst + 64 + ch0) + c);
+                        h[c] = make_float2(fmaf(wi.x, x, bi.x), fmaf(wi.y, x, bi.y));
+                    }
                     tc_wait_ld();   // the previous tile's TMEM reads of this thread are complete
                     publish(0, j);
                 }
                 for (int i = 0; i < L; i++, n_it++) {
                     const uint32_t ph = n_it & 1;
-                    const float* bl = biasL + i * BIAS_FLOATS;
+                    const int st = n_it & 1;
                     // ---- gate: z' = tanh(f + bf) * (1 + tanh(g/2 + bg/2))
                     mbar_wait(bar(B_FG_FULL + s), ph);
+                    const int inx = (i + 1 < L) ? i + 1 : 0, jnx = (i + 1 < L) ? j : j + 1;   // the next (layer, tile)
+                    if (M.kind[inx] == 1 && jnx >= 1 && jnx < a.ntiles && (warp & 7) == 0 && lane == 0) {
+                        // G1(i) has finished with the pre rows: fetch the 64 rows that precede tile jnx for layer inx
+                        fence_proxy_async();
+                        mbar_arrive_expect_tx(bar(B_PRE_FULL + s), PRE_BYTES);
+                        const uint8_t* src = ring64_s + (size_t)(M.ring_off[inx] * 2 + ((jnx - 1) & 1)) * PRE_BYTES;
+                        for (int c = 0; c < 8; c++) bulk_g2s(xs + c * X_CHUNK, src + c * 1024, 1024, bar(B_PRE_FULL + s));
+                    }
+                    __syncwarp();
+                    mbar_wait(bar(B_WRS_FULL + st), (n_it >> 1) & 1);      // this layer's biases are behind its Wrs
+                    const float* bl = reinterpret_cast<const float*>(smem + SM_WRS + st * WRS_STRIDE + WRS_BYTES);
                     tc_fence_after();
 #pragma unroll
-                    for (int cc = 0; cc < 2; cc++) {
-                        uint32_t f[32], g[32];
-                        tmem_ld32(lane_t + 128 * s + 32 * cc, f);
-                        tmem_ld32(lane_t + 128 * s + 64 + 32 * cc, g);
+                    for (int hh = 0; hh < 2; hh++) {
+                        uint32_t f[16], g[16];
+                        tmem_ld16(lane_t + 128 * s + ch0 + 16 * hh, f);
+                        tmem_ld16(lane_t + 128 * s + 64 + ch0 + 16 * hh, g);
                         tc_wait_ld();
-                        uint32_t pk[16];
+                        uint32_t pk[8];
 #pragma unroll
-                        for (int c = 0; c < 32; c += 2) {
-                            float tf0 = tanh_approx(__uint_as_float(f[c]) + bl[32 * cc + c]);
-                            float tg0 = tanh_approx(__uint_as_float(g[c]) + bl[64 + 32 * cc + c]);
-                            float tf1 = tanh_approx(__uint_as_float(f[c + 1]) + bl[32 * cc + c + 1]);
-                            float tg1 = tanh_approx(__uint_as_float(g[c + 1]) + bl[64 + 32 * cc + c + 1]);
-                            pk[c >> 1] = pack_half2(fmaf(tf0, tg0, tf0), fmaf(tf1, tg1, tf1));
+                        for (int c = 0; c < 8; c++) {
+                            float2 bf = *reinterpret_cast<const float2*>(bl + ch0 + 16 * hh + 2 * c);
+                            float2 bg = *reinterpret_cast<const float2*>(bl + 64 + ch0 + 16 * hh + 2 * c);
+                            float2 fa = add2(make_float2(__uint_as_float(f[2 * c]), __uint_as_float(f[2 * c + 1])), bf);
+                            float2 ga = add2(make_float2(__uint_as_float(g[2 * c]), __uint_as_float(g[2 * c + 1])), bg);
+                            float2 tf = make_float2(tanh_approx(fa.x), tanh_approx(fa.y));
+                            float2 tg = make_float2(tanh_approx(ga.x), tanh_approx(ga.y));
+                            float2 z = fma2(tf, tg, tf);
+                            pk[c] = pack_half2(z.x, z.y);
                         }
 #pragma unroll
-                        for (int c = 0; c < 4; c++)
-                            st_shared_v4(xs + (64 + r) * 16 + (4 * cc + c) * X_CHUNK, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2],
+                        for (int c = 0; c < 2; c++)
+                            st_shared_v4(xs + (64 + r) * 16 + (c0 + 2 * hh + c) * X_CHUNK, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2],
                                          pk[4 * c + 3]);
+                    }
+                    if (i < L - 1) {
+#pragma unroll
+                        for (int c = 0; c < 16; c++) h[c] = add2(h[c], *reinterpret_cast<const float2*>(bl + 128 + ch0 + 2 * c));
                     }
                     tc_fence_before();
                     fence_proxy_async_smem();
@@ -300,22 +399,20 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     mbar_wait(bar(B_RS_FULL + s), ph);
                     tc_fence_after();
                     if (i < L - 1) {
+                        uint32_t v[32];
+                        tmem_ld32(lane_t + 128 * s + ch0, v);
+                        tc_wait_ld();
 #pragma unroll
-                        for (int cc = 0; cc < 2; cc++) {
-                            uint32_t v[32];
-                            tmem_ld32(lane_t + 128 * s + 32 * cc, v);
-                            tc_wait_ld();
-#pragma unroll
-                            for (int c = 0; c < 32; c++) h[32 * cc + c] += __uint_as_float(v[c]) + bl[128 + 32 * cc + c];
-                        }
+                        for (int c = 0; c < 16; c++)
+                            h[c] = add2(h[c], make_float2(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1])));
                         publish(i + 1, j);
                     } else {
                         // u = ReLU(sum_i skip_i) -> fp16 tile in the workspace                       (C.1 step 3)
                         uint8_t* ut = a.u + (((size_t)wl * nb + b) * a.ntiles + j) * U_TILE_BYTES + r * 16;
 #pragma unroll
-                        for (int cc = 0; cc < 4; cc++) {
+                        for (int cc = 0; cc < 2; cc++) {
                             uint32_t v[32];
-                            tmem_ld32(lane_t + 256 + 128 * s + 32 * cc, v);
+                            tmem_ld32(lane_t + 256 + 128 * s + 64 * wg + 32 * cc, v);
                             tc_wait_ld();
                             if (valid) {
 #pragma unroll
@@ -324,11 +421,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 #pragma unroll
                                     for (int e = 0; e < 4; e++) {
                                         int col = 8 * c + 2 * e;
-                                        float u0 = fmaxf(__uint_as_float(v[col]) + __ldg(cst + 128 + 32 * cc + col), 0.f);
-                                        float u1 = fmaxf(__uint_as_float(v[col + 1]) + __ldg(cst + 128 + 32 * cc + col + 1), 0.f);
+                                        float2 bs = __ldg(reinterpret_cast<const float2*>(cst + 128 + 64 * wg + 32 * cc + col));
+                                        float u0 = fmaxf(__uint_as_float(v[col]) + bs.x, 0.f);
+                                        float u1 = fmaxf(__uint_as_float(v[col + 1]) + bs.y, 0.f);
                                         q[e] = pack_half2(u0, u1);
                                     }
-                                    *reinterpret_cast<uint4*>(ut + (4 * cc + c) * 2048) = make_uint4(q[0], q[1], q[2], q[3]);
+                                    *reinterpret_cast<uint4*>(ut + (8 * wg + 4 * cc + c) * 2048) = make_uint4(q[0], q[1], q[2], q[3]);
                                 }
                             }
                         }
@@ -339,7 +437,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 8) tmem_dealloc(tmem, 512);
+    if (warp == NEPI) tmem_dealloc(tmem, 512);
 }
 
 // ---- head kernel ---------------------------------------------------------------------------------------------------
@@ -449,7 +547,7 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
 // ---- host side: packing and launch -----------------------------------------------------------------------------------
 struct GwiTcPack {
     uint8_t *d_wfg = nullptr, *d_wrs = nullptr, *d_w1 = nullptr;
-    float *d_bias = nullptr, *d_cst = nullptr, *d_hc = nullptr;
+    float *d_cst = nullptr, *d_hc = nullptr;
     TcMeta meta;
     int num_sms = 148;
 };
@@ -460,7 +558,8 @@ bool gwi_tc_supported(const GwiArch& a)
     int stash = 0;
     for (int i = 0; i < a.L; i++) {
         int d = a.dil[i];
-        if (d <= 64) stash += d * 128;
+        if (d <= 32) stash += d * 128;
+        else if (d == 64) continue;
         else if (d % 128 != 0) return false;
     }
     return stash <= STASH_BYTES;
@@ -483,19 +582,21 @@ gwi_status gwi_tc_pack(gwi_model* m)
     TcMeta& M = p->meta;
     memset(&M, 0, sizeof(M));
     M.L = L, M.n_branch = nb;
-    int so = 0, ro = 0;
+    int so = 0, ro = 0, n64 = 0;
     for (int i = 0; i < L; i++) {
         M.dil[i] = a.dil[i];
-        M.big[i] = a.dil[i] > 64;
-        M.D[i] = M.big[i] ? a.dil[i] / 128 : 0;
-        M.stash_off[i] = so, M.ring_off[i] = ro;
-        if (M.big[i]) ro += M.D[i] + 1;
-        else so += a.dil[i] * 128;
+        M.kind[i] = a.dil[i] <= 32 ? 0 : (a.dil[i] == 64 ? 1 : 2);
+        M.D[i] = M.kind[i] == 2 ? a.dil[i] / 128 : 0;
+        M.stash_off[i] = so;
+        if (M.kind[i] == 2) M.ring_off[i] = ro, ro += M.D[i] + 1;
+        else if (M.kind[i] == 1) M.ring_off[i] = n64++;
+        else M.ring_off[i] = 0, so += a.dil[i] * 128;
     }
     M.ring_tiles = ro > 0 ? ro : 1;
+    M.n64 = n64 > 0 ? n64 : 1;
     const float* W = m->host_blob.data();
-    std::vector<uint16_t> wfg((size_t)nb * L * WFG_BYTES / 2), wrs((size_t)nb * L * WRS_BYTES / 2), w1((size_t)nb * U_TILE_BYTES / 2);
-    std::vector<float> bias((size_t)nb * L * BIAS_FLOATS), cst((size_t)nb * 256, 0.f), hc(257);
+    std::vector<uint16_t> wfg((size_t)nb * L * WFG_BYTES / 2), wrs((size_t)nb * L * WRS_STRIDE / 2), w1((size_t)nb * U_TILE_BYTES / 2);
+    std::vector<float> cst((size_t)nb * 256, 0.f), hc(257);
     for (int b = 0; b < nb; b++) {
         for (int c = 0; c < 64; c++) {
             cst[b * 256 + c] = W[m->off.W_in[b] + c];      // c_in = 1
@@ -511,18 +612,19 @@ gwi_status gwi_tc_pack(gwi_model* m)
                                      : 0.5f * W[lo.Wg + ((int64_t)(n - 64) * 64 + kin) * 2 + tap];
                     fg[(k / 8) * (128 * 8) + n * 8 + (k % 8)] = h16(v);
                 }
-            uint16_t* rs = wrs.data() + ((size_t)b * L + i) * (WRS_BYTES / 2);
+            uint16_t* rs = wrs.data() + ((size_t)b * L + i) * (WRS_STRIDE / 2);
             for (int n = 0; n < 192; n++)
                 for (int k = 0; k < 64; k++) {
                     float v = n < 128 ? 0.5f * W[lo.Ws + (int64_t)n * 64 + k] : 0.5f * W[lo.Wr + (int64_t)(n - 128) * 64 + k];
                     rs[(k / 8) * (192 * 8) + n * 8 + (k % 8)] = h16(v);
                 }
-            float* bl = bias.data() + ((size_t)b * L + i) * BIAS_FLOATS;
+            float bl[BIAS_FLOATS];
             for (int c = 0; c < 64; c++) {
                 bl[c] = W[lo.bf + c];
                 bl[64 + c] = 0.5f * W[lo.bg + c];
                 bl[128 + c] = W[lo.br + c];
             }
+            memcpy(rs + WRS_BYTES / 2, bl, sizeof(bl));   // the layer's biases travel behind its Wrs operand
             for (int q = 0; q < 128; q++) cst[b * 256 + 128 + q] += W[lo.bs + q];
         }
     }
@@ -538,7 +640,6 @@ gwi_status gwi_tc_pack(gwi_model* m)
     GWI_CUDA_CHECK(up((void**)&p->d_wfg, wfg.data(), wfg.size() * 2));
     GWI_CUDA_CHECK(up((void**)&p->d_wrs, wrs.data(), wrs.size() * 2));
     GWI_CUDA_CHECK(up((void**)&p->d_w1, w1.data(), w1.size() * 2));
-    GWI_CUDA_CHECK(up((void**)&p->d_bias, bias.data(), bias.size() * 4));
     GWI_CUDA_CHECK(up((void**)&p->d_cst, cst.data(), cst.size() * 4));
     GWI_CUDA_CHECK(up((void**)&p->d_hc, hc.data(), hc.size() * 4));
     cudaDeviceProp prop;
@@ -553,7 +654,7 @@ void gwi_tc_free(gwi_model* m)
 {
     GwiTcPack* p = m->tc;
     if (!p) return;
-    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_bias), cudaFree(p->d_cst), cudaFree(p->d_hc);
+    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_cst), cudaFree(p->d_hc);
     delete p;
     m->tc = nullptr;
 }
@@ -565,8 +666,9 @@ size_t gwi_tc_workspace_bytes(const gwi_model* m, int64_t B, int32_t T)
     const GwiTcPack* p = m->tc;
     int64_t ntiles = (T + TM - 1) / TM;
     size_t ring = (size_t)p->num_sms * 2 * p->meta.ring_tiles * PST_BYTES;
+    size_t ring64 = (size_t)p->num_sms * 2 * p->meta.n64 * 2 * PRE_BYTES;
     size_t u = (size_t)tc_chunk(B) * m->arch.n_branch * ntiles * U_TILE_BYTES;
-    return ring + u + 256;
+    return ring + ring64 + u + 512;
 }
 
 gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, int32_t T, float* d_prob, void* d_ws,
@@ -576,15 +678,17 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
     const int nb = m->arch.n_branch;
     const int ntiles = (T + TM - 1) / TM;
     size_t ring_bytes = ((size_t)p->num_sms * 2 * p->meta.ring_tiles * PST_BYTES + 255) & ~(size_t)255;
+    size_t ring64_bytes = ((size_t)p->num_sms * 2 * p->meta.n64 * 2 * PRE_BYTES + 255) & ~(size_t)255;
     uint8_t* ring = (uint8_t*)d_ws;
-    uint8_t* u = ring + ring_bytes;
+    uint8_t* ring64 = ring + ring_bytes;
+    uint8_t* u = ring64 + ring64_bytes;
     const int64_t Bc = tc_chunk(B);
     for (int64_t w0 = 0; w0 < B; w0 += Bc) {
         const int64_t nwin = (B - w0 < Bc) ? B - w0 : Bc;
         StackArgs sa;
-        sa.wfg = p->d_wfg, sa.wrs = p->d_wrs, sa.bias = p->d_bias, sa.cst = p->d_cst, sa.strain = d_strain;
+        sa.wfg = p->d_wfg, sa.wrs = p->d_wrs, sa.cst = p->d_cst, sa.strain = d_strain;
         sa.w0 = w0, sa.nwin = nwin, sa.T = T, sa.ntiles = ntiles, sa.C = nb * m->arch.c_in;
-        sa.ring = ring, sa.u = u, sa.meta = p->meta;
+        sa.ring = ring, sa.ring64 = ring64, sa.u = u, sa.meta = p->meta;
         int64_t njobs = ((nwin + 1) / 2) * nb;
         int grid = (int)(njobs < p->num_sms ? njobs : p->num_sms);
         k_stack<<<grid, NTHREADS, SM_TOTAL, st>>>(sa);
