@@ -2,7 +2,7 @@
 //
 // Two kernels, both hand-written tcgen05 (sm_100a) with accumulators in TMEM:
 //
-//  k_stack  one persistent CTA per SM walks jobs" = (pair of windows
+//  k_stack  one persistent CTA per SM walks "jobs" = (pair of windows, branch).  For every 128-timestep tile it runs
 //           the lift and all L gated residual blocks depth-first (DESIGN.md C.1 steps 1-3), so that
 //           no activation of a block ever goes to HBM:
 //             GEMM1  [128 x 128] = [h(t-d) | h(t)] [128 x 128] . [Wf|Wg/2]^T      (tcgen05.mma, fp32 accum in TMEM)
@@ -13,7 +13,7 @@
 //           buffer addressed d rows earlier (no-swizzle K-major layout, rows 16 bytes apart), so a dilation costs no
 //           data movement; the d rows that precede a tile come from a per-layer stash in shared memory (d <= 64) or,
 //           for d = 128, 256, 512, from an L2-resident ring in global memory that the bulk-copy engine prefetches.
-//           Two windows (slots") are in flight per CTA so that the tensor pipe works on one while the epilogue"
+//           Two windows ("slots") are in flight per CTA so that the tensor pipe works on one while the epilogue
 //           warps gate the other.  Output: u = ReLU(sum of skips) per branch, fp16, tile-major in the workspace.
 //  k_head   [128 x 128] = [u_H | u_L] . W1^T on tcgen05, then ReLU, dot with W2, sigmoid (C.1 steps 4-5).
 //
@@ -22,8 +22,8 @@
 #include <cstring>
 #include <vector>
 
-#include gwi_internal.h""
-#include gwi_tc_ptx.h""
+#include "gwi_internal.h"
+#include "gwi_tc_ptx.h"
 
 using namespace tc;
 
@@ -77,7 +77,7 @@ constexpr int SM_PST = SM_X + 2 * X_BYTES;                // 2 slots
 constexpr int SM_STASH = SM_PST + 2 * PST_BYTES;          // 2 slots
 constexpr int SM_BAR = SM_STASH + 2 * STASH_BYTES;
 constexpr int SM_TOTAL = SM_BAR + 256;
-static_assert(SM_TOTAL <= 232448, shared memory budget");"
+static_assert(SM_TOTAL <= 232448, "shared memory budget");
 
 enum { B_WFG_FULL = 0, B_WFG_FREE = 2, B_WRS_FULL = 4, B_WRS_FREE = 6, B_FG_FULL = 8, B_Z_READY = 10, B_RS_FULL = 12,
        B_H_READY = 14, B_PST_FULL = 16, B_PST_FREE = 18, B_PRE_FULL = 20, B_COUNT = 22 };
@@ -85,24 +85,24 @@ enum { B_WFG_FULL = 0, B_WFG_FREE = 2, B_WRS_FULL = 4, B_WRS_FREE = 6, B_FG_FULL
 __device__ __forceinline__ float2 add2(float2 a, float2 b)
 {
     float2 r;
-    asm({\n\t.reg .b64 ra
-        mov.b64 {%0
-        : =f"(r.x)
-        : f"(a.x)
+    asm("{\n\t.reg .b64 ra, rb, rc;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tadd.rn.f32x2 rc, ra, rb;\n\t"
+        "mov.b64 {%0, %1}, rc;\n\t}"
+        : "=f"(r.x), "=f"(r.y)
+        : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
     return r;
 }
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
 {
     float2 r;
-    asm({\n\t.reg .b64 ra
-        fma.rn.f32x2 rd
-        : =f"(r.x)
-        : f"(a.x)
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(r.x), "=f"(r.y)
+        : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
     return r;
 }
 
 // Schedule (one CTA per SM, persistent over jobs = (pair of windows, branch)).  The two windows of a job are two
-// slots" that run the same (tile
+// "slots" that run the same (tile, layer) sequence half a layer apart: the single MMA thread issues
 //     G1(slot 0, n)  G2(slot 1, n-1)  G1(slot 1, n)  G2(slot 0, n)          n = (tile, layer) iteration
 // so that while one slot's 8 epilogue warps gate (MUFU-bound), the tensor pipe and the other slot's warps work on the
 // other slot.  Weights (and the layer's biases) are double-buffered and shared by the two slots.
