@@ -19,7 +19,10 @@
 //
 // Roles in k_stack (320 threads): warps 0-3 epilogue of slot 0, warps 4-7 epilogue of slot 1 (warp % 4 = TMEM lane
 // quadrant), warp 8 lane 0 = bulk-copy producer (weights, ring tiles), warp 9 lane 0 = MMA issuer.
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
+#include <type_traits>
 #include <vector>
 
 #include "gwi_internal.h"
@@ -49,12 +52,27 @@ struct TcMeta {
     int dil[TC_MAX_L];
     int kind[TC_MAX_L];       // 0: d <= 32 (stash in shared memory), 1: d == 64 (pre rows through the global ring64),
                               // 2: d multiple of 128 (whole past tiles through the global ring)
-    int D[TC_MAX_L];          // d / 128 for kind 2
+    int lay[TC_MAX_L];        // kind | d << 2 (one constant load per GEMM in the MMA thread)
+    int D[TC_MAX_L];          // d / 128 for kind 2 (a power of two: the ring of a layer has D entries)
     int stash_off[TC_MAX_L];  // byte offset of the layer's stash inside the slot's stash area
     int ring_off[TC_MAX_L];   // kind 2: first ring entry (in tiles) of the layer; kind 1: index among the d = 64 layers
     int ring_tiles;           // ring entries per slot
     int n64;                  // number of d = 64 layers
 };
+
+#ifdef GWI_TC_TRACE
+// debug build only (-DGWI_TC_TRACE): the MMA issuer, the producer and lane 0 of every epilogue warp of CTA 0 record
+// (event, slot, iteration, clock) tuples, each into its own region (plain stores, no atomics)
+#define TRACE_CAP 4096
+__device__ uint4 g_trace[18 * TRACE_CAP];
+#define TRACE(ev, slot, n)                                                                                   \
+    do {                                                                                                     \
+        if (blockIdx.x == 0 && trace_k < TRACE_CAP)                                                          \
+            g_trace[trace_role * TRACE_CAP + trace_k++] = make_uint4((unsigned)(ev), (unsigned)(slot), (unsigned)(n), (unsigned)clock64()); \
+    } while (0)
+#else
+#define TRACE(ev, slot, n)
+#endif
 
 struct StackArgs {
     const uint8_t* wfg;   // [n_branch][L][WFG_BYTES]
@@ -137,6 +155,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
     uint32_t n_it = 0;                 // (job, tile, layer) iterations done
     uint32_t n_pst[2] = {0, 0};        // ring-tile loads done per slot
     uint32_t n_pre[2] = {0, 0};        // pre-row loads done per slot
+#ifdef GWI_TC_TRACE
+    unsigned trace_k = 0;
+    const int trace_role = warp == NEPI + 1 ? 0 : (warp == NEPI ? 17 : 1 + (warp & 15));
+#endif
 
     for (int64_t job = blockIdx.x; job < njobs; job += gridDim.x) {
         const int b = (int)(job % nb);
@@ -155,7 +177,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 
         if (warp == NEPI) {
             // =========================== producer: weights and ring tiles ===========================================
-            if (lane == 0) {
+            if (elect_one()) {
                 for (int n = 0; n < NI; n++, n_it++) {
                     const int i = n % L, j = n / L;
                     const int st = n_it & 1;
@@ -166,13 +188,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                              bar(B_WFG_FULL + st));
                     if (M.kind[i] == 2 && j >= M.D[i]) {
                         for (int s = 0; s < 2; s++) {
-                            // the tile was published (j - D) tiles ago, i.e. before G1 of the previous iteration of
-                            // this slot: waiting for that G1 keeps this thread from running ahead of the writer
-                            mbar_wait(bar(B_FG_FULL + s), (n_it - 1) & 1);
+                            // the tile was stored (j - D) tiles ago by the MMA thread, which waits for the completion
+                            // of its bulk stores before it issues GEMM2 of the same iteration: GEMM2 of the previous
+                            // iteration of this slot being done implies the tile is in L2
+                            mbar_wait(bar(B_RS_FULL + s), (n_it - 1) & 1);
                             mbar_wait(bar(B_PST_FREE + s), (n_pst[s] & 1) ^ 1);
                             mbar_arrive_expect_tx(bar(B_PST_FULL + s), PST_BYTES);
                             const uint8_t* src = a.ring + (((size_t)blockIdx.x * 2 + s) * M.ring_tiles + M.ring_off[i] +
-                                                           (j - M.D[i]) % (M.D[i] + 1)) * PST_BYTES;
+                                                           (j & (M.D[i] - 1))) * PST_BYTES;
                             bulk_g2s(sbase + SM_PST + s * PST_BYTES, src, PST_BYTES, bar(B_PST_FULL + s));
                             n_pst[s]++;
                         }
@@ -186,89 +209,124 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
             __syncwarp();
         } else if (warp == NEPI + 1) {
             // =========================== MMA issuer ===================================================================
-            if (lane == 0) {
+            if (elect_one()) {
                 const uint32_t idesc128 = make_idesc_f16(128, 128), idesc64 = make_idesc_f16(128, 64);
-                // GEMM1 of slot s, iteration n (global counter nit): f|g = [h(t-d) | h(t)] . Wfg^T
-                auto G1 = [&](int s, int n, uint32_t nit, bool release) {
-                    const int i = n % L, j = n / L;
-                    const int st = nit & 1;
-                    const int d = M.dil[i], kind = M.kind[i];
-                    const uint32_t wfg = sbase + SM_WFG + st * WFG_BYTES;
-                    const uint32_t xs = sbase + SM_X + s * X_BYTES;
-                    const uint32_t dt = tmem + 128 * s;
-                    uint32_t acc = 0;
-                    if (kind < 2) {
-                        if (kind == 1 && j >= 1) n_pre[s]++;
-                        tc_fence_after();
-                        for (int kk = 0; kk < 4; kk++, acc = 1)
-                            tc_mma_f16(dt, make_sdesc(xs + (64 - d) * 16 + 2 * kk * X_CHUNK, X_CHUNK, 128),
-                                       make_sdesc(wfg + 2 * kk * 2048, 2048, 128), idesc128, acc);
-                    } else if (j >= M.D[i]) {
-                        n_pst[s]++;
-                        tc_fence_after();
-                        const uint32_t ps = sbase + SM_PST + s * PST_BYTES;
-                        for (int kk = 0; kk < 4; kk++, acc = 1)
-                            tc_mma_f16(dt, make_sdesc(ps + 2 * kk * 2048, 2048, 128),
-                                       make_sdesc(wfg + 2 * kk * 2048, 2048, 128), idesc128, acc);
-                    } else {
-                        tc_fence_after();
-                    }
-                    for (int kk = 0; kk < 4; kk++, acc = 1)
-                        tc_mma_f16(dt, make_sdesc(xs + 64 * 16 + 2 * kk * X_CHUNK, X_CHUNK, 128),
-                                   make_sdesc(wfg + (8 + 2 * kk) * 2048, 2048, 128), idesc128, acc);
-                    tc_commit(bar(B_FG_FULL + s));
-                    if (kind == 2 && j >= M.D[i]) tc_commit(bar(B_PST_FREE + s));
-                    if (release) tc_commit(bar(B_WFG_FREE + st));
+                // Base descriptors, built once: the address field is the low 14 bits (16-byte units), so an operand at
+                // another offset is the base plus (bytes >> 4).  This thread is a single instruction stream whose
+                // latency bounds the MMA issue rate, hence no divisions, no arrays, no descriptor builds in the loop;
+                // under elect_one() the compiler keeps all of it in uniform registers.
+                const uint64_t dX = make_sdesc(sbase + SM_X + 64 * 16, X_CHUNK, 128);   // current rows; slot 1: + X_BYTES/16
+                const uint64_t dP = make_sdesc(sbase + SM_PST, 2048, 128);              // past tile;    slot 1: + PST_BYTES/16
+                const uint64_t dWfg = make_sdesc(sbase + SM_WFG, 2048, 128);            // stage 1: + WFG_BYTES/16
+                const uint64_t dWrs = make_sdesc(sbase + SM_WRS, 3072, 128);            // stage 1: + WRS_STRIDE/16
+                struct Slot {
+                    int i, j, op;          // layer, tile, next op (0: GEMM1, 1: GEMM2)
+                    uint32_t nit;          // global iteration counter of the next op
+                    uint32_t npst, npre;   // loads consumed so far (parities of PST_FULL / PRE_FULL)
+                    bool stored;           // a bulk store of this slot's history tile is in flight
                 };
-                // GEMM2 of slot s: skip += z' Ws'^T ; res = z' Wr'^T
-                auto G2 = [&](int s, int n, uint32_t nit, bool release) {
-                    const int i = n % L;
-                    const int st = nit & 1;
-                    const uint32_t wrs = sbase + SM_WRS + st * WRS_STRIDE;
-                    tc_fence_after();
-                    const uint32_t zs = sbase + SM_X + s * X_BYTES + 64 * 16;
-                    for (int kk = 0; kk < 4; kk++)
-                        tc_mma_f16(tmem + 256 + 128 * s, make_sdesc(zs + 2 * kk * X_CHUNK, X_CHUNK, 128),
-                                   make_sdesc(wrs + 2 * kk * 3072, 3072, 128), idesc128, (i > 0 || kk > 0) ? 1u : 0u);
-                    if (i < L - 1)   // reading A8: the last block's residual conv has no effect
-                        for (int kk = 0; kk < 4; kk++)
-                            tc_mma_f16(tmem + 128 * s, make_sdesc(zs + 2 * kk * X_CHUNK, X_CHUNK, 128),
-                                       make_sdesc(wrs + 128 * 16 + 2 * kk * 3072, 3072, 128), idesc64, kk > 0 ? 1u : 0u);
-                    tc_commit(bar(B_RS_FULL + s));
-                    if (release) tc_commit(bar(B_WRS_FREE + st));
-                };
-                // dynamic order: whichever slot's next GEMM has its operands ready is issued next
-                int sn[2] = {0, 0}, sop[2] = {0, 0};     // per slot: iteration inside the job, next op (0: G1, 1: G2)
+                Slot S0{0, 0, 0, n_it, n_pst[0], n_pre[0], false}, S1{0, 0, 0, n_it, n_pst[1], n_pre[1], false};
+                const uint32_t nit_start = n_it;
+                const uint32_t nit_end = n_it + (uint32_t)NI;
                 uint32_t idle = 0;
-                while (sn[0] < NI || sn[1] < NI) {
-                    bool any = false;
+                // issues the next GEMM of slot s if its operands are ready; dynamic order between the two slots
+                auto step = [&](auto SC, Slot& me, const Slot& ot) -> bool {
+                    constexpr int s = decltype(SC)::value;
+                    const uint32_t nit = me.nit, st = nit & 1, wpar = (nit >> 1) & 1, par = nit & 1;
+                    if (me.op == 0) {
+                        // ---- GEMM1: f|g = [h(t-d) | h(t)] . Wfg^T
+                        // stagger: slot 1 starts once slot 0 has gated its first tile-layer, so that afterwards one
+                        // slot's gate (MUFU) overlaps the other slot's GEMMs and residual update
+                        if (s == 1 && nit == nit_start && ot.nit == nit_start) return false;
+                        const int li = M.lay[me.i], kind = li & 3, d = li >> 2;
+                        const bool past = kind < 2 || me.j >= (d >> 7);
+                        if (!mbar_test(bar(B_WFG_FULL + st), wpar) || !mbar_test(bar(B_H_READY + s), par)) return false;
+                        if (kind == 1 && me.j >= 1 && !mbar_test(bar(B_PRE_FULL + s), me.npre & 1)) return false;
+                        if (kind == 2 && past && !mbar_test(bar(B_PST_FULL + s), me.npst & 1)) return false;
+                        tc_fence_after();
+                        TRACE(1, s + 10 * (idle > 9999 ? 9999 : idle), (int)(nit - nit_start));
+                        // history for later tiles: this thread copies the freshly published operand rows from shared
+                        // memory to the L2-resident rings with the bulk-copy engine (no per-thread global stores and
+                        // fences in the epilogue).  The ring entry of tile j is the one tile j - D was read from, and
+                        // that read has landed (PST_FULL above).
+                        if (kind == 2 && me.j + (d >> 7) < a.ntiles) {
+                            uint8_t* dst = a.ring + (((size_t)blockIdx.x * 2 + s) * M.ring_tiles + M.ring_off[me.i] +
+                                                     (me.j & ((d >> 7) - 1))) * PST_BYTES;
+                            const uint32_t src = sbase + SM_X + s * X_BYTES + 64 * 16;
 #pragma unroll
-                    for (int s = 0; s < 2; s++) {
-                        if (sn[s] >= NI) continue;
-                        const int n = sn[s];
-                        const uint32_t nit = n_it + n;
-                        const int st = nit & 1;
-                        if (sop[s] == 0) {
-                            const int i = n % L, j = n / L, kind = M.kind[i];
-                            bool ok = mbar_test(bar(B_WFG_FULL + st), (nit >> 1) & 1) && mbar_test(bar(B_H_READY + s), nit & 1);
-                            if (ok && kind == 1 && j >= 1) ok = mbar_test(bar(B_PRE_FULL + s), n_pre[s] & 1);
-                            if (ok && kind == 2 && j >= M.D[i]) ok = mbar_test(bar(B_PST_FULL + s), n_pst[s] & 1);
-                            if (!ok) continue;
-                            // the slot that issues G1(n) second releases the weight stage
-                            const int o = s ^ 1;
-                            G1(s, n, nit, sn[o] > n || (sn[o] == n && sop[o] == 1));
-                            sop[s] = 1, any = true;
-                        } else {
-                            if (!(mbar_test(bar(B_WRS_FULL + st), (nit >> 1) & 1) && mbar_test(bar(B_Z_READY + s), nit & 1))) continue;
-                            const int o = s ^ 1;
-                            G2(s, n, nit, sn[o] > n);
-                            sop[s] = 0, sn[s] = n + 1, any = true;
+                            for (int c = 0; c < 8; c++) bulk_s2g(dst + c * 2048, src + c * X_CHUNK, 2048);
+                            bulk_commit();
+                            me.stored = true;
+                        } else if (kind == 1 && me.j + 1 < a.ntiles) {
+                            uint8_t* dst = a.ring64 + ((((size_t)blockIdx.x * 2 + s) * M.n64 + M.ring_off[me.i]) * 2 + (me.j & 1)) * PRE_BYTES;
+                            const uint32_t src = sbase + SM_X + s * X_BYTES + 128 * 16;
+#pragma unroll
+                            for (int c = 0; c < 8; c++) bulk_s2g(dst + c * 1024, src + c * X_CHUNK, 1024);
+                            bulk_commit();
+                            me.stored = true;
                         }
+                        const uint32_t dt = tmem + 128 * s;
+                        const uint64_t bw = dWfg + st * (WFG_BYTES >> 4);
+                        const uint64_t ax = dX + s * (X_BYTES >> 4);
+                        uint32_t acc = 0;
+                        if (past) {
+                            const uint64_t ap = kind < 2 ? ax - d : dP + s * (PST_BYTES >> 4);
+                            const uint32_t ka = kind < 2 ? (2 * X_CHUNK) >> 4 : 4096 >> 4;
+#pragma unroll
+                            for (int kk = 0; kk < 4; kk++, acc = 1) tc_mma_f16(dt, ap + kk * ka, bw + kk * 256, idesc128, acc);
+                        }
+#pragma unroll
+                        for (int kk = 0; kk < 4; kk++, acc = 1)
+                            tc_mma_f16(dt, ax + kk * ((2 * X_CHUNK) >> 4), bw + 1024 + kk * 256, idesc128, acc);
+                        if (me.stored) bulk_wait_read();   // the gate overwrites these rows once it sees FG_FULL
+                        tc_commit(bar(B_FG_FULL + s));
+                        TRACE(2, s, (int)(nit - nit_start));
+                        if (kind == 2 && past) {
+                            tc_commit(bar(B_PST_FREE + s));
+                            me.npst++;
+                        }
+                        if (kind == 1 && me.j >= 1) me.npre++;
+                        // the slot that issues GEMM1 of an iteration second releases the weight stage
+                        if (ot.nit > nit || (ot.nit == nit && ot.op == 1)) tc_commit(bar(B_WFG_FREE + st));
+                        me.op = 1;
+                    } else {
+                        // ---- GEMM2: skip += z' Ws'^T ; res = z' Wr'^T
+                        if (!mbar_test(bar(B_WRS_FULL + st), wpar) || !mbar_test(bar(B_Z_READY + s), par)) return false;
+                        tc_fence_after();
+                        if (me.stored) {   // the ring write is complete before RS_FULL of this iteration (the producer's cue)
+                            bulk_wait_all();
+                            me.stored = false;
+                        }
+                        TRACE(3, s + 10 * (idle > 9999 ? 9999 : idle), (int)(nit - nit_start));
+                        const uint64_t bw = dWrs + st * (WRS_STRIDE >> 4);
+                        const uint64_t az = dX + s * (X_BYTES >> 4);
+#pragma unroll
+                        for (int kk = 0; kk < 4; kk++)
+                            tc_mma_f16(tmem + 256 + 128 * s, az + kk * ((2 * X_CHUNK) >> 4), bw + kk * 384, idesc128,
+                                       (me.i > 0 || kk > 0) ? 1u : 0u);
+                        if (me.i < L - 1) {  // reading A8: the last block's residual conv has no effect
+#pragma unroll
+                            for (int kk = 0; kk < 4; kk++)
+                                tc_mma_f16(tmem + 128 * s, az + kk * ((2 * X_CHUNK) >> 4), bw + 128 + kk * 384, idesc64,
+                                           kk > 0 ? 1u : 0u);
+                        }
+                        tc_commit(bar(B_RS_FULL + s));
+                        TRACE(4, s, (int)(nit - nit_start));
+                        if (ot.nit > nit) tc_commit(bar(B_WRS_FREE + st));
+                        me.op = 0, me.nit = nit + 1;
+                        if (++me.i == L) me.i = 0, me.j++;
                     }
+                    return true;
+                };
+                while (S0.nit != nit_end || S1.nit != nit_end) {
+                    bool any = false;
+                    if (S0.nit != nit_end) any |= step(std::integral_constant<int, 0>{}, S0, S1);
+                    if (S1.nit != nit_end) any |= step(std::integral_constant<int, 1>{}, S1, S0);
                     if (any) idle = 0;
                     else if (++idle > (1u << 27)) __trap();
                 }
-                n_it += NI;
+                n_it = nit_end;
+                n_pst[0] = S0.npst, n_pst[1] = S1.npst, n_pre[0] = S0.npre, n_pre[1] = S1.npre;
             }
             __syncwarp();
         } else {
@@ -282,7 +340,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
             const uint32_t xs = sbase + SM_X + s * X_BYTES;
             const uint32_t st0 = sbase + SM_STASH + s * STASH_BYTES;
             const uint32_t lane_t = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-            uint8_t* ring_s = a.ring + ((size_t)blockIdx.x * 2 + s) * M.ring_tiles * PST_BYTES;
             uint8_t* ring64_s = a.ring64 + ((size_t)blockIdx.x * 2 + s) * M.n64 * 2 * PRE_BYTES;
             const float* cst = a.cst + b * 256;
             float2 h[16];                                             // fp32 master of the residual stream, 32 channels
@@ -312,21 +369,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 #pragma unroll
                         for (int c = 0; c < 4; c++) st_shared_v4(xs + r * 16 + (c0 + c) * X_CHUNK, 0u, 0u, 0u, 0u);
                     }
-                    if (r >= 64) {
-                        uint8_t* g = ring64_s + (size_t)(M.ring_off[inext] * 2 + (j & 1)) * PRE_BYTES + (r - 64) * 16;
-#pragma unroll
-                        for (int c = 0; c < 4; c++)
-                            *reinterpret_cast<uint4*>(g + (c0 + c) * 1024) = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
-                        __threadfence_block();
-                        fence_proxy_async();
-                    }
-                } else {
-                    uint8_t* g = ring_s + (size_t)(M.ring_off[inext] + j % (M.D[inext] + 1)) * PST_BYTES + r * 16;
-#pragma unroll
-                    for (int c = 0; c < 4; c++)
-                        *reinterpret_cast<uint4*>(g + (c0 + c) * 2048) = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
-                    __threadfence_block();
-                    fence_proxy_async();
                 }
                 tc_fence_before();
                 fence_proxy_async_smem();
@@ -353,6 +395,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     const int st = n_it & 1;
                     // ---- gate: z' = tanh(f + bf) * (1 + tanh(g/2 + bg/2))
                     mbar_wait(bar(B_FG_FULL + s), ph);
+                    if (lane == 0) TRACE(5, 10 * (warp & 7) + s, j * L + i);
                     const int inx = (i + 1 < L) ? i + 1 : 0, jnx = (i + 1 < L) ? j : j + 1;   // the next (layer, tile)
                     if (M.kind[inx] == 1 && jnx >= 1 && jnx < a.ntiles && (warp & 7) == 0 && lane == 0) {
                         // G1(i) has finished with the pre rows: fetch the 64 rows that precede tile jnx for layer inx
@@ -395,8 +438,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     tc_fence_before();
                     fence_proxy_async_smem();
                     mbar_arrive(bar(B_Z_READY + s));
+                    if (lane == 0) TRACE(6, 10 * (warp & 7) + s, j * L + i);
                     // ---- residual update (or, after the last block, the branch output)
                     mbar_wait(bar(B_RS_FULL + s), ph);
+                    if (lane == 0) TRACE(7, 10 * (warp & 7) + s, j * L + i);
                     tc_fence_after();
                     if (i < L - 1) {
                         uint32_t v[32];
@@ -406,6 +451,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                         for (int c = 0; c < 16; c++)
                             h[c] = add2(h[c], make_float2(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1])));
                         publish(i + 1, j);
+                        if (lane == 0) TRACE(8, 10 * (warp & 7) + s, j * L + i);
                     } else {
                         // u = ReLU(sum_i skip_i) -> fp16 tile in the workspace                       (C.1 step 3)
                         uint8_t* ut = a.u + (((size_t)wl * nb + b) * a.ntiles + j) * U_TILE_BYTES + r * 16;
@@ -560,7 +606,7 @@ bool gwi_tc_supported(const GwiArch& a)
         int d = a.dil[i];
         if (d <= 32) stash += d * 128;
         else if (d == 64) continue;
-        else if (d % 128 != 0) return false;
+        else if (d % 128 != 0 || ((d / 128) & (d / 128 - 1)) != 0) return false;   // whole tiles, power of two
     }
     return stash <= STASH_BYTES;
 }
@@ -588,7 +634,8 @@ gwi_status gwi_tc_pack(gwi_model* m)
         M.kind[i] = a.dil[i] <= 32 ? 0 : (a.dil[i] == 64 ? 1 : 2);
         M.D[i] = M.kind[i] == 2 ? a.dil[i] / 128 : 0;
         M.stash_off[i] = so;
-        if (M.kind[i] == 2) M.ring_off[i] = ro, ro += M.D[i] + 1;
+        M.lay[i] = M.kind[i] | (a.dil[i] << 2);
+        if (M.kind[i] == 2) M.ring_off[i] = ro, ro += M.D[i];
         else if (M.kind[i] == 1) M.ring_off[i] = n64++;
         else M.ring_off[i] = 0, so += a.dil[i] * 128;
     }
@@ -700,6 +747,17 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
         k_head_tc<<<hgrid, HEAD_THREADS, 3 * nb * U_TILE_BYTES + 256, st>>>(ha);
         gwi_count_launch(2);
         GWI_CUDA_CHECK(cudaGetLastError());
+#ifdef GWI_TC_TRACE
+        if (const char* tp = getenv("GWI_TC_TRACE_FILE")) {
+            cudaStreamSynchronize(st);
+            std::vector<uint4> ev(18 * TRACE_CAP);
+            cudaMemcpyFromSymbol(ev.data(), g_trace, ev.size() * 16);
+            if (FILE* f = fopen(tp, "w")) {
+                for (auto& e : ev) fprintf(f, "%u %u %u %u\n", e.x, e.y, e.z, e.w);
+                fclose(f);
+            }
+        }
+#endif
     }
     return GWI_OK;
 }
