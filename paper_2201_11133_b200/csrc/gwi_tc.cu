@@ -45,7 +45,7 @@ constexpr int PRE_BYTES = 8 * 64 * 16;              // 8192: the 64 rows that pr
 constexpr int STASH_BYTES = 16384;                  // per slot: sum over layers with d <= 32 of d rows x 128 B
 constexpr int U_TILE_BYTES = 16 * 128 * 16;         // 32768: u tile, 16 chunks x 128 rows x 16 B
 constexpr int NEPI = 16;                            // epilogue warps: slot = w >> 3, column half = (w >> 2) & 1
-constexpr int NTHREADS = (NEPI + 2) * 32;           // + producer warp + MMA warp
+constexpr int NTHREADS = (NEPI + 3) * 32;           // + producer warp + one MMA issuer warp per slot
 
 struct TcMeta {
     int L, n_branch;
@@ -64,7 +64,7 @@ struct TcMeta {
 // debug build only (-DGWI_TC_TRACE): the MMA issuer, the producer and lane 0 of every epilogue warp of CTA 0 record
 // (event, slot, iteration, clock) tuples, each into its own region (plain stores, no atomics)
 #define TRACE_CAP 4096
-__device__ uint4 g_trace[18 * TRACE_CAP];
+__device__ uint4 g_trace[19 * TRACE_CAP];
 #define TRACE(ev, slot, n)                                                                                   \
     do {                                                                                                     \
         if (blockIdx.x == 0 && trace_k < TRACE_CAP)                                                          \
@@ -98,7 +98,7 @@ constexpr int SM_TOTAL = SM_BAR + 256;
 static_assert(SM_TOTAL <= 232448, "shared memory budget");
 
 enum { B_WFG_FULL = 0, B_WFG_FREE = 2, B_WRS_FULL = 4, B_WRS_FREE = 6, B_FG_FULL = 8, B_Z_READY = 10, B_RS_FULL = 12,
-       B_H_READY = 14, B_PST_FULL = 16, B_PST_FREE = 18, B_PRE_FULL = 20, B_COUNT = 22 };
+       B_H_READY = 14, B_PST_FULL = 16, B_PST_FREE = 18, B_PRE_FULL = 20, B_STAGGER = 22, B_COUNT = 23 };
 
 __device__ __forceinline__ float2 add2(float2 a, float2 b)
 {
@@ -137,6 +137,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
     if (threadIdx.x == 0) {
         for (int i = 0; i < B_COUNT; i++) {
             uint32_t cnt = (i >= B_Z_READY && i < B_Z_READY + 2) || (i >= B_H_READY && i < B_H_READY + 2) ? 256u : 1u;
+            if ((i >= B_WFG_FREE && i < B_WFG_FREE + 2) || (i >= B_WRS_FREE && i < B_WRS_FREE + 2)) cnt = 2u;   // both issuers
             mbar_init(bar(i), cnt);
         }
         mbar_fence_init();
@@ -155,14 +156,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
     uint32_t n_it = 0;                 // (job, tile, layer) iterations done
     uint32_t n_pst[2] = {0, 0};        // ring-tile loads done per slot
     uint32_t n_pre[2] = {0, 0};        // pre-row loads done per slot
+    uint32_t n_job = 0;                // jobs done by this CTA (parity of the STAGGER barrier)
 #ifdef GWI_TC_TRACE
     unsigned trace_k = 0;
-    const int trace_role = warp == NEPI + 1 ? 0 : (warp == NEPI ? 17 : 1 + (warp & 15));
+    const int trace_role = warp == NEPI + 1 ? 0 : (warp == NEPI ? 17 : (warp == NEPI + 2 ? 18 : 1 + (warp & 15)));
 #endif
 
     for (int64_t job = blockIdx.x; job < njobs; job += gridDim.x) {
         const int b = (int)(job % nb);
         const int64_t pair = job / nb;
+        const uint32_t job_par = n_job++ & 1;
         // ---- job prologue (all threads): zero the stashes and the X buffers (causal zero history, reading A4) --------
         __syncthreads();
         {
@@ -207,127 +210,110 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                 }
             }
             __syncwarp();
-        } else if (warp == NEPI + 1) {
-            // =========================== MMA issuer ===================================================================
+        } else if (warp == NEPI + 1 || warp == NEPI + 2) {
+            // =========================== MMA issuers: one thread per slot ===============================================
+            // Each slot has its own issuer (a single thread issues ~8 tcgen05.mma per GEMM in a dependent instruction
+            // stream; with one thread for both slots that stream was the bottleneck).  The two threads only meet in
+            // the tensor pipe and on the weight-stage barriers (WFG_FREE / WRS_FREE take one commit from each).
             if (elect_one()) {
                 const uint32_t idesc128 = make_idesc_f16(128, 128), idesc64 = make_idesc_f16(128, 64);
-                // Base descriptors, built once: the address field is the low 14 bits (16-byte units), so an operand at
-                // another offset is the base plus (bytes >> 4).  This thread is a single instruction stream whose
-                // latency bounds the MMA issue rate, hence no divisions, no arrays, no descriptor builds in the loop;
-                // under elect_one() the compiler keeps all of it in uniform registers.
-                const uint64_t dX = make_sdesc(sbase + SM_X + 64 * 16, X_CHUNK, 128);   // current rows; slot 1: + X_BYTES/16
-                const uint64_t dP = make_sdesc(sbase + SM_PST, 2048, 128);              // past tile;    slot 1: + PST_BYTES/16
-                const uint64_t dWfg = make_sdesc(sbase + SM_WFG, 2048, 128);            // stage 1: + WFG_BYTES/16
-                const uint64_t dWrs = make_sdesc(sbase + SM_WRS, 3072, 128);            // stage 1: + WRS_STRIDE/16
-                struct Slot {
-                    int i, j, op;          // layer, tile, next op (0: GEMM1, 1: GEMM2)
-                    uint32_t nit;          // global iteration counter of the next op
-                    uint32_t npst, npre;   // loads consumed so far (parities of PST_FULL / PRE_FULL)
-                    bool stored;           // a bulk store of this slot's history tile is in flight
-                };
-                Slot S0{0, 0, 0, n_it, n_pst[0], n_pre[0], false}, S1{0, 0, 0, n_it, n_pst[1], n_pre[1], false};
-                const uint32_t nit_start = n_it;
-                const uint32_t nit_end = n_it + (uint32_t)NI;
-                uint32_t idle = 0;
-                // issues the next GEMM of slot s if its operands are ready; dynamic order between the two slots
-                auto step = [&](auto SC, Slot& me, const Slot& ot) -> bool {
+                auto issuer = [&](auto SC) {
                     constexpr int s = decltype(SC)::value;
-                    const uint32_t nit = me.nit, st = nit & 1, wpar = (nit >> 1) & 1, par = nit & 1;
-                    if (me.op == 0) {
+                    // descriptors built once; the address field is the low 14 bits (16-byte units)
+                    const uint64_t ax = make_sdesc(sbase + SM_X + s * X_BYTES + 64 * 16, X_CHUNK, 128);   // current rows / z
+                    const uint64_t apst = make_sdesc(sbase + SM_PST + s * PST_BYTES, 2048, 128);           // past tile
+                    const uint64_t dWfg = make_sdesc(sbase + SM_WFG, 2048, 128);
+                    const uint64_t dWrs = make_sdesc(sbase + SM_WRS, 3072, 128);
+                    const uint32_t dt = tmem + 128 * s, dskip = tmem + 256 + 128 * s;
+                    const uint32_t xrows = sbase + SM_X + s * X_BYTES + 64 * 16;
+                    uint8_t* const ring_s = a.ring + ((size_t)blockIdx.x * 2 + s) * M.ring_tiles * PST_BYTES;
+                    uint8_t* const ring64_s = a.ring64 + ((size_t)blockIdx.x * 2 + s) * M.n64 * 2 * PRE_BYTES;
+                    uint32_t nit = n_it, npst = n_pst[s], npre = n_pre[s];
+                    int i = 0, j = 0;
+                    // stagger: slot 1 starts once slot 0 has gated its first tile-layer of the job, so that afterwards
+                    // one slot's gate (MUFU) overlaps the other slot's GEMMs and residual update
+                    if (s == 1) mbar_wait(bar(B_STAGGER), job_par);
+                    for (int n = 0; n < NI; n++, nit++) {
+                        const uint32_t st = nit & 1, wpar = (nit >> 1) & 1, par = nit & 1;
                         // ---- GEMM1: f|g = [h(t-d) | h(t)] . Wfg^T
-                        // stagger: slot 1 starts once slot 0 has gated its first tile-layer, so that afterwards one
-                        // slot's gate (MUFU) overlaps the other slot's GEMMs and residual update
-                        if (s == 1 && nit == nit_start && ot.nit == nit_start) return false;
-                        const int li = M.lay[me.i], kind = li & 3, d = li >> 2;
-                        const bool past = kind < 2 || me.j >= (d >> 7);
-                        if (!mbar_test(bar(B_WFG_FULL + st), wpar) || !mbar_test(bar(B_H_READY + s), par)) return false;
-                        if (kind == 1 && me.j >= 1 && !mbar_test(bar(B_PRE_FULL + s), me.npre & 1)) return false;
-                        if (kind == 2 && past && !mbar_test(bar(B_PST_FULL + s), me.npst & 1)) return false;
-                        tc_fence_after();
-                        TRACE(1, s + 10 * (idle > 9999 ? 9999 : idle), (int)(nit - nit_start));
-                        // history for later tiles: this thread copies the freshly published operand rows from shared
-                        // memory to the L2-resident rings with the bulk-copy engine (no per-thread global stores and
-                        // fences in the epilogue).  The ring entry of tile j is the one tile j - D was read from, and
-                        // that read has landed (PST_FULL above).
-                        if (kind == 2 && me.j + (d >> 7) < a.ntiles) {
-                            uint8_t* dst = a.ring + (((size_t)blockIdx.x * 2 + s) * M.ring_tiles + M.ring_off[me.i] +
-                                                     (me.j & ((d >> 7) - 1))) * PST_BYTES;
-                            const uint32_t src = sbase + SM_X + s * X_BYTES + 64 * 16;
-#pragma unroll
-                            for (int c = 0; c < 8; c++) bulk_s2g(dst + c * 2048, src + c * X_CHUNK, 2048);
-                            bulk_commit();
-                            me.stored = true;
-                        } else if (kind == 1 && me.j + 1 < a.ntiles) {
-                            uint8_t* dst = a.ring64 + ((((size_t)blockIdx.x * 2 + s) * M.n64 + M.ring_off[me.i]) * 2 + (me.j & 1)) * PRE_BYTES;
-                            const uint32_t src = sbase + SM_X + s * X_BYTES + 128 * 16;
-#pragma unroll
-                            for (int c = 0; c < 8; c++) bulk_s2g(dst + c * 1024, src + c * X_CHUNK, 1024);
-                            bulk_commit();
-                            me.stored = true;
+                        const int li = M.lay[i], kind = li & 3, d = li >> 2;
+                        const bool past = kind < 2 || j >= (d >> 7);
+                        mbar_wait(bar(B_WFG_FULL + st), wpar);
+                        mbar_wait(bar(B_H_READY + s), par);
+                        if (kind == 1 && j >= 1) {
+                            mbar_wait(bar(B_PRE_FULL + s), npre & 1);
+                            npre++;
                         }
-                        const uint32_t dt = tmem + 128 * s;
-                        const uint64_t bw = dWfg + st * (WFG_BYTES >> 4);
-                        const uint64_t ax = dX + s * (X_BYTES >> 4);
-                        uint32_t acc = 0;
-                        if (past) {
-                            const uint64_t ap = kind < 2 ? ax - d : dP + s * (PST_BYTES >> 4);
-                            const uint32_t ka = kind < 2 ? (2 * X_CHUNK) >> 4 : 4096 >> 4;
-#pragma unroll
-                            for (int kk = 0; kk < 4; kk++, acc = 1) tc_mma_f16(dt, ap + kk * ka, bw + kk * 256, idesc128, acc);
-                        }
-#pragma unroll
-                        for (int kk = 0; kk < 4; kk++, acc = 1)
-                            tc_mma_f16(dt, ax + kk * ((2 * X_CHUNK) >> 4), bw + 1024 + kk * 256, idesc128, acc);
-                        if (me.stored) bulk_wait_read();   // the gate overwrites these rows once it sees FG_FULL
-                        tc_commit(bar(B_FG_FULL + s));
-                        TRACE(2, s, (int)(nit - nit_start));
                         if (kind == 2 && past) {
-                            tc_commit(bar(B_PST_FREE + s));
-                            me.npst++;
+                            mbar_wait(bar(B_PST_FULL + s), npst & 1);
+                            npst++;
                         }
-                        if (kind == 1 && me.j >= 1) me.npre++;
-                        // the slot that issues GEMM1 of an iteration second releases the weight stage
-                        if (ot.nit > nit || (ot.nit == nit && ot.op == 1)) tc_commit(bar(B_WFG_FREE + st));
-                        me.op = 1;
-                    } else {
-                        // ---- GEMM2: skip += z' Ws'^T ; res = z' Wr'^T
-                        if (!mbar_test(bar(B_WRS_FULL + st), wpar) || !mbar_test(bar(B_Z_READY + s), par)) return false;
                         tc_fence_after();
-                        if (me.stored) {   // the ring write is complete before RS_FULL of this iteration (the producer's cue)
-                            bulk_wait_all();
-                            me.stored = false;
-                        }
-                        TRACE(3, s + 10 * (idle > 9999 ? 9999 : idle), (int)(nit - nit_start));
-                        const uint64_t bw = dWrs + st * (WRS_STRIDE >> 4);
-                        const uint64_t az = dX + s * (X_BYTES >> 4);
+                        TRACE(1, s, n);
+                        // history for later tiles: the freshly published operand rows go from shared memory to the
+                        // L2-resident rings through the bulk-copy engine.  The ring entry of tile j is the one tile
+                        // j - D was read from, and that read has landed (PST_FULL above).
+                        bool stored = false;
+                        if (kind == 2 && j + (d >> 7) < a.ntiles) {
+                            uint8_t* dst = ring_s + (size_t)(M.ring_off[i] + (j & ((d >> 7) - 1))) * PST_BYTES;
 #pragma unroll
-                        for (int kk = 0; kk < 4; kk++)
-                            tc_mma_f16(tmem + 256 + 128 * s, az + kk * ((2 * X_CHUNK) >> 4), bw + kk * 384, idesc128,
-                                       (me.i > 0 || kk > 0) ? 1u : 0u);
-                        if (me.i < L - 1) {  // reading A8: the last block's residual conv has no effect
+                            for (int c = 0; c < 8; c++) bulk_s2g(dst + c * 2048, xrows + c * X_CHUNK, 2048);
+                            bulk_commit();
+                            stored = true;
+                        } else if (kind == 1 && j + 1 < a.ntiles) {
+                            uint8_t* dst = ring64_s + (size_t)(M.ring_off[i] * 2 + (j & 1)) * PRE_BYTES;
+#pragma unroll
+                            for (int c = 0; c < 8; c++) bulk_s2g(dst + c * 1024, xrows + 64 * 16 + c * X_CHUNK, 1024);
+                            bulk_commit();
+                            stored = true;
+                        }
+                        {
+                            const uint64_t bw = dWfg + st * (WFG_BYTES >> 4);
+                            uint32_t acc = 0;
+                            if (past) {
+                                const uint64_t ap = kind < 2 ? ax - d : apst;
+                                const uint32_t ka = kind < 2 ? (2 * X_CHUNK) >> 4 : 4096 >> 4;
+#pragma unroll
+                                for (int kk = 0; kk < 4; kk++, acc = 1) tc_mma_f16(dt, ap + kk * ka, bw + kk * 256, idesc128, acc);
+                            }
+#pragma unroll
+                            for (int kk = 0; kk < 4; kk++, acc = 1)
+                                tc_mma_f16(dt, ax + kk * ((2 * X_CHUNK) >> 4), bw + 1024 + kk * 256, idesc128, acc);
+                        }
+                        if (stored) bulk_wait_read();   // the gate overwrites these rows once it sees FG_FULL
+                        tc_commit(bar(B_FG_FULL + s));
+                        if (kind == 2 && past) tc_commit(bar(B_PST_FREE + s));
+                        tc_commit(bar(B_WFG_FREE + st));          // one commit per slot frees the stage
+                        TRACE(2, s, n);
+                        // ---- GEMM2: skip += z' Ws'^T ; res = z' Wr'^T
+                        mbar_wait(bar(B_WRS_FULL + st), wpar);
+                        mbar_wait(bar(B_Z_READY + s), par);
+                        tc_fence_after();
+                        if (s == 0 && n == 0) mbar_arrive(bar(B_STAGGER));
+                        if (stored) bulk_wait_all();   // ring write complete before RS_FULL of this iteration (producer's cue)
+                        TRACE(3, s, n);
+                        {
+                            const uint64_t bw = dWrs + st * (WRS_STRIDE >> 4);
 #pragma unroll
                             for (int kk = 0; kk < 4; kk++)
-                                tc_mma_f16(tmem + 128 * s, az + kk * ((2 * X_CHUNK) >> 4), bw + 128 + kk * 384, idesc64,
-                                           kk > 0 ? 1u : 0u);
+                                tc_mma_f16(dskip, ax + kk * ((2 * X_CHUNK) >> 4), bw + kk * 384, idesc128, (i > 0 || kk > 0) ? 1u : 0u);
+                            if (i < L - 1) {  // reading A8: the last block's residual conv has no effect
+#pragma unroll
+                                for (int kk = 0; kk < 4; kk++)
+                                    tc_mma_f16(dt, ax + kk * ((2 * X_CHUNK) >> 4), bw + 128 + kk * 384, idesc64, kk > 0 ? 1u : 0u);
+                            }
                         }
                         tc_commit(bar(B_RS_FULL + s));
-                        TRACE(4, s, (int)(nit - nit_start));
-                        if (ot.nit > nit) tc_commit(bar(B_WRS_FREE + st));
-                        me.op = 0, me.nit = nit + 1;
-                        if (++me.i == L) me.i = 0, me.j++;
+                        tc_commit(bar(B_WRS_FREE + st));
+                        TRACE(4, s, n);
+                        if (++i == L) i = 0, j++;
                     }
-                    return true;
+                    n_pst[s] = npst, n_pre[s] = npre;
                 };
-                while (S0.nit != nit_end || S1.nit != nit_end) {
-                    bool any = false;
-                    if (S0.nit != nit_end) any |= step(std::integral_constant<int, 0>{}, S0, S1);
-                    if (S1.nit != nit_end) any |= step(std::integral_constant<int, 1>{}, S1, S0);
-                    if (any) idle = 0;
-                    else if (++idle > (1u << 27)) __trap();
-                }
-                n_it = nit_end;
-                n_pst[0] = S0.npst, n_pst[1] = S1.npst, n_pre[0] = S0.npre, n_pre[1] = S1.npre;
+                if (warp == NEPI + 1) issuer(std::integral_constant<int, 0>{});
+                else issuer(std::integral_constant<int, 1>{});
             }
+            n_it += NI;
             __syncwarp();
         } else {
             // =========================== epilogue: slot s, column half wg, row r =======================================
@@ -750,7 +736,7 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
 #ifdef GWI_TC_TRACE
         if (const char* tp = getenv("GWI_TC_TRACE_FILE")) {
             cudaStreamSynchronize(st);
-            std::vector<uint4> ev(18 * TRACE_CAP);
+            std::vector<uint4> ev(19 * TRACE_CAP);
             cudaMemcpyFromSymbol(ev.data(), g_trace, ev.size() * 16);
             if (FILE* f = fopen(tp, "w")) {
                 for (auto& e : ev) fprintf(f, "%u %u %u %u\n", e.x, e.y, e.z, e.w);
