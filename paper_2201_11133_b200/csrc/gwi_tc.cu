@@ -98,7 +98,7 @@ constexpr int SM_TOTAL = SM_BAR + 256;
 static_assert(SM_TOTAL <= 232448, "shared memory budget");
 
 enum { B_WFG_FULL = 0, B_WFG_FREE = 2, B_WRS_FULL = 4, B_WRS_FREE = 6, B_FG_FULL = 8, B_Z_READY = 10, B_RS_FULL = 12,
-       B_H_READY = 14, B_PST_FULL = 16, B_PST_FREE = 18, B_PRE_FULL = 20, B_STAGGER = 22, B_COUNT = 23 };
+       B_H_READY = 14, B_PST_FULL = 16, B_PST_FREE = 18, B_PRE_FULL = 20, B_SKD = 22, B_COUNT = 24 };
 
 __device__ __forceinline__ float2 add2(float2 a, float2 b)
 {
@@ -156,7 +156,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
     uint32_t n_it = 0;                 // (job, tile, layer) iterations done
     uint32_t n_pst[2] = {0, 0};        // ring-tile loads done per slot
     uint32_t n_pre[2] = {0, 0};        // pre-row loads done per slot
-    uint32_t n_job = 0;                // jobs done by this CTA (parity of the STAGGER barrier)
 #ifdef GWI_TC_TRACE
     unsigned trace_k = 0;
     const int trace_role = warp == NEPI + 1 ? 0 : (warp == NEPI ? 17 : (warp == NEPI + 2 ? 18 : 1 + (warp & 15)));
@@ -165,7 +164,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
     for (int64_t job = blockIdx.x; job < njobs; job += gridDim.x) {
         const int b = (int)(job % nb);
         const int64_t pair = job / nb;
-        const uint32_t job_par = n_job++ & 1;
         // ---- job prologue (all threads): zero the stashes and the X buffers (causal zero history, reading A4) --------
         __syncthreads();
         {
@@ -230,9 +228,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     uint8_t* const ring64_s = a.ring64 + ((size_t)blockIdx.x * 2 + s) * M.n64 * 2 * PRE_BYTES;
                     uint32_t nit = n_it, npst = n_pst[s], npre = n_pre[s];
                     int i = 0, j = 0;
-                    // stagger: slot 1 starts once slot 0 has gated its first tile-layer of the job, so that afterwards
-                    // one slot's gate (MUFU) overlaps the other slot's GEMMs and residual update
-                    if (s == 1) mbar_wait(bar(B_STAGGER), job_par);
                     for (int n = 0; n < NI; n++, nit++) {
                         const uint32_t st = nit & 1, wpar = (nit >> 1) & 1, par = nit & 1;
                         // ---- GEMM1: f|g = [h(t-d) | h(t)] . Wfg^T
@@ -289,21 +284,23 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                         mbar_wait(bar(B_WRS_FULL + st), wpar);
                         mbar_wait(bar(B_Z_READY + s), par);
                         tc_fence_after();
-                        if (s == 0 && n == 0) mbar_arrive(bar(B_STAGGER));
                         if (stored) bulk_wait_all();   // ring write complete before RS_FULL of this iteration (producer's cue)
                         TRACE(3, s, n);
                         {
+                            // the residual GEMM is on the critical path (next layer's operand), the skip GEMM is not:
+                            // residual first with its own commit, the skip sum runs under the residual epilogue
                             const uint64_t bw = dWrs + st * (WRS_STRIDE >> 4);
-#pragma unroll
-                            for (int kk = 0; kk < 4; kk++)
-                                tc_mma_f16(dskip, ax + kk * ((2 * X_CHUNK) >> 4), bw + kk * 384, idesc128, (i > 0 || kk > 0) ? 1u : 0u);
                             if (i < L - 1) {  // reading A8: the last block's residual conv has no effect
 #pragma unroll
                                 for (int kk = 0; kk < 4; kk++)
                                     tc_mma_f16(dt, ax + kk * ((2 * X_CHUNK) >> 4), bw + 128 + kk * 384, idesc64, kk > 0 ? 1u : 0u);
                             }
+                            tc_commit(bar(B_RS_FULL + s));
+#pragma unroll
+                            for (int kk = 0; kk < 4; kk++)
+                                tc_mma_f16(dskip, ax + kk * ((2 * X_CHUNK) >> 4), bw + kk * 384, idesc128, (i > 0 || kk > 0) ? 1u : 0u);
                         }
-                        tc_commit(bar(B_RS_FULL + s));
+                        tc_commit(bar(B_SKD + s));
                         tc_commit(bar(B_WRS_FREE + st));
                         TRACE(4, s, n);
                         if (++i == L) i = 0, j++;
@@ -379,8 +376,25 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                 for (int i = 0; i < L; i++, n_it++) {
                     const uint32_t ph = n_it & 1;
                     const int st = n_it & 1;
+                    // ---- off the critical path, while GEMM1 runs: this layer's biases (streamed behind its Wrs) and the
+                    // residual bias into the fp32 master
+                    mbar_wait(bar(B_WRS_FULL + st), (n_it >> 1) & 1);
+                    const float* bl = reinterpret_cast<const float*>(smem + SM_WRS + st * WRS_STRIDE + WRS_BYTES);
+                    if (i < L - 1) {
+#pragma unroll
+                        for (int c = 0; c < 16; c++) h[c] = add2(h[c], *reinterpret_cast<const float2*>(bl + 128 + ch0 + 2 * c));
+                    }
                     // ---- gate: z' = tanh(f + bf) * (1 + tanh(g/2 + bg/2))
                     mbar_wait(bar(B_FG_FULL + s), ph);
+#ifdef GWI_TC_ALTERNATE
+                    // optional: the gates of the two slots alternate (a gate starts when the other slot's previous gate
+                    // has ended) instead of drifting into lockstep
+                    if (s == 0) {
+                        if (j + i > 0) mbar_wait(bar(B_Z_READY + 1), (n_it - 1) & 1);
+                    } else {
+                        mbar_wait(bar(B_Z_READY + 0), n_it & 1);
+                    }
+#endif
                     if (lane == 0) TRACE(5, 10 * (warp & 7) + s, j * L + i);
                     const int inx = (i + 1 < L) ? i + 1 : 0, jnx = (i + 1 < L) ? j : j + 1;   // the next (layer, tile)
                     if (M.kind[inx] == 1 && jnx >= 1 && jnx < a.ntiles && (warp & 7) == 0 && lane == 0) {
@@ -391,35 +405,36 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                         for (int c = 0; c < 8; c++) bulk_g2s(xs + c * X_CHUNK, src + c * 1024, 1024, bar(B_PRE_FULL + s));
                     }
                     __syncwarp();
-                    mbar_wait(bar(B_WRS_FULL + st), (n_it >> 1) & 1);      // this layer's biases are behind its Wrs
-                    const float* bl = reinterpret_cast<const float*>(smem + SM_WRS + st * WRS_STRIDE + WRS_BYTES);
                     tc_fence_after();
+                    {
+                        // 4 chunks of 8 channels; the TMEM loads of chunk q+1 are in flight while chunk q is gated
+                        uint32_t fb[2][8], gb[2][8];
+                        const uint32_t tf0 = lane_t + 128 * s + ch0, tg0 = tf0 + 64;
+                        tmem_ld8(tf0, fb[0]);
+                        tmem_ld8(tg0, gb[0]);
 #pragma unroll
-                    for (int hh = 0; hh < 2; hh++) {
-                        uint32_t f[16], g[16];
-                        tmem_ld16(lane_t + 128 * s + ch0 + 16 * hh, f);
-                        tmem_ld16(lane_t + 128 * s + 64 + ch0 + 16 * hh, g);
-                        tc_wait_ld();
-                        uint32_t pk[8];
+                        for (int q = 0; q < 4; q++) {
+                            tc_wait_ld();
+                            if (q < 3) {
+                                tmem_ld8(tf0 + 8 * (q + 1), fb[(q + 1) & 1]);
+                                tmem_ld8(tg0 + 8 * (q + 1), gb[(q + 1) & 1]);
+                            }
+                            const uint32_t* f = fb[q & 1];
+                            const uint32_t* g = gb[q & 1];
+                            uint32_t pk[4];
 #pragma unroll
-                        for (int c = 0; c < 8; c++) {
-                            float2 bf = *reinterpret_cast<const float2*>(bl + ch0 + 16 * hh + 2 * c);
-                            float2 bg = *reinterpret_cast<const float2*>(bl + 64 + ch0 + 16 * hh + 2 * c);
-                            float2 fa = add2(make_float2(__uint_as_float(f[2 * c]), __uint_as_float(f[2 * c + 1])), bf);
-                            float2 ga = add2(make_float2(__uint_as_float(g[2 * c]), __uint_as_float(g[2 * c + 1])), bg);
-                            float2 tf = make_float2(tanh_approx(fa.x), tanh_approx(fa.y));
-                            float2 tg = make_float2(tanh_approx(ga.x), tanh_approx(ga.y));
-                            float2 z = fma2(tf, tg, tf);
-                            pk[c] = pack_half2(z.x, z.y);
+                            for (int c = 0; c < 4; c++) {
+                                float2 bf = *reinterpret_cast<const float2*>(bl + ch0 + 8 * q + 2 * c);
+                                float2 bg = *reinterpret_cast<const float2*>(bl + 64 + ch0 + 8 * q + 2 * c);
+                                float2 fa = add2(make_float2(__uint_as_float(f[2 * c]), __uint_as_float(f[2 * c + 1])), bf);
+                                float2 ga = add2(make_float2(__uint_as_float(g[2 * c]), __uint_as_float(g[2 * c + 1])), bg);
+                                float2 tf = make_float2(tanh_approx(fa.x), tanh_approx(fa.y));
+                                float2 tg = make_float2(tanh_approx(ga.x), tanh_approx(ga.y));
+                                float2 z = fma2(tf, tg, tf);
+                                pk[c] = pack_half2(z.x, z.y);
+                            }
+                            st_shared_v4(xs + (64 + r) * 16 + (c0 + q) * X_CHUNK, pk[0], pk[1], pk[2], pk[3]);
                         }
-#pragma unroll
-                        for (int c = 0; c < 2; c++)
-                            st_shared_v4(xs + (64 + r) * 16 + (c0 + 2 * hh + c) * X_CHUNK, pk[4 * c], pk[4 * c + 1], pk[4 * c + 2],
-                                         pk[4 * c + 3]);
-                    }
-                    if (i < L - 1) {
-#pragma unroll
-                        for (int c = 0; c < 16; c++) h[c] = add2(h[c], *reinterpret_cast<const float2*>(bl + 128 + ch0 + 2 * c));
                     }
                     tc_fence_before();
                     fence_proxy_async_smem();
@@ -436,10 +451,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 #pragma unroll
                         for (int c = 0; c < 16; c++)
                             h[c] = add2(h[c], make_float2(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1])));
+                        mbar_wait(bar(B_SKD + s), ph);   // the skip GEMM (issued after the residual GEMM) has read z
                         publish(i + 1, j);
                         if (lane == 0) TRACE(8, 10 * (warp & 7) + s, j * L + i);
                     } else {
                         // u = ReLU(sum_i skip_i) -> fp16 tile in the workspace                       (C.1 step 3)
+                        mbar_wait(bar(B_SKD + s), ph);
+                        tc_fence_after();
                         uint8_t* ut = a.u + (((size_t)wl * nb + b) * a.ntiles + j) * U_TILE_BYTES + r * 16;
 #pragma unroll
                         for (int cc = 0; cc < 2; cc++) {
