@@ -150,6 +150,13 @@ extern "C" gwi_status gwi_load_model(const char* path, gwi_precision prec, int d
             return st;
         }
     }
+    if (prec == GWI_FP16 && gwi_tiny_supported(m->arch)) {
+        st = gwi_tiny_pack(m);
+        if (st != GWI_OK) {
+            gwi_free_model(m);
+            return st;
+        }
+    }
     *out = m;
     return GWI_OK;
 }
@@ -158,6 +165,7 @@ extern "C" void gwi_free_model(gwi_model* m)
 {
     if (!m) return;
     gwi_tc_free(m);
+    gwi_tiny_free(m);
     if (m->d_blob) cudaFree(m->d_blob);
     if (m->d_off) cudaFree(m->d_off);
     delete m;

@@ -53,6 +53,8 @@ struct GwiDevModel {
 
 // Packed fp16 weights of the tcgen05 kernel (gwi_tc.cu); null when the architecture is not covered.
 struct GwiTcPack;
+// Packed fragments of the fused narrow-architecture stream kernel (gwi_tiny.cu); null when not covered / not FP16.
+struct GwiTinyPack;
 
 struct gwi_model {
     GwiArch arch;
@@ -63,6 +65,7 @@ struct gwi_model {
     float* d_blob = nullptr;
     GwiOffsets* d_off = nullptr; // copy of `off` in device memory
     GwiTcPack* tc = nullptr;
+    GwiTinyPack* tiny = nullptr;
 };
 
 // ---- generic CUDA-core path (gwi_generic.cu) ---------------------------------------------------------------
@@ -91,3 +94,11 @@ void gwi_tc_free(gwi_model* m);
 size_t gwi_tc_workspace_bytes(const gwi_model* m, int64_t B, int32_t T);
 gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, int32_t T, float* d_prob, void* d_ws,
                         size_t ws_bytes, cudaStream_t st);
+
+// ---- fused narrow-architecture stream kernel (gwi_tiny.cu) ----------------------------------------------------
+bool gwi_tiny_supported(const GwiArch& a);
+gwi_status gwi_tiny_pack(gwi_model* m);
+void gwi_tiny_free(gwi_model* m);
+int gwi_tiny_halo(const gwi_model* m);
+gwi_status gwi_tiny_stream(const gwi_model* m, const __half* d_x, int64_t ldx, int n, int64_t t0, const __half* xh_cur,
+                           __half* xh_next, float* d_prob, float* d_skip, int64_t lds, cudaStream_t st);

@@ -49,6 +49,11 @@ struct gwi_stream {
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr};
     int stage = 0;
     int64_t launches = 0;
+    // fused narrow-architecture kernel (FP16 mode, gwi_tiny.cu): carries only the last `halo` input samples
+    bool tiny = false;
+    int halo = 0;
+    __half* d_xh[2] = {nullptr, nullptr};   // [2 detectors][halo], ping-pong
+    int xh_cur = 0;
 };
 
 namespace {
@@ -63,9 +68,20 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
     for (int m = 0; m < s->M; m++) {
         const gwi_model* gm = s->models[m];
         float* skip0 = s->d_skip[m] + s->maxlag;
-        gwi_status rc = gwi_generic_stream_branches(gm, x, s->half_in, s->xcap, n, s->d_hA, s->d_hB, s->sub, skip0, s->lds,
-                                                    s->d_hist[s->hist_cur][m], s->d_hist[s->hist_cur ^ 1][m], 0, s->nb, st);
-        if (rc != GWI_OK) return rc;
+        gwi_status rc;
+        if (s->tiny) {
+            // fused kernel: zero lag only -> probabilities straight out of the kernel; with slides -> skip sums, the
+            // per-lag heads follow below
+            __half* xh_next = (m == 0) ? s->d_xh[s->xh_cur ^ 1] : nullptr;
+            rc = gwi_tiny_stream(gm, (const __half*)x, s->xcap, n, s->t_done, s->d_xh[s->xh_cur], xh_next,
+                                 nslides == 1 ? s->d_prob + (size_t)m * s->sub : nullptr, skip0, s->lds, st);
+            if (rc != GWI_OK) return rc;
+            if (nslides == 1) continue;
+        } else {
+            rc = gwi_generic_stream_branches(gm, x, s->half_in, s->xcap, n, s->d_hA, s->d_hB, s->sub, skip0, s->lds,
+                                             s->d_hist[s->hist_cur][m], s->d_hist[s->hist_cur ^ 1][m], 0, s->nb, st);
+            if (rc != GWI_OK) return rc;
+        }
         for (int k = 0; k < nslides; k++) {
             rc = gwi_generic_stream_head(gm, skip0, s->lds, s->lags[k], n, s->d_prob + ((size_t)k * s->M + m) * s->sub, st);
             if (rc != GWI_OK) return rc;
@@ -81,6 +97,7 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
         }
     }
     s->hist_cur ^= 1;
+    s->xh_cur ^= 1;
     for (int k = 0; k < nslides; k++) {
         const float* ptrs[GWI_MAX_MODELS];
         for (int m = 0; m < s->M; m++) ptrs[m] = s->d_prob + ((size_t)k * s->M + m) * s->sub;
@@ -175,6 +192,9 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     }
     s->N_total = n_total, s->min_len = min_len, s->theta = threshold, s->cap = capacity, s->d_pbar = d_pbar;
     s->R = m0->arch.R, s->S = m0->arch.S, s->nb = m0->arch.n_branch, s->Rf = m0->arch.receptive_field();
+    s->tiny = true;
+    for (int i = 0; i < n_models; i++) s->tiny = s->tiny && models[i]->tiny != nullptr;
+    s->halo = s->tiny ? gwi_tiny_halo(m0) : 0;
     s->xcap = std::max<int64_t>(std::min(max_chunk, n_total), std::min<int64_t>(n_total, s->maxlag + s->Rf - 1));
     // sub-chunk: bounds the activation workspace (2R floats per branch-sample) to ~2 GiB
     int64_t per = (int64_t)s->nb * 2 * s->R * 4;
@@ -218,6 +238,11 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     if ((e = cudaMalloc(&s->d_trig, (size_t)capacity * sizeof(gwi_trigger))) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_count, 4)) != cudaSuccess) return fail(e);
     if ((e = cudaMemset(s->d_count, 0, 4)) != cudaSuccess) return fail(e);
+    if (s->tiny)
+        for (int b = 0; b < 2; b++) {
+            if ((e = cudaMalloc(&s->d_xh[b], (size_t)2 * s->halo * 2)) != cudaSuccess) return fail(e);
+            if ((e = cudaMemset(s->d_xh[b], 0, (size_t)2 * s->halo * 2)) != cudaSuccess) return fail(e);
+        }
     if ((e = cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) return fail(e);
     for (int b = 0; b < 2; b++) {
         if ((e = cudaEventCreateWithFlags(&s->ev_copied[b], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
@@ -235,6 +260,7 @@ extern "C" void gwi_stream_destroy(gwi_stream* s)
     cudaDeviceSynchronize();
     for (int b = 0; b < 2; b++) {
         if (s->d_x[b]) cudaFree(s->d_x[b]);
+        if (s->d_xh[b]) cudaFree(s->d_xh[b]);
         for (float* p : s->d_hist[b])
             if (p) cudaFree(p);
         if (s->ev_copied[b]) cudaEventDestroy(s->ev_copied[b]);
@@ -276,9 +302,22 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
     // or it starts R_f - 1 samples before them
     for (int m = 0; m < s->M; m++) {
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
+        if (s->tiny) {
+            GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * s->halo * 2, st));
+            GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * s->halo * 2, st));
+        }
+        int xc = 0;
         for (int64_t o = 0; o < n_tail; o += s->sub) {
             int nn = (int)std::min<int64_t>(s->sub, n_tail - o);
-            gwi_status rc = gwi_generic_stream_branches(s->models[m], (const char*)s->d_x[0] + (size_t)o * elt(s), s->half_in,
+            gwi_status rc;
+            if (s->tiny) {
+                // both branches are evaluated; the H1 rows of the staging buffer hold nothing meaningful here and the
+                // H1 skip rows they produce are overwritten by the first real chunk
+                rc = gwi_tiny_stream(s->models[m], (const __half*)s->d_x[0] + o, s->xcap, nn, s->N_total - n_tail + o,
+                                     s->d_xh[xc], s->d_xh[xc ^ 1], nullptr, s->d_skip[m] + s->maxlag, s->lds, st);
+                xc ^= 1;
+            } else
+            rc = gwi_generic_stream_branches(s->models[m], (const char*)s->d_x[0] + (size_t)o * elt(s), s->half_in,
                                                         s->xcap, nn, s->d_hA, s->d_hB, s->sub, s->d_skip[m] + s->maxlag,
                                                         s->lds, s->d_hist[0][m], s->d_hist[1][m], 1, s->nb - 1, st);
             if (rc != GWI_OK) return rc;
@@ -295,6 +334,11 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
         // the real pass starts from zero history again
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[1][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
+    }
+    if (s->tiny) {
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * s->halo * 2, st));
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * s->halo * 2, st));
+        s->xh_cur = 0;
     }
     s->hist_cur = 0;
     s->primed = true;

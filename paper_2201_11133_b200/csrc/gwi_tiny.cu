@@ -1,0 +1,344 @@
+// gwi_tiny.cu -- fused FP16-mode stream kernel for the narrow ("config-1") architecture: n_branch = 2, c_in = 1,
+// R = 16, S = Hh = 32, k = 2, any dilation list whose receptive field fits the halo (sum d_i <= 64).
+//
+// The ensembles of BASELINE.json configs 3-5 are built from this architecture.  Its contractions are tiny (K = 32 and
+// K = 16 per block), so the path is bound by MUFU (256 tanh per output sample) and plain ALU work, not by the tensor
+// pipe.  One kernel evaluates lift -> L gated residual blocks -> skip sum -> ReLU ->
+// head -> sigmoid (DESIGN.md C.1 steps 1-5) for a tile of 128 - 16*HT consecutive stream samples per
+// CTA without writing any activation to global memory:
+//
+//   * time runs along the MMA M dimension, 16 rows per warp, 8 warps per CTA; the small channel contractions are
+//     warp-level m16n8k16 MMAs (fp16 operands, fp32 accumulate, reading A14) whose accumulator fragments are gated
+//     in registers and re-used directly as the A fragments of the next MMA (no shuffle, no shared-memory round trip);
+//   * the past tap h(t - d) of a dilated conv is the only cross-row access: every layer's fp16 operand tile is
+//     parked in shared memory (row stride 48 B: conflict-free fragment loads) and read back d rows earlier;
+//   * overlap reuse (row a-2): the first 16*HT rows of a tile are a halo that is recomputed from the carried last
+//     16*HT input samples of the previous chunk, so nothing but those samples is carried across chunks; rows at global
+//     time t < 0 are forced to zero at every layer input, which is exactly the causal padding of reading A4.
+//     Every output sample is an independent fixed-order computation, so chunked == unchunked bit for bit (reading A17).
+//
+// Output: either the per-sample probability (fused head, zero lag) or the per-branch skip sums for the time-slide
+// heads (reading A24), in the layout of the generic stream path.
+#include <cstring>
+#include <vector>
+
+#include "gwi_internal.h"
+
+namespace {
+
+constexpr int TW = 8;             // warps per CTA
+constexpr int ROWS = TW * 16;     // rows (time steps) per CTA tile, halo included
+constexpr int RS = 24;            // shared-memory row stride in halves (16 channels + 8 pad = 48 bytes)
+constexpr int PADROWS = 64;       // zero rows in front of the tile (reads at row - d of the first rows)
+constexpr int TINY_MAX_L = 8;
+
+struct TinyArgs {
+    const uint2* wfg;     // [nb][L][ks 2][nt 4][32]   B fragments of [past | current] x [f | g/2]
+    const uint2* wrs;     // [nb][L][nt 6][32]         B fragments of z' x [res | skip], both halved
+    const uint2* w1;      // [ks 4][nt 4][32]          B fragments of [u_H | u_L] x W1^T
+    const float* bias;    // [nb][L][80]: bf[16], bg/2[16], br[16], bs[32]
+    const float* cst;     // [nb][32]: W_in[16], b_in[16];  then head: b1[32], W2[32], b2
+    const __half* x;      // planar strain chunk: channel c at x + c * ldx, n samples
+    const __half* xh;     // [2][HALO] last HALO samples of the previous chunk (zeros at the stream start)
+    int64_t ldx;
+    int64_t t0;           // global index of sample 0 of this chunk
+    int n, L, halo;       // halo = 16 * HT rows
+    int dil[TINY_MAX_L];
+    float* prob;          // fused head: [n] probabilities (null in skip mode)
+    float* skip;          // skip mode: [nb][32][lds] skip sums incl. bias, pre-ReLU (null in fused mode)
+    int64_t lds;
+};
+
+__device__ __forceinline__ void mma16816(float (&c)[4], const uint32_t (&a)[4], uint2 b)
+{
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b.x), "r"(b.y));
+}
+__device__ __forceinline__ uint32_t pack2(float lo, float hi)
+{
+    __half2 h = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&h);
+}
+__device__ __forceinline__ float tanh_fast(float x)
+{
+    float y;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
+{
+    // two operand buffers (layer parity), each PADROWS zero rows + ROWS rows of 16 halves (+ pad)
+    __shared__ __align__(16) __half sm[2][(PADROWS + ROWS) * RS];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const int valid = ROWS - a.halo;                                    // output rows per CTA
+    const int64_t tile0 = (int64_t)blockIdx.x * valid - a.halo;          // chunk-local time of row 0
+    const int r0 = warp * 16 + g, r1 = r0 + 8;                           // this thread's two rows
+    const int64_t tl0 = tile0 + r0, tl1 = tile0 + r1;                    // chunk-local times
+    // rows before the stream start are zero at every layer input (reading A4)
+    const bool live0 = a.t0 + tl0 >= 0, live1 = a.t0 + tl1 >= 0;
+    for (int i = threadIdx.x; i < 2 * PADROWS * RS / 2; i += TW * 32) {
+        int buf = i / (PADROWS * RS / 2), k = i % (PADROWS * RS / 2);
+        reinterpret_cast<uint32_t*>(sm[buf])[k] = 0u;
+    }
+    const float* hcst = a.cst + 2 * 32;
+    uint32_t ua[2][2][4];                                                // head A fragments: [branch][k-step][4]
+
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+        // ---- lift (C.1 step 1): h0[r] = W_in[r] x + b_in[r]; fp32 master in accumulator-fragment layout
+        float x0 = 0.f, x1 = 0.f;
+        {
+            const __half* xc = a.x + (int64_t)b * a.ldx;
+            const __half* xp = a.xh + b * a.halo;
+            if (tl0 >= 0) { if (tl0 < a.n) x0 = __half2float(xc[tl0]); } else x0 = __half2float(xp[a.halo + tl0]);
+            if (tl1 >= 0) { if (tl1 < a.n) x1 = __half2float(xc[tl1]); } else x1 = __half2float(xp[a.halo + tl1]);
+        }
+        const float* cb = a.cst + b * 32;
+        float h[2][4];                                                   // [n-tile (8 channels)][c0..c3]
+#pragma unroll
+        for (int nt = 0; nt < 2; nt++) {
+            float2 w = __ldg(reinterpret_cast<const float2*>(cb + 8 * nt + 2 * t));
+            float2 bi = __ldg(reinterpret_cast<const float2*>(cb + 16 + 8 * nt + 2 * t));
+            h[nt][0] = live0 ? fmaf(w.x, x0, bi.x) : 0.f, h[nt][1] = live0 ? fmaf(w.y, x0, bi.y) : 0.f;
+            h[nt][2] = live1 ? fmaf(w.x, x1, bi.x) : 0.f, h[nt][3] = live1 ? fmaf(w.y, x1, bi.y) : 0.f;
+        }
+        float sk[4][4];                                                  // skip sum, 4 n-tiles of 8 channels
+#pragma unroll
+        for (int nt = 0; nt < 4; nt++) sk[nt][0] = sk[nt][1] = sk[nt][2] = sk[nt][3] = 0.f;
+
+        for (int i = 0; i < a.L; i++) {
+            const int d = a.dil[i];
+            __half* buf = sm[i & 1] + PADROWS * RS;
+            // ---- current-tap A fragment = this thread's own h values; parked in shared memory for the rows d later
+            uint32_t ac[4] = {pack2(h[0][0], h[0][1]), pack2(h[0][2], h[0][3]), pack2(h[1][0], h[1][1]), pack2(h[1][2], h[1][3])};
+            *reinterpret_cast<uint32_t*>(buf + r0 * RS + 2 * t) = ac[0];
+            *reinterpret_cast<uint32_t*>(buf + r1 * RS + 2 * t) = ac[1];
+            *reinterpret_cast<uint32_t*>(buf + r0 * RS + 8 + 2 * t) = ac[2];
+            *reinterpret_cast<uint32_t*>(buf + r1 * RS + 8 + 2 * t) = ac[3];
+            __syncthreads();   // one barrier per layer: the buffers alternate, so layer i+2 cannot overtake layer i readers
+            uint32_t ap[4];
+            ap[0] = *reinterpret_cast<const uint32_t*>(buf + (r0 - d) * RS + 2 * t);
+            ap[1] = *reinterpret_cast<const uint32_t*>(buf + (r1 - d) * RS + 2 * t);
+            ap[2] = *reinterpret_cast<const uint32_t*>(buf + (r0 - d) * RS + 8 + 2 * t);
+            ap[3] = *reinterpret_cast<const uint32_t*>(buf + (r1 - d) * RS + 8 + 2 * t);
+            // ---- f | g/2 = [h(t-d) | h(t)] . W^T + bias                                      (C.1 step 2)
+            const float* bl = a.bias + ((size_t)b * a.L + i) * 80;
+            const uint2* wf = a.wfg + ((size_t)b * a.L + i) * (2 * 4 * 32) + lane;
+            float fg[4][4];
+#pragma unroll
+            for (int nt = 0; nt < 4; nt++) {
+                float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 8 * nt + 2 * t));
+                fg[nt][0] = bb.x, fg[nt][1] = bb.y, fg[nt][2] = bb.x, fg[nt][3] = bb.y;
+                mma16816(fg[nt], ap, __ldg(wf + (0 * 4 + nt) * 32));
+                mma16816(fg[nt], ac, __ldg(wf + (1 * 4 + nt) * 32));
+            }
+            // ---- z' = tanh(f) (1 + tanh(g/2)) = 2 tanh(f) sigmoid(g); the 2 is folded into Wr/2, Ws/2
+            uint32_t az[4];
+            {
+                float z[2][4];
+#pragma unroll
+                for (int nt = 0; nt < 2; nt++)
+#pragma unroll
+                    for (int c = 0; c < 4; c++) {
+                        float tf = tanh_fast(fg[nt][c]), tg = tanh_fast(fg[nt + 2][c]);
+                        z[nt][c] = fmaf(tf, tg, tf);
+                    }
+                az[0] = pack2(z[0][0], z[0][1]), az[1] = pack2(z[0][2], z[0][3]);
+                az[2] = pack2(z[1][0], z[1][1]), az[3] = pack2(z[1][2], z[1][3]);
+            }
+            // ---- res | skip = z' . [Wr/2 | Ws/2]^T
+            const uint2* wr = a.wrs + ((size_t)b * a.L + i) * (6 * 32) + lane;
+            if (i < a.L - 1) {                                           // reading A8: the last residual conv is dead
+#pragma unroll
+                for (int nt = 0; nt < 2; nt++) {
+                    float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 32 + 8 * nt + 2 * t));
+                    float rr[4] = {bb.x, bb.y, bb.x, bb.y};
+                    mma16816(rr, az, __ldg(wr + nt * 32));
+                    h[nt][0] = live0 ? h[nt][0] + rr[0] : 0.f, h[nt][1] = live0 ? h[nt][1] + rr[1] : 0.f;
+                    h[nt][2] = live1 ? h[nt][2] + rr[2] : 0.f, h[nt][3] = live1 ? h[nt][3] + rr[3] : 0.f;
+                }
+            }
+#pragma unroll
+            for (int nt = 0; nt < 4; nt++) {
+                float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 48 + 8 * nt + 2 * t));
+                sk[nt][0] += bb.x, sk[nt][1] += bb.y, sk[nt][2] += bb.x, sk[nt][3] += bb.y;
+                mma16816(sk[nt], az, __ldg(wr + (2 + nt) * 32));
+            }
+        }
+        if (a.skip) {
+            // ---- time-slide mode: skip sums (pre-ReLU, fp32) for the per-lag heads, [branch][channel][time]
+            float* sp = a.skip + (size_t)b * 32 * a.lds;
+#pragma unroll
+            for (int nt = 0; nt < 4; nt++) {
+                const int q = 8 * nt + 2 * t;
+                if (r0 >= a.halo && tl0 < a.n) sp[(size_t)q * a.lds + tl0] = sk[nt][0], sp[(size_t)(q + 1) * a.lds + tl0] = sk[nt][1];
+                if (r1 >= a.halo && tl1 < a.n) sp[(size_t)q * a.lds + tl1] = sk[nt][2], sp[(size_t)(q + 1) * a.lds + tl1] = sk[nt][3];
+            }
+        } else {
+            // ---- u_b = ReLU(skip sum) as the A fragments of the head                        (C.1 steps 3, 4)
+#pragma unroll
+            for (int ks = 0; ks < 2; ks++) {
+                ua[b][ks][0] = pack2(fmaxf(sk[2 * ks][0], 0.f), fmaxf(sk[2 * ks][1], 0.f));
+                ua[b][ks][1] = pack2(fmaxf(sk[2 * ks][2], 0.f), fmaxf(sk[2 * ks][3], 0.f));
+                ua[b][ks][2] = pack2(fmaxf(sk[2 * ks + 1][0], 0.f), fmaxf(sk[2 * ks + 1][1], 0.f));
+                ua[b][ks][3] = pack2(fmaxf(sk[2 * ks + 1][2], 0.f), fmaxf(sk[2 * ks + 1][3], 0.f));
+            }
+        }
+        __syncthreads();   // the next branch starts again with buffer 0
+    }
+    if (a.skip) return;
+    // ---- head: v = ReLU(W1 [u_H; u_L] + b1), y = W2 . v + b2, p = sigmoid(y)                   (C.1 step 5)
+    float y0 = 0.f, y1 = 0.f;
+#pragma unroll
+    for (int nt = 0; nt < 4; nt++) {
+        float2 bb = __ldg(reinterpret_cast<const float2*>(hcst + 8 * nt + 2 * t));
+        float v[4] = {bb.x, bb.y, bb.x, bb.y};
+#pragma unroll
+        for (int ks = 0; ks < 4; ks++) mma16816(v, ua[ks >> 1][ks & 1], __ldg(a.w1 + (ks * 4 + nt) * 32 + lane));
+        float2 w2 = __ldg(reinterpret_cast<const float2*>(hcst + 32 + 8 * nt + 2 * t));
+        y0 = fmaf(w2.x, fmaxf(v[0], 0.f), y0), y0 = fmaf(w2.y, fmaxf(v[1], 0.f), y0);
+        y1 = fmaf(w2.x, fmaxf(v[2], 0.f), y1), y1 = fmaf(w2.y, fmaxf(v[3], 0.f), y1);
+    }
+    y0 += __shfl_xor_sync(0xffffffffu, y0, 1), y1 += __shfl_xor_sync(0xffffffffu, y1, 1);
+    y0 += __shfl_xor_sync(0xffffffffu, y0, 2), y1 += __shfl_xor_sync(0xffffffffu, y1, 2);
+    if (t == 0) {
+        const float b2 = __ldg(hcst + 64);
+        if (r0 >= a.halo && tl0 < a.n) a.prob[tl0] = 1.0f / (1.0f + __expf(-(y0 + b2)));
+        if (r1 >= a.halo && tl1 < a.n) a.prob[tl1] = 1.0f / (1.0f + __expf(-(y1 + b2)));
+    }
+}
+
+// keeps the last `halo` samples of each detector for the next chunk (older history shifts when n < halo)
+__global__ void k_tiny_xhist(const __half* x, int64_t ldx, int n, int halo, const __half* xh_old, __half* xh_new)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2 * halo) return;
+    int c = i / halo, k = i % halo;
+    int64_t p = (int64_t)n - halo + k;
+    xh_new[i] = p >= 0 ? x[c * ldx + p] : xh_old[c * halo + (halo + p)];
+}
+
+inline uint16_t h16(float v)
+{
+    __half h = __float2half_rn(v);
+    uint16_t u;
+    memcpy(&u, &h, 2);
+    return u;
+}
+
+} // namespace
+
+struct GwiTinyPack {
+    uint2 *d_wfg = nullptr, *d_wrs = nullptr, *d_w1 = nullptr;
+    float *d_bias = nullptr, *d_cst = nullptr;
+    int halo = 16;
+};
+
+bool gwi_tiny_supported(const GwiArch& a)
+{
+    if (a.n_branch != 2 || a.c_in != 1 || a.R != 16 || a.S != 32 || a.Hh != 32 || a.k != 2 || a.L > TINY_MAX_L) return false;
+    int s = 0;
+    for (int i = 0; i < a.L; i++) {
+        if (a.dil[i] > PADROWS) return false;
+        s += a.dil[i];
+    }
+    return s <= 64;
+}
+
+int gwi_tiny_halo(const gwi_model* m) { return m->tiny ? m->tiny->halo : 0; }
+
+gwi_status gwi_tiny_pack(gwi_model* m)
+{
+    const GwiArch& a = m->arch;
+    const int L = a.L, nb = 2;
+    GwiTinyPack* p = new GwiTinyPack();
+    m->tiny = p;
+    int sum = 0;
+    for (int i = 0; i < L; i++) sum += a.dil[i];
+    p->halo = ((sum + 15) / 16) * 16;
+    if (p->halo < 16) p->halo = 16;
+    const float* W = m->host_blob.data();
+    // B fragment of mma.m16n8k16 (col-major 16 x 8): lane (g = lane / 4, t = lane % 4) holds
+    //   b0 = {B[k = 2t][n = g], B[2t + 1][g]},  b1 = {B[2t + 8][g], B[2t + 9][g]}
+    auto frag = [&](auto&& B, int k0, int n0, int lane) {
+        int g = lane >> 2, t = lane & 3;
+        uint2 r;
+        r.x = (uint32_t)h16(B(k0 + 2 * t, n0 + g)) | ((uint32_t)h16(B(k0 + 2 * t + 1, n0 + g)) << 16);
+        r.y = (uint32_t)h16(B(k0 + 2 * t + 8, n0 + g)) | ((uint32_t)h16(B(k0 + 2 * t + 9, n0 + g)) << 16);
+        return r;
+    };
+    std::vector<uint2> wfg((size_t)nb * L * 8 * 32), wrs((size_t)nb * L * 6 * 32), w1(16 * 32);
+    std::vector<float> bias((size_t)nb * L * 80), cst(2 * 32 + 65);
+    for (int b = 0; b < nb; b++) {
+        for (int c = 0; c < 16; c++) cst[b * 32 + c] = W[m->off.W_in[b] + c], cst[b * 32 + 16 + c] = W[m->off.b_in[b] + c];
+        for (int i = 0; i < L; i++) {
+            const GwiLayerOff& lo = m->off.layer[b][i];
+            // B[k][n]: k < 16 past tap (tap 0) of channel k, k >= 16 current tap (tap 1); n < 16: f, n >= 16: g / 2
+            auto Bfg = [&](int k, int n) {
+                int tap = k < 16 ? 0 : 1, kin = k & 15;
+                return n < 16 ? W[lo.Wf + ((int64_t)n * 16 + kin) * 2 + tap] : 0.5f * W[lo.Wg + ((int64_t)(n - 16) * 16 + kin) * 2 + tap];
+            };
+            for (int ks = 0; ks < 2; ks++)
+                for (int nt = 0; nt < 4; nt++)
+                    for (int l = 0; l < 32; l++) wfg[(((size_t)b * L + i) * 8 + ks * 4 + nt) * 32 + l] = frag(Bfg, 16 * ks, 8 * nt, l);
+            // B[k][n]: n < 16: Wr[n][k] / 2, n >= 16: Ws[n - 16][k] / 2
+            auto Brs = [&](int k, int n) { return n < 16 ? 0.5f * W[lo.Wr + (int64_t)n * 16 + k] : 0.5f * W[lo.Ws + (int64_t)(n - 16) * 16 + k]; };
+            for (int nt = 0; nt < 6; nt++)
+                for (int l = 0; l < 32; l++) wrs[(((size_t)b * L + i) * 6 + nt) * 32 + l] = frag(Brs, 0, 8 * nt, l);
+            float* bl = bias.data() + ((size_t)b * L + i) * 80;
+            for (int c = 0; c < 16; c++) bl[c] = W[lo.bf + c], bl[16 + c] = 0.5f * W[lo.bg + c], bl[32 + c] = W[lo.br + c];
+            for (int q = 0; q < 32; q++) bl[48 + q] = W[lo.bs + q];
+        }
+    }
+    auto B1 = [&](int k, int n) { return W[m->off.W1 + (int64_t)n * 64 + k]; };   // k over [u_H(32) | u_L(32)]
+    for (int ks = 0; ks < 4; ks++)
+        for (int nt = 0; nt < 4; nt++)
+            for (int l = 0; l < 32; l++) w1[(ks * 4 + nt) * 32 + l] = frag(B1, 16 * ks, 8 * nt, l);
+    for (int c = 0; c < 32; c++) cst[64 + c] = W[m->off.b1 + c], cst[96 + c] = W[m->off.W2 + c];
+    cst[128] = W[m->off.b2];
+    auto up = [&](void** dst, const void* src, size_t bytes) -> cudaError_t {
+        cudaError_t e = cudaMalloc(dst, bytes);
+        if (e != cudaSuccess) return e;
+        return cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice);
+    };
+    GWI_CUDA_CHECK(up((void**)&p->d_wfg, wfg.data(), wfg.size() * 8));
+    GWI_CUDA_CHECK(up((void**)&p->d_wrs, wrs.data(), wrs.size() * 8));
+    GWI_CUDA_CHECK(up((void**)&p->d_w1, w1.data(), w1.size() * 8));
+    GWI_CUDA_CHECK(up((void**)&p->d_bias, bias.data(), bias.size() * 4));
+    GWI_CUDA_CHECK(up((void**)&p->d_cst, cst.data(), cst.size() * 4));
+    return GWI_OK;
+}
+
+void gwi_tiny_free(gwi_model* m)
+{
+    GwiTinyPack* p = m->tiny;
+    if (!p) return;
+    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_bias), cudaFree(p->d_cst);
+    delete p;
+    m->tiny = nullptr;
+}
+
+// One chunk of n samples of a planar fp16 stream through one model.  xh_cur / xh_next: [2][halo] carried input samples
+// (xh_next may be null: no update).  prob: fused-head output [n], or null with skip != null (time-slide mode).
+gwi_status gwi_tiny_stream(const gwi_model* m, const __half* d_x, int64_t ldx, int n, int64_t t0, const __half* xh_cur,
+                           __half* xh_next, float* d_prob, float* d_skip, int64_t lds, cudaStream_t st)
+{
+    const GwiTinyPack* p = m->tiny;
+    TinyArgs a;
+    a.wfg = p->d_wfg, a.wrs = p->d_wrs, a.w1 = p->d_w1, a.bias = p->d_bias, a.cst = p->d_cst;
+    a.x = d_x, a.xh = xh_cur, a.ldx = ldx, a.t0 = t0, a.n = n, a.L = m->arch.L, a.halo = p->halo;
+    for (int i = 0; i < m->arch.L; i++) a.dil[i] = m->arch.dil[i];
+    a.prob = d_prob, a.skip = d_prob ? nullptr : d_skip, a.lds = lds;
+    const int valid = ROWS - p->halo;
+    const int grid = (n + valid - 1) / valid;
+    k_tiny<<<grid, TW * 32, 0, st>>>(a);
+    gwi_count_launch(1);
+    if (xh_next) {
+        k_tiny_xhist<<<(2 * p->halo + 127) / 128, 128, 0, st>>>(d_x, ldx, n, p->halo, xh_cur, xh_next);
+        gwi_count_launch(1);
+    }
+    GWI_CUDA_CHECK(cudaGetLastError());
+    return GWI_OK;
+}
