@@ -101,4 +101,6 @@ gwi_status gwi_tiny_pack(gwi_model* m);
 void gwi_tiny_free(gwi_model* m);
 int gwi_tiny_halo(const gwi_model* m);
 gwi_status gwi_tiny_stream(const gwi_model* m, const __half* d_x, int64_t ldx, int n, int64_t t0, const __half* xh_cur,
-                           __half* xh_next, float* d_prob, float* d_skip, int64_t lds, cudaStream_t st);
+                           __half* xh_next, float* d_prob, __half* d_u16, int64_t lds, cudaStream_t st);
+gwi_status gwi_tiny_heads(const gwi_model* m, const __half* d_u16, int64_t lds, int n, const int64_t* d_lags, int n_lags,
+                          float* d_prob, int64_t stride_k, cudaStream_t st);

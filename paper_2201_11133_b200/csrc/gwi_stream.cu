@@ -54,6 +54,8 @@ struct gwi_stream {
     int halo = 0;
     __half* d_xh[2] = {nullptr, nullptr};   // [2 detectors][halo], ping-pong
     int xh_cur = 0;
+    std::vector<__half*> d_u16;             // time slides: per model [2][lds][32] fp16 branch features, time-major
+    int64_t* d_lags = nullptr;              // device copy of the lag list
 };
 
 namespace {
@@ -67,16 +69,24 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
     const char* x = (const char*)s->d_x[xb] + (size_t)x0 * elt(s);
     for (int m = 0; m < s->M; m++) {
         const gwi_model* gm = s->models[m];
-        float* skip0 = s->d_skip[m] + s->maxlag;
+        float* skip0 = s->tiny ? nullptr : s->d_skip[m] + s->maxlag;
         gwi_status rc;
         if (s->tiny) {
             // fused kernel: zero lag only -> probabilities straight out of the kernel; with slides -> skip sums, the
             // per-lag heads follow below
             __half* xh_next = (m == 0) ? s->d_xh[s->xh_cur ^ 1] : nullptr;
+            __half* u0 = nslides > 1 ? s->d_u16[m] + (size_t)s->maxlag * 32 : nullptr;
             rc = gwi_tiny_stream(gm, (const __half*)x, s->xcap, n, s->t_done, s->d_xh[s->xh_cur], xh_next,
-                                 nslides == 1 ? s->d_prob + (size_t)m * s->sub : nullptr, skip0, s->lds, st);
+                                 nslides == 1 ? s->d_prob + (size_t)m * s->sub : nullptr, u0, s->lds, st);
             if (rc != GWI_OK) return rc;
             if (nslides == 1) continue;
+            rc = gwi_tiny_heads(gm, u0, s->lds, n, s->d_lags, nslides, s->d_prob + (size_t)m * s->sub, (int64_t)s->M * s->sub, st);
+            if (rc != GWI_OK) return rc;
+            // ring shift: the last maxlag rows of the L1 features move to the front
+            __half* base = s->d_u16[m] + (size_t)s->lds * 32;
+            GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_tmp, base + (size_t)n * 32, (size_t)s->maxlag * 64, cudaMemcpyDeviceToDevice, st));
+            GWI_CUDA_CHECK(cudaMemcpyAsync(base, s->d_tmp, (size_t)s->maxlag * 64, cudaMemcpyDeviceToDevice, st));
+            continue;
         } else {
             rc = gwi_generic_stream_branches(gm, x, s->half_in, s->xcap, n, s->d_hA, s->d_hB, s->sub, skip0, s->lds,
                                              s->d_hist[s->hist_cur][m], s->d_hist[s->hist_cur ^ 1][m], 0, s->nb, st);
@@ -199,6 +209,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     // sub-chunk: bounds the activation workspace (2R floats per branch-sample) to ~2 GiB
     int64_t per = (int64_t)s->nb * 2 * s->R * 4;
     int64_t sub = std::max<int64_t>(4096, (2LL << 30) / per);
+    if (s->tiny) sub = std::max<int64_t>(4096, (1LL << 30) / ((int64_t)(1 + n_lags) * n_models * 4));   // ~1 GiB of probabilities
     sub = std::min<int64_t>(sub, 1 << 24);
     sub = std::min<int64_t>(sub, s->xcap);
     s->sub = (int)sub;
@@ -215,12 +226,14 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     for (int b = 0; b < 2; b++)
         if ((e = cudaMalloc(&s->d_x[b], (size_t)C * s->xcap * elt(s))) != cudaSuccess) return fail(e);
     size_t hbytes = (size_t)s->nb * s->R * s->sub * 4;
-    if ((e = cudaMalloc(&s->d_hA, hbytes)) != cudaSuccess) return fail(e);
-    if ((e = cudaMalloc(&s->d_hB, hbytes)) != cudaSuccess) return fail(e);
+    if (!s->tiny) {   // activation workspace of the generic per-layer kernels
+        if ((e = cudaMalloc(&s->d_hA, hbytes)) != cudaSuccess) return fail(e);
+        if ((e = cudaMalloc(&s->d_hB, hbytes)) != cudaSuccess) return fail(e);
+    }
     size_t histb = (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(m0)) * 4;
     s->d_skip.assign(s->M, nullptr);
     s->d_hist[0].assign(s->M, nullptr), s->d_hist[1].assign(s->M, nullptr);
-    for (int m = 0; m < s->M; m++) {
+    for (int m = 0; m < s->M && !s->tiny; m++) {
         size_t sb = (size_t)s->nb * s->S * s->lds * 4;
         if ((e = cudaMalloc(&s->d_skip[m], sb)) != cudaSuccess) return fail(e);
         if ((e = cudaMemset(s->d_skip[m], 0, sb)) != cudaSuccess) return fail(e);
@@ -238,11 +251,22 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     if ((e = cudaMalloc(&s->d_trig, (size_t)capacity * sizeof(gwi_trigger))) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_count, 4)) != cudaSuccess) return fail(e);
     if ((e = cudaMemset(s->d_count, 0, 4)) != cudaSuccess) return fail(e);
-    if (s->tiny)
+    if (s->tiny) {
         for (int b = 0; b < 2; b++) {
             if ((e = cudaMalloc(&s->d_xh[b], (size_t)2 * s->halo * 2)) != cudaSuccess) return fail(e);
             if ((e = cudaMemset(s->d_xh[b], 0, (size_t)2 * s->halo * 2)) != cudaSuccess) return fail(e);
         }
+        if (nslides > 1) {
+            s->d_u16.assign(s->M, nullptr);
+            for (int m = 0; m < s->M; m++) {
+                size_t ub = (size_t)2 * s->lds * 32 * 2;
+                if ((e = cudaMalloc(&s->d_u16[m], ub)) != cudaSuccess) return fail(e);
+                if ((e = cudaMemset(s->d_u16[m], 0, ub)) != cudaSuccess) return fail(e);
+            }
+            if ((e = cudaMalloc(&s->d_lags, (size_t)nslides * 8)) != cudaSuccess) return fail(e);
+            if ((e = cudaMemcpy(s->d_lags, s->lags.data(), (size_t)nslides * 8, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+        }
+    }
     if ((e = cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) return fail(e);
     for (int b = 0; b < 2; b++) {
         if ((e = cudaEventCreateWithFlags(&s->ev_copied[b], cudaEventDisableTiming)) != cudaSuccess) return fail(e);
@@ -268,6 +292,9 @@ extern "C" void gwi_stream_destroy(gwi_stream* s)
     }
     for (float* p : s->d_skip)
         if (p) cudaFree(p);
+    for (__half* p : s->d_u16)
+        if (p) cudaFree(p);
+    if (s->d_lags) cudaFree(s->d_lags);
     if (s->d_hA) cudaFree(s->d_hA);
     if (s->d_hB) cudaFree(s->d_hB);
     if (s->d_tmp) cudaFree(s->d_tmp);
@@ -301,7 +328,8 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
     // features of the tail: zero history is exact for the last maxlag samples because either the tail starts at t = 0
     // or it starts R_f - 1 samples before them
     for (int m = 0; m < s->M; m++) {
-        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
+        if (!s->tiny)
+            GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
         if (s->tiny) {
             GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * s->halo * 2, st));
             GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * s->halo * 2, st));
@@ -314,8 +342,13 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
                 // both branches are evaluated; the H1 rows of the staging buffer hold nothing meaningful here and the
                 // H1 skip rows they produce are overwritten by the first real chunk
                 rc = gwi_tiny_stream(s->models[m], (const __half*)s->d_x[0] + o, s->xcap, nn, s->N_total - n_tail + o,
-                                     s->d_xh[xc], s->d_xh[xc ^ 1], nullptr, s->d_skip[m] + s->maxlag, s->lds, st);
+                                     s->d_xh[xc], s->d_xh[xc ^ 1], nullptr, s->d_u16[m] + (size_t)s->maxlag * 32, s->lds, st);
                 xc ^= 1;
+                if (rc != GWI_OK) return rc;
+                __half* base16 = s->d_u16[m] + (size_t)s->lds * 32;
+                GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_tmp, base16 + (size_t)nn * 32, (size_t)s->maxlag * 64, cudaMemcpyDeviceToDevice, st));
+                GWI_CUDA_CHECK(cudaMemcpyAsync(base16, s->d_tmp, (size_t)s->maxlag * 64, cudaMemcpyDeviceToDevice, st));
+                continue;
             } else
             rc = gwi_generic_stream_branches(s->models[m], (const char*)s->d_x[0] + (size_t)o * elt(s), s->half_in,
                                                         s->xcap, nn, s->d_hA, s->d_hB, s->sub, s->d_skip[m] + s->maxlag,
@@ -332,6 +365,7 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
             std::swap(s->d_hist[0][m], s->d_hist[1][m]);
         }
         // the real pass starts from zero history again
+        if (s->tiny) continue;
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[1][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
     }

@@ -45,8 +45,8 @@ struct TinyArgs {
     int n, L, halo;       // halo = 16 * HT rows
     int dil[TINY_MAX_L];
     float* prob;          // fused head: [n] probabilities (null in skip mode)
-    float* skip;          // skip mode: [nb][32][lds] skip sums incl. bias, pre-ReLU (null in fused mode)
-    int64_t lds;
+    __half* u16;          // time-slide mode: [nb][lds][32] branch features u = ReLU(skip sum), fp16, time-major
+    int64_t lds;          //   (null in fused mode); row 0 = sample 0 of this chunk
 };
 
 __device__ __forceinline__ void mma16816(float (&c)[4], const uint32_t (&a)[4], uint2 b)
@@ -167,14 +167,16 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
                 mma16816(sk[nt], az, __ldg(wr + (2 + nt) * 32));
             }
         }
-        if (a.skip) {
-            // ---- time-slide mode: skip sums (pre-ReLU, fp32) for the per-lag heads, [branch][channel][time]
-            float* sp = a.skip + (size_t)b * 32 * a.lds;
+        if (a.u16) {
+            // ---- time-slide mode: u_b = ReLU(skip sum) in fp16, time-major, for the per-lag heads (k_tiny_heads)
+            __half* up = a.u16 + (size_t)b * a.lds * 32;
 #pragma unroll
             for (int nt = 0; nt < 4; nt++) {
                 const int q = 8 * nt + 2 * t;
-                if (r0 >= a.halo && tl0 < a.n) sp[(size_t)q * a.lds + tl0] = sk[nt][0], sp[(size_t)(q + 1) * a.lds + tl0] = sk[nt][1];
-                if (r1 >= a.halo && tl1 < a.n) sp[(size_t)q * a.lds + tl1] = sk[nt][2], sp[(size_t)(q + 1) * a.lds + tl1] = sk[nt][3];
+                if (r0 >= a.halo && tl0 < a.n)
+                    *reinterpret_cast<uint32_t*>(up + tl0 * 32 + q) = pack2(fmaxf(sk[nt][0], 0.f), fmaxf(sk[nt][1], 0.f));
+                if (r1 >= a.halo && tl1 < a.n)
+                    *reinterpret_cast<uint32_t*>(up + tl1 * 32 + q) = pack2(fmaxf(sk[nt][2], 0.f), fmaxf(sk[nt][3], 0.f));
             }
         } else {
             // ---- u_b = ReLU(skip sum) as the A fragments of the head                        (C.1 steps 3, 4)
@@ -188,7 +190,7 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
         }
         __syncthreads();   // the next branch starts again with buffer 0
     }
-    if (a.skip) return;
+    if (a.u16) return;
     // ---- head: v = ReLU(W1 [u_H; u_L] + b1), y = W2 . v + b2, p = sigmoid(y)                   (C.1 step 5)
     float y0 = 0.f, y1 = 0.f;
 #pragma unroll
@@ -207,6 +209,87 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
         const float b2 = __ldg(hcst + 64);
         if (r0 >= a.halo && tl0 < a.n) a.prob[tl0] = 1.0f / (1.0f + __expf(-(y0 + b2)));
         if (r1 >= a.halo && tl1 < a.n) a.prob[tl1] = 1.0f / (1.0f + __expf(-(y1 + b2)));
+    }
+}
+
+// Time-slide heads (reading A24): p_k[t] = head(u_H1[t], u_L1[t - lag_k]) for every lag of the list, from the fp16
+// time-major branch features.  W1 [u_H; u_L] is split by linearity: the H1 half of the contraction is done once per
+// 16-row tile and re-used for every lag, each lag adds its L1 half (same accumulation order as the fused head of
+// k_tiny, so lag 0 reproduces it bit for bit).  u16 row 0 = sample 0 of the chunk; L1 rows at negative indices are the
+// ring of the previous max-lag samples.
+struct HeadsArgs {
+    const uint2* w1;
+    const float* hcst;      // b1[32], W2[32], b2
+    const __half* u16;      // [2][lds][32], pointing at row 0 of this chunk
+    int64_t lds;
+    int n, n_lags;
+    const int64_t* lags;    // device array
+    float* prob;            // [n_lags][stride_k] ; this model's slice starts at prob
+    int64_t stride_k;
+};
+
+__global__ void __launch_bounds__(256) k_tiny_heads(const HeadsArgs a)
+{
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const int64_t row0 = ((int64_t)blockIdx.x * 8 + warp) * 16;
+    if (row0 >= a.n) return;
+    const int64_t ra = row0 + g, rb = ra + 8;
+    const int64_t ca = ra < a.n ? ra : a.n - 1, cb = rb < a.n ? rb : a.n - 1;   // clamp loads of the ragged tail
+    const __half* uH = a.u16;
+    const __half* uL = a.u16 + a.lds * 32;
+    // H1 half: acc = b1 + W1[:, 0:32] u_H
+    float acc[4][4];
+    {
+        uint32_t ah[2][4];
+#pragma unroll
+        for (int ks = 0; ks < 2; ks++) {
+            ah[ks][0] = *reinterpret_cast<const uint32_t*>(uH + ca * 32 + 16 * ks + 2 * t);
+            ah[ks][1] = *reinterpret_cast<const uint32_t*>(uH + cb * 32 + 16 * ks + 2 * t);
+            ah[ks][2] = *reinterpret_cast<const uint32_t*>(uH + ca * 32 + 16 * ks + 8 + 2 * t);
+            ah[ks][3] = *reinterpret_cast<const uint32_t*>(uH + cb * 32 + 16 * ks + 8 + 2 * t);
+        }
+#pragma unroll
+        for (int nt = 0; nt < 4; nt++) {
+            float2 bb = __ldg(reinterpret_cast<const float2*>(a.hcst + 8 * nt + 2 * t));
+            acc[nt][0] = bb.x, acc[nt][1] = bb.y, acc[nt][2] = bb.x, acc[nt][3] = bb.y;
+#pragma unroll
+            for (int ks = 0; ks < 2; ks++) mma16816(acc[nt], ah[ks], __ldg(a.w1 + (ks * 4 + nt) * 32 + lane));
+        }
+    }
+    uint2 wl[2][4];
+    float2 w2[4];
+#pragma unroll
+    for (int nt = 0; nt < 4; nt++) {
+        wl[0][nt] = __ldg(a.w1 + (2 * 4 + nt) * 32 + lane), wl[1][nt] = __ldg(a.w1 + (3 * 4 + nt) * 32 + lane);
+        w2[nt] = __ldg(reinterpret_cast<const float2*>(a.hcst + 32 + 8 * nt + 2 * t));
+    }
+    const float b2 = __ldg(a.hcst + 64);
+    for (int k = 0; k < a.n_lags; k++) {
+        const int64_t lag = a.lags[k];
+        uint32_t al[2][4];
+#pragma unroll
+        for (int ks = 0; ks < 2; ks++) {
+            al[ks][0] = *reinterpret_cast<const uint32_t*>(uL + (ca - lag) * 32 + 16 * ks + 2 * t);
+            al[ks][1] = *reinterpret_cast<const uint32_t*>(uL + (cb - lag) * 32 + 16 * ks + 2 * t);
+            al[ks][2] = *reinterpret_cast<const uint32_t*>(uL + (ca - lag) * 32 + 16 * ks + 8 + 2 * t);
+            al[ks][3] = *reinterpret_cast<const uint32_t*>(uL + (cb - lag) * 32 + 16 * ks + 8 + 2 * t);
+        }
+        float y0 = 0.f, y1 = 0.f;
+#pragma unroll
+        for (int nt = 0; nt < 4; nt++) {
+            float v[4] = {acc[nt][0], acc[nt][1], acc[nt][2], acc[nt][3]};
+            mma16816(v, al[0], wl[0][nt]);
+            mma16816(v, al[1], wl[1][nt]);
+            y0 = fmaf(w2[nt].x, fmaxf(v[0], 0.f), y0), y0 = fmaf(w2[nt].y, fmaxf(v[1], 0.f), y0);
+            y1 = fmaf(w2[nt].x, fmaxf(v[2], 0.f), y1), y1 = fmaf(w2[nt].y, fmaxf(v[3], 0.f), y1);
+        }
+        y0 += __shfl_xor_sync(0xffffffffu, y0, 1), y1 += __shfl_xor_sync(0xffffffffu, y1, 1);
+        y0 += __shfl_xor_sync(0xffffffffu, y0, 2), y1 += __shfl_xor_sync(0xffffffffu, y1, 2);
+        if (t == 0) {
+            float* pk = a.prob + (size_t)k * a.stride_k;
+            if (ra < a.n) pk[ra] = 1.0f / (1.0f + __expf(-(y0 + b2)));
+            if (rb < a.n) pk[rb] = 1.0f / (1.0f + __expf(-(y1 + b2)));
+        }
     }
 }
 
@@ -321,16 +404,17 @@ void gwi_tiny_free(gwi_model* m)
 }
 
 // One chunk of n samples of a planar fp16 stream through one model.  xh_cur / xh_next: [2][halo] carried input samples
-// (xh_next may be null: no update).  prob: fused-head output [n], or null with skip != null (time-slide mode).
+// (xh_next may be null: no update).  prob: fused-head output [n], or null with d_u16 != null (time-slide mode:
+// d_u16 = row of sample 0 inside a [2][lds][32] fp16 buffer).
 gwi_status gwi_tiny_stream(const gwi_model* m, const __half* d_x, int64_t ldx, int n, int64_t t0, const __half* xh_cur,
-                           __half* xh_next, float* d_prob, float* d_skip, int64_t lds, cudaStream_t st)
+                           __half* xh_next, float* d_prob, __half* d_u16, int64_t lds, cudaStream_t st)
 {
     const GwiTinyPack* p = m->tiny;
     TinyArgs a;
     a.wfg = p->d_wfg, a.wrs = p->d_wrs, a.w1 = p->d_w1, a.bias = p->d_bias, a.cst = p->d_cst;
     a.x = d_x, a.xh = xh_cur, a.ldx = ldx, a.t0 = t0, a.n = n, a.L = m->arch.L, a.halo = p->halo;
     for (int i = 0; i < m->arch.L; i++) a.dil[i] = m->arch.dil[i];
-    a.prob = d_prob, a.skip = d_prob ? nullptr : d_skip, a.lds = lds;
+    a.prob = d_prob, a.u16 = d_prob ? nullptr : d_u16, a.lds = lds;
     const int valid = ROWS - p->halo;
     const int grid = (n + valid - 1) / valid;
     k_tiny<<<grid, TW * 32, 0, st>>>(a);
@@ -339,6 +423,20 @@ gwi_status gwi_tiny_stream(const gwi_model* m, const __half* d_x, int64_t ldx, i
         k_tiny_xhist<<<(2 * p->halo + 127) / 128, 128, 0, st>>>(d_x, ldx, n, p->halo, xh_cur, xh_next);
         gwi_count_launch(1);
     }
+    GWI_CUDA_CHECK(cudaGetLastError());
+    return GWI_OK;
+}
+
+// Heads of all lags for one model on one chunk (time-slide mode).  d_u16: row of sample 0; d_lags: device array.
+gwi_status gwi_tiny_heads(const gwi_model* m, const __half* d_u16, int64_t lds, int n, const int64_t* d_lags, int n_lags,
+                          float* d_prob, int64_t stride_k, cudaStream_t st)
+{
+    const GwiTinyPack* p = m->tiny;
+    HeadsArgs a;
+    a.w1 = p->d_w1, a.hcst = p->d_cst + 64, a.u16 = d_u16, a.lds = lds, a.n = n, a.n_lags = n_lags, a.lags = d_lags;
+    a.prob = d_prob, a.stride_k = stride_k;
+    k_tiny_heads<<<(n + 127) / 128, 256, 0, st>>>(a);
+    gwi_count_launch(1);
     GWI_CUDA_CHECK(cudaGetLastError());
     return GWI_OK;
 }
