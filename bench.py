@@ -71,6 +71,59 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(self.rows)}
 
 
+def stream_bench(dev, work, rank, n_chunks=744):
+    """Extra, reported beside the headline: the streaming ensemble path (gwi_stream_*) on the config-1 architecture.
+    hour  = BASELINE.json configs[2]: 4-model ensemble, 1 h two-detector stream resident in HBM, one push + finish.
+    month = configs[4]: 744 one-hour chunks pushed from pinned host buffers (H2D on the side stream inside the timed
+            region), triggers read back at the end.  Two distinct seeded hour chunks rotate as the host source."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    N1 = 3600 * gs.FS
+    models = []
+    for sd in range(4):
+        pth = os.path.join(work, f"bench_cfg1_seed{sd}_r{rank}.gwim")
+        gs.make_model_file(pth, gs.CFG1_ARCH, seed=sd)
+        models.append(gwi.load_model(pth, gwi.FP16, dev.index))
+    host = [torch.from_numpy(gs.stream_noise(1, c * N1, N1)).pin_memory() for c in range(2)]
+    xd = host[0].to(dev)
+    out = {}
+    # ---- hour, device resident
+    times = []
+    for rep in range(5):
+        st = gwi.Stream(models, N1, N1, THETA, LMIN, capacity=4096)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        st.push(xd[0], xd[1])
+        e1.record()
+        n, _ = st.finish()
+        times.append(e0.elapsed_time(e1))
+        st.close()
+    ms = float(np.median(times[2:]))
+    mufu_ops = N1 * 4 * (gs.CFG1_ARCH.tanh_per_timestep() if hasattr(gs.CFG1_ARCH, "tanh_per_timestep") else 256)
+    floor_ms = mufu_ops / (16 * 148 * 1.965e9) * 1e3
+    out["hour"] = {"workload": "configs[2]: 4 models (config-1 arch), 1 h stream, FP16, resident in HBM", "ms": ms,
+                   "strain_seconds_per_s": 3600 / (ms * 1e-3), "triggers": n,
+                   "bound": "alu (MUFU tanh: 256 per sample per model at 16/clk/SM x 148 SMs x 1.965 GHz)",
+                   "mufu_floor_ms": floor_ms, "frac_of_mufu_floor": floor_ms / ms}
+    # ---- month, host -> device streaming
+    st = gwi.Stream(models, n_chunks * N1, N1, THETA, LMIN, capacity=65536)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for c in range(n_chunks):
+        h = host[c & 1]
+        st.push(h[0], h[1])
+    n, _ = st.finish()
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    st.close()
+    out["month"] = {"workload": f"configs[4]: {n_chunks / 24:.0f} days x 4096 Hz x 2 detectors FP16 in {n_chunks} one-hour chunks from pinned host "
+                                "memory (2 distinct seeded chunks rotating), 4-model ensemble + trigger clustering",
+                    "wall_s": dt, "strain_seconds_per_s": n_chunks * 3600 / dt, "h2d_bytes": n_chunks * N1 * 2 * 2,
+                    "h2d_gb_per_s": n_chunks * N1 * 4 / dt / 1e9, "triggers": n}
+    return out
+
+
 def oracle_sample(model_path, x16, n_windows):
     """Times the oracle as it stands on the host cores over `n_windows` windows of the workload."""
     from oracle import gwo
@@ -116,6 +169,8 @@ def main():
     ap.add_argument("--windows", type=int, default=1024)
     ap.add_argument("--impl", default="gwi")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stream", action="store_true", help="skip the extra streaming-ensemble measurements")
+    ap.add_argument("--stream-chunks", type=int, default=744, help="one-hour chunks of the month-long stream leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -217,6 +272,12 @@ def main():
         e2e_s = float(tt.item())
     sampler.stop_flag = True
     sampler.join(timeout=3)
+    stream_extra = None
+    if not args.no_stream and world == 1:
+        try:
+            stream_extra = stream_bench(dev, work, rank, args.stream_chunks)
+        except Exception as ex:  # the headline line must still come out
+            stream_extra = {"error": repr(ex)}
 
     if rank != 0:
         return
@@ -243,6 +304,8 @@ def main():
                      "kernel": "gwi_infer (all launches of one call)", "flops_per_launch": flops_per_step,
                      "infer_ms": infer_ms, "frac_of_nominal_2250": tflops / 2250.0},
     }
+    if stream_extra is not None:
+        line["stream"] = stream_extra
     if not args.no_cpu_baseline and world == 1:
         nthreads = os.cpu_count() or 1
         nwin = max(1, min(3 * nthreads, 48))
