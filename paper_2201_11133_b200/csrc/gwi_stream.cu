@@ -11,8 +11,10 @@
 //   a-8..a-10  per slide: ensemble mean, strict threshold, run clustering with the run carried across chunks
 //   a-11 trigger records copied to the host at finish, sorted by (slide, start)
 //
-// The branch stacks run on the generic CUDA-core kernels (gwi_generic.cu) for every architecture: each output sample
-// is an independent, fixed-order fp32 accumulation, which is what makes chunked == unchunked exact.
+// Two back ends: the fused narrow-architecture kernel (gwi_tiny.cu; FP16 mode, config-1 widths: the ensembles of
+// BASELINE.json configs 3-5), and the generic CUDA-core kernels (gwi_generic.cu) for every other architecture and for
+// FP32 mode.  In both, each output sample is an independent fixed-order computation, which is what makes
+// chunked == unchunked exact.
 #include <algorithm>
 #include <new>
 #include <vector>

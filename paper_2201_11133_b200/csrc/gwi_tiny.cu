@@ -17,8 +17,8 @@
 //     time t < 0 are forced to zero at every layer input, which is exactly the causal padding of reading A4.
 //     Every output sample is an independent fixed-order computation, so chunked == unchunked bit for bit (reading A17).
 //
-// Output: either the per-sample probability (fused head, zero lag) or the per-branch skip sums for the time-slide
-// heads (reading A24), in the layout of the generic stream path.
+// Output: either the per-sample probability (fused head, zero lag) or, for time slides (reading A24), the branch
+// features u = ReLU(skip sum) as fp16 time-major rows, from which k_tiny_heads evaluates the head for every lag.
 #include <cstring>
 #include <vector>
 

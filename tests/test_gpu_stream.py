@@ -182,3 +182,29 @@ def test_stream_argument_errors(tmpdir_s):
     assert n == len(recs)
     with pytest.raises(gwi.GwiError):
         gwi.Stream(gms, 1000, 500, lags=[1000])
+
+
+def test_full_hour_sampled_against_oracle(tmpdir_s):
+    """configs[2] at full size, in the launch configuration bench.py times (one 1 h push, 4 models, FP16): the mean
+    probability on sampled spans against the oracle evaluated on those spans alone (valid R_f - 1 samples in)."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1, 2, 3], gwi.FP16)
+    N = 3600 * 4096
+    g = torch.Generator().manual_seed(5)
+    xt = torch.randn((2, N), generator=g).to(torch.float16)
+    st = gwi.Stream(gms, N, N, 0.5, 2048, capacity=4096, want_pbar=True)
+    xd = xt.cuda()
+    st.push(xd[0], xd[1])
+    n, recs = st.finish()
+    x = xt.numpy()
+    rf = gms[0].receptive_field
+    for s0 in [0, 111, 4096 * 1800 - 7, N - 5000]:
+        span = x[:, s0:s0 + 5000].astype(np.float64)
+        want = gwo.ensemble_mean([om.stream(span) for om in oms])
+        got = st.pbar[0, s0:s0 + 5000].cpu().numpy()
+        lo = 0 if s0 == 0 else rf - 1
+        assert np.max(np.abs(got[lo:] - want[lo:])) <= 2e-3
+    pb = st.pbar[0].cpu().numpy()
+    assert np.isfinite(pb).all() and 0.0 <= pb.min() and pb.max() <= 1.0
+    st.close()

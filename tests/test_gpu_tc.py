@@ -81,3 +81,17 @@ def test_many_windows_more_jobs_than_sms(tmpdir_s):
     x2[1::2] = x[::2]
     got2 = _run(gm, x2)
     assert np.array_equal(got2[::2], got[1::2]) and np.array_equal(got2[1::2], got[::2])   # bit-identical per window
+
+
+def test_full_batch_sampled_against_oracle(tmpdir_s):
+    """BASELINE.json configs[1] at full size in the launch configuration bench.py times (1024 windows x 4096, one
+    gwi_infer call): sampled windows against the oracle; every probability finite and inside [0, 1]."""
+    import paper_2201_11133_b200 as gwi
+    a = gs.PAPER_ARCH
+    om, gm = model_pair(tmpdir_s, "tc_full", a, gs.xavier_tensors(a, 0), gwi.FP16)
+    x, inj = gs.cfg2_windows(seed=1, B=1024, T=4096)
+    got = _run(gm, x)
+    assert np.isfinite(got).all() and got.min() >= 0.0 and got.max() <= 1.0
+    sel = sorted({0, 1, 295, 296, 511, 1022, 1023, int(inj[0]), int(inj[-1])})
+    want = om.infer_windows(x[sel].astype(np.float64))
+    assert np.max(np.abs(got[sel] - want)) <= TOL16
