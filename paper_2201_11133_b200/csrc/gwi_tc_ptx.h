@@ -56,7 +56,11 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t spins = 0;
+#ifdef GWI_SPIN_TEST
+    while (!mbar_test(bar, parity)) {
+#else
     while (!mbar_try_wait(bar, parity)) {
+#endif
         if (++spins > (1u << 26)) __trap();
     }
 }

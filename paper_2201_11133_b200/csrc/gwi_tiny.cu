@@ -77,13 +77,15 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
     const int r0 = warp * 16 + g, r1 = r0 + 8;                           // this thread's two rows
     const int64_t tl0 = tile0 + r0, tl1 = tile0 + r1;                    // chunk-local times
     // rows before the stream start are zero at every layer input (reading A4)
+    const bool premask = a.t0 + tile0 < 0;                               // CTA-uniform: only the first tile of a stream
     const bool live0 = a.t0 + tl0 >= 0, live1 = a.t0 + tl1 >= 0;
     for (int i = threadIdx.x; i < 2 * PADROWS * RS / 2; i += TW * 32) {
         int buf = i / (PADROWS * RS / 2), k = i % (PADROWS * RS / 2);
         reinterpret_cast<uint32_t*>(sm[buf])[k] = 0u;
     }
     const float* hcst = a.cst + 2 * 32;
-    uint32_t ua[2][2][4];                                                // head A fragments: [branch][k-step][4]
+    uint32_t ua[2][4];                                                   // head A fragments of the current branch
+    __shared__ uint4 sm_u[2][TW * 32];                                   // branch 0's fragments, parked while branch 1 runs
 
 #pragma unroll
     for (int b = 0; b < 2; b++) {
@@ -101,14 +103,24 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
         for (int nt = 0; nt < 2; nt++) {
             float2 w = __ldg(reinterpret_cast<const float2*>(cb + 8 * nt + 2 * t));
             float2 bi = __ldg(reinterpret_cast<const float2*>(cb + 16 + 8 * nt + 2 * t));
-            h[nt][0] = live0 ? fmaf(w.x, x0, bi.x) : 0.f, h[nt][1] = live0 ? fmaf(w.y, x0, bi.y) : 0.f;
-            h[nt][2] = live1 ? fmaf(w.x, x1, bi.x) : 0.f, h[nt][3] = live1 ? fmaf(w.y, x1, bi.y) : 0.f;
+            h[nt][0] = fmaf(w.x, x0, bi.x), h[nt][1] = fmaf(w.y, x0, bi.y);
+            h[nt][2] = fmaf(w.x, x1, bi.x), h[nt][3] = fmaf(w.y, x1, bi.y);
+            if (premask) {
+                if (!live0) h[nt][0] = h[nt][1] = 0.f;
+                if (!live1) h[nt][2] = h[nt][3] = 0.f;
+            }
         }
         float sk[4][4];                                                  // skip sum, 4 n-tiles of 8 channels
 #pragma unroll
-        for (int nt = 0; nt < 4; nt++) sk[nt][0] = sk[nt][1] = sk[nt][2] = sk[nt][3] = 0.f;
+        for (int nt = 0; nt < 4; nt++) {                                 // starts at sum_i bs_i (summed on the host)
+            float2 bb = __ldg(reinterpret_cast<const float2*>(a.cst + 2 * 32 + 66 + b * 32 + 8 * nt + 2 * t));
+            sk[nt][0] = bb.x, sk[nt][1] = bb.y, sk[nt][2] = bb.x, sk[nt][3] = bb.y;
+        }
 
-        for (int i = 0; i < a.L; i++) {
+        const float* bl = a.bias + (size_t)b * a.L * 80;
+        const uint2* wf = a.wfg + (size_t)b * a.L * (2 * 4 * 32) + lane;
+        const uint2* wr = a.wrs + (size_t)b * a.L * (6 * 32) + lane;
+        for (int i = 0; i < a.L; i++, bl += 80, wf += 2 * 4 * 32, wr += 6 * 32) {
             const int d = a.dil[i];
             __half* buf = sm[i & 1] + PADROWS * RS;
             // ---- current-tap A fragment = this thread's own h values; parked in shared memory for the rows d later
@@ -124,8 +136,6 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
             ap[2] = *reinterpret_cast<const uint32_t*>(buf + (r0 - d) * RS + 8 + 2 * t);
             ap[3] = *reinterpret_cast<const uint32_t*>(buf + (r1 - d) * RS + 8 + 2 * t);
             // ---- f | g/2 = [h(t-d) | h(t)] . W^T + bias                                      (C.1 step 2)
-            const float* bl = a.bias + ((size_t)b * a.L + i) * 80;
-            const uint2* wf = a.wfg + ((size_t)b * a.L + i) * (2 * 4 * 32) + lane;
             float fg[4][4];
 #pragma unroll
             for (int nt = 0; nt < 4; nt++) {
@@ -149,21 +159,21 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
                 az[2] = pack2(z[1][0], z[1][1]), az[3] = pack2(z[1][2], z[1][3]);
             }
             // ---- res | skip = z' . [Wr/2 | Ws/2]^T
-            const uint2* wr = a.wrs + ((size_t)b * a.L + i) * (6 * 32) + lane;
             if (i < a.L - 1) {                                           // reading A8: the last residual conv is dead
 #pragma unroll
                 for (int nt = 0; nt < 2; nt++) {
                     float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 32 + 8 * nt + 2 * t));
                     float rr[4] = {bb.x, bb.y, bb.x, bb.y};
                     mma16816(rr, az, __ldg(wr + nt * 32));
-                    h[nt][0] = live0 ? h[nt][0] + rr[0] : 0.f, h[nt][1] = live0 ? h[nt][1] + rr[1] : 0.f;
-                    h[nt][2] = live1 ? h[nt][2] + rr[2] : 0.f, h[nt][3] = live1 ? h[nt][3] + rr[3] : 0.f;
+                    h[nt][0] += rr[0], h[nt][1] += rr[1], h[nt][2] += rr[2], h[nt][3] += rr[3];
+                    if (premask) {
+                        if (!live0) h[nt][0] = h[nt][1] = 0.f;
+                        if (!live1) h[nt][2] = h[nt][3] = 0.f;
+                    }
                 }
             }
 #pragma unroll
             for (int nt = 0; nt < 4; nt++) {
-                float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 48 + 8 * nt + 2 * t));
-                sk[nt][0] += bb.x, sk[nt][1] += bb.y, sk[nt][2] += bb.x, sk[nt][3] += bb.y;
                 mma16816(sk[nt], az, __ldg(wr + (2 + nt) * 32));
             }
         }
@@ -182,10 +192,11 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
             // ---- u_b = ReLU(skip sum) as the A fragments of the head                        (C.1 steps 3, 4)
 #pragma unroll
             for (int ks = 0; ks < 2; ks++) {
-                ua[b][ks][0] = pack2(fmaxf(sk[2 * ks][0], 0.f), fmaxf(sk[2 * ks][1], 0.f));
-                ua[b][ks][1] = pack2(fmaxf(sk[2 * ks][2], 0.f), fmaxf(sk[2 * ks][3], 0.f));
-                ua[b][ks][2] = pack2(fmaxf(sk[2 * ks + 1][0], 0.f), fmaxf(sk[2 * ks + 1][1], 0.f));
-                ua[b][ks][3] = pack2(fmaxf(sk[2 * ks + 1][2], 0.f), fmaxf(sk[2 * ks + 1][3], 0.f));
+                ua[ks][0] = pack2(fmaxf(sk[2 * ks][0], 0.f), fmaxf(sk[2 * ks][1], 0.f));
+                ua[ks][1] = pack2(fmaxf(sk[2 * ks][2], 0.f), fmaxf(sk[2 * ks][3], 0.f));
+                ua[ks][2] = pack2(fmaxf(sk[2 * ks + 1][0], 0.f), fmaxf(sk[2 * ks + 1][1], 0.f));
+                ua[ks][3] = pack2(fmaxf(sk[2 * ks + 1][2], 0.f), fmaxf(sk[2 * ks + 1][3], 0.f));
+                if (b == 0) sm_u[ks][threadIdx.x] = make_uint4(ua[ks][0], ua[ks][1], ua[ks][2], ua[ks][3]);
             }
         }
         __syncthreads();   // the next branch starts again with buffer 0
@@ -198,7 +209,13 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
         float2 bb = __ldg(reinterpret_cast<const float2*>(hcst + 8 * nt + 2 * t));
         float v[4] = {bb.x, bb.y, bb.x, bb.y};
 #pragma unroll
-        for (int ks = 0; ks < 4; ks++) mma16816(v, ua[ks >> 1][ks & 1], __ldg(a.w1 + (ks * 4 + nt) * 32 + lane));
+        for (int ks = 0; ks < 2; ks++) {                                 // H1 half (parked), then L1 half
+            uint4 p = sm_u[ks][threadIdx.x];
+            uint32_t ah[4] = {p.x, p.y, p.z, p.w};
+            mma16816(v, ah, __ldg(a.w1 + (ks * 4 + nt) * 32 + lane));
+        }
+#pragma unroll
+        for (int ks = 0; ks < 2; ks++) mma16816(v, ua[ks], __ldg(a.w1 + ((2 + ks) * 4 + nt) * 32 + lane));
         float2 w2 = __ldg(reinterpret_cast<const float2*>(hcst + 32 + 8 * nt + 2 * t));
         y0 = fmaf(w2.x, fmaxf(v[0], 0.f), y0), y0 = fmaf(w2.y, fmaxf(v[1], 0.f), y0);
         y1 = fmaf(w2.x, fmaxf(v[2], 0.f), y1), y1 = fmaf(w2.y, fmaxf(v[3], 0.f), y1);
@@ -353,7 +370,7 @@ gwi_status gwi_tiny_pack(gwi_model* m)
         return r;
     };
     std::vector<uint2> wfg((size_t)nb * L * 8 * 32), wrs((size_t)nb * L * 6 * 32), w1(16 * 32);
-    std::vector<float> bias((size_t)nb * L * 80), cst(2 * 32 + 65);
+    std::vector<float> bias((size_t)nb * L * 80), cst(2 * 32 + 65 + 1 + 2 * 32, 0.f);   // + pad + sum_i bs_i per branch
     for (int b = 0; b < nb; b++) {
         for (int c = 0; c < 16; c++) cst[b * 32 + c] = W[m->off.W_in[b] + c], cst[b * 32 + 16 + c] = W[m->off.b_in[b] + c];
         for (int i = 0; i < L; i++) {
@@ -372,7 +389,7 @@ gwi_status gwi_tiny_pack(gwi_model* m)
                 for (int l = 0; l < 32; l++) wrs[(((size_t)b * L + i) * 6 + nt) * 32 + l] = frag(Brs, 0, 8 * nt, l);
             float* bl = bias.data() + ((size_t)b * L + i) * 80;
             for (int c = 0; c < 16; c++) bl[c] = W[lo.bf + c], bl[16 + c] = 0.5f * W[lo.bg + c], bl[32 + c] = W[lo.br + c];
-            for (int q = 0; q < 32; q++) bl[48 + q] = W[lo.bs + q];
+            for (int q = 0; q < 32; q++) bl[48 + q] = W[lo.bs + q], cst[2 * 32 + 66 + b * 32 + q] += W[lo.bs + q];
         }
     }
     auto B1 = [&](int k, int n) { return W[m->off.W1 + (int64_t)n * 64 + k]; };   // k over [u_H(32) | u_L(32)]
