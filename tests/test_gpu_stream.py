@@ -208,3 +208,32 @@ def test_full_hour_sampled_against_oracle(tmpdir_s):
     pb = st.pbar[0].cpu().numpy()
     assert np.isfinite(pb).all() and 0.0 <= pb.min() and pb.max() <= 1.0
     st.close()
+
+
+@pytest.mark.parametrize("prec_name,tol", [("FP16", 2e-3), ("FP32", 1e-5)])
+@pytest.mark.parametrize("N,chunks,lags", [(1, [1], []), (5, [1, 1, 1, 1, 1], [3]), (17, [16, 1], [16]),
+                                           (113, [112, 1], []), (225, [1, 111, 113], [1, 224]),
+                                           (4096, [4096], [4095])])
+def test_stream_degenerate_sizes(tmpdir_s, prec_name, tol, N, chunks, lags):
+    """Streams shorter than the receptive field / the kernel halo / one tile, one-sample chunks, lags next to N."""
+    import paper_2201_11133_b200 as gwi
+    prec = getattr(gwi, prec_name)
+    oms, gms = _models(tmpdir_s, [0, 1], prec, bias="random")
+    dt = np.float16 if prec == gwi.FP16 else np.float32
+    x = gs.stream_noise(21, 0, N, dtype=dt)
+    want = _oracle_slides(oms, x, lags)
+    n, recs, pbar = _run_stream(gms, x, chunks, lags, 0.5, 1)
+    assert np.max(np.abs(pbar - want)) <= tol
+    assert trig_tuples(recs) == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 1)
+
+
+def test_stream_generic_path_paper_scale_fp32(tmpdir_s):
+    """The generic back end (any architecture) on the paper-scale model: carried per-layer history over dilations up
+    to 512, chunks shorter than the receptive field."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0], gwi.FP32, bias="random", arch=gs.PAPER_ARCH)
+    N = 5000
+    x = gs.stream_noise(23, 0, N, dtype=np.float32)
+    want = _oracle_slides(oms, x, [4096])
+    n, recs, pbar = _run_stream(gms, x, _ragged(N, 4, 100, 900), [4096], 0.5, 4, max_chunk=900)
+    assert np.max(np.abs(pbar - want)) <= 1e-5
