@@ -104,3 +104,4 @@ gwi_status gwi_tiny_stream(const gwi_model* m, const __half* d_x, int64_t ldx, i
                            __half* xh_next, float* d_prob, __half* d_u16, int64_t lds, cudaStream_t st);
 gwi_status gwi_tiny_heads(const gwi_model* m, const __half* d_u16, int64_t lds, int n, const int64_t* d_lags, int n_lags,
                           float* d_prob, int64_t stride_k, cudaStream_t st);
+gwi_status gwi_xhist_update(const __half* d_x, int64_t ldx, int n, int halo, const __half* xh_cur, __half* xh_next, cudaStream_t st);

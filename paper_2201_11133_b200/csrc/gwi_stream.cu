@@ -58,9 +58,48 @@ struct gwi_stream {
     int xh_cur = 0;
     std::vector<__half*> d_u16;             // time slides: per model [2][lds][32] fp16 branch features, time-major
     int64_t* d_lags = nullptr;              // device copy of the lag list
+    // tensor-core back end (paper-scale models, FP16 mode, zero lag only)
+    bool tcb = false;
+    int seg = 0, segT = 0, segH = 0;        // outputs per segment, window length H + seg, warm-up H = R_f - 1
+    __half2* d_segx = nullptr;              // [B][segT][2] channels-last batch
+    float* d_segp = nullptr;                // [B][segT] probabilities of the batch
+    void* d_tcws = nullptr;
+    size_t tcws_bytes = 0;
 };
 
 namespace {
+
+// ---- tensor-core back end (paper-scale models, FP16 mode, zero lag): the chunk is cut into segments of SEG outputs;
+// segment w > 0 is evaluated as a window of T = H + SEG samples whose first H = R_f - 1 samples are warm-up that is
+// recomputed from the input (exact: no output after the warm-up sees the window's zero padding), segment 0 of the
+// STREAM is a window without warm-up (its zero padding is the stream's, reading A4), segment 0 of a later chunk takes
+// its warm-up from the carried last H samples of the previous chunk.  All segments of a chunk go through the fused
+// tcgen05 kernel (gwi_tc.cu) as one batch of windows.
+__global__ void k_seg_gather(const __half* __restrict__ x, int64_t ldx, const __half* __restrict__ xh, int n, int SEG, int H,
+                             int T, int stream_start, __half2* __restrict__ out, int64_t total)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // (window, t)
+    if (i >= total) return;
+    int w = (int)(i / T), t = (int)(i % T);
+    int64_t src = (w == 0 && stream_start) ? t : (int64_t)w * SEG - H + t;   // chunk-local sample
+    __half a = __float2half(0.f), b = a;
+    if (src >= n) {
+    } else if (src >= 0) {
+        a = x[src], b = x[ldx + src];
+    } else {
+        a = xh[H + src], b = xh[H + H + src];
+    }
+    out[i] = __halves2half2(a, b);
+}
+__global__ void k_seg_scatter(const float* __restrict__ pb, int n, int SEG, int H, int T, int stream_start,
+                              float* __restrict__ prob)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // chunk-local output sample
+    if (i >= n) return;
+    int w = (int)(i / SEG), o = (int)(i % SEG);
+    int t = (w == 0 && stream_start) ? o : H + o;
+    prob[i] = pb[(int64_t)w * T + t];
+}
 
 size_t elt(const gwi_stream* s) { return s->half_in ? 2 : 4; }
 
@@ -71,8 +110,25 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
     const char* x = (const char*)s->d_x[xb] + (size_t)x0 * elt(s);
     for (int m = 0; m < s->M; m++) {
         const gwi_model* gm = s->models[m];
-        float* skip0 = s->tiny ? nullptr : s->d_skip[m] + s->maxlag;
+        float* skip0 = (s->tiny || s->tcb) ? nullptr : s->d_skip[m] + s->maxlag;
         gwi_status rc;
+        if (s->tcb) {
+            const int B = (n + s->seg - 1) / s->seg;
+            const int start = s->t_done == 0 ? 1 : 0;
+            if (m == 0) {
+                int64_t total = (int64_t)B * s->segT;
+                k_seg_gather<<<(unsigned)((total + 255) / 256), 256, 0, st>>>((const __half*)x, s->xcap, s->d_xh[s->xh_cur], n, s->seg,
+                                                                             s->segH, s->segT, start, s->d_segx, total);
+                rc = gwi_xhist_update((const __half*)x, s->xcap, n, s->segH, s->d_xh[s->xh_cur], s->d_xh[s->xh_cur ^ 1], st);
+                if (rc != GWI_OK) return rc;
+            }
+            rc = gwi_tc_infer(gm, (const __half*)s->d_segx, B, s->segT, s->d_segp, s->d_tcws, s->tcws_bytes, st);
+            if (rc != GWI_OK) return rc;
+            k_seg_scatter<<<(n + 255) / 256, 256, 0, st>>>(s->d_segp, n, s->seg, s->segH, s->segT, start, s->d_prob + (size_t)m * s->sub);
+            gwi_count_launch(m == 0 ? 2 : 1);
+            GWI_CUDA_CHECK(cudaGetLastError());
+            continue;
+        }
         if (s->tiny) {
             // fused kernel: zero lag only -> probabilities straight out of the kernel; with slides -> skip sums, the
             // per-lag heads follow below
@@ -207,11 +263,21 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     s->tiny = true;
     for (int i = 0; i < n_models; i++) s->tiny = s->tiny && models[i]->tiny != nullptr;
     s->halo = s->tiny ? gwi_tiny_halo(m0) : 0;
+    s->tcb = s->half_in && n_lags == 0 && !s->tiny && m0->arch.n_branch == 2 && m0->arch.c_in == 1;
+    for (int i = 0; i < n_models; i++) s->tcb = s->tcb && models[i]->tc != nullptr;
+    if (s->tcb) {
+        s->segH = s->Rf - 1;
+        s->segT = ((s->segH + 8192 + 127) / 128) * 128;    // >= 8192 outputs per segment, whole tiles
+        if (s->segT < 16384) s->segT = 16384;
+        s->seg = s->segT - s->segH;
+        s->halo = s->segH;
+    }
     s->xcap = std::max<int64_t>(std::min(max_chunk, n_total), std::min<int64_t>(n_total, s->maxlag + s->Rf - 1));
     // sub-chunk: bounds the activation workspace (2R floats per branch-sample) to ~2 GiB
     int64_t per = (int64_t)s->nb * 2 * s->R * 4;
     int64_t sub = std::max<int64_t>(4096, (2LL << 30) / per);
     if (s->tiny) sub = std::max<int64_t>(4096, (1LL << 30) / ((int64_t)(1 + n_lags) * n_models * 4));   // ~1 GiB of probabilities
+    if (s->tcb) sub = 1 << 24;
     sub = std::min<int64_t>(sub, 1 << 24);
     sub = std::min<int64_t>(sub, s->xcap);
     s->sub = (int)sub;
@@ -228,14 +294,25 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     for (int b = 0; b < 2; b++)
         if ((e = cudaMalloc(&s->d_x[b], (size_t)C * s->xcap * elt(s))) != cudaSuccess) return fail(e);
     size_t hbytes = (size_t)s->nb * s->R * s->sub * 4;
-    if (!s->tiny) {   // activation workspace of the generic per-layer kernels
+    if (s->tcb) {
+        const int64_t Bmax = (s->sub + s->seg - 1) / s->seg;
+        if ((e = cudaMalloc(&s->d_segx, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);
+        if ((e = cudaMalloc(&s->d_segp, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);
+        s->tcws_bytes = gwi_tc_workspace_bytes(m0, Bmax, s->segT);
+        if ((e = cudaMalloc(&s->d_tcws, s->tcws_bytes)) != cudaSuccess) return fail(e);
+        for (int b = 0; b < 2; b++) {
+            if ((e = cudaMalloc(&s->d_xh[b], (size_t)2 * s->segH * 2)) != cudaSuccess) return fail(e);
+            if ((e = cudaMemset(s->d_xh[b], 0, (size_t)2 * s->segH * 2)) != cudaSuccess) return fail(e);
+        }
+    }
+    if (!s->tiny && !s->tcb) {   // activation workspace of the generic per-layer kernels
         if ((e = cudaMalloc(&s->d_hA, hbytes)) != cudaSuccess) return fail(e);
         if ((e = cudaMalloc(&s->d_hB, hbytes)) != cudaSuccess) return fail(e);
     }
     size_t histb = (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(m0)) * 4;
     s->d_skip.assign(s->M, nullptr);
     s->d_hist[0].assign(s->M, nullptr), s->d_hist[1].assign(s->M, nullptr);
-    for (int m = 0; m < s->M && !s->tiny; m++) {
+    for (int m = 0; m < s->M && !s->tiny && !s->tcb; m++) {
         size_t sb = (size_t)s->nb * s->S * s->lds * 4;
         if ((e = cudaMalloc(&s->d_skip[m], sb)) != cudaSuccess) return fail(e);
         if ((e = cudaMemset(s->d_skip[m], 0, sb)) != cudaSuccess) return fail(e);
@@ -297,6 +374,9 @@ extern "C" void gwi_stream_destroy(gwi_stream* s)
     for (__half* p : s->d_u16)
         if (p) cudaFree(p);
     if (s->d_lags) cudaFree(s->d_lags);
+    if (s->d_segx) cudaFree(s->d_segx);
+    if (s->d_segp) cudaFree(s->d_segp);
+    if (s->d_tcws) cudaFree(s->d_tcws);
     if (s->d_hA) cudaFree(s->d_hA);
     if (s->d_hB) cudaFree(s->d_hB);
     if (s->d_tmp) cudaFree(s->d_tmp);

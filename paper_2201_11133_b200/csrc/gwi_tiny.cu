@@ -457,3 +457,12 @@ gwi_status gwi_tiny_heads(const gwi_model* m, const __half* d_u16, int64_t lds, 
     GWI_CUDA_CHECK(cudaGetLastError());
     return GWI_OK;
 }
+
+// carried input samples, any halo length (used by the stream back ends that recompute their warm-up from the input)
+gwi_status gwi_xhist_update(const __half* d_x, int64_t ldx, int n, int halo, const __half* xh_cur, __half* xh_next, cudaStream_t st)
+{
+    k_tiny_xhist<<<(2 * halo + 127) / 128, 128, 0, st>>>(d_x, ldx, n, halo, xh_cur, xh_next);
+    gwi_count_launch(1);
+    GWI_CUDA_CHECK(cudaGetLastError());
+    return GWI_OK;
+}

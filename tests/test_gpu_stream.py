@@ -237,3 +237,20 @@ def test_stream_generic_path_paper_scale_fp32(tmpdir_s):
     want = _oracle_slides(oms, x, [4096])
     n, recs, pbar = _run_stream(gms, x, _ragged(N, 4, 100, 900), [4096], 0.5, 4, max_chunk=900)
     assert np.max(np.abs(pbar - want)) <= 1e-5
+
+
+def test_stream_paper_scale_tensor_core_back_end(tmpdir_s):
+    """FP16 stream of paper-scale models: segments with recomputed warm-up through the fused tcgen05 kernel.  Parity
+    with the oracle's one-pass definition, and chunked == unchunked bit for bit."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1], gwi.FP16, arch=gs.PAPER_ARCH)
+    assert all(g.uses_tensor_cores for g in gms)
+    N = 40000
+    x = gs.stream_noise(31, 0, N, dtype=np.float16)
+    want = _oracle_slides(oms, x, [])
+    n0, r0, p0 = _run_stream(gms, x, [N], [], 0.5, 16)
+    assert np.max(np.abs(p0 - want)) <= 2e-3
+    n1, r1, p1 = _run_stream(gms, x, _ragged(N, 2, 1000, 17000), [], 0.5, 16, max_chunk=17000)
+    assert np.array_equal(p0, p1)
+    assert trig_tuples(r0) == trig_tuples(r1)
+    assert trig_tuples(r0) == _oracle_triggers(p0.astype(np.float64), float(np.float32(0.5)), 16)
