@@ -106,6 +106,32 @@ def stream_bench(dev, work, rank, n_chunks=744):
                    "strain_seconds_per_s": 3600 / (ms * 1e-3), "triggers": n,
                    "bound": "alu (MUFU tanh: 256 per sample per model at 16/clk/SM x 148 SMs x 1.965 GHz)",
                    "mufu_floor_ms": floor_ms, "frac_of_mufu_floor": floor_ms / ms}
+    # ---- hour, 4 paper-scale models (SURVEY.md 8(f) NEXT-2 in the small): tensor-core stream back end
+    try:
+        pm = []
+        for sd in range(4):
+            pth = os.path.join(work, f"bench_paper_seed{sd}_s{rank}.gwim")
+            gs.make_model_file(pth, gs.PAPER_ARCH, seed=sd)
+            pm.append(gwi.load_model(pth, gwi.FP16, dev.index))
+        times = []
+        for rep in range(3):
+            st = gwi.Stream(pm, N1, N1, THETA, LMIN, capacity=4096)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            st.push(xd[0], xd[1])
+            e1.record()
+            n, _ = st.finish()
+            times.append(e0.elapsed_time(e1))
+            st.close()
+        ms = float(np.median(times[1:]))
+        out["hour_paper_scale"] = {"workload": "4 paper-scale models (2x20 blocks, R64/S128), 1 h stream, FP16, resident in HBM; "
+                                               "segments of 14338 outputs + 2046 recomputed warm-up samples through k_stack",
+                                   "ms": ms, "strain_seconds_per_s": 3600 / (ms * 1e-3), "triggers": n,
+                                   "tflops_algorithmic": gs.PAPER_ARCH.flops_per_timestep() * N1 * 4 / (ms * 1e-3) / 1e12}
+        del pm
+    except Exception as ex:
+        out["hour_paper_scale"] = {"error": repr(ex)}
     # ---- month, host -> device streaming
     st = gwi.Stream(models, n_chunks * N1, N1, THETA, LMIN, capacity=65536)
     torch.cuda.synchronize()
