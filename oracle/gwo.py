@@ -22,6 +22,10 @@ class Trigger(C.Structure):
                 ("peak_p", C.c_double), ("mean_p", C.c_double)]
 
 
+class Event(C.Structure):
+    _fields_ = [("t_first", C.c_int64), ("t_last", C.c_int64), ("n_triggers", C.c_int32), ("slide", C.c_int32)]
+
+
 def build(force=False):
     """gcc -O2 -fopenmp -ffp-contract=off: no FMA contraction, so the sums are the ones the source spells."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
@@ -54,6 +58,9 @@ def lib():
         L.gwo_triggers.restype = C.c_long
         L.gwo_triggers.argtypes = [_dp, C.c_long, C.c_double, C.c_long, C.c_int, C.c_long, C.POINTER(_dp), C.c_int,
                                    C.POINTER(Trigger), C.c_long]
+        L.gwo_coincidence.restype = C.c_long
+        L.gwo_coincidence.argtypes = [C.POINTER(C.POINTER(C.c_long)), C.POINTER(C.c_int), C.c_int, C.c_long, C.c_int,
+                                      C.POINTER(Event), C.c_long]
         L.gwo_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -189,3 +196,14 @@ def triggers(pbar, theta, Lmin, slide=0, t0=0, pm=None, cap=1 << 16):
 
 def num_threads():
     return lib().gwo_num_threads()
+
+
+def coincidence(ends, window, slide=0, cap=1 << 14):
+    """ends: list (one per model) of lists of trigger end times -> [(t_first, t_last, n_triggers)] (reading A34)."""
+    M = len(ends)
+    arrs = [(C.c_long * max(len(e), 1))(*[int(v) for v in e]) for e in ends]
+    ptrs = (C.POINTER(C.c_long) * M)(*[C.cast(a, C.POINTER(C.c_long)) for a in arrs])
+    n = (C.c_int * M)(*[len(e) for e in ends])
+    out = (Event * cap)()
+    k = lib().gwo_coincidence(ptrs, n, M, int(window), int(slide), out, cap)
+    return [(o.t_first, o.t_last, o.n_triggers) for o in out[:min(k, cap)]]

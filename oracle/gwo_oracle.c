@@ -19,7 +19,8 @@
  * P4 dilation<->polyphase and shift, P5/P6 hand-worked examples (tests/golden), P7 closed forms,
  * P8 windowed==stream, P9 branch independence + slide reuse, P10 channel permutation, P11 batch
  * independence, P12 numpy.convolve cross-check, P13/P14 clustering worked example + brute force,
- * P16 sign pass-through closed form.  PARITY UNPINNED: the absolute probability values for the
+ * P16 sign pass-through closed form, P17 coincidence worked example + tuple brute force + invariances.
+ * PARITY UNPINNED: the absolute probability values for the
  * random-weight configs have no external reference (no trained weights / LIGO data in this container).
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC gwo_oracle.c -o libgwo_oracle.so -lm
@@ -340,6 +341,53 @@ long gwo_triggers(const double *pbar, long N, double theta, long Lmin, int slide
             count++;
         }
     }
+    return count;
+}
+
+/* ---- all-model coincidence of per-model triggers ("Triggers that were reported by all AI models in
+ * the ensemble, and which were coincident within a time window of 0.5 seconds were flagged as gravitational wave
+ * events"; reading A34) ------------------------------------------------------------------------------------------
+ * ends[m][i], i < n[m]: merger-time estimates (trigger ends) of model m, any order.
+ * A time a is an ANCHOR iff a is one of the ends and every model has an end in [a, a + W].
+ * Anchors are sorted; a new event starts at an anchor that is more than W after the previous anchor.
+ * Event: t_first = its first anchor, t_last = the largest end (any model) in [t_first, last anchor + W],
+ * n_triggers = number of ends (all models) in [t_first, last anchor + W].  Plain O(n^2) scans.           */
+typedef struct { int64_t t_first, t_last; int32_t n_triggers, slide; } gwo_event;
+
+long gwo_coincidence(const long *const *ends, const int *n, int M, long W, int slide, gwo_event *out, long cap)
+{
+    long na = 0, tot = 0;
+    for (int m = 0; m < M; m++) tot += n[m];
+    long *anch = (long *)malloc((size_t)(tot > 0 ? tot : 1) * sizeof(long));
+    for (int m = 0; m < M; m++)
+        for (int i = 0; i < n[m]; i++) {
+            long a = ends[m][i];
+            int all = 1;
+            for (int q = 0; q < M && all; q++) {
+                int found = 0;
+                for (int j = 0; j < n[q]; j++) if (ends[q][j] >= a && ends[q][j] <= a + W) found = 1;
+                all = found;
+            }
+            if (all) anch[na++] = a;
+        }
+    for (long i = 1; i < na; i++) {                      /* insertion sort */
+        long v = anch[i], j = i - 1;
+        while (j >= 0 && anch[j] > v) { anch[j + 1] = anch[j]; j--; }
+        anch[j + 1] = v;
+    }
+    long count = 0, i = 0;
+    while (i < na) {
+        long first = anch[i], last = anch[i];
+        while (i + 1 < na && anch[i + 1] - last <= W) { i++; last = anch[i]; }
+        i++;
+        long tl = first; int nt = 0;
+        for (int m = 0; m < M; m++)
+            for (int j = 0; j < n[m]; j++)
+                if (ends[m][j] >= first && ends[m][j] <= last + W) { nt++; if (ends[m][j] > tl) tl = ends[m][j]; }
+        if (count < cap) { out[count].t_first = first; out[count].t_last = tl; out[count].n_triggers = nt; out[count].slide = slide; }
+        count++;
+    }
+    free(anch);
     return count;
 }
 
