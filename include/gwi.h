@@ -165,6 +165,31 @@ gwi_status gwi_stream_push_host(gwi_stream* s, const void* h_h1, const void* h_l
 gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, int32_t capacity, int32_t* h_count,
                              void* cuda_stream);
 int64_t gwi_stream_samples_done(const gwi_stream* s);
+
+/* ---- the paper's decision rule: per-model triggers + all-model coincidence (reading A34) ------
+ *
+ * gwi_stream_set_rule   before the first push.  GWI_RULE_MEAN (default): triggers of the ensemble-mean probability
+ *                     (BASELINE.json configs 3-5).  GWI_RULE_PER_MODEL: every model's own probability is thresholded
+ *                     and clustered separately (same threshold, min_len, run carry); each record carries its slide and
+ *                     model_mask = 1 << model.  In this mode d_pbar, if given at create, is [1 + n_lags][n_models][n_total]
+ *                     and receives every model's probabilities.
+ * gwi_coincidence     HOST function on HOST records (as gwi_stream_finish returns them in GWI_RULE_PER_MODEL mode, any
+ *                     order).  Per slide: an end time a of some trigger is an anchor iff every one of the n_models
+ *                     models has a trigger whose end lies in [a, a + window]; anchors more than `window` apart start
+ *                     a new event; an event reports t_first = its first anchor, t_last = the largest trigger end in
+ *                     [t_first, last anchor + window], n_triggers = the number of trigger ends in that span.
+ *                     Events sorted by (slide, t_first); *n_events = total (GWI_ERR_CAPACITY if > capacity, the first
+ *                     `capacity` are valid).  `end` is the merger-time estimate of a trigger.       */
+typedef enum { GWI_RULE_MEAN = 0, GWI_RULE_PER_MODEL = 1 } gwi_rule;
+typedef struct {
+    int64_t t_first;
+    int64_t t_last;
+    int32_t n_triggers;
+    int32_t slide;
+} gwi_event;
+gwi_status gwi_stream_set_rule(gwi_stream* s, gwi_rule rule);
+gwi_status gwi_coincidence(const gwi_trigger* h_triggers, int32_t n_triggers, int32_t n_models, int64_t window,
+                           gwi_event* h_events, int32_t capacity, int32_t* n_events);
 void gwi_stream_destroy(gwi_stream* s);
 
 /* ---- misc ---------------------------------------------------------------------------------------------- */

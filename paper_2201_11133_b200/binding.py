@@ -13,7 +13,8 @@ EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_m
                     "gwi_infer_workspace_bytes", "gwi_infer", "gwi_carry_bytes", "gwi_triggers_workspace_bytes",
                     "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
                     "gwi_stream_tail_samples", "gwi_stream_prime", "gwi_stream_push", "gwi_stream_push_host",
-                    "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_destroy"]
+                    "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_destroy", "gwi_stream_set_rule",
+                    "gwi_coincidence"]
 
 
 class GwiError(RuntimeError):
@@ -78,6 +79,10 @@ def lib():
     L.gwi_stream_samples_done.argtypes = [vp]
     L.gwi_stream_destroy.restype = None
     L.gwi_stream_destroy.argtypes = [vp]
+    L.gwi_stream_set_rule.restype = C.c_int
+    L.gwi_stream_set_rule.argtypes = [vp, C.c_int]
+    L.gwi_coincidence.restype = C.c_int
+    L.gwi_coincidence.argtypes = [vp, C.c_int32, C.c_int32, C.c_int64, vp, C.c_int32, i32p]
     L.gwi_last_error.restype = C.c_char_p
     L.gwi_version.restype = C.c_int
     L.gwi_launch_count.restype = C.c_int64
@@ -198,6 +203,22 @@ def new_carry(device=0):
     return torch.zeros(lib().gwi_carry_bytes(), dtype=torch.uint8, device=f"cuda:{device}" if isinstance(device, int) else device)
 
 
+RULE_MEAN, RULE_PER_MODEL = 0, 1
+
+
+class Event(C.Structure):
+    _fields_ = [("t_first", C.c_int64), ("t_last", C.c_int64), ("n_triggers", C.c_int32), ("slide", C.c_int32)]
+
+
+def coincidence(records, n_models, window, capacity=4096):
+    """gwi_coincidence on a list of Trigger records (per-model rule) -> [Event...] sorted by (slide, t_first)."""
+    arr = (Trigger * max(len(records), 1))(*records)
+    out = (Event * max(capacity, 1))()
+    n = C.c_int32(0)
+    _check(lib().gwi_coincidence(arr, len(records), int(n_models), int(window), out, int(capacity), C.byref(n)))
+    return [Event.from_buffer_copy(out[i]) for i in range(n.value)]
+
+
 class Stream:
     """Handle on a gwi_stream (gwi_stream_create ... gwi_stream_destroy).  Marshalling only.
 
@@ -205,19 +226,22 @@ class Stream:
     max_chunk: largest push; want_pbar: keep the mean probability of every slide ([1+n_lags][n_total] float32 device
     tensor in .pbar) for parity tests."""
 
-    def __init__(self, models, n_total, max_chunk, threshold=0.5, min_len=2048, lags=(), capacity=4096, want_pbar=False):
+    def __init__(self, models, n_total, max_chunk, threshold=0.5, min_len=2048, lags=(), capacity=4096, want_pbar=False,
+                 rule=RULE_MEAN):
         self.models = list(models)
         self.device = torch.device("cuda", self.models[0].device)
         self.dtype = torch.float16 if self.models[0].precision == FP16 else torch.float32
         self.capacity = int(capacity)
-        self.pbar = (torch.zeros((1 + len(lags), int(n_total)), dtype=torch.float32, device=self.device)
-                     if want_pbar else None)
+        shape = (1 + len(lags), int(n_total)) if rule == RULE_MEAN else (1 + len(lags), len(self.models), int(n_total))
+        self.pbar = torch.zeros(shape, dtype=torch.float32, device=self.device) if want_pbar else None
         mp = (C.c_void_p * len(self.models))(*[m._h for m in self.models])
         lg = (C.c_int64 * max(len(lags), 1))(*[int(v) for v in lags])
         self._h = C.c_void_p()
         _check(lib().gwi_stream_create(mp, len(self.models), lg, len(lags), int(n_total), int(max_chunk), float(threshold),
                                        int(min_len), self.capacity,
                                        C.c_void_p(self.pbar.data_ptr()) if want_pbar else None, C.byref(self._h)))
+        if rule != RULE_MEAN:
+            _check(lib().gwi_stream_set_rule(self._h, int(rule)))
 
     @property
     def tail_samples(self):

@@ -58,6 +58,8 @@ struct gwi_stream {
     int xh_cur = 0;
     std::vector<__half*> d_u16;             // time slides: per model [2][lds][32] fp16 branch features, time-major
     int64_t* d_lags = nullptr;              // device copy of the lag list
+    int rule = 0;                           // GWI_RULE_MEAN / GWI_RULE_PER_MODEL
+    void* d_carry_pm = nullptr;             // per-model rule: [n_slides][M] carry blocks
     // tensor-core back end (paper-scale models, FP16 mode, zero lag only)
     bool tcb = false;
     int seg = 0, segT = 0, segH = 0;        // outputs per segment, window length H + seg, warm-up H = R_f - 1
@@ -166,6 +168,21 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
     }
     s->hist_cur ^= 1;
     s->xh_cur ^= 1;
+    if (s->rule == GWI_RULE_PER_MODEL) {
+        // the paper's rule: every model thresholded and clustered on its own; slide k and model m are
+        // packed into the record's slide field (k | m << 20) and unpacked at finish
+        for (int k = 0; k < nslides; k++)
+            for (int m = 0; m < s->M; m++) {
+                const float* ptr1[1] = {s->d_prob + ((size_t)k * s->M + m) * s->sub};
+                float* pb = s->d_pbar ? s->d_pbar + ((size_t)k * s->M + m) * s->N_total + s->t_done : nullptr;
+                gwi_status rc = gwi_post_run(ptr1, 1, n, s->t_done, s->theta, s->min_len, k | (m << 20), last ? 1 : 0,
+                                             (char*)s->d_carry_pm + ((size_t)k * s->M + m) * gwi_carry_bytes(), s->d_trig, s->cap,
+                                             s->d_count, 1, pb, s->d_post_ws, s->post_ws_bytes, st);
+                if (rc != GWI_OK) return rc;
+            }
+        s->t_done += n;
+        return GWI_OK;
+    }
     for (int k = 0; k < nslides; k++) {
         const float* ptrs[GWI_MAX_MODELS];
         for (int m = 0; m < s->M; m++) ptrs[m] = s->d_prob + ((size_t)k * s->M + m) * s->sub;
@@ -325,6 +342,8 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     if ((e = cudaMalloc(&s->d_prob, (size_t)nslides * s->M * s->sub * 4)) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_carry, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
     if ((e = cudaMemset(s->d_carry, 0, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc(&s->d_carry_pm, (size_t)nslides * s->M * gwi_carry_bytes())) != cudaSuccess) return fail(e);
+    if ((e = cudaMemset(s->d_carry_pm, 0, (size_t)nslides * s->M * gwi_carry_bytes())) != cudaSuccess) return fail(e);
     s->post_ws_bytes = gwi_triggers_workspace_bytes(s->sub);
     if ((e = cudaMalloc(&s->d_post_ws, s->post_ws_bytes)) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_trig, (size_t)capacity * sizeof(gwi_trigger))) != cudaSuccess) return fail(e);
@@ -382,6 +401,7 @@ extern "C" void gwi_stream_destroy(gwi_stream* s)
     if (s->d_tmp) cudaFree(s->d_tmp);
     if (s->d_prob) cudaFree(s->d_prob);
     if (s->d_carry) cudaFree(s->d_carry);
+    if (s->d_carry_pm) cudaFree(s->d_carry_pm);
     if (s->d_post_ws) cudaFree(s->d_post_ws);
     if (s->d_trig) cudaFree(s->d_trig);
     if (s->d_count) cudaFree(s->d_count);
@@ -530,6 +550,11 @@ extern "C" gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, 
         GWI_CUDA_CHECK(cudaMemcpyAsync(recs.data(), s->d_trig, (size_t)have * sizeof(gwi_trigger), cudaMemcpyDeviceToHost, st));
         GWI_CUDA_CHECK(cudaStreamSynchronize(st));
     }
+    if (s->rule == GWI_RULE_PER_MODEL)
+        for (auto& r : recs) {
+            r.model_mask = 1 << (r.slide >> 20);
+            r.slide &= (1 << 20) - 1;
+        }
     // records arrive grouped by sub-chunk; the list is sorted by (slide, start)
     std::stable_sort(recs.begin(), recs.end(), [](const gwi_trigger& a, const gwi_trigger& b) {
         return a.slide != b.slide ? a.slide < b.slide : a.start < b.start;
@@ -546,3 +571,73 @@ extern "C" gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, 
 }
 
 extern "C" int64_t gwi_stream_samples_done(const gwi_stream* s) { return s ? s->t_done : -1; }
+
+extern "C" gwi_status gwi_stream_set_rule(gwi_stream* s, gwi_rule rule)
+{
+    if (!s || (rule != GWI_RULE_MEAN && rule != GWI_RULE_PER_MODEL) || s->t_done != 0) {
+        gwi_set_error("gwi_stream_set_rule: bad argument (must be called before the first push)");
+        return GWI_ERR_ARG;
+    }
+    s->rule = (int)rule;
+    return GWI_OK;
+}
+
+// Host-side coincidence of per-model triggers (include/gwi.h; reading A34).  Two-pointer sweeps over the per-model end
+// lists, O(n log n) for the sorts.
+extern "C" gwi_status gwi_coincidence(const gwi_trigger* h_triggers, int32_t n_triggers, int32_t n_models, int64_t window,
+                                      gwi_event* h_events, int32_t capacity, int32_t* n_events)
+{
+    if (n_triggers < 0 || (n_triggers > 0 && !h_triggers) || n_models < 1 || n_models > GWI_MAX_MODELS || window < 0 ||
+        capacity < 0 || (capacity > 0 && !h_events) || !n_events) {
+        gwi_set_error("gwi_coincidence: bad argument");
+        return GWI_ERR_ARG;
+    }
+    std::vector<int32_t> slides;
+    for (int i = 0; i < n_triggers; i++) slides.push_back(h_triggers[i].slide);
+    std::sort(slides.begin(), slides.end());
+    slides.erase(std::unique(slides.begin(), slides.end()), slides.end());
+    int64_t total = 0;
+    for (int32_t sl : slides) {
+        std::vector<std::vector<int64_t>> ends(n_models);
+        std::vector<int64_t> all;
+        for (int i = 0; i < n_triggers; i++) {
+            const gwi_trigger& t = h_triggers[i];
+            if (t.slide != sl) continue;
+            for (int m = 0; m < n_models; m++)
+                if (t.model_mask & (1 << m)) ends[m].push_back(t.end);
+            all.push_back(t.end);
+        }
+        for (auto& e : ends) std::sort(e.begin(), e.end());
+        std::sort(all.begin(), all.end());
+        // anchors: ends a such that every model has an end in [a, a + window]
+        std::vector<int64_t> anchors;
+        for (int64_t a : all) {
+            bool ok = true;
+            for (int m = 0; m < n_models && ok; m++) {
+                auto it = std::lower_bound(ends[m].begin(), ends[m].end(), a);
+                ok = it != ends[m].end() && *it <= a + window;
+            }
+            if (ok && (anchors.empty() || anchors.back() != a)) anchors.push_back(a);
+        }
+        size_t i = 0;
+        while (i < anchors.size()) {
+            int64_t first = anchors[i], last = anchors[i];
+            while (i + 1 < anchors.size() && anchors[i + 1] - last <= window) last = anchors[++i];
+            i++;
+            auto lo = std::lower_bound(all.begin(), all.end(), first);
+            auto hi = std::upper_bound(all.begin(), all.end(), last + window);
+            if (total < capacity) {
+                gwi_event ev;
+                ev.t_first = first, ev.t_last = *(hi - 1), ev.n_triggers = (int32_t)(hi - lo), ev.slide = sl;
+                h_events[total] = ev;
+            }
+            total++;
+        }
+    }
+    *n_events = (int32_t)total;
+    if (total > capacity) {
+        gwi_set_error("gwi_coincidence: %lld events > capacity %d", (long long)total, capacity);
+        return GWI_ERR_CAPACITY;
+    }
+    return GWI_OK;
+}

@@ -254,3 +254,45 @@ def test_stream_paper_scale_tensor_core_back_end(tmpdir_s):
     assert np.array_equal(p0, p1)
     assert trig_tuples(r0) == trig_tuples(r1)
     assert trig_tuples(r0) == _oracle_triggers(p0.astype(np.float64), float(np.float32(0.5)), 16)
+
+
+def test_per_model_rule_and_coincidence(tmpdir_s):
+    """The paper's decision rule (reading A34) end to end: per-model triggers from the stream in
+    GWI_RULE_PER_MODEL mode, all-model coincidence on the host, against the oracle on the same probabilities."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1, 2], gwi.FP16)
+    N = 30000
+    x = gs.stream_noise(41, 0, N, dtype=np.float16)
+    st = gwi.Stream(gms, N, 7000, 0.5, 3, lags=[4096], capacity=1 << 16, want_pbar=True, rule=gwi.RULE_PER_MODEL)
+    import torch
+    xt = torch.from_numpy(x)
+    st.prime(xt[1, N - st.tail_samples:].contiguous())
+    pos = 0
+    for n in _ragged(N, 9, 500, 7000):
+        st.push(xt[0, pos:pos + n].contiguous().cuda(), xt[1, pos:pos + n].contiguous().cuda())
+        pos += n
+    cnt, recs = st.finish()
+    p = st.pbar.cpu().numpy()                                   # [slide][model][N]
+    st.close()
+    assert cnt == len(recs) and cnt > 10
+    # per-model probabilities against the oracle's definition
+    for m, om in enumerate(oms):
+        p0, u = om.stream(x.astype(np.float64), want_u=True)
+        assert np.max(np.abs(p[0, m] - p0)) <= 2e-3
+        assert np.max(np.abs(p[1, m] - om.head_slide(u, 4096))) <= 2e-3
+    # threshold at each model's own median so that every model has many runs
+    # (records were produced with theta = 0.5; compare those against the oracle's clustering of the same arrays)
+    want_recs = []
+    for k in range(2):
+        for m in range(3):
+            _, rr = gwo.triggers(p[k, m].astype(np.float64), float(np.float32(0.5)), 3, slide=k)
+            want_recs += [(k, 1 << m, r[1], r[2]) for r in rr]
+    got_recs = sorted((r.slide, r.model_mask, r.start, r.end) for r in recs)
+    assert got_recs == sorted(want_recs)
+    # coincidence within 0.5 s
+    ev = gwi.coincidence(recs, 3, 2048)
+    want_ev = []
+    for k in range(2):
+        ends = [[r[3] for r in want_recs if r[0] == k and r[1] == 1 << m] for m in range(3)]
+        want_ev += [(k,) + e for e in gwo.coincidence(ends, 2048, slide=k)]
+    assert [(e.slide, e.t_first, e.t_last, e.n_triggers) for e in ev] == want_ev

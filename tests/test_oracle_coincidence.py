@@ -71,3 +71,25 @@ def test_p17_tuple_brute_force_and_invariances():
         wide = gwo.coincidence(ends, W + 5)
         for a, b, _ in ev:
             assert any(a2 <= a and b <= b2 for a2, b2, _ in wide)
+
+
+def test_library_coincidence_matches_oracle_on_host():
+    """gwi_coincidence is a host function (two-pointer sweeps): exact agreement with the oracle's O(n^2) definition on
+    random per-model trigger lists, several slides, records in random order."""
+    import paper_2201_11133_b200 as gwi
+    rs = np.random.RandomState(11)
+    for trial in range(100):
+        M = int(rs.randint(1, 5))
+        W = int(rs.randint(0, 60))
+        recs, want = [], []
+        for slide in range(int(rs.randint(1, 4))):
+            ends = _rand_ends(rs, M, 8, 300)
+            for m, e in enumerate(ends):
+                for v in e:
+                    recs.append(gwi.Trigger(slide=slide, model_mask=1 << m, start=v - 5, end=v, peak_p=1.0, mean_p=1.0))
+            want += [(slide,) + ev for ev in gwo.coincidence(ends, W, slide=slide)]
+        rs.shuffle(recs)
+        got = [(e.slide, e.t_first, e.t_last, e.n_triggers) for e in gwi.coincidence(recs, M, W)]
+        assert got == want
+    with np.testing.assert_raises(gwi.GwiError):
+        gwi.coincidence([], 0, 5)
