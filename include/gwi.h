@@ -192,6 +192,19 @@ gwi_status gwi_coincidence(const gwi_trigger* h_triggers, int32_t n_triggers, in
                            gwi_event* h_events, int32_t capacity, int32_t* n_events);
 void gwi_stream_destroy(gwi_stream* s);
 
+/* ---- trigger counts at many thresholds in one pass (ROC sweep) ---------------
+ * counts[j] = number of maximal runs of the ensemble mean (same fixed fp32 expression as gwi_ensemble_triggers) that are
+ * strictly above thresholds[j] for at least min_len samples, for a WHOLE stream of N samples (no chunk carry).
+ * d_prob: HOST array of n_models DEVICE pointers to [N] float.  d_thresholds: DEVICE [n_thresholds] float, ascending,
+ * 1 <= n_thresholds <= 1024.  d_counts: DEVICE [n_thresholds] int64.  1 <= min_len <= 16384.
+ * d_workspace: DEVICE, >= gwi_sweep_workspace_bytes(n_thresholds), 256 B aligned.
+ * Method: one sliding-window minimum m[t] over min_len samples; count(theta) = rising edges of (m > theta).
+ * Errors: GWI_ERR_ARG, GWI_ERR_NOMEM, GWI_ERR_UNSUPPORTED (min_len > 16384), GWI_ERR_CUDA. */
+size_t gwi_sweep_workspace_bytes(int32_t n_thresholds);
+gwi_status gwi_threshold_sweep(const float* const* d_prob, int32_t n_models, int64_t N, const float* d_thresholds,
+                               int32_t n_thresholds, int64_t min_len, int64_t* d_counts, void* d_workspace,
+                               size_t workspace_bytes, void* cuda_stream);
+
 /* ---- misc ---------------------------------------------------------------------------------------------- */
 const char* gwi_last_error(void);
 int gwi_version(void);

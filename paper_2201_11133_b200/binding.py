@@ -14,7 +14,7 @@ EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_m
                     "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
                     "gwi_stream_tail_samples", "gwi_stream_prime", "gwi_stream_push", "gwi_stream_push_host",
                     "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_destroy", "gwi_stream_set_rule",
-                    "gwi_coincidence"]
+                    "gwi_coincidence", "gwi_sweep_workspace_bytes", "gwi_threshold_sweep"]
 
 
 class GwiError(RuntimeError):
@@ -83,6 +83,10 @@ def lib():
     L.gwi_stream_set_rule.argtypes = [vp, C.c_int]
     L.gwi_coincidence.restype = C.c_int
     L.gwi_coincidence.argtypes = [vp, C.c_int32, C.c_int32, C.c_int64, vp, C.c_int32, i32p]
+    L.gwi_sweep_workspace_bytes.restype = C.c_size_t
+    L.gwi_sweep_workspace_bytes.argtypes = [C.c_int32]
+    L.gwi_threshold_sweep.restype = C.c_int
+    L.gwi_threshold_sweep.argtypes = [C.POINTER(vp), C.c_int32, C.c_int64, vp, C.c_int32, C.c_int64, vp, vp, C.c_size_t, vp]
     L.gwi_last_error.restype = C.c_char_p
     L.gwi_version.restype = C.c_int
     L.gwi_launch_count.restype = C.c_int64
@@ -197,6 +201,21 @@ def ensemble_triggers(probs, threshold, min_len, t0=0, slide_id=0, last_chunk=Tr
         e.count, e.records = n, recs
         raise e
     return n, recs, pbar
+
+
+def threshold_sweep(probs, thresholds, min_len):
+    """gwi_threshold_sweep: probs = list of [N] float32 device tensors, thresholds ascending -> int64 device tensor [K]."""
+    dev = probs[0].device
+    probs = [p.contiguous() for p in probs]
+    N = probs[0].numel()
+    ptrs = (C.c_void_p * len(probs))(*[p.data_ptr() for p in probs])
+    th = torch.as_tensor(thresholds, dtype=torch.float32).to(dev).contiguous()
+    K = th.numel()
+    counts = torch.zeros(K, dtype=torch.int64, device=dev)
+    ws = torch.empty(max(lib().gwi_sweep_workspace_bytes(K), 256), dtype=torch.uint8, device=dev)
+    _check(lib().gwi_threshold_sweep(ptrs, len(probs), N, C.c_void_p(th.data_ptr()), K, int(min_len),
+                                     C.c_void_p(counts.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(dev)))
+    return counts
 
 
 def new_carry(device=0):

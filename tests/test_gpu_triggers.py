@@ -113,3 +113,20 @@ def test_capacity_overflow_gives_valid_prefix():
         _gpu(ps, 0.5, 8, capacity=7)
     assert e.value.status == 7 and e.value.count == n
     assert trig_tuples(e.value.records) == [(r[0], r[1], r[2]) for r in recs[:7]]
+
+
+@pytest.mark.parametrize("N,lmin,M", [(1, 1, 1), (10, 11, 2), (5000, 1, 4), (100003, 100, 4), (300000, 2048, 4),
+                                      (40000, 4097, 3), (70000, 16384, 2), (1 << 20, 2048, 4)])
+def test_threshold_sweep_equals_per_threshold_clustering(N, lmin, M):
+    """gwi_threshold_sweep (one sliding-window-minimum pass) against the oracle's trigger count at every threshold."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    ps = _noisy(N + lmin + M, N, M=M, corr=max(16, min(lmin // 2, 700)))
+    pb = gwo.ensemble_mean_f32(ps).astype(np.float64)
+    th = np.unique(np.concatenate([np.linspace(0.0, 0.9998, 97), [0.3, 0.5, 0.7, float(pb.min()), float(pb.max())]])
+                   .astype(np.float32))
+    got = gwi.threshold_sweep([torch.from_numpy(p).cuda() for p in ps], th, lmin).cpu().numpy()
+    want = [gwo.triggers(pb, float(t), lmin, cap=1)[0] for t in th]
+    assert got.tolist() == want
+    if N >= 5000:
+        assert max(want) > 0
