@@ -11,9 +11,10 @@
 // For sorted thresholds an edge from m[t-1] to m[t] > m[t-1] raises exactly the thresholds theta_j with
 // m[t-1] <= theta_j < m[t]: a range, recorded in a difference array and prefix-summed at the end.
 //
-// k_sweep: each CTA loads TT + L_min - 1 samples of the ensemble mean (fixed fp32 expression, as in gwi_post.cu) into
-// shared memory, builds the window minimum by doubling (min over 2^k, then two overlapping 2^k windows), and scans
-// its outputs for rising edges.  HBM-bound: 4 M bytes per sample, read (1 + (L_min - 1) / TT) times.
+// k_sweep / k_sweep_vh: each CTA loads TT + L_min samples of the ensemble mean (fixed fp32 expression, as in
+// gwi_post.cu) into shared memory, builds the window minimum (k_sweep: by doubling, min over 2^k then two overlapping
+// 2^k windows; k_sweep_vh: prefix / suffix minima per block of L_min), and scans its outputs for rising edges.
+// HBM-bound by design: 4 M bytes per sample, read (1 + L_min / TT) times.
 #include "gwi_internal.h"
 
 namespace {
@@ -75,8 +76,129 @@ __global__ void __launch_bounds__(SW_THREADS) k_sweep(SwPtrs P, int M, int64_t N
     for (int o = threadIdx.x; o < (int)(t_hi - t_lo); o += SW_THREADS) {
         const int e = L + o;                                     // a-index of output t = t_lo + o
         const float cur_m = wmin(e);
-        int i0 = 0;
-        if (t_lo + o > L - 1) i0 = idx(wmin(e - 1));             // the very first window has no predecessor
+        const bool first = !(t_lo + o > L - 1);                  // the very first window has no predecessor
+        const float prev_m = first ? -INFINITY : wmin(e - 1);
+        if (!(cur_m > prev_m)) continue;                         // only a rising minimum can raise a threshold
+        const int i0 = first ? 0 : idx(prev_m);
+        const int i1 = idx(cur_m);
+        if (i1 > i0) {
+            atomicAdd(&diff[i0], 1);
+            atomicAdd(&diff[i1], -1);
+        }
+    }
+}
+
+// van Herk / Gil-Werman form for long windows: the tile is cut into blocks of L samples; G = prefix minimum inside each
+// block, H = suffix minimum inside each block; the window [e - L + 1, e] spans at most two blocks, so
+// m = min(H[e - L + 1], G[e]).  One warp per (block, direction): every lane scans its own contiguous chunk twice
+// (chunk minimum, warp scan of the 32 chunk minima, then the running minimum).  The arrays are padded by one word per
+// 32 so that the lanes' strided chunk walks spread over the banks.
+__device__ __forceinline__ int padi(int j) { return j + (j >> 5); }
+
+__global__ void __launch_bounds__(SW_THREADS) k_sweep_vh(SwPtrs P, int M, int64_t N, int L, int TT, const float* __restrict__ thr, int K,
+                                                         int* __restrict__ diff, int vec)
+{
+    extern __shared__ float sm[];
+    constexpr int OFF = 3;               // a-index 0 is sample blockIdx * TT - 4: 16-byte aligned tiles when TT % 4 == 0
+    const int cap = padi(TT + L + OFF) + 1;
+    float* G = sm;
+    float* H = sm + cap;
+    float* th = H + cap;
+    const int64_t t_lo = (int64_t)blockIdx.x * TT + (L - 1);
+    if (t_lo >= N) return;
+    const int64_t t_hi = min(t_lo + TT, N);
+    const int64_t base = t_lo - L - OFF;                         // sample index of a-index 0
+    const int len = (int)(t_hi - base);
+    const float fM = (float)M;
+    for (int i = threadIdx.x; i < K; i += SW_THREADS) th[i] = thr[i];
+    if (vec) {
+        // four samples per thread and load instruction (all pointers 16-byte aligned, TT % 4 == 0)
+        for (int i4 = threadIdx.x; 4 * i4 < len; i4 += SW_THREADS) {
+            const int64_t t = base + 4 * i4;
+            float v[4] = {INFINITY, INFINITY, INFINITY, INFINITY};
+            if (t >= 0 && t + 3 < N) {
+                float4 s = *reinterpret_cast<const float4*>(P.p[0] + t);
+                for (int j = 1; j < M; j++) {
+                    float4 q = *reinterpret_cast<const float4*>(P.p[j] + t);
+                    s.x = __fadd_rn(s.x, q.x), s.y = __fadd_rn(s.y, q.y), s.z = __fadd_rn(s.z, q.z), s.w = __fadd_rn(s.w, q.w);
+                }
+                v[0] = __fdiv_rn(s.x, fM), v[1] = __fdiv_rn(s.y, fM), v[2] = __fdiv_rn(s.z, fM), v[3] = __fdiv_rn(s.w, fM);
+            } else {
+                for (int e = 0; e < 4; e++)
+                    if (t + e >= 0 && t + e < N) {
+                        float s = P.p[0][t + e];
+                        for (int j = 1; j < M; j++) s = __fadd_rn(s, P.p[j][t + e]);
+                        v[e] = __fdiv_rn(s, fM);
+                    }
+            }
+            for (int e = 0; e < 4; e++)
+                if (4 * i4 + e < len) G[padi(4 * i4 + e)] = v[e], H[padi(4 * i4 + e)] = v[e];
+        }
+    } else {
+#pragma unroll 4
+        for (int i = threadIdx.x; i < len; i += SW_THREADS) {
+            int64_t t = base + i;
+            float v = INFINITY;
+            if (t >= 0) {
+                float s = P.p[0][t];
+                for (int j = 1; j < M; j++) s = __fadd_rn(s, P.p[j][t]);
+                v = __fdiv_rn(s, fM);
+            }
+            G[padi(i)] = v;
+            H[padi(i)] = v;
+        }
+    }
+    __syncthreads();
+    {
+        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        const int nbk = (len - OFF + L - 1) / L, C = (L + 31) / 32;
+        for (int task = warp; task < 2 * nbk; task += SW_THREADS / 32) {
+            const int q = task >> 1, back = task & 1;
+            const int b0 = OFF + q * L, b1 = min(b0 + L, len);         // block [b0, b1)
+            const int c0 = min(b0 + lane * C, b1), c1 = min(c0 + C, b1);   // this lane's chunk [c0, c1)
+            float* A = back ? H : G;
+            float tot = INFINITY;
+            for (int j = c0; j < c1; j++) tot = fminf(tot, A[padi(j)]);
+            // exclusive scan of the chunk minima over the lanes (forward: lanes below, backward: lanes above)
+            float inc = tot;
+            for (int o = 1; o < 32; o <<= 1) {
+                float v = back ? __shfl_down_sync(0xffffffffu, inc, o) : __shfl_up_sync(0xffffffffu, inc, o);
+                if (back ? (lane + o < 32) : (lane >= o)) inc = fminf(inc, v);
+            }
+            float carry = back ? __shfl_down_sync(0xffffffffu, inc, 1) : __shfl_up_sync(0xffffffffu, inc, 1);
+            if (back ? lane == 31 : lane == 0) carry = INFINITY;
+            float run = carry;
+            if (!back) {
+                for (int j = c0; j < c1; j++) {
+                    run = fminf(run, A[padi(j)]);
+                    A[padi(j)] = run;
+                }
+            } else {
+                for (int j = c1 - 1; j >= c0; j--) {
+                    run = fminf(run, A[padi(j)]);
+                    A[padi(j)] = run;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    auto wmin = [&](int e) { return fminf(H[padi(e - L + 1)], G[padi(e)]); };
+    auto idx = [&](float v) {
+        int lo = 0, hi = K;
+        while (lo < hi) {
+            int mid = (lo + hi) >> 1;
+            if (th[mid] < v) lo = mid + 1;
+            else hi = mid;
+        }
+        return lo;
+    };
+    for (int o = threadIdx.x; o < (int)(t_hi - t_lo); o += SW_THREADS) {
+        const int e = OFF + L + o;
+        const float cur_m = wmin(e);
+        const bool first = !(t_lo + o > L - 1);                  // the very first window has no predecessor
+        const float prev_m = first ? -INFINITY : wmin(e - 1);
+        if (!(cur_m > prev_m)) continue;                         // only a rising minimum can raise a threshold
+        const int i0 = first ? 0 : idx(prev_m);
         const int i1 = idx(cur_m);
         if (i1 > i0) {
             atomicAdd(&diff[i0], 1);
@@ -129,12 +251,24 @@ extern "C" gwi_status gwi_threshold_sweep(const float* const* d_prob, int32_t n_
     const int L = (int)min_len;
     if (N >= L) {
         // 2 (TT + L) floats + thresholds: two CTAs per SM (2 x ~108 KB) when the window allows, else one
-        const int TT = ((L <= 6144 ? 13500 : 27000) - L) / 256 * 256;
-        size_t smem = (size_t)(2 * (TT + L) + n_thresholds) * sizeof(float);
-        GWI_CUDA_CHECK(cudaFuncSetAttribute(k_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        const int budget = L <= 6144 ? 13000 : 26000;
         int64_t nout = N - (L - 1);
-        unsigned grid = (unsigned)((nout + TT - 1) / TT);
-        k_sweep<<<grid, SW_THREADS, smem, st>>>(P, n_models, N, L, TT, d_thresholds, n_thresholds, diff);
+        if (L >= 256 && L <= 8192) {
+            // long windows: prefix / suffix minima per block of L, TT a multiple of L (>= L for these L)
+            const int TT = (budget - L) / L * L;
+            size_t smem = (size_t)(2 * ((TT + L + 3) + ((TT + L + 3) >> 5) + 1) + n_thresholds) * sizeof(float);
+            int vec = (TT & 3) == 0;
+            for (int j = 0; j < n_models; j++) vec = vec && (((uintptr_t)d_prob[j] & 15) == 0);
+            GWI_CUDA_CHECK(cudaFuncSetAttribute(k_sweep_vh, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            unsigned grid = (unsigned)((nout + TT - 1) / TT);
+            k_sweep_vh<<<grid, SW_THREADS, smem, st>>>(P, n_models, N, L, TT, d_thresholds, n_thresholds, diff, vec);
+        } else {
+            const int TT = (budget - L) / 256 * 256;
+            size_t smem = (size_t)(2 * (TT + L) + n_thresholds) * sizeof(float);
+            GWI_CUDA_CHECK(cudaFuncSetAttribute(k_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            unsigned grid = (unsigned)((nout + TT - 1) / TT);
+            k_sweep<<<grid, SW_THREADS, smem, st>>>(P, n_models, N, L, TT, d_thresholds, n_thresholds, diff);
+        }
         gwi_count_launch(1);
     }
     k_sweep_scan<<<1, 32, 0, st>>>(diff, n_thresholds, d_counts);
