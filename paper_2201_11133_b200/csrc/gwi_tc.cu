@@ -719,7 +719,17 @@ void gwi_tc_free(gwi_model* m)
     m->tc = nullptr;
 }
 
-static int64_t tc_chunk(int64_t B) { return B < 1024 ? B : 1024; }
+// Windows per launch: the u workspace (32 KB per window-branch-tile) is bounded to ~16 GiB; a batch is cut into equal
+// launches so that no launch is left with a handful of windows (one job is a whole window pair: a short launch would
+// run on a few SMs for as long as a full one).
+static int64_t tc_chunk(int64_t B, int nb, int64_t ntiles)
+{
+    int64_t cap = (16LL << 30) / ((int64_t)nb * ntiles * U_TILE_BYTES);
+    if (cap < 296) cap = 296;
+    if (B <= cap) return B;
+    int64_t launches = (B + cap - 1) / cap;
+    return (B + launches - 1) / launches;
+}
 
 size_t gwi_tc_workspace_bytes(const gwi_model* m, int64_t B, int32_t T)
 {
@@ -727,7 +737,7 @@ size_t gwi_tc_workspace_bytes(const gwi_model* m, int64_t B, int32_t T)
     int64_t ntiles = (T + TM - 1) / TM;
     size_t ring = (size_t)p->num_sms * 2 * p->meta.ring_tiles * PST_BYTES;
     size_t ring64 = (size_t)p->num_sms * 2 * p->meta.n64 * 2 * PRE_BYTES;
-    size_t u = (size_t)tc_chunk(B) * m->arch.n_branch * ntiles * U_TILE_BYTES;
+    size_t u = (size_t)tc_chunk(B, m->arch.n_branch, ntiles) * m->arch.n_branch * ntiles * U_TILE_BYTES;
     return ring + ring64 + u + 512;
 }
 
@@ -742,7 +752,7 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
     uint8_t* ring = (uint8_t*)d_ws;
     uint8_t* ring64 = ring + ring_bytes;
     uint8_t* u = ring64 + ring64_bytes;
-    const int64_t Bc = tc_chunk(B);
+    const int64_t Bc = tc_chunk(B, nb, ntiles);
     for (int64_t w0 = 0; w0 < B; w0 += Bc) {
         const int64_t nwin = (B - w0 < Bc) ? B - w0 : Bc;
         StackArgs sa;
