@@ -26,19 +26,11 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
 __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;
-#ifdef GWI_WAIT_HINT
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(bar), "r"(parity), "r"((uint32_t)GWI_WAIT_HINT)
-        : "memory");
-#else
     asm volatile(
         "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(ok)
         : "r"(bar), "r"(parity)
         : "memory");
-#endif
     return ok != 0;
 }
 // non-blocking test (for the MMA issuer, which polls the barriers of both slots)
@@ -56,11 +48,7 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t spins = 0;
-#ifdef GWI_SPIN_TEST
-    while (!mbar_test(bar, parity)) {
-#else
     while (!mbar_try_wait(bar, parity)) {
-#endif
         if (++spins > (1u << 26)) __trap();
     }
 }
