@@ -95,3 +95,18 @@ def test_full_batch_sampled_against_oracle(tmpdir_s):
     sel = sorted({0, 1, 295, 296, 511, 1022, 1023, int(inj[0]), int(inj[-1])})
     want = om.infer_windows(x[sel].astype(np.float64))
     assert np.max(np.abs(got[sel] - want)) <= TOL16
+
+
+def test_repeated_launches_are_bitwise_identical(tmpdir_s):
+    """The kernel's barrier protocol leaves no room for a data race to change a result: the same batch through
+    gwi_infer several times, with another shape in between, gives bit-identical probabilities."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    a = gs.PAPER_ARCH
+    om, gm = model_pair(tmpdir_s, "tc_rep", a, gs.xavier_tensors(a, 5, bias="random"), gwi.FP16)
+    x = torch.from_numpy(rand_windows(9, 300, 1100, dtype=np.float16)).cuda()
+    y = torch.from_numpy(rand_windows(10, 7, 260, dtype=np.float16)).cuda()
+    ref = gm.infer(x).clone()
+    for _ in range(4):
+        gm.infer(y)
+        assert torch.equal(gm.infer(x), ref)
