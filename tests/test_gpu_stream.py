@@ -296,3 +296,19 @@ def test_per_model_rule_and_coincidence(tmpdir_s):
         ends = [[r[3] for r in want_recs if r[0] == k and r[1] == 1 << m] for m in range(3)]
         want_ev += [(k,) + e for e in gwo.coincidence(ends, 2048, slide=k)]
     assert [(e.slide, e.t_first, e.t_last, e.n_triggers) for e in ev] == want_ev
+
+
+def test_config3_recipe_32_slides(tmpdir_s):
+    """BASELINE.json configs[3] recipe at a size the oracle finishes: coloured-then-whitened noise (reading A27), the
+    4-model ensemble, circular lags k x 1 s for k = 1..32 (reading A24, A25), all slides in one pass."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1, 2, 3], gwi.FP16)
+    N = 33 * 4096 + 1234
+    x = np.stack([gs.coloured_whitened_noise(2 + d, d, N, seg_len=1 << 16) for d in range(2)])
+    assert x.dtype == np.float16 and abs(float(x.astype(np.float64).std()) - 1.0) < 0.05
+    lags = [k * 4096 for k in range(1, 33)]
+    want = _oracle_slides(oms, x, lags)
+    n, recs, pbar = _run_stream(gms, x, _ragged(N, 12, 9000, 40000), lags, 0.5, 64, max_chunk=40000)
+    assert np.max(np.abs(pbar - want)) <= 2e-3
+    got = trig_tuples(recs)
+    assert got == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 64) and got == sorted(got)
