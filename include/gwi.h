@@ -110,8 +110,8 @@ size_t gwi_triggers_workspace_bytes(int64_t N);
  *          before the first chunk; it carries the open run across calls on consecutive chunks.
  * last_chunk != 0: a run still open at the end of this chunk is closed there (reading A21).
  * d_triggers / d_count: device; records sorted by start; *d_count = number of qualifying runs closed by this
- *          call (may exceed capacity; then only the first `capacity` are written and the status, reported by
- *          gwi_triggers_status after synchronising, is GWI_ERR_CAPACITY).
+ *          call (may exceed capacity; then only the first `capacity` are written: the call itself is asynchronous and
+ *          returns GWI_OK, the caller compares *d_count with capacity after synchronising the stream).
  * d_pbar: optional device [N] float, receives the mean probability (NULL: not written).
  * 1 <= n_models <= 16, N >= 1.  Errors: GWI_ERR_ARG, GWI_ERR_NOMEM, GWI_ERR_CUDA. */
 gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0,
