@@ -130,8 +130,9 @@ gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t n_models, i
  *   gives bit-identical results to pushing it whole (reading A17).
  *
  * Back ends (chosen at create, same results contract): FP16-mode ensembles of the narrow config-1 architecture run on a
- * fused kernel; FP16-mode paper-scale models without slides run on the tcgen05 kernel over segments with recomputed
- * warm-up; everything else (FP32 mode, other architectures, slides on paper-scale models) runs on the generic kernels.
+ * fused kernel; FP16-mode paper-scale models run on the tcgen05 kernel over segments with recomputed warm-up (with
+ * slides when the lags and n_total are multiples of 128 samples and n_total >= max lag + R_f - 1); everything else
+ * (FP32 mode, other architectures) runs on the generic kernels.
  *
  * gwi_stream_create   models: HOST array of n_models loaded models sharing device, precision and architecture
  *                     (1..16).  lags: HOST array of n_lags lags in SAMPLES, each in [1, n_total) (n_lags = 0: zero lag

@@ -67,6 +67,14 @@ struct gwi_stream {
     float* d_segp = nullptr;                // [B][segT] probabilities of the batch
     void* d_tcws = nullptr;
     size_t tcws_bytes = 0;
+    // ... with time slides (lags, n_total multiples of 128): incoming chunks are re-blocked into whole segments, the L1
+    // feature tiles of the last max-lag samples are kept as history, one head launch per lag on the u tiles
+    bool tcs = false;
+    int Rt = 0;                             // history tiles = maxlag / 128
+    __half* d_acc = nullptr;                // [2][acc_cap] samples received but not yet processed (+ the new chunk)
+    int64_t acc_cap = 0, pend = 0, t_recv = 0;
+    std::vector<uint8_t*> d_hist_t[2];      // per model [R][32 KB] L1 feature tiles that precede the next block, ping-pong
+    int hist_t_cur = 0;
 };
 
 namespace {
@@ -103,7 +111,27 @@ __global__ void k_seg_scatter(const float* __restrict__ pb, int n, int SEG, int 
     prob[i] = pb[(int64_t)w * T + t];
 }
 
+// history of L1 feature tiles: new[i] = tile (nq - R + i) of the block just processed (branch 1, segment layout), or the
+// old history when that index is negative
+__global__ void k_hist_tiles(const uint8_t* __restrict__ u, int ntiles, int64_t nq, int R, int seg_tiles, int warm_tiles,
+                             int stream_start, const uint8_t* __restrict__ hold, uint8_t* __restrict__ hnew)
+{
+    const int64_t i = blockIdx.x, q = nq - R + i;
+    const uint8_t* src;
+    if (q >= 0) {
+        const int64_t w = q / seg_tiles, tl = q % seg_tiles + ((w == 0 && stream_start) ? 0 : warm_tiles);
+        src = u + ((size_t)(w * 2 + 1) * ntiles + tl) * 32768;
+    } else {
+        src = hold + (size_t)(i + nq) * 32768;
+    }
+    const uint4* s4 = reinterpret_cast<const uint4*>(src);
+    uint4* d4 = reinterpret_cast<uint4*>(hnew + (size_t)i * 32768);
+    for (int k = threadIdx.x; k < 2048; k += blockDim.x) d4[k] = s4[k];
+}
+
 size_t elt(const gwi_stream* s) { return s->half_in ? 2 : 4; }
+
+gwi_status post_block(gwi_stream* s, int n, bool last, cudaStream_t st);
 
 // one sub-chunk of n <= sub samples, already in staging buffer `xb` at column `x0`
 gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStream_t st)
@@ -112,7 +140,7 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
     const char* x = (const char*)s->d_x[xb] + (size_t)x0 * elt(s);
     for (int m = 0; m < s->M; m++) {
         const gwi_model* gm = s->models[m];
-        float* skip0 = (s->tiny || s->tcb) ? nullptr : s->d_skip[m] + s->maxlag;
+        float* skip0 = (s->tiny || s->tcb || s->tcs) ? nullptr : s->d_skip[m] + s->maxlag;
         gwi_status rc;
         if (s->tcb) {
             const int B = (n + s->seg - 1) / s->seg;
@@ -168,6 +196,13 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
     }
     s->hist_cur ^= 1;
     s->xh_cur ^= 1;
+    return post_block(s, n, last, st);
+}
+
+// ensemble mean / per-model rule, threshold, clustering of one processed block for every slide; advances t_done
+gwi_status post_block(gwi_stream* s, int n, bool last, cudaStream_t st)
+{
+    const int nslides = (int)s->lags.size();
     if (s->rule == GWI_RULE_PER_MODEL) {
         // the paper's rule: every model thresholded and clustered on its own; slide k and model m are
         // packed into the record's slide field (k | m << 20) and unpacked at finish
@@ -207,13 +242,77 @@ gwi_status run_chunk(gwi_stream* s, int xb, int64_t n, cudaStream_t st)
     return GWI_OK;
 }
 
+// ---- tensor-core back end with time slides: one block of n samples (whole segments, or the stream's last samples) that
+// sit at the front of d_acc
+gwi_status tcs_block(gwi_stream* s, int n, bool last, cudaStream_t st)
+{
+    const int nslides = (int)s->lags.size();
+    const int B = (n + s->seg - 1) / s->seg, start = s->t_done == 0 ? 1 : 0;
+    const int ntiles = s->segT / 128, seg_tiles = s->seg / 128, warm_tiles = s->segH / 128;
+    const int64_t nq = (n + 127) / 128, total = (int64_t)B * s->segT;
+    k_seg_gather<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(s->d_acc, s->acc_cap, s->d_xh[s->xh_cur], n, s->seg, s->segH, s->segT,
+                                                                 start, s->d_segx, total);
+    gwi_count_launch(1);
+    gwi_status rc = gwi_xhist_update(s->d_acc, s->acc_cap, n, s->segH, s->d_xh[s->xh_cur], s->d_xh[s->xh_cur ^ 1], st);
+    if (rc != GWI_OK) return rc;
+    s->xh_cur ^= 1;
+    for (int m = 0; m < s->M; m++) {
+        const uint8_t* u = nullptr;
+        rc = gwi_tc_stack(s->models[m], (const __half*)s->d_segx, B, s->segT, s->d_tcws, s->tcws_bytes, st, &u);
+        if (rc != GWI_OK) return rc;
+        for (int k = 0; k < nslides; k++) {
+            rc = gwi_tc_head_stream(s->models[m], u, ntiles, s->d_hist_t[s->hist_t_cur][m], s->Rt, nq, s->lags[k] / 128, seg_tiles,
+                                    warm_tiles, start, n, s->d_prob + ((size_t)k * s->M + m) * s->sub, st);
+            if (rc != GWI_OK) return rc;
+        }
+        if (s->Rt > 0) {
+            k_hist_tiles<<<s->Rt, 256, 0, st>>>(u, ntiles, nq, s->Rt, seg_tiles, warm_tiles, start, s->d_hist_t[s->hist_t_cur][m],
+                                               s->d_hist_t[s->hist_t_cur ^ 1][m]);
+            gwi_count_launch(1);
+        }
+    }
+    s->hist_t_cur ^= 1;
+    GWI_CUDA_CHECK(cudaGetLastError());
+    return GWI_OK;
+}
+
+// appends the n samples of staging buffer xb to the pending ones and processes every whole segment (everything at the end
+// of the stream); what is left moves to the front
+gwi_status tcs_append_and_run(gwi_stream* s, int xb, int64_t n, cudaStream_t st)
+{
+    const size_t rowb = (size_t)s->xcap * 2;
+    GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_acc + s->pend, (size_t)s->acc_cap * 2, s->d_x[xb], rowb, (size_t)n * 2, 2,
+                                     cudaMemcpyDeviceToDevice, st));
+    s->pend += n, s->t_recv += n;
+    const bool final = s->t_recv == s->N_total;
+    while (s->pend >= s->seg || (final && s->pend > 0)) {
+        int64_t proc = final ? s->pend : (s->pend / s->seg) * s->seg;
+        if (proc > s->sub) proc = s->sub;
+        const bool last = final && proc == s->pend;
+        gwi_status rc = tcs_block(s, (int)proc, last, st);
+        if (rc != GWI_OK) return rc;
+        rc = post_block(s, (int)proc, last, st);
+        if (rc != GWI_OK) return rc;
+        const int64_t rest = s->pend - proc;
+        if (rest > 0) {
+            // the remainder moves to the front; staged through the (now free) segment batch buffer because the ranges can overlap
+            GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_segx, (size_t)rest * 2, s->d_acc + proc, (size_t)s->acc_cap * 2, (size_t)rest * 2, 2,
+                                             cudaMemcpyDeviceToDevice, st));
+            GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_acc, (size_t)s->acc_cap * 2, s->d_segx, (size_t)rest * 2, (size_t)rest * 2, 2,
+                                             cudaMemcpyDeviceToDevice, st));
+        }
+        s->pend = rest;
+    }
+    return GWI_OK;
+}
+
 gwi_status check_push(gwi_stream* s, const void* a, const void* b, int64_t n, const char* who)
 {
     if (!s || !a || (s->nb > 1 && !b) || n < 1) {
         gwi_set_error("%s: bad argument", who);
         return GWI_ERR_ARG;
     }
-    if (s->finished || s->t_done + n > s->N_total) {
+    if (s->finished || (s->tcs ? s->t_recv : s->t_done) + n > s->N_total) {
         gwi_set_error("%s: %lld samples pushed + %lld > stream length %lld (or stream finished)", who, (long long)s->t_done,
                       (long long)n, (long long)s->N_total);
         return GWI_ERR_ARG;
@@ -289,14 +388,31 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
         s->seg = s->segT - s->segH;
         s->halo = s->segH;
     }
+    // the same back end with time slides: everything on the 128-sample tile grid
+    s->tcs = s->half_in && n_lags > 0 && !s->tiny && m0->arch.n_branch == 2 && m0->arch.c_in == 1 && n_total % 128 == 0 &&
+             n_total >= s->maxlag + s->Rf - 1;
+    for (int i = 0; i < n_models; i++) s->tcs = s->tcs && models[i]->tc != nullptr;
+    for (int i = 0; i < n_lags; i++) s->tcs = s->tcs && lags[i] % 128 == 0;
+    if (s->tcs) {
+        s->segH = ((s->Rf - 1 + 127) / 128) * 128;
+        s->segT = s->segH + 8192 < 16384 ? 16384 : s->segH + 8192;
+        s->seg = s->segT - s->segH;
+        s->halo = s->segH;
+        s->Rt = (int)(s->maxlag / 128);
+    }
     s->xcap = std::max<int64_t>(std::min(max_chunk, n_total), std::min<int64_t>(n_total, s->maxlag + s->Rf - 1));
     // sub-chunk: bounds the activation workspace (2R floats per branch-sample) to ~2 GiB
     int64_t per = (int64_t)s->nb * 2 * s->R * 4;
     int64_t sub = std::max<int64_t>(4096, (2LL << 30) / per);
     if (s->tiny) sub = std::max<int64_t>(4096, (1LL << 30) / ((int64_t)(1 + n_lags) * n_models * 4));   // ~1 GiB of probabilities
     if (s->tcb) sub = 1 << 24;
+    if (s->tcs) {
+        int64_t maxw = gwi_tc_max_windows(m0, s->segT);
+        sub = std::min<int64_t>(1 << 24, maxw * s->seg) / s->seg * s->seg;
+        if (sub < s->maxlag) s->tcs = false;               // the priming pass runs the tail as one block
+    }
     sub = std::min<int64_t>(sub, 1 << 24);
-    sub = std::min<int64_t>(sub, s->xcap);
+    if (!s->tcs) sub = std::min<int64_t>(sub, s->xcap);
     s->sub = (int)sub;
     s->lds = s->maxlag + s->sub;
     const int nslides = (int)s->lags.size();
@@ -322,14 +438,32 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
             if ((e = cudaMemset(s->d_xh[b], 0, (size_t)2 * s->segH * 2)) != cudaSuccess) return fail(e);
         }
     }
-    if (!s->tiny && !s->tcb) {   // activation workspace of the generic per-layer kernels
+    if (s->tcs) {
+        const int64_t Bmax = s->sub / s->seg + 1;
+        s->acc_cap = s->sub + s->seg + s->xcap;
+        if ((e = cudaMalloc(&s->d_segx, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);
+        s->tcws_bytes = gwi_tc_workspace_bytes(m0, Bmax, s->segT);
+        if ((e = cudaMalloc(&s->d_tcws, s->tcws_bytes)) != cudaSuccess) return fail(e);
+        if ((e = cudaMalloc(&s->d_acc, (size_t)2 * s->acc_cap * 2)) != cudaSuccess) return fail(e);
+        if ((e = cudaMemset(s->d_acc, 0, (size_t)2 * s->acc_cap * 2)) != cudaSuccess) return fail(e);
+        for (int b = 0; b < 2; b++) {
+            if ((e = cudaMalloc(&s->d_xh[b], (size_t)2 * s->segH * 2)) != cudaSuccess) return fail(e);
+            if ((e = cudaMemset(s->d_xh[b], 0, (size_t)2 * s->segH * 2)) != cudaSuccess) return fail(e);
+            s->d_hist_t[b].assign(s->M, nullptr);
+            for (int m = 0; m < s->M; m++) {
+                if ((e = cudaMalloc(&s->d_hist_t[b][m], (size_t)s->Rt * 32768)) != cudaSuccess) return fail(e);
+                if ((e = cudaMemset(s->d_hist_t[b][m], 0, (size_t)s->Rt * 32768)) != cudaSuccess) return fail(e);
+            }
+        }
+    }
+    if (!s->tiny && !s->tcb && !s->tcs) {   // activation workspace of the generic per-layer kernels
         if ((e = cudaMalloc(&s->d_hA, hbytes)) != cudaSuccess) return fail(e);
         if ((e = cudaMalloc(&s->d_hB, hbytes)) != cudaSuccess) return fail(e);
     }
     size_t histb = (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(m0)) * 4;
     s->d_skip.assign(s->M, nullptr);
     s->d_hist[0].assign(s->M, nullptr), s->d_hist[1].assign(s->M, nullptr);
-    for (int m = 0; m < s->M && !s->tiny && !s->tcb; m++) {
+    for (int m = 0; m < s->M && !s->tiny && !s->tcb && !s->tcs; m++) {
         size_t sb = (size_t)s->nb * s->S * s->lds * 4;
         if ((e = cudaMalloc(&s->d_skip[m], sb)) != cudaSuccess) return fail(e);
         if ((e = cudaMemset(s->d_skip[m], 0, sb)) != cudaSuccess) return fail(e);
@@ -338,7 +472,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
             if ((e = cudaMemset(s->d_hist[b][m], 0, histb)) != cudaSuccess) return fail(e);   // zero history == A4 padding
         }
     }
-    if (s->maxlag > 0 && (e = cudaMalloc(&s->d_tmp, (size_t)(s->nb - 1) * s->S * s->maxlag * 4)) != cudaSuccess) return fail(e);
+    if (s->maxlag > 0 && !s->tcs && (e = cudaMalloc(&s->d_tmp, (size_t)(s->nb - 1) * s->S * s->maxlag * 4)) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_prob, (size_t)nslides * s->M * s->sub * 4)) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_carry, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
     if ((e = cudaMemset(s->d_carry, 0, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
@@ -396,6 +530,10 @@ extern "C" void gwi_stream_destroy(gwi_stream* s)
     if (s->d_segx) cudaFree(s->d_segx);
     if (s->d_segp) cudaFree(s->d_segp);
     if (s->d_tcws) cudaFree(s->d_tcws);
+    if (s->d_acc) cudaFree(s->d_acc);
+    for (int b = 0; b < 2; b++)
+        for (uint8_t* p : s->d_hist_t[b])
+            if (p) cudaFree(p);
     if (s->d_hA) cudaFree(s->d_hA);
     if (s->d_hB) cudaFree(s->d_hB);
     if (s->d_tmp) cudaFree(s->d_tmp);
@@ -423,6 +561,35 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     GWI_CUDA_CHECK(cudaSetDevice(s->device));
+    if (s->tcs) {
+        // tail = L1[N - maxlag - (R_f - 1), N): the first R_f - 1 samples are the warm-up of the history tiles (the segment
+        // warm-up is R_f - 1 rounded up to whole tiles, the front of it stays zero and is never looked at by an output)
+        const int pre = s->Rf - 1, H = s->segH;
+        const int64_t n = s->maxlag;
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * H * 2, st));
+        GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_xh[0] + H + (H - pre), l1_tail, (size_t)pre * 2, cudaMemcpyDefault, st));
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_acc, 0, (size_t)n * 2, st));
+        GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_acc + s->acc_cap, (const __half*)l1_tail + pre, (size_t)n * 2, cudaMemcpyDefault, st));
+        const int B = (int)((n + s->seg - 1) / s->seg);
+        const int64_t total = (int64_t)B * s->segT;
+        k_seg_gather<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(s->d_acc, s->acc_cap, s->d_xh[0], (int)n, s->seg, H, s->segT, 0,
+                                                                     s->d_segx, total);
+        gwi_count_launch(1);
+        for (int m = 0; m < s->M; m++) {
+            const uint8_t* u = nullptr;
+            gwi_status rc = gwi_tc_stack(s->models[m], (const __half*)s->d_segx, B, s->segT, s->d_tcws, s->tcws_bytes, st, &u);
+            if (rc != GWI_OK) return rc;
+            k_hist_tiles<<<s->Rt, 256, 0, st>>>(u, s->segT / 128, s->Rt, s->Rt, s->seg / 128, H / 128, 0, s->d_hist_t[1][m],
+                                               s->d_hist_t[0][m]);
+            gwi_count_launch(1);
+        }
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * H * 2, st));
+        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * H * 2, st));
+        GWI_CUDA_CHECK(cudaGetLastError());
+        s->xh_cur = 0, s->hist_t_cur = 0, s->pend = 0;
+        s->primed = true;
+        return GWI_OK;
+    }
     const int c_in = s->models[0]->arch.c_in;
     // the tail goes to the branch-1 rows of staging buffer 0 (cudaMemcpyDefault: host or device source)
     GWI_CUDA_CHECK(cudaMemcpy2DAsync((char*)s->d_x[0] + (size_t)c_in * s->xcap * elt(s), s->xcap * elt(s), l1_tail,
@@ -496,7 +663,7 @@ extern "C" gwi_status gwi_stream_push(gwi_stream* s, const void* d_h1, const voi
     if (s->nb > 1)
         GWI_CUDA_CHECK(cudaMemcpy2DAsync((char*)s->d_x[b] + c_in * rowb, rowb, d_l1, n * elt(s), n * elt(s),
                                          (size_t)c_in * (s->nb - 1), cudaMemcpyDeviceToDevice, st));
-    rc = run_chunk(s, b, n, st);
+    rc = s->tcs ? tcs_append_and_run(s, b, n, st) : run_chunk(s, b, n, st);
     if (rc != GWI_OK) return rc;
     GWI_CUDA_CHECK(cudaEventRecord(s->ev_consumed[b], st));
     s->stage ^= 1;
@@ -521,7 +688,7 @@ extern "C" gwi_status gwi_stream_push_host(gwi_stream* s, const void* h_h1, cons
                                          (size_t)c_in * (s->nb - 1), cudaMemcpyHostToDevice, s->copy_stream));
     GWI_CUDA_CHECK(cudaEventRecord(s->ev_copied[b], s->copy_stream));
     GWI_CUDA_CHECK(cudaStreamWaitEvent(st, s->ev_copied[b], 0));
-    rc = run_chunk(s, b, n, st);
+    rc = s->tcs ? tcs_append_and_run(s, b, n, st) : run_chunk(s, b, n, st);
     if (rc != GWI_OK) return rc;
     GWI_CUDA_CHECK(cudaEventRecord(s->ev_consumed[b], st));
     s->stage ^= 1;

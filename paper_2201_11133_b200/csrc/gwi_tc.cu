@@ -507,6 +507,14 @@ struct HeadArgs {
     float* prob;          // [B][T]
     int64_t w0, nwin;
     int T, ntiles, n_branch;
+    // stream mode (mode = 1, gwi_stream.cu tensor-core back end with time slides, reading A24): the items are the nq
+    // output tiles of a block of segments; output tile q lives in window q / seg_tiles at tile q % seg_tiles +
+    // warm_tiles (no warm-up in the first window of the stream); the L1 tile is taken lag_tiles earlier, from the
+    // block or, before its start, from hist = the R L1 tiles that precede the block.
+    int mode;
+    const uint8_t* hist;
+    int64_t nq, lag_tiles;
+    int R, seg_tiles, warm_tiles, stream_start, n_valid;
 };
 constexpr int HEAD_THREADS = 192;   // warps 0-3 epilogue, warp 4 producer, warp 5 MMA
 
@@ -530,7 +538,14 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    const int64_t nitems = a.nwin * a.ntiles;
+    const int64_t nitems = a.mode ? a.nq : a.nwin * a.ntiles;
+    // stream mode: address of the u tile of branch b that holds block-local output tile q (q < 0: history)
+    auto stream_tile = [&](int64_t q, int b) -> const uint8_t* {
+        if (q < 0) return a.hist + (size_t)(a.R + q) * U_TILE_BYTES;
+        const int64_t w = q / a.seg_tiles;
+        const int64_t tl = q % a.seg_tiles + ((w == 0 && a.stream_start) ? 0 : a.warm_tiles);
+        return a.u + (((size_t)w * nb + b) * a.ntiles + tl) * U_TILE_BYTES;
+    };
 
     if (warp == 4) {
         if (lane == 0) {
@@ -542,9 +557,11 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
                 const int64_t wl = it / a.ntiles, j = it % a.ntiles;
                 mbar_wait(bar(3 + st), ((n >> 1) & 1) ^ 1);
                 mbar_arrive_expect_tx(bar(1 + st), W1B);
-                for (int b = 0; b < nb; b++)
-                    bulk_g2s(sbase + OFF_U + st * W1B + b * U_TILE_BYTES,
-                             a.u + (((size_t)wl * nb + b) * a.ntiles + j) * U_TILE_BYTES, U_TILE_BYTES, bar(1 + st));
+                for (int b = 0; b < nb; b++) {
+                    const uint8_t* src = a.mode ? stream_tile(b == 0 ? it : it - a.lag_tiles, b)
+                                                : a.u + (((size_t)wl * nb + b) * a.ntiles + j) * U_TILE_BYTES;
+                    bulk_g2s(sbase + OFF_U + st * W1B + b * U_TILE_BYTES, src, U_TILE_BYTES, bar(1 + st));
+                }
             }
         }
         __syncwarp();
@@ -592,8 +609,13 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
             }
             tc_fence_before();
             mbar_arrive(bar(7 + st));
-            const int t = (int)j * TM + r;
-            if (t < a.T) a.prob[(size_t)(a.w0 + wl) * a.T + t] = 1.0f / (1.0f + __expf(-y));
+            if (a.mode) {
+                const int64_t t = it * TM + r;
+                if (t < a.n_valid) a.prob[t] = 1.0f / (1.0f + __expf(-y));
+            } else {
+                const int t = (int)j * TM + r;
+                if (t < a.T) a.prob[(size_t)(a.w0 + wl) * a.T + t] = 1.0f / (1.0f + __expf(-y));
+            }
         }
     }
     tc_fence_before();
@@ -764,7 +786,8 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
         k_stack<<<grid, NTHREADS, SM_TOTAL, st>>>(sa);
         HeadArgs ha;
         ha.w1 = p->d_w1, ha.hc = p->d_hc, ha.u = u, ha.prob = d_prob, ha.w0 = w0, ha.nwin = nwin, ha.T = T, ha.ntiles = ntiles,
-        ha.n_branch = nb;
+        ha.n_branch = nb, ha.mode = 0, ha.hist = nullptr, ha.nq = 0, ha.lag_tiles = 0, ha.R = 0, ha.seg_tiles = 0, ha.warm_tiles = 0,
+        ha.stream_start = 0, ha.n_valid = 0;
         int64_t nitems = nwin * ntiles;
         int hgrid = (int)(nitems < p->num_sms ? nitems : p->num_sms);
         k_head_tc<<<hgrid, HEAD_THREADS, 3 * nb * U_TILE_BYTES + 256, st>>>(ha);
@@ -782,5 +805,60 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
         }
 #endif
     }
+    return GWI_OK;
+}
+
+// ---- pieces for the streaming back end with time slides (gwi_stream.cu) ---------------------------------------------
+int64_t gwi_tc_max_windows(const gwi_model* m, int32_t T)
+{
+    const int64_t ntiles = (T + TM - 1) / TM;
+    int64_t cap = (16LL << 30) / ((int64_t)m->arch.n_branch * ntiles * U_TILE_BYTES);
+    return cap < 296 ? 296 : cap;
+}
+
+// Branch stacks only: B windows (B <= gwi_tc_max_windows) -> u tiles [B][n_branch][ntiles][U_TILE_BYTES] at *u_out
+// inside the workspace (same layout as gwi_tc_infer uses between its two kernels).
+gwi_status gwi_tc_stack(const gwi_model* m, const __half* d_strain, int64_t B, int32_t T, void* d_ws, size_t ws_bytes,
+                        cudaStream_t st, const uint8_t** u_out)
+{
+    const GwiTcPack* p = m->tc;
+    const int nb = m->arch.n_branch;
+    const int ntiles = (T + TM - 1) / TM;
+    if (B > gwi_tc_max_windows(m, T) || ws_bytes < gwi_tc_workspace_bytes(m, B, T)) {
+        gwi_set_error("gwi_tc_stack: batch of %lld windows does not fit one launch / the workspace", (long long)B);
+        return GWI_ERR_NOMEM;
+    }
+    size_t ring_bytes = ((size_t)p->num_sms * 2 * p->meta.ring_tiles * PST_BYTES + 255) & ~(size_t)255;
+    size_t ring64_bytes = ((size_t)p->num_sms * 2 * p->meta.n64 * 2 * PRE_BYTES + 255) & ~(size_t)255;
+    uint8_t* ring = (uint8_t*)d_ws;
+    uint8_t* ring64 = ring + ring_bytes;
+    uint8_t* u = ring64 + ring64_bytes;
+    StackArgs sa;
+    sa.wfg = p->d_wfg, sa.wrs = p->d_wrs, sa.cst = p->d_cst, sa.strain = d_strain;
+    sa.w0 = 0, sa.nwin = B, sa.T = T, sa.ntiles = ntiles, sa.C = nb * m->arch.c_in;
+    sa.ring = ring, sa.ring64 = ring64, sa.u = u, sa.meta = p->meta;
+    int64_t njobs = ((B + 1) / 2) * nb;
+    int grid = (int)(njobs < p->num_sms ? njobs : p->num_sms);
+    k_stack<<<grid, NTHREADS, SM_TOTAL, st>>>(sa);
+    gwi_count_launch(1);
+    GWI_CUDA_CHECK(cudaGetLastError());
+    *u_out = u;
+    return GWI_OK;
+}
+
+// Head of one lag over the nq output tiles of a block (see HeadArgs, stream mode).
+gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, const uint8_t* hist, int R, int64_t nq,
+                              int64_t lag_tiles, int seg_tiles, int warm_tiles, int stream_start, int n_valid, float* d_prob,
+                              cudaStream_t st)
+{
+    const GwiTcPack* p = m->tc;
+    HeadArgs ha;
+    ha.w1 = p->d_w1, ha.hc = p->d_hc, ha.u = u, ha.prob = d_prob, ha.w0 = 0, ha.nwin = 0, ha.T = 0, ha.ntiles = ntiles;
+    ha.n_branch = m->arch.n_branch, ha.mode = 1, ha.hist = hist, ha.nq = nq, ha.lag_tiles = lag_tiles, ha.R = R;
+    ha.seg_tiles = seg_tiles, ha.warm_tiles = warm_tiles, ha.stream_start = stream_start, ha.n_valid = n_valid;
+    int hgrid = (int)(nq < p->num_sms ? nq : p->num_sms);
+    k_head_tc<<<hgrid, HEAD_THREADS, 3 * ha.n_branch * U_TILE_BYTES + 256, st>>>(ha);
+    gwi_count_launch(1);
+    GWI_CUDA_CHECK(cudaGetLastError());
     return GWI_OK;
 }

@@ -312,3 +312,20 @@ def test_config3_recipe_32_slides(tmpdir_s):
     assert np.max(np.abs(pbar - want)) <= 2e-3
     got = trig_tuples(recs)
     assert got == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 64) and got == sorted(got)
+
+
+def test_stream_paper_scale_slides_tensor_core_back_end(tmpdir_s):
+    """FP16 stream of paper-scale models WITH time slides: chunks re-blocked into whole segments, L1 feature tiles kept
+    as history, one tcgen05 head launch per lag.  Parity with the oracle; chunked == unchunked bit for bit."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1], gwi.FP16, arch=gs.PAPER_ARCH)
+    N = 128 * 300
+    x = gs.stream_noise(33, 0, N, dtype=np.float16)
+    lags = [4096, 12800]
+    want = _oracle_slides(oms, x, lags)
+    n0, r0, p0 = _run_stream(gms, x, [N], lags, 0.5, 16)
+    assert np.max(np.abs(p0 - want)) <= 2e-3
+    n1, r1, p1 = _run_stream(gms, x, _ragged(N, 3, 1, 20000), lags, 0.5, 16, max_chunk=20000)
+    assert np.array_equal(p0, p1)
+    assert trig_tuples(r0) == trig_tuples(r1)
+    assert trig_tuples(r0) == _oracle_triggers(p0.astype(np.float64), float(np.float32(0.5)), 16)
