@@ -206,6 +206,20 @@ gwi_status gwi_threshold_sweep(const float* const* d_prob, int32_t n_models, int
                                int32_t n_thresholds, int64_t min_len, int64_t* d_counts, void* d_workspace,
                                size_t workspace_bytes, void* cuda_stream);
 
+/* ---- whitening front end (reading A35) ----------------------------------------
+ * One segment of n raw strain samples of one detector -> whitened, unit-variance samples (what gwi_infer / gwi_stream_*
+ * take as input): Welch estimate of the segment's own PSD (frames of nper samples every nper/2, symmetric Hann window,
+ * mean of the squared magnitudes), linear interpolation of it to the segment's frequencies, division of the spectrum
+ * by its square root, inverse transform, division by the population standard deviation.
+ * d_raw: DEVICE [n] float (not modified).  d_out: DEVICE [n], float, or __half when out_is_half != 0 (may not alias
+ * d_raw).  n, nper even, 4 <= nper <= n <= 2^30.  d_workspace: DEVICE, >= gwi_whiten_workspace_bytes(n, nper), 256 B
+ * aligned.  The FFTs are cuFFT transforms; the library is loaded on first use (GWI_ERR_UNSUPPORTED if it cannot be).
+ * The call enqueues on cuda_stream and waits for it before returning (the FFT plans are released).
+ * Errors: GWI_ERR_ARG, GWI_ERR_NOMEM, GWI_ERR_UNSUPPORTED, GWI_ERR_CUDA. */
+size_t gwi_whiten_workspace_bytes(int64_t n, int32_t nper);
+gwi_status gwi_whiten(const float* d_raw, int64_t n, int32_t nper, void* d_out, int out_is_half, void* d_workspace,
+                      size_t workspace_bytes, void* cuda_stream);
+
 /* ---- misc ---------------------------------------------------------------------------------------------- */
 const char* gwi_last_error(void);
 int gwi_version(void);

@@ -14,7 +14,8 @@ EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_m
                     "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
                     "gwi_stream_tail_samples", "gwi_stream_prime", "gwi_stream_push", "gwi_stream_push_host",
                     "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_destroy", "gwi_stream_set_rule",
-                    "gwi_coincidence", "gwi_sweep_workspace_bytes", "gwi_threshold_sweep"]
+                    "gwi_coincidence", "gwi_sweep_workspace_bytes", "gwi_threshold_sweep", "gwi_whiten_workspace_bytes",
+                    "gwi_whiten"]
 
 
 class GwiError(RuntimeError):
@@ -87,6 +88,10 @@ def lib():
     L.gwi_sweep_workspace_bytes.argtypes = [C.c_int32]
     L.gwi_threshold_sweep.restype = C.c_int
     L.gwi_threshold_sweep.argtypes = [C.POINTER(vp), C.c_int32, C.c_int64, vp, C.c_int32, C.c_int64, vp, vp, C.c_size_t, vp]
+    L.gwi_whiten_workspace_bytes.restype = C.c_size_t
+    L.gwi_whiten_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
+    L.gwi_whiten.restype = C.c_int
+    L.gwi_whiten.argtypes = [vp, C.c_int64, C.c_int32, vp, C.c_int, vp, C.c_size_t, vp]
     L.gwi_last_error.restype = C.c_char_p
     L.gwi_version.restype = C.c_int
     L.gwi_launch_count.restype = C.c_int64
@@ -216,6 +221,17 @@ def threshold_sweep(probs, thresholds, min_len):
     _check(lib().gwi_threshold_sweep(ptrs, len(probs), N, C.c_void_p(th.data_ptr()), K, int(min_len),
                                      C.c_void_p(counts.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(dev)))
     return counts
+
+
+def whiten(raw, nper, half=True):
+    """gwi_whiten: raw [n] float32 device tensor -> whitened unit-variance [n] tensor (float16 or float32)."""
+    raw = raw.contiguous()
+    n = raw.numel()
+    out = torch.empty(n, dtype=torch.float16 if half else torch.float32, device=raw.device)
+    ws = torch.empty(max(lib().gwi_whiten_workspace_bytes(n, int(nper)), 256), dtype=torch.uint8, device=raw.device)
+    _check(lib().gwi_whiten(C.c_void_p(raw.data_ptr()), n, int(nper), C.c_void_p(out.data_ptr()), int(bool(half)),
+                            C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(raw.device)))
+    return out
 
 
 def new_carry(device=0):

@@ -1,0 +1,220 @@
+// gwi_whiten.cu -- whitening front end (PSD estimate of the strain, whitening with
+// it, standard deviation normalised to one; parameters by reading A35).
+//
+// One segment of n raw samples -> whitened samples ready for gwi_stream_push / gwi_infer:
+//   1. Welch estimate: frames of nper samples every nper/2, symmetric Hann window, P = mean |rfft(frame)|^2
+//   2. P interpolated linearly to the n/2+1 frequencies of the segment
+//   3. Y = rfft(x) / sqrt(P_interp), y = irfft(Y)
+//   4. out = y / std(y)  (population standard deviation), written as float or __half
+// The FFTs are plain library transforms (cuFFT: a batched R2C of the frames, one R2C and one C2R of the segment); the
+// windowing, the periodogram mean, the interpolation + division, the statistics and the output scaling are kernels of
+// this file.  cuFFT is loaded with dlopen on first use, so that libgwi.so itself has no link-time dependency on it:
+// without the library gwi_whiten returns GWI_ERR_UNSUPPORTED and nothing else is affected.
+#include <cufft.h>
+#include <dlfcn.h>
+
+#include "gwi_internal.h"
+
+namespace {
+
+struct CufftApi {
+    cufftResult (*Plan1d)(cufftHandle*, int, cufftType, int) = nullptr;
+    cufftResult (*SetStream)(cufftHandle, cudaStream_t) = nullptr;
+    cufftResult (*ExecR2C)(cufftHandle, cufftReal*, cufftComplex*) = nullptr;
+    cufftResult (*ExecC2R)(cufftHandle, cufftComplex*, cufftReal*) = nullptr;
+    cufftResult (*Destroy)(cufftHandle) = nullptr;
+    bool ok = false;
+};
+
+CufftApi& cufft_api()
+{
+    static CufftApi api;
+    static bool tried = false;
+    if (tried) return api;
+    tried = true;
+    void* h = nullptr;
+    for (const char* name : {"libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so.11"}) {
+        h = dlopen(name, RTLD_NOW | RTLD_LOCAL);
+        if (h) break;
+    }
+    if (!h) return api;
+    api.Plan1d = (decltype(api.Plan1d))dlsym(h, "cufftPlan1d");
+    api.SetStream = (decltype(api.SetStream))dlsym(h, "cufftSetStream");
+    api.ExecR2C = (decltype(api.ExecR2C))dlsym(h, "cufftExecR2C");
+    api.ExecC2R = (decltype(api.ExecC2R))dlsym(h, "cufftExecC2R");
+    api.Destroy = (decltype(api.Destroy))dlsym(h, "cufftDestroy");
+    api.ok = api.Plan1d && api.SetStream && api.ExecR2C && api.ExecC2R && api.Destroy;
+    return api;
+}
+
+// 1 / rms of the raw segment: raw strain is ~1e-21, whose squares underflow fp32; the whitened output does not depend
+// on the input's scale, so everything is computed on x / rms(x)
+__device__ __forceinline__ float raw_scale(const double* stats, int64_t n)
+{
+    const double ms = stats[1] / (double)n;
+    return ms > 0.0 ? (float)(1.0 / sqrt(ms)) : 1.0f;
+}
+
+// frames[k][i] = scale * x[k * step + i] * hann(i)
+__global__ void k_frames(const float* __restrict__ x, int nper, int K, float* __restrict__ frames, const double* __restrict__ rs,
+                         int64_t n)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (int64_t)K * nper) return;
+    const int k = (int)(idx / nper), i = (int)(idx % nper);
+    const float w = 0.5f - 0.5f * cospif(2.0f * (float)i / (float)(nper - 1));
+    frames[idx] = x[(int64_t)k * (nper / 2) + i] * raw_scale(rs, n) * w;
+}
+
+// P[j] = mean over frames of |F[k][j]|^2
+__global__ void k_periodogram(const float2* __restrict__ F, int nf, int K, float* __restrict__ P)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= nf) return;
+    double acc = 0.0;
+    for (int k = 0; k < K; k++) {
+        float2 v = F[(int64_t)k * nf + j];
+        acc += (double)v.x * v.x + (double)v.y * v.y;
+    }
+    P[j] = (float)(acc / K);
+}
+
+// X[i] /= sqrt(P interpolated at i * nper / n)
+__global__ void k_divide(float2* __restrict__ X, int64_t nx, int64_t n, int nper, const float* __restrict__ P,
+                         const double* __restrict__ rs)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nx) return;
+    const double pos = (double)i * nper / (double)n;
+    int j = (int)pos;
+    if (j > nper / 2 - 1) j = nper / 2 - 1;
+    const float frac = (float)(pos - j);
+    const float p = P[j] * (1.0f - frac) + P[j + 1] * frac;
+    const float s = rsqrtf(fmaxf(p, 1e-30f)) * raw_scale(rs, n);
+    float2 v = X[i];
+    X[i] = make_float2(v.x * s, v.y * s);
+}
+
+// stats[0] += sum y, stats[1] += sum y^2 (double)
+__global__ void k_stats_y(const float* __restrict__ y, int64_t n, double* __restrict__ stats)
+{
+    __shared__ double s0[256], s1[256];
+    double a = 0.0, b = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        double v = y[i];
+        a += v, b += v * v;
+    }
+    s0[threadIdx.x] = a, s1[threadIdx.x] = b;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) s0[threadIdx.x] += s0[threadIdx.x + o], s1[threadIdx.x] += s1[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        atomicAdd(&stats[0], s0[0]);
+        atomicAdd(&stats[1], s1[0]);
+    }
+}
+
+template <typename OT>
+__global__ void k_scale_out(const float* __restrict__ y, int64_t n, const double* __restrict__ stats, OT* __restrict__ out)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double mean = stats[0] / (double)n;
+    const double var = stats[1] / (double)n - mean * mean;
+    const float inv = (float)(1.0 / sqrt(var > 0.0 ? var : 1.0));
+    out[i] = (OT)(y[i] * inv);
+}
+
+struct WsLayout {
+    size_t frames, spec, P, X, y, stats, total;
+    int K;
+};
+WsLayout ws_layout(int64_t n, int nper)
+{
+    WsLayout L;
+    L.K = (int)((n - nper) / (nper / 2) + 1);
+    size_t o = 0;
+    auto take = [&](size_t b) { size_t at = o; o += (b + 255) & ~(size_t)255; return at; };
+    L.frames = take((size_t)L.K * nper * 4);
+    L.spec = take((size_t)L.K * (nper / 2 + 1) * 8);
+    L.P = take((size_t)(nper / 2 + 2) * 4);
+    L.X = take((size_t)(n / 2 + 1) * 8);
+    L.y = take((size_t)n * 4);
+    L.stats = take(32);
+    L.total = o;
+    return L;
+}
+
+} // namespace
+
+extern "C" size_t gwi_whiten_workspace_bytes(int64_t n, int32_t nper)
+{
+    if (n < 4 || nper < 4 || (n & 1) || (nper & 1) || nper > n) return 0;
+    return ws_layout(n, nper).total;
+}
+
+extern "C" gwi_status gwi_whiten(const float* d_raw, int64_t n, int32_t nper, void* d_out, int out_is_half, void* d_workspace,
+                                 size_t workspace_bytes, void* cuda_stream)
+{
+    if (!d_raw || !d_out || !d_workspace || n < 4 || nper < 4 || (n & 1) || (nper & 1) || nper > n || n > (1LL << 30) ||
+        ((uintptr_t)d_workspace & 255)) {
+        gwi_set_error("gwi_whiten: bad argument (n and nper even, 4 <= nper <= n <= 2^30)");
+        return GWI_ERR_ARG;
+    }
+    WsLayout L = ws_layout(n, nper);
+    if (workspace_bytes < L.total) {
+        gwi_set_error("gwi_whiten: workspace %zu < %zu bytes", workspace_bytes, L.total);
+        return GWI_ERR_NOMEM;
+    }
+    CufftApi& fft = cufft_api();
+    if (!fft.ok) {
+        gwi_set_error("gwi_whiten: cuFFT (libcufft.so.11) could not be loaded");
+        return GWI_ERR_UNSUPPORTED;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char* ws = (char*)d_workspace;
+    float* frames = (float*)(ws + L.frames);
+    float2* spec = (float2*)(ws + L.spec);
+    float* P = (float*)(ws + L.P);
+    float2* X = (float2*)(ws + L.X);
+    float* y = (float*)(ws + L.y);
+    double* stats = (double*)(ws + L.stats);
+    const int K = L.K, nf = nper / 2 + 1;
+    cufftHandle pf = 0, pr = 0, pi = 0;
+    auto fail = [&](const char* what) {
+        if (pf) fft.Destroy(pf);
+        if (pr) fft.Destroy(pr);
+        if (pi) fft.Destroy(pi);
+        gwi_set_error("gwi_whiten: cuFFT %s failed", what);
+        return GWI_ERR_CUDA;
+    };
+    if (fft.Plan1d(&pf, nper, CUFFT_R2C, K) != CUFFT_SUCCESS) return fail("plan (frames)");
+    if (fft.Plan1d(&pr, (int)n, CUFFT_R2C, 1) != CUFFT_SUCCESS) return fail("plan (forward)");
+    if (fft.Plan1d(&pi, (int)n, CUFFT_C2R, 1) != CUFFT_SUCCESS) return fail("plan (inverse)");
+    fft.SetStream(pf, st), fft.SetStream(pr, st), fft.SetStream(pi, st);
+    const int64_t nfr = (int64_t)K * nper;
+    cudaMemsetAsync(stats, 0, 32, st);
+    k_stats_y<<<592, 256, 0, st>>>(d_raw, n, stats + 2);          // stats[2..3]: sum and sum of squares of the raw input
+    k_frames<<<(unsigned)((nfr + 255) / 256), 256, 0, st>>>(d_raw, nper, K, frames, stats + 2, n);
+    if (fft.ExecR2C(pf, frames, (cufftComplex*)spec) != CUFFT_SUCCESS) return fail("exec (frames)");
+    k_periodogram<<<(nf + 127) / 128, 128, 0, st>>>(spec, nf, K, P);
+    // cuFFT R2C is out of place here: the raw input stays untouched
+    if (fft.ExecR2C(pr, const_cast<float*>(d_raw), (cufftComplex*)X) != CUFFT_SUCCESS) return fail("exec (forward)");
+    k_divide<<<(unsigned)((n / 2 + 1 + 255) / 256), 256, 0, st>>>(X, n / 2 + 1, n, nper, P, stats + 2);
+    if (fft.ExecC2R(pi, (cufftComplex*)X, y) != CUFFT_SUCCESS) return fail("exec (inverse)");
+    k_stats_y<<<592, 256, 0, st>>>(y, n, stats);
+    if (out_is_half) k_scale_out<__half><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(y, n, stats, (__half*)d_out);
+    else k_scale_out<float><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(y, n, stats, (float*)d_out);
+    gwi_count_launch(6);
+    cudaError_t e = cudaGetLastError();
+    // the plans own work areas that the enqueued transforms use: release them once the stream has drained
+    cudaStreamSynchronize(st);
+    fft.Destroy(pf), fft.Destroy(pr), fft.Destroy(pi);
+    if (e != cudaSuccess) {
+        gwi_set_error("gwi_whiten: %s", cudaGetErrorString(e));
+        return GWI_ERR_CUDA;
+    }
+    return GWI_OK;
+}
