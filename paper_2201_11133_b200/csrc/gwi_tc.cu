@@ -192,6 +192,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     mbar_arrive_expect_tx(bar(B_WFG_FULL + st), WFG_BYTES);
                     bulk_g2s(sbase + SM_WFG + st * WFG_BYTES, a.wfg + ((size_t)b * L + i) * WFG_BYTES, WFG_BYTES,
                              bar(B_WFG_FULL + st));
+                    mbar_wait(bar(B_WRS_FREE + st), wph ^ 1);
+                    mbar_arrive_expect_tx(bar(B_WRS_FULL + st), WRS_STRIDE);
+                    bulk_g2s(sbase + SM_WRS + st * WRS_STRIDE, a.wrs + ((size_t)b * L + i) * WRS_STRIDE, WRS_STRIDE,
+                             bar(B_WRS_FULL + st));
+                    // the past tiles last: their waits (GEMM2 of the previous iteration of both slots) must not hold back
+                    // the weights and biases of this iteration, which the gate needs first
                     if (M.kind[i] == 2 && j >= M.D[i]) {
                         for (int s = 0; s < 2; s++) {
                             // the tile was stored (j - D) tiles ago by the MMA thread, which waits for the completion
@@ -206,10 +212,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                             n_pst[s]++;
                         }
                     }
-                    mbar_wait(bar(B_WRS_FREE + st), wph ^ 1);
-                    mbar_arrive_expect_tx(bar(B_WRS_FULL + st), WRS_STRIDE);
-                    bulk_g2s(sbase + SM_WRS + st * WRS_STRIDE, a.wrs + ((size_t)b * L + i) * WRS_STRIDE, WRS_STRIDE,
-                             bar(B_WRS_FULL + st));
                 }
             }
             __syncwarp();
