@@ -365,24 +365,27 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                 mbar_arrive(bar(B_H_READY + s));
             };
 
-            for (int j = 0; j < a.ntiles; j++) {
-                // ---- lift: h0 = W_in x + b_in                                                   (C.1 step 1)
-                {
-                    const int t = j * TM + r;
-                    float x = 0.f;
-                    if (t < a.T) x = __half2float(a.strain[((size_t)w * a.T + t) * a.C + b]);
+            // ---- lift of tile j: h0 = W_in x + b_in, published as the operand of layer 0            (C.1 step 1)
+            auto load_x = [&](int j) {
+                const int t = j * TM + r;
+                return t < a.T ? __half2float(a.strain[((size_t)w * a.T + t) * a.C + b]) : 0.f;
+            };
+            auto lift = [&](int j, float x) {
 #pragma unroll
-                    for (int c = 0; c < 16; c++) {
-                        float2 wi = __ldg(reinterpret_cast<const float2*>(cst + ch0) + c);
-                        float2 bi = __ldg(reinterpret_cast<const float2*>(cst + 64 + ch0) + c);
-                        h[c] = make_float2(fmaf(wi.x, x, bi.x), fmaf(wi.y, x, bi.y));
-                    }
-                    tc_wait_ld();   // the previous tile's TMEM reads of this thread are complete
-                    publish(0, j);
+                for (int c = 0; c < 16; c++) {
+                    float2 wi = __ldg(reinterpret_cast<const float2*>(cst + ch0) + c);
+                    float2 bi = __ldg(reinterpret_cast<const float2*>(cst + 64 + ch0) + c);
+                    h[c] = make_float2(fmaf(wi.x, x, bi.x), fmaf(wi.y, x, bi.y));
                 }
+                publish(0, j);
+            };
+            lift(0, load_x(0));
+            float xnext = 0.f;
+            for (int j = 0; j < a.ntiles; j++) {
                 for (int i = 0; i < L; i++, n_it++) {
                     const uint32_t ph = n_it & 1;
                     const int st = n_it & 1;
+                    if (i == L - 1 && j + 1 < a.ntiles) xnext = load_x(j + 1);   // strain of the next tile, a whole layer early
                     // ---- off the critical path, while GEMM1 runs: this layer's biases (streamed behind its Wrs) and the
                     // residual bias into the fp32 master
                     mbar_wait(bar(B_WRS_FULL + st), (n_it >> 1) & 1);
@@ -469,6 +472,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                         // u = ReLU(sum_i skip_i) -> fp16 tile in the workspace                       (C.1 step 3)
                         mbar_wait(bar(B_SKD + s), ph);
                         tc_fence_after();
+                        // the next tile starts first (its GEMM1 runs under the u output below; its first skip GEMM, which
+                        // overwrites the skip sum, needs this warp's gate of layer 0, i.e. comes after the reads below)
+                        if (j + 1 < a.ntiles) lift(j + 1, xnext);
                         uint8_t* ut = a.u + (((size_t)wl * nb + b) * a.ntiles + j) * U_TILE_BYTES + r * 16;
 #pragma unroll
                         for (int cc = 0; cc < 2; cc++) {
