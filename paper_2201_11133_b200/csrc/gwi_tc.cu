@@ -98,7 +98,8 @@ constexpr int SM_X = SM_WRS + 2 * WRS_STRIDE;             // 2 slots
 constexpr int SM_PST = SM_X + 2 * X_BYTES;                // 2 slots
 constexpr int SM_STASH = SM_PST + 2 * PST_BYTES;          // 2 slots
 constexpr int SM_BAR = SM_STASH + 2 * STASH_BYTES;
-constexpr int SM_TOTAL = SM_BAR + 256;
+constexpr int SM_CST = SM_BAR + 256;                      // the branch's lift weights and skip-bias sum (256 floats)
+constexpr int SM_TOTAL = SM_CST + 1024;
 static_assert(SM_TOTAL <= 232448, "shared memory budget");
 
 enum { B_WFG_FULL = 0, B_WFG_FREE = 2, B_WRS_FULL = 4, B_WRS_FREE = 6, B_FG_FULL = 8, B_Z_READY = 10, B_RS_FULL = 12,
@@ -177,6 +178,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
             for (int i = threadIdx.x; i < 2 * STASH_BYTES / 16; i += NTHREADS) zs[i] = z4;
             uint4* zx = reinterpret_cast<uint4*>(smem + SM_X);
             for (int i = threadIdx.x; i < 2 * X_BYTES / 16; i += NTHREADS) zx[i] = z4;
+            if (threadIdx.x < 256) reinterpret_cast<float*>(smem + SM_CST)[threadIdx.x] = a.cst[b * 256 + threadIdx.x];
         }
         fence_proxy_async_smem();
         __syncthreads();
@@ -303,6 +305,19 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                                     tc_mma_f16(dt, ax + kk * ((2 * X_CHUNK) >> 4), bw + 128 + kk * 384, idesc64, kk > 0 ? 1u : 0u);
                             }
                             tc_commit(bar(B_RS_FULL + s));
+                            {
+                                // pre rows of the next iteration (d = 64 layers): GEMM1 of this iteration is done with them
+                                // (its gate has ended), and this thread's own bulk store of the entry (a tile ago) has
+                                // completed (bulk_wait_all above, in that iteration)
+                                const int inx = (i + 1 < L) ? i + 1 : 0, jnx = (i + 1 < L) ? j : j + 1;
+                                if ((M.lay[inx] & 3) == 1 && jnx >= 1 && jnx < a.ntiles) {
+                                    const uint8_t* src = ring64_s + (size_t)(M.ring_off[inx] * 2 + ((jnx - 1) & 1)) * PRE_BYTES;
+                                    mbar_arrive_expect_tx(bar(B_PRE_FULL + s), PRE_BYTES);
+#pragma unroll
+                                    for (int c = 0; c < 8; c++)
+                                        bulk_g2s(xrows - 64 * 16 + c * X_CHUNK, src + c * 1024, 1024, bar(B_PRE_FULL + s));
+                                }
+                            }
 #pragma unroll
                             for (int kk = 0; kk < 4; kk++)
                                 tc_mma_f16(dskip, ax + kk * ((2 * X_CHUNK) >> 4), bw + kk * 384, idesc128, (i > 0 || kk > 0) ? 1u : 0u);
@@ -330,8 +345,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
             const uint32_t xs = sbase + SM_X + s * X_BYTES;
             const uint32_t st0 = sbase + SM_STASH + s * STASH_BYTES;
             const uint32_t lane_t = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-            uint8_t* ring64_s = a.ring64 + ((size_t)blockIdx.x * 2 + s) * M.n64 * 2 * PRE_BYTES;
-            const float* cst = a.cst + b * 256;
+            const float* cst = reinterpret_cast<const float*>(smem + SM_CST);   // W_in[64], b_in[64], sum_i bs_i[128]
             float2 h[16];                                             // fp32 master of the residual stream, 32 channels
 
             // writes the fp16 copy of h as the operand of layer `inext` for tile j, maintains stash / rings, signals MMA
@@ -373,8 +387,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
             auto lift = [&](int j, float x) {
 #pragma unroll
                 for (int c = 0; c < 16; c++) {
-                    float2 wi = __ldg(reinterpret_cast<const float2*>(cst + ch0) + c);
-                    float2 bi = __ldg(reinterpret_cast<const float2*>(cst + 64 + ch0) + c);
+                    float2 wi = *(reinterpret_cast<const float2*>(cst + ch0) + c);
+                    float2 bi = *(reinterpret_cast<const float2*>(cst + 64 + ch0) + c);
                     h[c] = make_float2(fmaf(wi.x, x, bi.x), fmaf(wi.y, x, bi.y));
                 }
                 publish(0, j);
@@ -407,14 +421,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     }
 #endif
                     if (lane == 0) TRACE(5, 10 * (warp & 7) + s, j * L + i);
-                    const int inx = (i + 1 < L) ? i + 1 : 0, jnx = (i + 1 < L) ? j : j + 1;   // the next (layer, tile)
-                    if (M.kind[inx] == 1 && jnx >= 1 && jnx < a.ntiles && (warp & 7) == 0 && lane == 0) {
-                        // G1(i) has finished with the pre rows: fetch the 64 rows that precede tile jnx for layer inx
-                        fence_proxy_async();
-                        mbar_arrive_expect_tx(bar(B_PRE_FULL + s), PRE_BYTES);
-                        const uint8_t* src = ring64_s + (size_t)(M.ring_off[inx] * 2 + ((jnx - 1) & 1)) * PRE_BYTES;
-                        for (int c = 0; c < 8; c++) bulk_g2s(xs + c * X_CHUNK, src + c * 1024, 1024, bar(B_PRE_FULL + s));
-                    }
                     __syncwarp();
                     tc_fence_after();
                     {
@@ -488,7 +494,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 #pragma unroll
                                     for (int e = 0; e < 4; e++) {
                                         int col = 8 * c + 2 * e;
-                                        float2 bs = __ldg(reinterpret_cast<const float2*>(cst + 128 + 64 * wg + 32 * cc + col));
+                                        float2 bs = *reinterpret_cast<const float2*>(cst + 128 + 64 * wg + 32 * cc + col);
                                         float u0 = fmaxf(__uint_as_float(v[col]) + bs.x, 0.f);
                                         float u1 = fmaxf(__uint_as_float(v[col + 1]) + bs.y, 0.f);
                                         q[e] = pack_half2(u0, u1);
