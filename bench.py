@@ -150,6 +150,56 @@ def stream_bench(dev, work, rank, n_chunks=744):
         del pm
     except Exception as ex:
         out["hour_paper_scale"] = {"error": repr(ex)}
+    # ---- configs[3]: 1 day, 32 circular one-second slides, all lags in one pass (slid-strain-seconds/s)
+    try:
+        n_hours = 24 if n_chunks >= 24 else max(n_chunks, 1)
+        xc = torch.from_numpy(np.stack([gs.coloured_whitened_noise(2 + d, d, N1, seg_len=N1) for d in range(2)])).to(dev)
+        lags = [gs.FS * k for k in range(1, 33)]
+        st = gwi.Stream(models, n_hours * N1, N1, THETA, LMIN, lags=lags, capacity=65536)
+        st.prime(xc[1, N1 - st.tail_samples:].contiguous())
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for c in range(n_hours):
+            st.push(xc[0], xc[1])
+        e1.record()
+        n, _ = st.finish()
+        ms = e0.elapsed_time(e1)
+        st.close()
+        out["day_32_slides"] = {"workload": f"configs[3]: {n_hours} h of coloured-then-whitened noise (reading A27; one seeded hour per detector "
+                                            "pushed repeatedly, resident in HBM), 4 models (config-1 arch), zero lag + 32 circular lags of "
+                                            "k x 1 s, all lags in one pass", "ms": ms,
+                                "strain_seconds_per_s": n_hours * 3600 / (ms * 1e-3),
+                                "slid_strain_seconds_per_s": 33 * n_hours * 3600 / (ms * 1e-3), "triggers": n}
+        del xc
+    except Exception as ex:
+        out["day_32_slides"] = {"error": repr(ex)}
+    # ---- standalone post-processing (a-8..a-10) on materialised probabilities: HBM-bound, algorithmic bytes = M x N x 4
+    try:
+        Np = 1 << 27
+        g = torch.Generator(device=dev)
+        g.manual_seed(7)
+        probs = [torch.rand(Np, generator=g, device=dev, dtype=torch.float32) * 0.45 for _ in range(4)]
+        for k in range(16):                                    # 16 plateaus of 1 s above the threshold -> 16 triggers
+            for pm_ in probs:
+                pm_[(k + 1) * 7_000_003:(k + 1) * 7_000_003 + gs.FS] = 0.9
+        times = []
+        for rep in range(6):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            cnt, _, _ = gwi.ensemble_triggers(probs, THETA, LMIN, capacity=4096, sync=False)
+            e1.record()
+            torch.cuda.synchronize()
+            times.append(e0.elapsed_time(e1))
+        ms = float(np.median(times[2:]))
+        hbm = peaks()[0].get("hbm_gbs", 6650.0)
+        gbs = 4 * Np * 4 / (ms * 1e-3) / 1e9
+        out["post"] = {"workload": "gwi_ensemble_triggers on 4 x 2^27 float32 probabilities (2.1 GB > L2): mean, threshold, run clustering",
+                       "ms": ms, "triggers": int(cnt.item()), "bound": "hbm", "achieved_gb_per_s": gbs, "peak_gb_per_s": hbm,
+                       "frac": gbs / hbm, "samples_per_s": Np / (ms * 1e-3)}
+        del probs
+    except Exception as ex:
+        out["post"] = {"error": repr(ex)}
     # ---- month, host -> device streaming
     st = gwi.Stream(models, n_chunks * N1, N1, THETA, LMIN, capacity=65536)
     torch.cuda.synchronize()

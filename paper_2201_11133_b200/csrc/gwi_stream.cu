@@ -404,7 +404,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     // sub-chunk: bounds the activation workspace (2R floats per branch-sample) to ~2 GiB
     int64_t per = (int64_t)s->nb * 2 * s->R * 4;
     int64_t sub = std::max<int64_t>(4096, (2LL << 30) / per);
-    if (s->tiny) sub = std::max<int64_t>(4096, (1LL << 30) / ((int64_t)(1 + n_lags) * n_models * 4));   // ~1 GiB of probabilities
+    if (s->tiny) sub = std::max<int64_t>(4096, (4LL << 30) / ((int64_t)(1 + n_lags) * n_models * 4));   // <= 4 GiB of probabilities
     if (s->tcb) sub = 1 << 24;
     if (s->tcs) {
         int64_t maxw = gwi_tc_max_windows(m0, s->segT);

@@ -231,11 +231,10 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
 
 // Time-slide heads (reading A24): p_k[t] = head(u_H1[t], u_L1[t - lag_k]) for every lag of the list, from the fp16
 // time-major branch features.  W1 [u_H; u_L] is split by linearity: the H1 half of the contraction is done once per
-// 16-row tile and re-used for every lag, each lag adds its L1 half (same accumulation order as the fused head of
-// k_tiny, so lag 0 reproduces it bit for bit).  u16 row 0 = sample 0 of the chunk; L1 rows at negative indices are the
+// 16-row tile and re-used for every lag, each lag adds its L1 half.  u16 row 0 = sample 0 of the chunk; L1 rows at negative indices are the
 // ring of the previous max-lag samples.
 struct HeadsArgs {
-    const uint2* w1;
+    const uint2* w1p;       // [ks 4][nt 4][32] B fragments of W1^T in the k order of the 16-byte row loads (see the kernel)
     const float* hcst;      // b1[32], W2[32], b2
     const __half* u16;      // [2][lds][32], pointing at row 0 of this chunk
     int64_t lds;
@@ -252,61 +251,53 @@ __global__ void __launch_bounds__(256) k_tiny_heads(const HeadsArgs a)
     if (row0 >= a.n) return;
     const int64_t ra = row0 + g, rb = ra + 8;
     const int64_t ca = ra < a.n ? ra : a.n - 1, cb = rb < a.n ? rb : a.n - 1;   // clamp loads of the ragged tail
-    const __half* uH = a.u16;
-    const __half* uL = a.u16 + a.lds * 32;
+    // a feature row is 32 halves = 4 x 16 bytes; lane (g, t) loads bytes 16 t .. 16 t + 15 of rows g and g + 8 with one
+    // 16-byte load each and uses them as the A fragments of two k-steps whose k order is permuted accordingly (w1p)
+    const uint4* uH = reinterpret_cast<const uint4*>(a.u16);
+    const uint4* uL = reinterpret_cast<const uint4*>(a.u16 + a.lds * 32);
     // H1 half: acc = b1 + W1[:, 0:32] u_H
     float acc[4][4];
     {
-        uint32_t ah[2][4];
-#pragma unroll
-        for (int ks = 0; ks < 2; ks++) {
-            ah[ks][0] = *reinterpret_cast<const uint32_t*>(uH + ca * 32 + 16 * ks + 2 * t);
-            ah[ks][1] = *reinterpret_cast<const uint32_t*>(uH + cb * 32 + 16 * ks + 2 * t);
-            ah[ks][2] = *reinterpret_cast<const uint32_t*>(uH + ca * 32 + 16 * ks + 8 + 2 * t);
-            ah[ks][3] = *reinterpret_cast<const uint32_t*>(uH + cb * 32 + 16 * ks + 8 + 2 * t);
-        }
+        const uint4 ha = uH[ca * 4 + t], hb = uH[cb * 4 + t];
+        const uint32_t ah0[4] = {ha.x, hb.x, ha.y, hb.y}, ah1[4] = {ha.z, hb.z, ha.w, hb.w};
 #pragma unroll
         for (int nt = 0; nt < 4; nt++) {
             float2 bb = __ldg(reinterpret_cast<const float2*>(a.hcst + 8 * nt + 2 * t));
             acc[nt][0] = bb.x, acc[nt][1] = bb.y, acc[nt][2] = bb.x, acc[nt][3] = bb.y;
-#pragma unroll
-            for (int ks = 0; ks < 2; ks++) mma16816(acc[nt], ah[ks], __ldg(a.w1 + (ks * 4 + nt) * 32 + lane));
+            mma16816(acc[nt], ah0, __ldg(a.w1p + (0 * 4 + nt) * 32 + lane));
+            mma16816(acc[nt], ah1, __ldg(a.w1p + (1 * 4 + nt) * 32 + lane));
         }
     }
     uint2 wl[2][4];
     float2 w2[4];
 #pragma unroll
     for (int nt = 0; nt < 4; nt++) {
-        wl[0][nt] = __ldg(a.w1 + (2 * 4 + nt) * 32 + lane), wl[1][nt] = __ldg(a.w1 + (3 * 4 + nt) * 32 + lane);
+        wl[0][nt] = __ldg(a.w1p + (2 * 4 + nt) * 32 + lane), wl[1][nt] = __ldg(a.w1p + (3 * 4 + nt) * 32 + lane);
         w2[nt] = __ldg(reinterpret_cast<const float2*>(a.hcst + 32 + 8 * nt + 2 * t));
     }
     const float b2 = __ldg(a.hcst + 64);
+    // after the butterfly every lane of a group holds both rows' sums: lane t = 0 finishes row g, lane t = 1 row g + 8
+    const int64_t rst = (t & 1) ? rb : ra;
+    const bool store = t < 2 && rst < a.n;
+#pragma unroll 2
     for (int k = 0; k < a.n_lags; k++) {
-        const int64_t lag = a.lags[k];
-        uint32_t al[2][4];
-#pragma unroll
-        for (int ks = 0; ks < 2; ks++) {
-            al[ks][0] = *reinterpret_cast<const uint32_t*>(uL + (ca - lag) * 32 + 16 * ks + 2 * t);
-            al[ks][1] = *reinterpret_cast<const uint32_t*>(uL + (cb - lag) * 32 + 16 * ks + 2 * t);
-            al[ks][2] = *reinterpret_cast<const uint32_t*>(uL + (ca - lag) * 32 + 16 * ks + 8 + 2 * t);
-            al[ks][3] = *reinterpret_cast<const uint32_t*>(uL + (cb - lag) * 32 + 16 * ks + 8 + 2 * t);
-        }
+        const int64_t lag = __ldg(a.lags + k);
+        const uint4 la = uL[(ca - lag) * 4 + t], lb = uL[(cb - lag) * 4 + t];
+        const uint32_t al0[4] = {la.x, lb.x, la.y, lb.y}, al1[4] = {la.z, lb.z, la.w, lb.w};
         float y0 = 0.f, y1 = 0.f;
 #pragma unroll
         for (int nt = 0; nt < 4; nt++) {
             float v[4] = {acc[nt][0], acc[nt][1], acc[nt][2], acc[nt][3]};
-            mma16816(v, al[0], wl[0][nt]);
-            mma16816(v, al[1], wl[1][nt]);
+            mma16816(v, al0, wl[0][nt]);
+            mma16816(v, al1, wl[1][nt]);
             y0 = fmaf(w2[nt].x, fmaxf(v[0], 0.f), y0), y0 = fmaf(w2[nt].y, fmaxf(v[1], 0.f), y0);
             y1 = fmaf(w2[nt].x, fmaxf(v[2], 0.f), y1), y1 = fmaf(w2[nt].y, fmaxf(v[3], 0.f), y1);
         }
         y0 += __shfl_xor_sync(0xffffffffu, y0, 1), y1 += __shfl_xor_sync(0xffffffffu, y1, 1);
         y0 += __shfl_xor_sync(0xffffffffu, y0, 2), y1 += __shfl_xor_sync(0xffffffffu, y1, 2);
-        if (t == 0) {
-            float* pk = a.prob + (size_t)k * a.stride_k;
-            if (ra < a.n) pk[ra] = 1.0f / (1.0f + __expf(-(y0 + b2)));
-            if (rb < a.n) pk[rb] = 1.0f / (1.0f + __expf(-(y1 + b2)));
-        }
+        const float y = ((t & 1) ? y1 : y0) + b2;
+        const float p = __fdividef(1.0f, 1.0f + __expf(-y));
+        if (store) a.prob[(size_t)k * a.stride_k + rst] = p;
     }
 }
 
@@ -331,7 +322,7 @@ inline uint16_t h16(float v)
 } // namespace
 
 struct GwiTinyPack {
-    uint2 *d_wfg = nullptr, *d_wrs = nullptr, *d_w1 = nullptr;
+    uint2 *d_wfg = nullptr, *d_wrs = nullptr, *d_w1 = nullptr, *d_w1p = nullptr;
     float *d_bias = nullptr, *d_cst = nullptr;
     int halo = 16;
 };
@@ -396,6 +387,19 @@ gwi_status gwi_tiny_pack(gwi_model* m)
     for (int ks = 0; ks < 4; ks++)
         for (int nt = 0; nt < 4; nt++)
             for (int l = 0; l < 32; l++) w1[(ks * 4 + nt) * 32 + l] = frag(B1, 16 * ks, 8 * nt, l);
+    // the same for k_tiny_heads, whose A fragments come from 16-byte row loads: k-step kk of half hb (0: u_H, 1: u_L) pairs
+    // fragment position (2t, 2t+1) with channels 8t + 4kk + (0, 1) and position (2t+8, 2t+9) with channels 8t + 4kk + (2, 3)
+    std::vector<uint2> w1p(16 * 32);
+    for (int hb = 0; hb < 2; hb++)
+        for (int kk = 0; kk < 2; kk++)
+            for (int nt = 0; nt < 4; nt++)
+                for (int l = 0; l < 32; l++) {
+                    const int g = l >> 2, t = l & 3, c0 = 32 * hb + 8 * t + 4 * kk, n = 8 * nt + g;
+                    uint2 r;
+                    r.x = (uint32_t)h16(B1(c0, n)) | ((uint32_t)h16(B1(c0 + 1, n)) << 16);
+                    r.y = (uint32_t)h16(B1(c0 + 2, n)) | ((uint32_t)h16(B1(c0 + 3, n)) << 16);
+                    w1p[((2 * hb + kk) * 4 + nt) * 32 + l] = r;
+                }
     for (int c = 0; c < 32; c++) cst[64 + c] = W[m->off.b1 + c], cst[96 + c] = W[m->off.W2 + c];
     cst[128] = W[m->off.b2];
     auto up = [&](void** dst, const void* src, size_t bytes) -> cudaError_t {
@@ -406,6 +410,7 @@ gwi_status gwi_tiny_pack(gwi_model* m)
     GWI_CUDA_CHECK(up((void**)&p->d_wfg, wfg.data(), wfg.size() * 8));
     GWI_CUDA_CHECK(up((void**)&p->d_wrs, wrs.data(), wrs.size() * 8));
     GWI_CUDA_CHECK(up((void**)&p->d_w1, w1.data(), w1.size() * 8));
+    GWI_CUDA_CHECK(up((void**)&p->d_w1p, w1p.data(), w1p.size() * 8));
     GWI_CUDA_CHECK(up((void**)&p->d_bias, bias.data(), bias.size() * 4));
     GWI_CUDA_CHECK(up((void**)&p->d_cst, cst.data(), cst.size() * 4));
     return GWI_OK;
@@ -415,7 +420,7 @@ void gwi_tiny_free(gwi_model* m)
 {
     GwiTinyPack* p = m->tiny;
     if (!p) return;
-    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_bias), cudaFree(p->d_cst);
+    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_w1p), cudaFree(p->d_bias), cudaFree(p->d_cst);
     delete p;
     m->tiny = nullptr;
 }
@@ -450,7 +455,7 @@ gwi_status gwi_tiny_heads(const gwi_model* m, const __half* d_u16, int64_t lds, 
 {
     const GwiTinyPack* p = m->tiny;
     HeadsArgs a;
-    a.w1 = p->d_w1, a.hcst = p->d_cst + 64, a.u16 = d_u16, a.lds = lds, a.n = n, a.n_lags = n_lags, a.lags = d_lags;
+    a.w1p = p->d_w1p, a.hcst = p->d_cst + 64, a.u16 = d_u16, a.lds = lds, a.n = n, a.n_lags = n_lags, a.lags = d_lags;
     a.prob = d_prob, a.stride_k = stride_k;
     k_tiny_heads<<<(n + 127) / 128, 256, 0, st>>>(a);
     gwi_count_launch(1);
