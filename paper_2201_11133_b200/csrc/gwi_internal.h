@@ -85,8 +85,8 @@ int64_t gwi_tc_max_windows(const gwi_model* m, int32_t T);
 gwi_status gwi_tc_stack(const gwi_model* m, const __half* d_strain, int64_t B, int32_t T, void* d_ws, size_t ws_bytes,
                         cudaStream_t st, const uint8_t** u_out);
 gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, const uint8_t* hist, int R, int64_t nq,
-                              int64_t lag_tiles, int seg_tiles, int warm_tiles, int stream_start, int n_valid, float* d_prob,
-                              cudaStream_t st);
+                              const int64_t* d_lags, int n_lags, int seg_tiles, int warm_tiles, int stream_start, int n_valid,
+                              float* d_prob, int64_t stride_k, cudaStream_t st);
 
 // ---- post-processing (gwi_post.cu) ---------------------------------------------------------------------------
 gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0, float threshold,

@@ -260,11 +260,9 @@ gwi_status tcs_block(gwi_stream* s, int n, bool last, cudaStream_t st)
         const uint8_t* u = nullptr;
         rc = gwi_tc_stack(s->models[m], (const __half*)s->d_segx, B, s->segT, s->d_tcws, s->tcws_bytes, st, &u);
         if (rc != GWI_OK) return rc;
-        for (int k = 0; k < nslides; k++) {
-            rc = gwi_tc_head_stream(s->models[m], u, ntiles, s->d_hist_t[s->hist_t_cur][m], s->Rt, nq, s->lags[k] / 128, seg_tiles,
-                                    warm_tiles, start, n, s->d_prob + ((size_t)k * s->M + m) * s->sub, st);
-            if (rc != GWI_OK) return rc;
-        }
+        rc = gwi_tc_head_stream(s->models[m], u, ntiles, s->d_hist_t[s->hist_t_cur][m], s->Rt, nq, s->d_lags, nslides, seg_tiles,
+                                warm_tiles, start, n, s->d_prob + (size_t)m * s->sub, (int64_t)s->M * s->sub, st);
+        if (rc != GWI_OK) return rc;
         if (s->Rt > 0) {
             k_hist_tiles<<<s->Rt, 256, 0, st>>>(u, ntiles, nq, s->Rt, seg_tiles, warm_tiles, start, s->d_hist_t[s->hist_t_cur][m],
                                                s->d_hist_t[s->hist_t_cur ^ 1][m]);
@@ -439,6 +437,8 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
         }
     }
     if (s->tcs) {
+        if ((e = cudaMalloc(&s->d_lags, (size_t)nslides * 8)) != cudaSuccess) return fail(e);
+        if ((e = cudaMemcpy(s->d_lags, s->lags.data(), (size_t)nslides * 8, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
         const int64_t Bmax = s->sub / s->seg + 1;
         s->acc_cap = s->sub + s->seg + s->xcap;
         if ((e = cudaMalloc(&s->d_segx, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);

@@ -523,13 +523,17 @@ struct HeadArgs {
     int T, ntiles, n_branch;
     // stream mode (mode = 1, gwi_stream.cu tensor-core back end with time slides, reading A24): the items are the nq
     // output tiles of a block of segments; output tile q lives in window q / seg_tiles at tile q % seg_tiles +
-    // warm_tiles (no warm-up in the first window of the stream); the L1 tile is taken lag_tiles earlier, from the
-    // block or, before its start, from hist = the R L1 tiles that precede the block.
+    // warm_tiles (no warm-up in the first window of the stream).  Every lag of the list is evaluated while the H1 tile
+    // of the item sits in shared memory: the L1 tile of lag k is taken lags[k] / 128 tiles earlier, from the block or,
+    // before its start, from hist = the R L1 tiles that precede the block (those tiles were read by the items just
+    // before, so they come from L2); probabilities of lag k go to prob + k * stride_k.
     int mode;
     const uint8_t* hist;
-    int64_t nq, lag_tiles;
-    int R, seg_tiles, warm_tiles, stream_start, n_valid;
+    const int64_t* lags;      // device, samples, multiples of 128
+    int64_t nq, stride_k;
+    int n_lags, R, seg_tiles, warm_tiles, stream_start, n_valid;
 };
+constexpr int HEAD_SMEM_EXTRA = 2048;   // barriers, TMEM slot, b1 | W2 | b2
 constexpr int HEAD_THREADS = 192;   // warps 0-3 epilogue, warp 4 producer, warp 5 MMA
 
 __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
@@ -540,13 +544,16 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
     const int nb = a.n_branch;
     const int W1B = nb * U_TILE_BYTES;            // bytes of W1 blob == bytes of one u stage
     const int OFF_U = W1B, OFF_BAR = W1B + 2 * W1B;
-    // barriers: 0 w1_full, 1-2 u_full[st], 3-4 u_free[st], 5-6 acc_full[st], 7-8 acc_free[st]
+    // barriers: 0 w1_full, 1-2 u_full[st], 3-4 u_free[st], 5-6 acc_full[st], 7-8 acc_free[st]; stream mode: stage st holds
+    // an H1 tile (first half; 9-10 h_full, 11-12 h_free, one per item) and an L1 tile (second half; 1-4, one per lag)
     auto bar = [&](int i) { return sbase + OFF_BAR + 8 * i; };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * 9);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * 13);
+    float* hcs = reinterpret_cast<float*>(smem + OFF_BAR + 256);            // b1[128], W2[128], b2
     if (threadIdx.x == 0) {
-        for (int i = 0; i < 9; i++) mbar_init(bar(i), (i == 7 || i == 8) ? 128u : 1u);
+        for (int i = 0; i < 13; i++) mbar_init(bar(i), (i == 7 || i == 8) ? 128u : 1u);
         mbar_fence_init();
     }
+    for (int i = threadIdx.x; i < 257; i += HEAD_THREADS) hcs[i] = __ldg(a.hc + i);
     if (warp == 4) tmem_alloc(smem_u32(tmem_slot), 256);
     tc_fence_before();
     __syncthreads();
@@ -565,17 +572,29 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
         if (lane == 0) {
             mbar_arrive_expect_tx(bar(0), W1B);
             bulk_g2s(sbase, a.w1, W1B, bar(0));
-            uint32_t n = 0;
+            uint32_t n = 0, c = 0;
             for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x, n++) {
+                if (a.mode) {
+                    const int hs = n & 1;
+                    mbar_wait(bar(11 + hs), ((n >> 1) & 1) ^ 1);
+                    mbar_arrive_expect_tx(bar(9 + hs), U_TILE_BYTES);
+                    bulk_g2s(sbase + OFF_U + hs * W1B, stream_tile(it, 0), U_TILE_BYTES, bar(9 + hs));
+                    for (int k = 0; k < a.n_lags; k++, c++) {
+                        const int ls = c & 1;
+                        mbar_wait(bar(3 + ls), ((c >> 1) & 1) ^ 1);
+                        mbar_arrive_expect_tx(bar(1 + ls), U_TILE_BYTES);
+                        bulk_g2s(sbase + OFF_U + ls * W1B + U_TILE_BYTES, stream_tile(it - __ldg(a.lags + k) / TM, 1), U_TILE_BYTES,
+                                 bar(1 + ls));
+                    }
+                    continue;
+                }
                 const int st = n & 1;
                 const int64_t wl = it / a.ntiles, j = it % a.ntiles;
                 mbar_wait(bar(3 + st), ((n >> 1) & 1) ^ 1);
                 mbar_arrive_expect_tx(bar(1 + st), W1B);
-                for (int b = 0; b < nb; b++) {
-                    const uint8_t* src = a.mode ? stream_tile(b == 0 ? it : it - a.lag_tiles, b)
-                                                : a.u + (((size_t)wl * nb + b) * a.ntiles + j) * U_TILE_BYTES;
-                    bulk_g2s(sbase + OFF_U + st * W1B + b * U_TILE_BYTES, src, U_TILE_BYTES, bar(1 + st));
-                }
+                for (int b = 0; b < nb; b++)
+                    bulk_g2s(sbase + OFF_U + st * W1B + b * U_TILE_BYTES, a.u + (((size_t)wl * nb + b) * a.ntiles + j) * U_TILE_BYTES,
+                             U_TILE_BYTES, bar(1 + st));
             }
         }
         __syncwarp();
@@ -583,8 +602,29 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
         if (lane == 0) {
             const uint32_t idesc = make_idesc_f16(128, 128);
             mbar_wait(bar(0), 0);
-            uint32_t n = 0;
+            uint32_t n = 0, c = 0;
             for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x, n++) {
+                if (a.mode) {
+                    const int hs = n & 1;
+                    mbar_wait(bar(9 + hs), (n >> 1) & 1);
+                    for (int k = 0; k < a.n_lags; k++, c++) {
+                        const int ls = c & 1;
+                        const uint32_t ph = (c >> 1) & 1;
+                        mbar_wait(bar(1 + ls), ph);
+                        mbar_wait(bar(7 + ls), ph ^ 1);
+                        tc_fence_after();
+                        for (int kk = 0; kk < 8; kk++)
+                            tc_mma_f16(tmem + 128 * ls, make_sdesc(sbase + OFF_U + hs * W1B + 2 * kk * 2048, 2048, 128),
+                                       make_sdesc(sbase + 2 * kk * 2048, 2048, 128), idesc, kk > 0 ? 1u : 0u);
+                        for (int kk = 0; kk < 8; kk++)
+                            tc_mma_f16(tmem + 128 * ls, make_sdesc(sbase + OFF_U + ls * W1B + U_TILE_BYTES + 2 * kk * 2048, 2048, 128),
+                                       make_sdesc(sbase + 2 * (8 + kk) * 2048, 2048, 128), idesc, 1u);
+                        tc_commit(bar(5 + ls));
+                        tc_commit(bar(3 + ls));
+                    }
+                    tc_commit(bar(11 + hs));
+                    continue;
+                }
                 const int st = n & 1;
                 const uint32_t ph = (n >> 1) & 1;
                 mbar_wait(bar(1 + st), ph);
@@ -601,35 +641,49 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
     } else {
         const int r = warp * 32 + lane;
         const uint32_t lane_t = tmem + ((uint32_t)(warp * 32) << 16);
-        const float b2 = __ldg(a.hc + 256);
-        uint32_t n = 0;
-        for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x, n++) {
-            const int st = n & 1;
-            const uint32_t ph = (n >> 1) & 1;
-            const int64_t wl = it / a.ntiles, j = it % a.ntiles;
-            mbar_wait(bar(5 + st), ph);
-            tc_fence_after();
+        const float4* b1s = reinterpret_cast<const float4*>(hcs);
+        const float4* w2s = reinterpret_cast<const float4*>(hcs + 128);
+        const float b2 = hcs[256];
+        // y = W2 . ReLU(acc + b1) + b2 of this thread's row from accumulator buffer `as`, then the buffer is released
+        auto finish = [&](int as) {
             float y = b2;
 #pragma unroll
             for (int cc = 0; cc < 4; cc++) {
                 uint32_t v[32];
-                tmem_ld32(lane_t + 128 * st + 32 * cc, v);
+                tmem_ld32(lane_t + 128 * as + 32 * cc, v);
                 tc_wait_ld();
 #pragma unroll
-                for (int c = 0; c < 32; c++) {
-                    float hv = fmaxf(__uint_as_float(v[c]) + __ldg(a.hc + 32 * cc + c), 0.f);
-                    y = fmaf(__ldg(a.hc + 128 + 32 * cc + c), hv, y);
+                for (int c = 0; c < 8; c++) {
+                    const float4 bb = b1s[8 * cc + c], ww = w2s[8 * cc + c];
+                    y = fmaf(ww.x, fmaxf(__uint_as_float(v[4 * c]) + bb.x, 0.f), y);
+                    y = fmaf(ww.y, fmaxf(__uint_as_float(v[4 * c + 1]) + bb.y, 0.f), y);
+                    y = fmaf(ww.z, fmaxf(__uint_as_float(v[4 * c + 2]) + bb.z, 0.f), y);
+                    y = fmaf(ww.w, fmaxf(__uint_as_float(v[4 * c + 3]) + bb.w, 0.f), y);
                 }
             }
             tc_fence_before();
-            mbar_arrive(bar(7 + st));
+            mbar_arrive(bar(7 + as));
+            return 1.0f / (1.0f + __expf(-y));
+        };
+        uint32_t n = 0, c = 0;
+        for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x, n++) {
             if (a.mode) {
                 const int64_t t = it * TM + r;
-                if (t < a.n_valid) a.prob[t] = 1.0f / (1.0f + __expf(-y));
-            } else {
-                const int t = (int)j * TM + r;
-                if (t < a.T) a.prob[(size_t)(a.w0 + wl) * a.T + t] = 1.0f / (1.0f + __expf(-y));
+                for (int k = 0; k < a.n_lags; k++, c++) {
+                    mbar_wait(bar(5 + (c & 1)), (c >> 1) & 1);
+                    tc_fence_after();
+                    const float pr = finish(c & 1);
+                    if (t < a.n_valid) a.prob[(size_t)k * a.stride_k + t] = pr;
+                }
+                continue;
             }
+            const int st = n & 1;
+            const int64_t wl = it / a.ntiles, j = it % a.ntiles;
+            mbar_wait(bar(5 + st), (n >> 1) & 1);
+            tc_fence_after();
+            const float pr = finish(st);
+            const int t = (int)j * TM + r;
+            if (t < a.T) a.prob[(size_t)(a.w0 + wl) * a.T + t] = pr;
         }
     }
     tc_fence_before();
@@ -742,7 +796,7 @@ gwi_status gwi_tc_pack(gwi_model* m)
     GWI_CUDA_CHECK(cudaGetDeviceProperties(&prop, m->device));
     p->num_sms = prop.multiProcessorCount;
     GWI_CUDA_CHECK(cudaFuncSetAttribute(k_stack, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_TOTAL));
-    GWI_CUDA_CHECK(cudaFuncSetAttribute(k_head_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 2 * U_TILE_BYTES + 256));
+    GWI_CUDA_CHECK(cudaFuncSetAttribute(k_head_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 2 * U_TILE_BYTES + HEAD_SMEM_EXTRA));
     return GWI_OK;
 }
 
@@ -800,11 +854,11 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
         k_stack<<<grid, NTHREADS, SM_TOTAL, st>>>(sa);
         HeadArgs ha;
         ha.w1 = p->d_w1, ha.hc = p->d_hc, ha.u = u, ha.prob = d_prob, ha.w0 = w0, ha.nwin = nwin, ha.T = T, ha.ntiles = ntiles,
-        ha.n_branch = nb, ha.mode = 0, ha.hist = nullptr, ha.nq = 0, ha.lag_tiles = 0, ha.R = 0, ha.seg_tiles = 0, ha.warm_tiles = 0,
-        ha.stream_start = 0, ha.n_valid = 0;
+        ha.n_branch = nb, ha.mode = 0, ha.hist = nullptr, ha.lags = nullptr, ha.nq = 0, ha.stride_k = 0, ha.n_lags = 0, ha.R = 0,
+        ha.seg_tiles = 0, ha.warm_tiles = 0, ha.stream_start = 0, ha.n_valid = 0;
         int64_t nitems = nwin * ntiles;
         int hgrid = (int)(nitems < p->num_sms ? nitems : p->num_sms);
-        k_head_tc<<<hgrid, HEAD_THREADS, 3 * nb * U_TILE_BYTES + 256, st>>>(ha);
+        k_head_tc<<<hgrid, HEAD_THREADS, 3 * nb * U_TILE_BYTES + HEAD_SMEM_EXTRA, st>>>(ha);
         gwi_count_launch(2);
         GWI_CUDA_CHECK(cudaGetLastError());
 #ifdef GWI_TC_TRACE
@@ -860,18 +914,23 @@ gwi_status gwi_tc_stack(const gwi_model* m, const __half* d_strain, int64_t B, i
     return GWI_OK;
 }
 
-// Head of one lag over the nq output tiles of a block (see HeadArgs, stream mode).
+// Heads of all lags over the nq output tiles of a block (see HeadArgs, stream mode); d_lags: device array of n_lags lags
+// in samples (multiples of 128); probabilities of lag k at d_prob + k * stride_k.
 gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, const uint8_t* hist, int R, int64_t nq,
-                              int64_t lag_tiles, int seg_tiles, int warm_tiles, int stream_start, int n_valid, float* d_prob,
-                              cudaStream_t st)
+                              const int64_t* d_lags, int n_lags, int seg_tiles, int warm_tiles, int stream_start, int n_valid,
+                              float* d_prob, int64_t stride_k, cudaStream_t st)
 {
     const GwiTcPack* p = m->tc;
+    if (m->arch.n_branch != 2) {
+        gwi_set_error("gwi_tc_head_stream: two branches expected");
+        return GWI_ERR_UNSUPPORTED;
+    }
     HeadArgs ha;
     ha.w1 = p->d_w1, ha.hc = p->d_hc, ha.u = u, ha.prob = d_prob, ha.w0 = 0, ha.nwin = 0, ha.T = 0, ha.ntiles = ntiles;
-    ha.n_branch = m->arch.n_branch, ha.mode = 1, ha.hist = hist, ha.nq = nq, ha.lag_tiles = lag_tiles, ha.R = R;
+    ha.n_branch = 2, ha.mode = 1, ha.hist = hist, ha.lags = d_lags, ha.nq = nq, ha.stride_k = stride_k, ha.n_lags = n_lags, ha.R = R;
     ha.seg_tiles = seg_tiles, ha.warm_tiles = warm_tiles, ha.stream_start = stream_start, ha.n_valid = n_valid;
     int hgrid = (int)(nq < p->num_sms ? nq : p->num_sms);
-    k_head_tc<<<hgrid, HEAD_THREADS, 3 * ha.n_branch * U_TILE_BYTES + 256, st>>>(ha);
+    k_head_tc<<<hgrid, HEAD_THREADS, 3 * ha.n_branch * U_TILE_BYTES + HEAD_SMEM_EXTRA, st>>>(ha);
     gwi_count_launch(1);
     GWI_CUDA_CHECK(cudaGetLastError());
     return GWI_OK;
