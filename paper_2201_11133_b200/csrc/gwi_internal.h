@@ -82,6 +82,7 @@ gwi_status gwi_generic_stream_head(const gwi_model* m, const float* skip, int64_
                                    cudaStream_t st);
 
 int64_t gwi_tc_max_windows(const gwi_model* m, int32_t T);
+int gwi_tc_num_sms(const gwi_model* m);
 gwi_status gwi_tc_stack(const gwi_model* m, const __half* d_strain, int64_t B, int32_t T, void* d_ws, size_t ws_bytes,
                         cudaStream_t st, const uint8_t** u_out);
 gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, const uint8_t* hist, int R, int64_t nq,

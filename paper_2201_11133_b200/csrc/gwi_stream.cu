@@ -62,7 +62,8 @@ struct gwi_stream {
     void* d_carry_pm = nullptr;             // per-model rule: [n_slides][M] carry blocks
     // tensor-core back end (paper-scale models, FP16 mode, zero lag only)
     bool tcb = false;
-    int seg = 0, segT = 0, segH = 0;        // outputs per segment, window length H + seg, warm-up H = R_f - 1
+    int seg = 0, segT = 0, segH = 0;        // outputs per segment, window length H + seg, warm-up H = R_f - 1 (seg, segT: of the
+    int segT0 = 0;                          // current block, chosen by pick_seg; segT0 = the shortest window length)
     __half2* d_segx = nullptr;              // [B][segT][2] channels-last batch
     float* d_segp = nullptr;                // [B][segT] probabilities of the batch
     void* d_tcws = nullptr;
@@ -133,6 +134,27 @@ size_t elt(const gwi_stream* s) { return s->half_in ? 2 : 4; }
 
 gwi_status post_block(gwi_stream* s, int n, bool last, cudaStream_t st);
 
+constexpr int SEGT_MAX = 131072;   // longest segment window (samples)
+
+// Segment length for a block of n samples (tensor-core back ends).  The persistent k_stack grid works through
+// jobs = 2 branches x pairs of segments in ceil(jobs / SMs) rounds, each as long as one segment window, and every
+// segment recomputes segH warm-up samples: the window length (whole tiles) with the smallest rounds x length wins,
+// ties go to the shorter one.  An hour of 4096 Hz data gives 148 segments of 101 760 samples (one round, 2 % warm-up)
+// instead of 1029 of 16 384 (seven rounds, 12.5 % warm-up).  Results do not depend on the segmentation: every output
+// sees its whole receptive field either way.
+void pick_seg(gwi_stream* s, int64_t n)
+{
+    const int sms = gwi_tc_num_sms(s->models[0]);
+    int best = s->segT0;
+    int64_t best_cost = INT64_MAX;
+    for (int segT = s->segT0; segT <= SEGT_MAX; segT += 128) {
+        const int64_t seg = segT - s->segH;
+        const int64_t B = (n + seg - 1) / seg, jobs = ((B + 1) / 2) * 2, rounds = (jobs + sms - 1) / sms;
+        if (rounds * segT < best_cost) best_cost = rounds * segT, best = segT;
+    }
+    s->segT = best, s->seg = best - s->segH;
+}
+
 // one sub-chunk of n <= sub samples, already in staging buffer `xb` at column `x0`
 gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStream_t st)
 {
@@ -143,6 +165,7 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
         float* skip0 = (s->tiny || s->tcb || s->tcs) ? nullptr : s->d_skip[m] + s->maxlag;
         gwi_status rc;
         if (s->tcb) {
+            if (m == 0) pick_seg(s, n);
             const int B = (n + s->seg - 1) / s->seg;
             const int start = s->t_done == 0 ? 1 : 0;
             if (m == 0) {
@@ -283,9 +306,12 @@ gwi_status tcs_append_and_run(gwi_stream* s, int xb, int64_t n, cudaStream_t st)
                                      cudaMemcpyDeviceToDevice, st));
     s->pend += n, s->t_recv += n;
     const bool final = s->t_recv == s->N_total;
-    while (s->pend >= s->seg || (final && s->pend > 0)) {
-        int64_t proc = final ? s->pend : (s->pend / s->seg) * s->seg;
-        if (proc > s->sub) proc = s->sub;
+    const int seg0 = s->segT0 - s->segH;
+    while (s->pend >= seg0 || (final && s->pend > 0)) {
+        const int64_t avail = std::min<int64_t>(s->pend, s->sub);
+        pick_seg(s, avail);
+        int64_t proc = (final && avail == s->pend) ? avail : (avail / s->seg) * s->seg;
+        if (proc == 0) s->segT = s->segT0, s->seg = seg0, proc = (avail / seg0) * seg0;
         const bool last = final && proc == s->pend;
         gwi_status rc = tcs_block(s, (int)proc, last, st);
         if (rc != GWI_OK) return rc;
@@ -383,6 +409,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
         s->segH = s->Rf - 1;
         s->segT = ((s->segH + 8192 + 127) / 128) * 128;    // >= 8192 outputs per segment, whole tiles
         if (s->segT < 16384) s->segT = 16384;
+        s->segT0 = s->segT;
         s->seg = s->segT - s->segH;
         s->halo = s->segH;
     }
@@ -394,6 +421,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     if (s->tcs) {
         s->segH = ((s->Rf - 1 + 127) / 128) * 128;
         s->segT = s->segH + 8192 < 16384 ? 16384 : s->segH + 8192;
+        s->segT0 = s->segT;
         s->seg = s->segT - s->segH;
         s->halo = s->segH;
         s->Rt = (int)(s->maxlag / 128);
@@ -426,7 +454,8 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
         if ((e = cudaMalloc(&s->d_x[b], (size_t)C * s->xcap * elt(s))) != cudaSuccess) return fail(e);
     size_t hbytes = (size_t)s->nb * s->R * s->sub * 4;
     if (s->tcb) {
-        const int64_t Bmax = (s->sub + s->seg - 1) / s->seg;
+        // any segment length of pick_seg: B * segT <= n * segT0 / seg0 + SEGT_MAX samples
+        const int64_t Bmax = ((int64_t)((double)s->sub * s->segT0 / s->seg) + 2 * SEGT_MAX) / s->segT0 + 1;
         if ((e = cudaMalloc(&s->d_segx, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);
         if ((e = cudaMalloc(&s->d_segp, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);
         s->tcws_bytes = gwi_tc_workspace_bytes(m0, Bmax, s->segT);
@@ -439,8 +468,8 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     if (s->tcs) {
         if ((e = cudaMalloc(&s->d_lags, (size_t)nslides * 8)) != cudaSuccess) return fail(e);
         if ((e = cudaMemcpy(s->d_lags, s->lags.data(), (size_t)nslides * 8, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
-        const int64_t Bmax = s->sub / s->seg + 1;
-        s->acc_cap = s->sub + s->seg + s->xcap;
+        const int64_t Bmax = ((int64_t)((double)s->sub * s->segT0 / s->seg) + 2 * SEGT_MAX) / s->segT0 + 1;
+        s->acc_cap = s->sub + SEGT_MAX + s->xcap;
         if ((e = cudaMalloc(&s->d_segx, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);
         s->tcws_bytes = gwi_tc_workspace_bytes(m0, Bmax, s->segT);
         if ((e = cudaMalloc(&s->d_tcws, s->tcws_bytes)) != cudaSuccess) return fail(e);
@@ -570,6 +599,7 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
         GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_xh[0] + H + (H - pre), l1_tail, (size_t)pre * 2, cudaMemcpyDefault, st));
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_acc, 0, (size_t)n * 2, st));
         GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_acc + s->acc_cap, (const __half*)l1_tail + pre, (size_t)n * 2, cudaMemcpyDefault, st));
+        pick_seg(s, n);
         const int B = (int)((n + s->seg - 1) / s->seg);
         const int64_t total = (int64_t)B * s->segT;
         k_seg_gather<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(s->d_acc, s->acc_cap, s->d_xh[0], (int)n, s->seg, H, s->segT, 0,

@@ -884,6 +884,8 @@ int64_t gwi_tc_max_windows(const gwi_model* m, int32_t T)
     return cap < 296 ? 296 : cap;
 }
 
+int gwi_tc_num_sms(const gwi_model* m) { return m->tc->num_sms; }
+
 // Branch stacks only: B windows (B <= gwi_tc_max_windows) -> u tiles [B][n_branch][ntiles][U_TILE_BYTES] at *u_out
 // inside the workspace (same layout as gwi_tc_infer uses between its two kernels).
 gwi_status gwi_tc_stack(const gwi_model* m, const __half* d_strain, int64_t B, int32_t T, void* d_ws, size_t ws_bytes,

@@ -329,3 +329,39 @@ def test_stream_paper_scale_slides_tensor_core_back_end(tmpdir_s):
     assert np.array_equal(p0, p1)
     assert trig_tuples(r0) == trig_tuples(r1)
     assert trig_tuples(r0) == _oracle_triggers(p0.astype(np.float64), float(np.float32(0.5)), 16)
+
+
+@pytest.mark.parametrize("lags", [[], [4096, 12800]])
+def test_paper_scale_long_block_segment_choice(tmpdir_s, lags):
+    """A block long enough that the tensor-core back ends pick segments longer than the minimum (pick_seg: > 296
+    minimum-length segments per launch): one 6 M-sample push against the same stream in 1 M-sample pushes (minimum-length
+    segments) bit for bit, and sampled spans against the oracle evaluated on those spans alone."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0], gwi.FP16, arch=gs.PAPER_ARCH)
+    N = 128 * 46872
+    g = torch.Generator().manual_seed(11)
+    xt = torch.randn((2, N), generator=g).to(torch.float16)
+    xd = xt.cuda()
+    outs = []
+    for chunk in (N, 1 << 20):
+        st = gwi.Stream(gms, N, chunk, 0.5, 2048, lags=lags, capacity=4096, want_pbar=True)
+        if lags:
+            st.prime(xd[1, N - st.tail_samples:].contiguous())
+        for p in range(0, N, chunk):
+            st.push(xd[0, p:p + chunk].contiguous(), xd[1, p:p + chunk].contiguous())
+        n, recs = st.finish()
+        outs.append((n, trig_tuples(recs), st.pbar.cpu().numpy()))
+        st.close()
+    assert outs[0][0] == outs[1][0] and outs[0][1] == outs[1][1]
+    assert np.array_equal(outs[0][2], outs[1][2])
+    pb = outs[0][2]
+    assert np.isfinite(pb).all() and 0.0 <= pb.min() and pb.max() <= 1.0
+    x = xt.numpy()
+    rf = gms[0].receptive_field
+    for s0 in [0, 40578 - 2100, 2_999_000, N - rf - 300]:
+        span = x[:, s0:s0 + rf + 300].astype(np.float64)
+        want = oms[0].stream(span)
+        lo = 0 if s0 == 0 else rf - 1
+        got = pb[0, s0:s0 + rf + 300]
+        assert np.max(np.abs(got[lo:] - want[lo:])) <= 2e-3
