@@ -534,7 +534,7 @@ struct HeadArgs {
     int n_lags, R, seg_tiles, warm_tiles, stream_start, n_valid;
 };
 constexpr int HEAD_SMEM_EXTRA = 2048;   // barriers, TMEM slot, b1 | W2 | b2
-constexpr int HEAD_THREADS = 192;   // warps 0-3 epilogue, warp 4 producer, warp 5 MMA
+constexpr int HEAD_THREADS = 320;   // warps 0-7 epilogue (warps 0-3: accumulator buffer 0, warps 4-7: buffer 1), warp 8 producer, warp 9 MMA
 
 __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
 {
@@ -554,7 +554,7 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
         mbar_fence_init();
     }
     for (int i = threadIdx.x; i < 257; i += HEAD_THREADS) hcs[i] = __ldg(a.hc + i);
-    if (warp == 4) tmem_alloc(smem_u32(tmem_slot), 256);
+    if (warp == 8) tmem_alloc(smem_u32(tmem_slot), 256);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -568,7 +568,7 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
         return a.u + (((size_t)w * nb + b) * a.ntiles + tl) * U_TILE_BYTES;
     };
 
-    if (warp == 4) {
+    if (warp == 8) {
         if (lane == 0) {
             mbar_arrive_expect_tx(bar(0), W1B);
             bulk_g2s(sbase, a.w1, W1B, bar(0));
@@ -598,7 +598,7 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
             }
         }
         __syncwarp();
-    } else if (warp == 5) {
+    } else if (warp == 9) {
         if (lane == 0) {
             const uint32_t idesc = make_idesc_f16(128, 128);
             mbar_wait(bar(0), 0);
@@ -639,14 +639,16 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
         }
         __syncwarp();
     } else {
-        const int r = warp * 32 + lane;
-        const uint32_t lane_t = tmem + ((uint32_t)(warp * 32) << 16);
+        // the two accumulator buffers alternate, each has its own four warps (one per TMEM lane quadrant), so that the
+        // epilogue of one tile overlaps the whole MMA time of the next
+        const int set = warp >> 2, r = (warp & 3) * 32 + lane;
+        const uint32_t lane_t = tmem + ((uint32_t)((warp & 3) * 32) << 16);
         const float4* b1s = reinterpret_cast<const float4*>(hcs);
         const float4* w2s = reinterpret_cast<const float4*>(hcs + 128);
         const float b2 = hcs[256];
         // y = W2 . ReLU(acc + b1) + b2 of this thread's row from accumulator buffer `as`, then the buffer is released
         auto finish = [&](int as) {
-            float y = b2;
+            float y0 = 0.f, y1 = 0.f, y2 = 0.f, y3 = 0.f;       // four independent chains over the 128 channels
 #pragma unroll
             for (int cc = 0; cc < 4; cc++) {
                 uint32_t v[32];
@@ -655,12 +657,13 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
 #pragma unroll
                 for (int c = 0; c < 8; c++) {
                     const float4 bb = b1s[8 * cc + c], ww = w2s[8 * cc + c];
-                    y = fmaf(ww.x, fmaxf(__uint_as_float(v[4 * c]) + bb.x, 0.f), y);
-                    y = fmaf(ww.y, fmaxf(__uint_as_float(v[4 * c + 1]) + bb.y, 0.f), y);
-                    y = fmaf(ww.z, fmaxf(__uint_as_float(v[4 * c + 2]) + bb.z, 0.f), y);
-                    y = fmaf(ww.w, fmaxf(__uint_as_float(v[4 * c + 3]) + bb.w, 0.f), y);
+                    y0 = fmaf(ww.x, fmaxf(__uint_as_float(v[4 * c]) + bb.x, 0.f), y0);
+                    y1 = fmaf(ww.y, fmaxf(__uint_as_float(v[4 * c + 1]) + bb.y, 0.f), y1);
+                    y2 = fmaf(ww.z, fmaxf(__uint_as_float(v[4 * c + 2]) + bb.z, 0.f), y2);
+                    y3 = fmaf(ww.w, fmaxf(__uint_as_float(v[4 * c + 3]) + bb.w, 0.f), y3);
                 }
             }
+            const float y = ((y0 + y1) + (y2 + y3)) + b2;
             tc_fence_before();
             mbar_arrive(bar(7 + as));
             return 1.0f / (1.0f + __expf(-y));
@@ -670,25 +673,26 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
             if (a.mode) {
                 const int64_t t = it * TM + r;
                 for (int k = 0; k < a.n_lags; k++, c++) {
-                    mbar_wait(bar(5 + (c & 1)), (c >> 1) & 1);
+                    if ((int)(c & 1) != set) continue;
+                    mbar_wait(bar(5 + set), (c >> 1) & 1);
                     tc_fence_after();
-                    const float pr = finish(c & 1);
+                    const float pr = finish(set);
                     if (t < a.n_valid) a.prob[(size_t)k * a.stride_k + t] = pr;
                 }
                 continue;
             }
-            const int st = n & 1;
+            if ((int)(n & 1) != set) continue;
             const int64_t wl = it / a.ntiles, j = it % a.ntiles;
-            mbar_wait(bar(5 + st), (n >> 1) & 1);
+            mbar_wait(bar(5 + set), (n >> 1) & 1);
             tc_fence_after();
-            const float pr = finish(st);
+            const float pr = finish(set);
             const int t = (int)j * TM + r;
             if (t < a.T) a.prob[(size_t)(a.w0 + wl) * a.T + t] = pr;
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 4) tmem_dealloc(tmem, 256);
+    if (warp == 8) tmem_dealloc(tmem, 256);
 }
 
 } // namespace
