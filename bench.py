@@ -126,7 +126,7 @@ def stream_bench(dev, work, rank, n_chunks=744):
             st.close()
         ms = float(np.median(times[1:]))
         out["hour_paper_scale"] = {"workload": "4 paper-scale models (2x20 blocks, R64/S128), 1 h stream, FP16, resident in HBM; "
-                                               "segments of 14338 outputs + 2046 recomputed warm-up samples through k_stack",
+                                               "148 segments of 99714 outputs + 2046 recomputed warm-up samples through k_stack in one launch per model",
                                    "ms": ms, "strain_seconds_per_s": 3600 / (ms * 1e-3), "triggers": n,
                                    "tflops_algorithmic": gs.PAPER_ARCH.flops_per_timestep() * N1 * 4 / (ms * 1e-3) / 1e12}
         # the same with 32 one-second time slides (paper-scale background estimation)
