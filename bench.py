@@ -71,7 +71,7 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(self.rows)}
 
 
-def stream_bench(dev, work, rank, n_chunks=744):
+def stream_bench(dev, work, rank, n_chunks=744, paper_month=False):
     """Extra, reported beside the headline: the streaming ensemble path (gwi_stream_*) on the config-1 architecture.
     hour  = BASELINE.json configs[2]: 4-model ensemble, 1 h two-detector stream resident in HBM, one push + finish.
     month = configs[4]: 744 one-hour chunks pushed from pinned host buffers (H2D on the side stream inside the timed
@@ -147,6 +147,25 @@ def stream_bench(dev, work, rank, n_chunks=744):
         out["hour_paper_scale_32_slides"] = {"workload": "4 paper-scale models, 1 h stream, zero lag + 32 circular lags of k x 1 s, FP16",
                                              "ms": ms, "strain_seconds_per_s": 3600 / (ms * 1e-3),
                                              "slid_strain_seconds_per_s": 33 * 3600 / (ms * 1e-3), "triggers": n}
+        if paper_month:
+            # the month through the 4 x paper-scale ensemble, streamed from pinned host memory
+            for name, lg in (("month_paper_scale", []), ("month_paper_scale_32_slides", lags)):
+                st = gwi.Stream(pm, n_chunks * N1, N1, THETA, LMIN, lags=lg, capacity=65536)
+                if lg:
+                    st.prime(host[(n_chunks - 1) & 1][1, N1 - st.tail_samples:].contiguous())
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                for c in range(n_chunks):
+                    h = host[c & 1]
+                    st.push(h[0], h[1])
+                n, _ = st.finish()
+                torch.cuda.synchronize()
+                dt = time.perf_counter() - t0
+                st.close()
+                out[name] = {"workload": f"{n_chunks} one-hour chunks from pinned host memory, 4 paper-scale models, "
+                                         f"{1 + len(lg)} slide(s), FP16", "wall_s": dt,
+                             "strain_seconds_per_s": n_chunks * 3600 / dt,
+                             "slid_strain_seconds_per_s": (1 + len(lg)) * n_chunks * 3600 / dt, "triggers": n}
         del pm
     except Exception as ex:
         out["hour_paper_scale"] = {"error": repr(ex)}
@@ -265,6 +284,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stream", action="store_true", help="skip the extra streaming-ensemble measurements")
     ap.add_argument("--stream-chunks", type=int, default=744, help="one-hour chunks of the month-long stream leg")
+    ap.add_argument("--paper-month", action="store_true",
+                    help="also stream the month through the 4 x paper-scale ensemble, without and with 32 slides (about 7 minutes)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -369,7 +390,7 @@ def main():
     stream_extra = None
     if not args.no_stream and world == 1:
         try:
-            stream_extra = stream_bench(dev, work, rank, args.stream_chunks)
+            stream_extra = stream_bench(dev, work, rank, args.stream_chunks, args.paper_month)
         except Exception as ex:  # the headline line must still come out
             stream_extra = {"error": repr(ex)}
 
