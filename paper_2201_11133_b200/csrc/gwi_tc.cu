@@ -534,6 +534,7 @@ struct HeadArgs {
     int n_lags, R, seg_tiles, warm_tiles, stream_start, n_valid;
 };
 constexpr int HEAD_SMEM_EXTRA = 2048;   // barriers, TMEM slot, b1 | W2 | b2
+constexpr int HEAD_SMEM = 7 * U_TILE_BYTES + HEAD_SMEM_EXTRA;   // W1 (2 tiles) + 5 feature-tile buffers
 constexpr int HEAD_THREADS = 320;   // warps 0-7 epilogue (warps 0-3: accumulator buffer 0, warps 4-7: buffer 1), warp 8 producer, warp 9 MMA
 
 __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
@@ -543,14 +544,18 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nb = a.n_branch;
     const int W1B = nb * U_TILE_BYTES;            // bytes of W1 blob == bytes of one u stage
-    const int OFF_U = W1B, OFF_BAR = W1B + 2 * W1B;
-    // barriers: 0 w1_full, 1-2 u_full[st], 3-4 u_free[st], 5-6 acc_full[st], 7-8 acc_free[st]; stream mode: stage st holds
-    // an H1 tile (first half; 9-10 h_full, 11-12 h_free, one per item) and an L1 tile (second half; 1-4, one per lag)
+    const int OFF_U = W1B, OFF_BAR = 7 * U_TILE_BYTES;
+    const int OFF_L = OFF_U + 2 * U_TILE_BYTES;   // stream mode: two H1 tile buffers at OFF_U, three L1 tile buffers at OFF_L
+    // barriers: 0 w1_full, 1-2 u_full[st], 3-4 u_free[st], 5-6 acc_full[st], 7-8 acc_free[st]; stream mode: H1 tiles (one
+    // per item) 9-10 h_full, 11-12 h_free; L1 tiles (one per lag, three buffers: a 32 KB tile takes about two MMA
+    // times to arrive from L2) l_full 1, 2, 13 and l_free 3, 4, 14
     auto bar = [&](int i) { return sbase + OFF_BAR + 8 * i; };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * 13);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * 16);
+    auto l_full = [&](int ls) { return bar(ls < 2 ? 1 + ls : 13); };
+    auto l_free = [&](int ls) { return bar(ls < 2 ? 3 + ls : 14); };
     float* hcs = reinterpret_cast<float*>(smem + OFF_BAR + 256);            // b1[128], W2[128], b2
     if (threadIdx.x == 0) {
-        for (int i = 0; i < 13; i++) mbar_init(bar(i), (i == 7 || i == 8) ? 128u : 1u);
+        for (int i = 0; i < 15; i++) mbar_init(bar(i), (i == 7 || i == 8) ? 128u : 1u);
         mbar_fence_init();
     }
     for (int i = threadIdx.x; i < 257; i += HEAD_THREADS) hcs[i] = __ldg(a.hc + i);
@@ -578,13 +583,13 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
                     const int hs = n & 1;
                     mbar_wait(bar(11 + hs), ((n >> 1) & 1) ^ 1);
                     mbar_arrive_expect_tx(bar(9 + hs), U_TILE_BYTES);
-                    bulk_g2s(sbase + OFF_U + hs * W1B, stream_tile(it, 0), U_TILE_BYTES, bar(9 + hs));
+                    bulk_g2s(sbase + OFF_U + hs * U_TILE_BYTES, stream_tile(it, 0), U_TILE_BYTES, bar(9 + hs));
                     for (int k = 0; k < a.n_lags; k++, c++) {
-                        const int ls = c & 1;
-                        mbar_wait(bar(3 + ls), ((c >> 1) & 1) ^ 1);
-                        mbar_arrive_expect_tx(bar(1 + ls), U_TILE_BYTES);
-                        bulk_g2s(sbase + OFF_U + ls * W1B + U_TILE_BYTES, stream_tile(it - __ldg(a.lags + k) / TM, 1), U_TILE_BYTES,
-                                 bar(1 + ls));
+                        const int ls = c % 3;
+                        mbar_wait(l_free(ls), ((c / 3) & 1) ^ 1);
+                        mbar_arrive_expect_tx(l_full(ls), U_TILE_BYTES);
+                        bulk_g2s(sbase + OFF_L + ls * U_TILE_BYTES, stream_tile(it - __ldg(a.lags + k) / TM, 1), U_TILE_BYTES,
+                                 l_full(ls));
                     }
                     continue;
                 }
@@ -599,28 +604,33 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
         }
         __syncwarp();
     } else if (warp == 9) {
-        if (lane == 0) {
+        // one elected thread issues; under elect_one() the compiler keeps the descriptors in uniform registers and the
+        // unrolled tcgen05.mma go out back to back (the address field of a descriptor counts 16-byte units)
+        if (elect_one()) {
             const uint32_t idesc = make_idesc_f16(128, 128);
+            const uint64_t dW = make_sdesc(sbase, 2048, 128);
+            const uint64_t dU = make_sdesc(sbase + OFF_U, 2048, 128);
+            const uint64_t dL = make_sdesc(sbase + OFF_L, 2048, 128);
             mbar_wait(bar(0), 0);
             uint32_t n = 0, c = 0;
             for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x, n++) {
                 if (a.mode) {
                     const int hs = n & 1;
                     mbar_wait(bar(9 + hs), (n >> 1) & 1);
+                    const uint64_t dh = dU + hs * (U_TILE_BYTES >> 4);
                     for (int k = 0; k < a.n_lags; k++, c++) {
-                        const int ls = c & 1;
-                        const uint32_t ph = (c >> 1) & 1;
-                        mbar_wait(bar(1 + ls), ph);
-                        mbar_wait(bar(7 + ls), ph ^ 1);
+                        const int ls = c % 3, as = c & 1;
+                        mbar_wait(l_full(ls), (c / 3) & 1);
+                        mbar_wait(bar(7 + as), ((c >> 1) & 1) ^ 1);
                         tc_fence_after();
-                        for (int kk = 0; kk < 8; kk++)
-                            tc_mma_f16(tmem + 128 * ls, make_sdesc(sbase + OFF_U + hs * W1B + 2 * kk * 2048, 2048, 128),
-                                       make_sdesc(sbase + 2 * kk * 2048, 2048, 128), idesc, kk > 0 ? 1u : 0u);
-                        for (int kk = 0; kk < 8; kk++)
-                            tc_mma_f16(tmem + 128 * ls, make_sdesc(sbase + OFF_U + ls * W1B + U_TILE_BYTES + 2 * kk * 2048, 2048, 128),
-                                       make_sdesc(sbase + 2 * (8 + kk) * 2048, 2048, 128), idesc, 1u);
-                        tc_commit(bar(5 + ls));
-                        tc_commit(bar(3 + ls));
+                        const uint64_t dl = dL + ls * (U_TILE_BYTES >> 4);
+                        const uint32_t dt = tmem + 128 * as;
+#pragma unroll
+                        for (int kk = 0; kk < 8; kk++) tc_mma_f16(dt, dh + kk * 256, dW + kk * 256, idesc, kk > 0 ? 1u : 0u);
+#pragma unroll
+                        for (int kk = 0; kk < 8; kk++) tc_mma_f16(dt, dl + kk * 256, dW + (8 + kk) * 256, idesc, 1u);
+                        tc_commit(bar(5 + as));
+                        tc_commit(l_free(ls));
                     }
                     tc_commit(bar(11 + hs));
                     continue;
@@ -630,9 +640,14 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
                 mbar_wait(bar(1 + st), ph);
                 mbar_wait(bar(7 + st), ph ^ 1);
                 tc_fence_after();
-                for (int kk = 0; kk < nb * 8; kk++)
-                    tc_mma_f16(tmem + 128 * st, make_sdesc(sbase + OFF_U + st * W1B + 2 * kk * 2048, 2048, 128),
-                               make_sdesc(sbase + 2 * kk * 2048, 2048, 128), idesc, kk > 0 ? 1u : 0u);
+                const uint64_t du = dU + st * (W1B >> 4);
+                const uint32_t dt = tmem + 128 * st;
+#pragma unroll
+                for (int kk = 0; kk < 8; kk++) tc_mma_f16(dt, du + kk * 256, dW + kk * 256, idesc, kk > 0 ? 1u : 0u);
+                if (nb == 2) {
+#pragma unroll
+                    for (int kk = 8; kk < 16; kk++) tc_mma_f16(dt, du + kk * 256, dW + kk * 256, idesc, 1u);
+                }
                 tc_commit(bar(5 + st));
                 tc_commit(bar(3 + st));
             }
@@ -800,7 +815,7 @@ gwi_status gwi_tc_pack(gwi_model* m)
     GWI_CUDA_CHECK(cudaGetDeviceProperties(&prop, m->device));
     p->num_sms = prop.multiProcessorCount;
     GWI_CUDA_CHECK(cudaFuncSetAttribute(k_stack, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_TOTAL));
-    GWI_CUDA_CHECK(cudaFuncSetAttribute(k_head_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 2 * U_TILE_BYTES + HEAD_SMEM_EXTRA));
+    GWI_CUDA_CHECK(cudaFuncSetAttribute(k_head_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, HEAD_SMEM));
     return GWI_OK;
 }
 
@@ -862,7 +877,7 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
         ha.seg_tiles = 0, ha.warm_tiles = 0, ha.stream_start = 0, ha.n_valid = 0;
         int64_t nitems = nwin * ntiles;
         int hgrid = (int)(nitems < p->num_sms ? nitems : p->num_sms);
-        k_head_tc<<<hgrid, HEAD_THREADS, 3 * nb * U_TILE_BYTES + HEAD_SMEM_EXTRA, st>>>(ha);
+        k_head_tc<<<hgrid, HEAD_THREADS, HEAD_SMEM, st>>>(ha);
         gwi_count_launch(2);
         GWI_CUDA_CHECK(cudaGetLastError());
 #ifdef GWI_TC_TRACE
@@ -936,7 +951,7 @@ gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, 
     ha.n_branch = 2, ha.mode = 1, ha.hist = hist, ha.lags = d_lags, ha.nq = nq, ha.stride_k = stride_k, ha.n_lags = n_lags, ha.R = R;
     ha.seg_tiles = seg_tiles, ha.warm_tiles = warm_tiles, ha.stream_start = stream_start, ha.n_valid = n_valid;
     int hgrid = (int)(nq < p->num_sms ? nq : p->num_sms);
-    k_head_tc<<<hgrid, HEAD_THREADS, 3 * ha.n_branch * U_TILE_BYTES + HEAD_SMEM_EXTRA, st>>>(ha);
+    k_head_tc<<<hgrid, HEAD_THREADS, HEAD_SMEM, st>>>(ha);
     gwi_count_launch(1);
     GWI_CUDA_CHECK(cudaGetLastError());
     return GWI_OK;
