@@ -516,7 +516,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 // ---- head kernel ---------------------------------------------------------------------------------------------------
 struct HeadArgs {
     const uint8_t* w1;    // B operand: N = 128 x K = n_branch*128, chunk-column (chunk stride 2048)
-    const float* hc;      // b1[128], W2[128], b2
+    float b1[128], w2[128], b2;   // head constants by value: read as constant-bank operands, not through shared memory
     const uint8_t* u;     // [nwin][n_branch][ntiles][U_TILE_BYTES]
     float* prob;          // [B][T]
     int64_t w0, nwin;
@@ -547,19 +547,21 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
     const int OFF_U = W1B, OFF_BAR = 7 * U_TILE_BYTES;
     const int OFF_L = OFF_U + 2 * U_TILE_BYTES;   // stream mode: two H1 tile buffers at OFF_U, three L1 tile buffers at OFF_L
     // barriers: 0 w1_full, 1-2 u_full[st], 3-4 u_free[st], 5-6 acc_full[st], 7-8 acc_free[st]; stream mode: H1 tiles (one
-    // per item) 9-10 h_full, 11-12 h_free; L1 tiles (one per lag, three buffers: a 32 KB tile takes about two MMA
-    // times to arrive from L2) l_full 1, 2, 13 and l_free 3, 4, 14
+    // per item) 9-10 h_full, 11-12 h_free; L1 tiles (one per lag, three buffers) l_full 1, 2, 13 and l_free 3, 4, 14;
+    // the H1 half of the contraction (one per item, TMEM columns 0-255) 15-16 ah_full, 17-18 ah_free; the L1 halves
+    // (one per lag, TMEM columns 256-511) use 5-8.
+    // The SS-mode MMAs read 128 B/clk of shared memory, all there is: whatever else goes through shared memory (the
+    // bulk copies of the tiles, epilogue constants) adds to the MMA time, so the H1 half W1[:, :128] u_H is contracted
+    // once per item and only the K = 128 of the L1 half per lag, and the epilogue takes b1 and W2 from the constant bank.
     auto bar = [&](int i) { return sbase + OFF_BAR + 8 * i; };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * 16);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * 20);
     auto l_full = [&](int ls) { return bar(ls < 2 ? 1 + ls : 13); };
     auto l_free = [&](int ls) { return bar(ls < 2 ? 3 + ls : 14); };
-    float* hcs = reinterpret_cast<float*>(smem + OFF_BAR + 256);            // b1[128], W2[128], b2
     if (threadIdx.x == 0) {
-        for (int i = 0; i < 15; i++) mbar_init(bar(i), (i == 7 || i == 8) ? 128u : 1u);
+        for (int i = 0; i < 19; i++) mbar_init(bar(i), (i == 7 || i == 8) ? 128u : (i == 17 || i == 18) ? 256u : 1u);
         mbar_fence_init();
     }
-    for (int i = threadIdx.x; i < 257; i += HEAD_THREADS) hcs[i] = __ldg(a.hc + i);
-    if (warp == 8) tmem_alloc(smem_u32(tmem_slot), 256);
+    if (warp == 8) tmem_alloc(smem_u32(tmem_slot), 512);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -616,23 +618,27 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
             for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x, n++) {
                 if (a.mode) {
                     const int hs = n & 1;
-                    mbar_wait(bar(9 + hs), (n >> 1) & 1);
+                    const uint32_t hp = (n >> 1) & 1;
+                    mbar_wait(bar(9 + hs), hp);
+                    mbar_wait(bar(17 + hs), hp ^ 1);
+                    tc_fence_after();
                     const uint64_t dh = dU + hs * (U_TILE_BYTES >> 4);
+#pragma unroll
+                    for (int kk = 0; kk < 8; kk++) tc_mma_f16(tmem + 128 * hs, dh + kk * 256, dW + kk * 256, idesc, kk > 0 ? 1u : 0u);
+                    tc_commit(bar(15 + hs));
+                    tc_commit(bar(11 + hs));
                     for (int k = 0; k < a.n_lags; k++, c++) {
                         const int ls = c % 3, as = c & 1;
                         mbar_wait(l_full(ls), (c / 3) & 1);
                         mbar_wait(bar(7 + as), ((c >> 1) & 1) ^ 1);
                         tc_fence_after();
                         const uint64_t dl = dL + ls * (U_TILE_BYTES >> 4);
-                        const uint32_t dt = tmem + 128 * as;
+                        const uint32_t dt = tmem + 256 + 128 * as;
 #pragma unroll
-                        for (int kk = 0; kk < 8; kk++) tc_mma_f16(dt, dh + kk * 256, dW + kk * 256, idesc, kk > 0 ? 1u : 0u);
-#pragma unroll
-                        for (int kk = 0; kk < 8; kk++) tc_mma_f16(dt, dl + kk * 256, dW + (8 + kk) * 256, idesc, 1u);
+                        for (int kk = 0; kk < 8; kk++) tc_mma_f16(dt, dl + kk * 256, dW + (8 + kk) * 256, idesc, kk > 0 ? 1u : 0u);
                         tc_commit(bar(5 + as));
                         tc_commit(l_free(ls));
                     }
-                    tc_commit(bar(11 + hs));
                     continue;
                 }
                 const int st = n & 1;
@@ -658,56 +664,66 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
         // epilogue of one tile overlaps the whole MMA time of the next
         const int set = warp >> 2, r = (warp & 3) * 32 + lane;
         const uint32_t lane_t = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-        const float4* b1s = reinterpret_cast<const float4*>(hcs);
-        const float4* w2s = reinterpret_cast<const float4*>(hcs + 128);
-        const float b2 = hcs[256];
-        // y = W2 . ReLU(acc + b1) + b2 of this thread's row from accumulator buffer `as`, then the buffer is released
-        auto finish = [&](int as) {
-            float y0 = 0.f, y1 = 0.f, y2 = 0.f, y3 = 0.f;       // four independent chains over the 128 channels
+        // y = W2 . ReLU(acc + b1) + b2 of this thread's row; acc = accumulator columns at `ta` (+ those at `tb` when
+        // SPLIT: the H1 half of the contraction); four independent chains over the 128 channels
+        auto finish = [&](uint32_t ta, uint32_t tb, auto SPLIT) {
+            float y0 = 0.f, y1 = 0.f, y2 = 0.f, y3 = 0.f;
 #pragma unroll
             for (int cc = 0; cc < 4; cc++) {
-                uint32_t v[32];
-                tmem_ld32(lane_t + 128 * as + 32 * cc, v);
+                uint32_t v[32], w[32];
+                tmem_ld32(lane_t + ta + 32 * cc, v);
+                if (decltype(SPLIT)::value) tmem_ld32(lane_t + tb + 32 * cc, w);
                 tc_wait_ld();
 #pragma unroll
-                for (int c = 0; c < 8; c++) {
-                    const float4 bb = b1s[8 * cc + c], ww = w2s[8 * cc + c];
-                    y0 = fmaf(ww.x, fmaxf(__uint_as_float(v[4 * c]) + bb.x, 0.f), y0);
-                    y1 = fmaf(ww.y, fmaxf(__uint_as_float(v[4 * c + 1]) + bb.y, 0.f), y1);
-                    y2 = fmaf(ww.z, fmaxf(__uint_as_float(v[4 * c + 2]) + bb.z, 0.f), y2);
-                    y3 = fmaf(ww.w, fmaxf(__uint_as_float(v[4 * c + 3]) + bb.w, 0.f), y3);
+                for (int c = 0; c < 32; c += 4) {
+                    float x0 = __uint_as_float(v[c]), x1 = __uint_as_float(v[c + 1]), x2 = __uint_as_float(v[c + 2]),
+                          x3 = __uint_as_float(v[c + 3]);
+                    if (decltype(SPLIT)::value)
+                        x0 += __uint_as_float(w[c]), x1 += __uint_as_float(w[c + 1]), x2 += __uint_as_float(w[c + 2]),
+                            x3 += __uint_as_float(w[c + 3]);
+                    y0 = fmaf(a.w2[32 * cc + c], fmaxf(x0 + a.b1[32 * cc + c], 0.f), y0);
+                    y1 = fmaf(a.w2[32 * cc + c + 1], fmaxf(x1 + a.b1[32 * cc + c + 1], 0.f), y1);
+                    y2 = fmaf(a.w2[32 * cc + c + 2], fmaxf(x2 + a.b1[32 * cc + c + 2], 0.f), y2);
+                    y3 = fmaf(a.w2[32 * cc + c + 3], fmaxf(x3 + a.b1[32 * cc + c + 3], 0.f), y3);
                 }
             }
-            const float y = ((y0 + y1) + (y2 + y3)) + b2;
-            tc_fence_before();
-            mbar_arrive(bar(7 + as));
+            const float y = ((y0 + y1) + (y2 + y3)) + a.b2;
             return 1.0f / (1.0f + __expf(-y));
         };
         uint32_t n = 0, c = 0;
         for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x, n++) {
             if (a.mode) {
                 const int64_t t = it * TM + r;
+                const int hs = n & 1;
                 for (int k = 0; k < a.n_lags; k++, c++) {
                     if ((int)(c & 1) != set) continue;
+                    mbar_wait(bar(15 + hs), (n >> 1) & 1);
                     mbar_wait(bar(5 + set), (c >> 1) & 1);
                     tc_fence_after();
-                    const float pr = finish(set);
+                    const float pr = finish(256 + 128 * set, 128 * hs, std::true_type{});
+                    tc_fence_before();
+                    mbar_arrive(bar(7 + set));
                     if (t < a.n_valid) a.prob[(size_t)k * a.stride_k + t] = pr;
                 }
+                // both sets have read the H1 half of this item (n_lags >= 2: each set had at least one lag)
+                tc_fence_before();
+                mbar_arrive(bar(17 + hs));
                 continue;
             }
             if ((int)(n & 1) != set) continue;
             const int64_t wl = it / a.ntiles, j = it % a.ntiles;
             mbar_wait(bar(5 + set), (n >> 1) & 1);
             tc_fence_after();
-            const float pr = finish(set);
+            const float pr = finish(128 * set, 0, std::false_type{});
+            tc_fence_before();
+            mbar_arrive(bar(7 + set));
             const int t = (int)j * TM + r;
             if (t < a.T) a.prob[(size_t)(a.w0 + wl) * a.T + t] = pr;
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 8) tmem_dealloc(tmem, 256);
+    if (warp == 8) tmem_dealloc(tmem, 512);
 }
 
 } // namespace
@@ -715,7 +731,8 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
 // ---- host side: packing and launch -----------------------------------------------------------------------------------
 struct GwiTcPack {
     uint8_t *d_wfg = nullptr, *d_wrs = nullptr, *d_w1 = nullptr;
-    float *d_cst = nullptr, *d_hc = nullptr;
+    float *d_cst = nullptr;
+    float h_hc[257];        // b1[128], W2[128], b2 (passed to k_head_tc by value)
     TcMeta meta;
     int num_sms = 148;
 };
@@ -810,7 +827,7 @@ gwi_status gwi_tc_pack(gwi_model* m)
     GWI_CUDA_CHECK(up((void**)&p->d_wrs, wrs.data(), wrs.size() * 2));
     GWI_CUDA_CHECK(up((void**)&p->d_w1, w1.data(), w1.size() * 2));
     GWI_CUDA_CHECK(up((void**)&p->d_cst, cst.data(), cst.size() * 4));
-    GWI_CUDA_CHECK(up((void**)&p->d_hc, hc.data(), hc.size() * 4));
+    memcpy(p->h_hc, hc.data(), sizeof(p->h_hc));
     cudaDeviceProp prop;
     GWI_CUDA_CHECK(cudaGetDeviceProperties(&prop, m->device));
     p->num_sms = prop.multiProcessorCount;
@@ -823,7 +840,7 @@ void gwi_tc_free(gwi_model* m)
 {
     GwiTcPack* p = m->tc;
     if (!p) return;
-    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_cst), cudaFree(p->d_hc);
+    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_cst);
     delete p;
     m->tc = nullptr;
 }
@@ -872,7 +889,8 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
         int grid = (int)(njobs < p->num_sms ? njobs : p->num_sms);
         k_stack<<<grid, NTHREADS, SM_TOTAL, st>>>(sa);
         HeadArgs ha;
-        ha.w1 = p->d_w1, ha.hc = p->d_hc, ha.u = u, ha.prob = d_prob, ha.w0 = w0, ha.nwin = nwin, ha.T = T, ha.ntiles = ntiles,
+        memcpy(ha.b1, p->h_hc, 128 * 4), memcpy(ha.w2, p->h_hc + 128, 128 * 4), ha.b2 = p->h_hc[256];
+        ha.w1 = p->d_w1, ha.u = u, ha.prob = d_prob, ha.w0 = w0, ha.nwin = nwin, ha.T = T, ha.ntiles = ntiles,
         ha.n_branch = nb, ha.mode = 0, ha.hist = nullptr, ha.lags = nullptr, ha.nq = 0, ha.stride_k = 0, ha.n_lags = 0, ha.R = 0,
         ha.seg_tiles = 0, ha.warm_tiles = 0, ha.stream_start = 0, ha.n_valid = 0;
         int64_t nitems = nwin * ntiles;
@@ -942,12 +960,13 @@ gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, 
                               float* d_prob, int64_t stride_k, cudaStream_t st)
 {
     const GwiTcPack* p = m->tc;
-    if (m->arch.n_branch != 2) {
-        gwi_set_error("gwi_tc_head_stream: two branches expected");
+    if (m->arch.n_branch != 2 || n_lags < 2) {
+        gwi_set_error("gwi_tc_head_stream: two branches and at least two slides (zero lag + one lag) expected");
         return GWI_ERR_UNSUPPORTED;
     }
     HeadArgs ha;
-    ha.w1 = p->d_w1, ha.hc = p->d_hc, ha.u = u, ha.prob = d_prob, ha.w0 = 0, ha.nwin = 0, ha.T = 0, ha.ntiles = ntiles;
+    memcpy(ha.b1, p->h_hc, 128 * 4), memcpy(ha.w2, p->h_hc + 128, 128 * 4), ha.b2 = p->h_hc[256];
+    ha.w1 = p->d_w1, ha.u = u, ha.prob = d_prob, ha.w0 = 0, ha.nwin = 0, ha.T = 0, ha.ntiles = ntiles;
     ha.n_branch = 2, ha.mode = 1, ha.hist = hist, ha.lags = d_lags, ha.nq = nq, ha.stride_k = stride_k, ha.n_lags = n_lags, ha.R = R;
     ha.seg_tiles = seg_tiles, ha.warm_tiles = warm_tiles, ha.stream_start = stream_start, ha.n_valid = n_valid;
     int hgrid = (int)(nq < p->num_sms ? nq : p->num_sms);
