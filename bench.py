@@ -440,8 +440,8 @@ def main():
                        "step i (two device buffers); count + records read back every step"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "tensor", "achieved": tflops, "peak": peak_tf, "unit": "TFLOP/s", "frac": tflops / peak_tf,
-                     "traffic": 8.77e9, "traffic_note": "dram__bytes_read+write of k_stack per launch, ncu --set full, "
-                     "profiles/r1_v4_summary.md (u tiles 2.15 GB + history-ring tiles evicted from L2)", "peak_kind": f"bf16 cuBLAS sustained, {pk_kind}; fp16 = same tensor rate",
+                     "traffic": 5.25e9, "traffic_note": "dram__bytes_read+write of k_stack per launch, ncu --set full, "
+                     "profiles/r1_v5_k_stack_dram.md (u tiles 2.15 GB + history-ring tiles evicted from L2)", "peak_kind": f"bf16 cuBLAS sustained, {pk_kind}; fp16 = same tensor rate",
                      "kernel": "gwi_infer (all launches of one call)", "flops_per_launch": flops_per_step,
                      "infer_ms": infer_ms, "frac_of_nominal_2250": tflops / 2250.0},
     }

@@ -28,6 +28,21 @@
 #include "gwi_internal.h"
 #include "gwi_tc_ptx.h"
 
+// L2 residency hints: the history rings (66 MB for the whole grid, re-read 1-4 tile times after they are written) are
+// stored and loaded evict-last, the u tiles (2 GB per launch, read by the next kernel) are stored evict-first
+#ifndef GWI_TC_L2HINT
+#define GWI_TC_L2HINT 1
+#endif
+#if GWI_TC_L2HINT
+#define GWI_RING_G2S(dst, src, bytes, bar) bulk_g2s_hint(dst, src, bytes, bar, ring_pol)
+#define GWI_RING_S2G(dst, src, bytes) bulk_s2g_hint(dst, src, bytes, ring_pol)
+#define GWI_U_STORE(ptr, val) __stcs(ptr, val)
+#else
+#define GWI_RING_G2S(dst, src, bytes, bar) bulk_g2s(dst, src, bytes, bar)
+#define GWI_RING_S2G(dst, src, bytes) bulk_s2g(dst, src, bytes)
+#define GWI_U_STORE(ptr, val) (*(ptr) = (val))
+#endif
+
 using namespace tc;
 
 namespace {
@@ -138,6 +153,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
     const int L = M.L, nb = M.n_branch;
     auto bar = [&](int i) { return sbase + SM_BAR + 8 * i; };
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + SM_BAR + 8 * B_COUNT);
+#if GWI_TC_L2HINT
+    const uint64_t ring_pol = l2_policy_evict_last();
+#endif
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < B_COUNT; i++) {
@@ -210,7 +228,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                             mbar_arrive_expect_tx(bar(B_PST_FULL + s), PST_BYTES);
                             const uint8_t* src = a.ring + (((size_t)blockIdx.x * 2 + s) * M.ring_tiles + M.ring_off[i] +
                                                            (j & (M.D[i] - 1))) * PST_BYTES;
-                            bulk_g2s(sbase + SM_PST + s * PST_BYTES, src, PST_BYTES, bar(B_PST_FULL + s));
+                            GWI_RING_G2S(sbase + SM_PST + s * PST_BYTES, src, PST_BYTES, bar(B_PST_FULL + s));
                             n_pst[s]++;
                         }
                     }
@@ -261,13 +279,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                         if (kind == 2 && j + (d >> 7) < a.ntiles) {
                             uint8_t* dst = ring_s + (size_t)(M.ring_off[i] + (j & ((d >> 7) - 1))) * PST_BYTES;
 #pragma unroll
-                            for (int c = 0; c < 8; c++) bulk_s2g(dst + c * 2048, xrows + c * X_CHUNK, 2048);
+                            for (int c = 0; c < 8; c++) GWI_RING_S2G(dst + c * 2048, xrows + c * X_CHUNK, 2048);
                             bulk_commit();
                             stored = true;
                         } else if (kind == 1 && j + 1 < a.ntiles) {
                             uint8_t* dst = ring64_s + (size_t)(M.ring_off[i] * 2 + (j & 1)) * PRE_BYTES;
 #pragma unroll
-                            for (int c = 0; c < 8; c++) bulk_s2g(dst + c * 1024, xrows + 64 * 16 + c * X_CHUNK, 1024);
+                            for (int c = 0; c < 8; c++) GWI_RING_S2G(dst + c * 1024, xrows + 64 * 16 + c * X_CHUNK, 1024);
                             bulk_commit();
                             stored = true;
                         }
@@ -315,7 +333,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                                     mbar_arrive_expect_tx(bar(B_PRE_FULL + s), PRE_BYTES);
 #pragma unroll
                                     for (int c = 0; c < 8; c++)
-                                        bulk_g2s(xrows - 64 * 16 + c * X_CHUNK, src + c * 1024, 1024, bar(B_PRE_FULL + s));
+                                        GWI_RING_G2S(xrows - 64 * 16 + c * X_CHUNK, src + c * 1024, 1024, bar(B_PRE_FULL + s));
                                 }
                             }
 #pragma unroll
@@ -499,7 +517,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                                         float u1 = fmaxf(__uint_as_float(v[col + 1]) + bs.y, 0.f);
                                         q[e] = pack_half2(u0, u1);
                                     }
-                                    *reinterpret_cast<uint4*>(ut + (8 * wg + 4 * cc + c) * 2048) = make_uint4(q[0], q[1], q[2], q[3]);
+                                    GWI_U_STORE(reinterpret_cast<uint4*>(ut + (8 * wg + 4 * cc + c) * 2048), make_uint4(q[0], q[1], q[2], q[3]));
                                 }
                             }
                         }
