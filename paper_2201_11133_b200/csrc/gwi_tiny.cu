@@ -234,7 +234,7 @@ __global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
 // 16-row tile and re-used for every lag, each lag adds its L1 half.  u16 row 0 = sample 0 of the chunk; L1 rows at negative indices are the
 // ring of the previous max-lag samples.
 struct HeadsArgs {
-    const uint2* w1p;       // [ks 4][nt 4][32] B fragments of W1^T in the k order of the 16-byte row loads (see the kernel)
+    const uint4* w1t;       // [half 2][mt 2][kk 2][32] A fragments of W1 in the k order of the 16-byte row loads (see the kernel)
     const float* hcst;      // b1[32], W2[32], b2
     const __half* u16;      // [2][lds][32], pointing at row 0 of this chunk
     int64_t lds;
@@ -249,55 +249,76 @@ __global__ void __launch_bounds__(256) k_tiny_heads(const HeadsArgs a)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int64_t row0 = ((int64_t)blockIdx.x * 8 + warp) * 16;
     if (row0 >= a.n) return;
+    // The contraction is done transposed, D[channel][time] = W1 . u^T: the weights are the A operand (two m-tiles of 16
+    // hidden channels), eight feature rows the B operand.  A lane's B fragments of both k-steps are then the 16 bytes
+    // at offset 16 t of feature row g, one load and no register shuffling (the k order of the packed weights w1t is
+    // permuted to match).  The warp handles two groups of eight rows.
     const int64_t ra = row0 + g, rb = ra + 8;
     const int64_t ca = ra < a.n ? ra : a.n - 1, cb = rb < a.n ? rb : a.n - 1;   // clamp loads of the ragged tail
-    // a feature row is 32 halves = 4 x 16 bytes; lane (g, t) loads bytes 16 t .. 16 t + 15 of rows g and g + 8 with one
-    // 16-byte load each and uses them as the A fragments of two k-steps whose k order is permuted accordingly (w1p)
     const uint4* uH = reinterpret_cast<const uint4*>(a.u16);
     const uint4* uL = reinterpret_cast<const uint4*>(a.u16 + a.lds * 32);
-    // H1 half: acc = b1 + W1[:, 0:32] u_H
-    float acc[4][4];
+    // H1 half: acc[group][m-tile] = b1 + W1[:, 0:32] u_H; c0, c1: channel 16 mt + g, c2, c3: channel 16 mt + g + 8
+    float acc[2][2][4];
     {
         const uint4 ha = uH[ca * 4 + t], hb = uH[cb * 4 + t];
-        const uint32_t ah0[4] = {ha.x, hb.x, ha.y, hb.y}, ah1[4] = {ha.z, hb.z, ha.w, hb.w};
 #pragma unroll
-        for (int nt = 0; nt < 4; nt++) {
-            float2 bb = __ldg(reinterpret_cast<const float2*>(a.hcst + 8 * nt + 2 * t));
-            acc[nt][0] = bb.x, acc[nt][1] = bb.y, acc[nt][2] = bb.x, acc[nt][3] = bb.y;
-            mma16816(acc[nt], ah0, __ldg(a.w1p + (0 * 4 + nt) * 32 + lane));
-            mma16816(acc[nt], ah1, __ldg(a.w1p + (1 * 4 + nt) * 32 + lane));
+        for (int mt = 0; mt < 2; mt++) {
+            const float b_lo = __ldg(a.hcst + 16 * mt + g), b_hi = __ldg(a.hcst + 16 * mt + g + 8);
+            const uint4 w0 = __ldg(a.w1t + (mt * 2 + 0) * 32 + lane), w1 = __ldg(a.w1t + (mt * 2 + 1) * 32 + lane);
+            const uint32_t a0[4] = {w0.x, w0.y, w0.z, w0.w}, a1[4] = {w1.x, w1.y, w1.z, w1.w};
+#pragma unroll
+            for (int gr = 0; gr < 2; gr++) {
+                const uint4 h = gr ? hb : ha;
+                acc[gr][mt][0] = b_lo, acc[gr][mt][1] = b_lo, acc[gr][mt][2] = b_hi, acc[gr][mt][3] = b_hi;
+                mma16816(acc[gr][mt], a0, make_uint2(h.x, h.y));
+                mma16816(acc[gr][mt], a1, make_uint2(h.z, h.w));
+            }
         }
     }
-    uint2 wl[2][4];
-    float2 w2[4];
+    uint32_t wl[2][2][4];
+    float w2lo[2], w2hi[2];
 #pragma unroll
-    for (int nt = 0; nt < 4; nt++) {
-        wl[0][nt] = __ldg(a.w1p + (2 * 4 + nt) * 32 + lane), wl[1][nt] = __ldg(a.w1p + (3 * 4 + nt) * 32 + lane);
-        w2[nt] = __ldg(reinterpret_cast<const float2*>(a.hcst + 32 + 8 * nt + 2 * t));
+    for (int mt = 0; mt < 2; mt++) {
+#pragma unroll
+        for (int kk = 0; kk < 2; kk++) {
+            const uint4 w = __ldg(a.w1t + ((2 + mt) * 2 + kk) * 32 + lane);
+            wl[mt][kk][0] = w.x, wl[mt][kk][1] = w.y, wl[mt][kk][2] = w.z, wl[mt][kk][3] = w.w;
+        }
+        w2lo[mt] = __ldg(a.hcst + 32 + 16 * mt + g), w2hi[mt] = __ldg(a.hcst + 32 + 16 * mt + g + 8);
     }
     const float b2 = __ldg(a.hcst + 64);
-    // after the butterfly every lane of a group holds both rows' sums: lane t = 0 finishes row g, lane t = 1 row g + 8
-    const int64_t rst = (t & 1) ? rb : ra;
-    const bool store = t < 2 && rst < a.n;
+    // after the reduction over the eight channel lanes, lane (g, t) holds the row 8 (g >> 2) + 2 t + ((g >> 1) & 1)
+    const bool hi16 = lane & 16, hi8 = lane & 8;
+    const int64_t rst = row0 + 8 * (g >> 2) + 2 * t + ((g >> 1) & 1);
+    const bool store = !(g & 1) && rst < a.n;
 #pragma unroll 2
     for (int k = 0; k < a.n_lags; k++) {
         const int64_t lag = __ldg(a.lags + k);
         const uint4 la = uL[(ca - lag) * 4 + t], lb = uL[(cb - lag) * 4 + t];
-        const uint32_t al0[4] = {la.x, lb.x, la.y, lb.y}, al1[4] = {la.z, lb.z, la.w, lb.w};
-        float y0 = 0.f, y1 = 0.f;
+        float p[4];                                  // group A time 2t, 2t + 1; group B time 2t, 2t + 1
 #pragma unroll
-        for (int nt = 0; nt < 4; nt++) {
-            float v[4] = {acc[nt][0], acc[nt][1], acc[nt][2], acc[nt][3]};
-            mma16816(v, al0, wl[0][nt]);
-            mma16816(v, al1, wl[1][nt]);
-            y0 = fmaf(w2[nt].x, fmaxf(v[0], 0.f), y0), y0 = fmaf(w2[nt].y, fmaxf(v[1], 0.f), y0);
-            y1 = fmaf(w2[nt].x, fmaxf(v[2], 0.f), y1), y1 = fmaf(w2[nt].y, fmaxf(v[3], 0.f), y1);
+        for (int gr = 0; gr < 2; gr++) {
+            const uint4 l = gr ? lb : la;
+            float y0 = 0.f, y1 = 0.f;
+#pragma unroll
+            for (int mt = 0; mt < 2; mt++) {
+                float v[4] = {acc[gr][mt][0], acc[gr][mt][1], acc[gr][mt][2], acc[gr][mt][3]};
+                mma16816(v, wl[mt][0], make_uint2(l.x, l.y));
+                mma16816(v, wl[mt][1], make_uint2(l.z, l.w));
+                y0 = fmaf(w2lo[mt], fmaxf(v[0], 0.f), y0), y0 = fmaf(w2hi[mt], fmaxf(v[2], 0.f), y0);
+                y1 = fmaf(w2lo[mt], fmaxf(v[1], 0.f), y1), y1 = fmaf(w2hi[mt], fmaxf(v[3], 0.f), y1);
+            }
+            p[2 * gr] = y0, p[2 * gr + 1] = y1;
         }
-        y0 += __shfl_xor_sync(0xffffffffu, y0, 1), y1 += __shfl_xor_sync(0xffffffffu, y1, 1);
-        y0 += __shfl_xor_sync(0xffffffffu, y0, 2), y1 += __shfl_xor_sync(0xffffffffu, y1, 2);
-        const float y = ((t & 1) ? y1 : y0) + b2;
-        const float p = __fdividef(1.0f, 1.0f + __expf(-y));
-        if (store) a.prob[(size_t)k * a.stride_k + rst] = p;
+        // sum over the 8 channel lanes (lane bits 2-4), halving the number of values at each step
+        const float r0 = __shfl_xor_sync(0xffffffffu, hi16 ? p[0] : p[2], 16);
+        const float r1 = __shfl_xor_sync(0xffffffffu, hi16 ? p[1] : p[3], 16);
+        const float k0 = (hi16 ? p[2] : p[0]) + r0, k1 = (hi16 ? p[3] : p[1]) + r1;
+        const float r2 = __shfl_xor_sync(0xffffffffu, hi8 ? k0 : k1, 8);
+        float y = (hi8 ? k1 : k0) + r2;
+        y += __shfl_xor_sync(0xffffffffu, y, 4);
+        const float pr = __fdividef(1.0f, 1.0f + __expf(-(y + b2)));
+        if (store) a.prob[(size_t)k * a.stride_k + rst] = pr;
     }
 }
 
@@ -322,7 +343,8 @@ inline uint16_t h16(float v)
 } // namespace
 
 struct GwiTinyPack {
-    uint2 *d_wfg = nullptr, *d_wrs = nullptr, *d_w1 = nullptr, *d_w1p = nullptr;
+    uint2 *d_wfg = nullptr, *d_wrs = nullptr, *d_w1 = nullptr;
+    uint4* d_w1t = nullptr;
     float *d_bias = nullptr, *d_cst = nullptr;
     int halo = 16;
 };
@@ -387,18 +409,17 @@ gwi_status gwi_tiny_pack(gwi_model* m)
     for (int ks = 0; ks < 4; ks++)
         for (int nt = 0; nt < 4; nt++)
             for (int l = 0; l < 32; l++) w1[(ks * 4 + nt) * 32 + l] = frag(B1, 16 * ks, 8 * nt, l);
-    // the same for k_tiny_heads, whose A fragments come from 16-byte row loads: k-step kk of half hb (0: u_H, 1: u_L) pairs
-    // fragment position (2t, 2t+1) with channels 8t + 4kk + (0, 1) and position (2t+8, 2t+9) with channels 8t + 4kk + (2, 3)
-    std::vector<uint2> w1p(16 * 32);
+    // k_tiny_heads contracts transposed (weights = A operand, 8 feature rows = B operand, see the kernel): A fragment of
+    // half hb (0: u_H, 1: u_L), m-tile mt, k-step kk; fragment position (2t, 2t+1) <-> input channels 8t + 4kk + (0, 1),
+    // position (2t+8, 2t+9) <-> channels 8t + 4kk + (2, 3)
+    std::vector<uint4> w1t(16 * 32);
     for (int hb = 0; hb < 2; hb++)
-        for (int kk = 0; kk < 2; kk++)
-            for (int nt = 0; nt < 4; nt++)
+        for (int mt = 0; mt < 2; mt++)
+            for (int kk = 0; kk < 2; kk++)
                 for (int l = 0; l < 32; l++) {
-                    const int g = l >> 2, t = l & 3, c0 = 32 * hb + 8 * t + 4 * kk, n = 8 * nt + g;
-                    uint2 r;
-                    r.x = (uint32_t)h16(B1(c0, n)) | ((uint32_t)h16(B1(c0 + 1, n)) << 16);
-                    r.y = (uint32_t)h16(B1(c0 + 2, n)) | ((uint32_t)h16(B1(c0 + 3, n)) << 16);
-                    w1p[((2 * hb + kk) * 4 + nt) * 32 + l] = r;
+                    const int g = l >> 2, t = l & 3, c0 = 32 * hb + 8 * t + 4 * kk, n0 = 16 * mt + g;
+                    auto pk = [&](int k, int n) { return (uint32_t)h16(B1(k, n)) | ((uint32_t)h16(B1(k + 1, n)) << 16); };
+                    w1t[((hb * 2 + mt) * 2 + kk) * 32 + l] = make_uint4(pk(c0, n0), pk(c0, n0 + 8), pk(c0 + 2, n0), pk(c0 + 2, n0 + 8));
                 }
     for (int c = 0; c < 32; c++) cst[64 + c] = W[m->off.b1 + c], cst[96 + c] = W[m->off.W2 + c];
     cst[128] = W[m->off.b2];
@@ -410,7 +431,7 @@ gwi_status gwi_tiny_pack(gwi_model* m)
     GWI_CUDA_CHECK(up((void**)&p->d_wfg, wfg.data(), wfg.size() * 8));
     GWI_CUDA_CHECK(up((void**)&p->d_wrs, wrs.data(), wrs.size() * 8));
     GWI_CUDA_CHECK(up((void**)&p->d_w1, w1.data(), w1.size() * 8));
-    GWI_CUDA_CHECK(up((void**)&p->d_w1p, w1p.data(), w1p.size() * 8));
+    GWI_CUDA_CHECK(up((void**)&p->d_w1t, w1t.data(), w1t.size() * 16));
     GWI_CUDA_CHECK(up((void**)&p->d_bias, bias.data(), bias.size() * 4));
     GWI_CUDA_CHECK(up((void**)&p->d_cst, cst.data(), cst.size() * 4));
     return GWI_OK;
@@ -420,7 +441,7 @@ void gwi_tiny_free(gwi_model* m)
 {
     GwiTinyPack* p = m->tiny;
     if (!p) return;
-    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_w1p), cudaFree(p->d_bias), cudaFree(p->d_cst);
+    cudaFree(p->d_wfg), cudaFree(p->d_wrs), cudaFree(p->d_w1), cudaFree(p->d_w1t), cudaFree(p->d_bias), cudaFree(p->d_cst);
     delete p;
     m->tiny = nullptr;
 }
@@ -455,7 +476,7 @@ gwi_status gwi_tiny_heads(const gwi_model* m, const __half* d_u16, int64_t lds, 
 {
     const GwiTinyPack* p = m->tiny;
     HeadsArgs a;
-    a.w1p = p->d_w1p, a.hcst = p->d_cst + 64, a.u16 = d_u16, a.lds = lds, a.n = n, a.n_lags = n_lags, a.lags = d_lags;
+    a.w1t = p->d_w1t, a.hcst = p->d_cst + 64, a.u16 = d_u16, a.lds = lds, a.n = n, a.n_lags = n_lags, a.lags = d_lags;
     a.prob = d_prob, a.stride_k = stride_k;
     k_tiny_heads<<<(n + 127) / 128, 256, 0, st>>>(a);
     gwi_count_launch(1);
