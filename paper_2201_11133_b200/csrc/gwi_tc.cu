@@ -71,6 +71,9 @@ struct TcMeta {
     int D[TC_MAX_L];          // d / 128 for kind 2 (a power of two: the ring of a layer has D entries)
     int stash_off[TC_MAX_L];  // byte offset of the layer's stash inside the slot's stash area
     int ring_off[TC_MAX_L];   // kind 2: first ring entry (in tiles) of the layer; kind 1: index among the d = 64 layers
+    int zp[TC_MAX_L];         // 1: the layer's gate output z goes to the slot's past-tile buffer instead of the operand rows
+                              // (the buffer is idle: neither this layer nor the next one is kind 2), so that the residual
+                              // update may overwrite the operand rows while the skip GEMM still reads z
     int ring_tiles;           // ring entries per slot
     int n64;                  // number of d = 64 layers
 };
@@ -317,10 +320,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                             // the residual GEMM is on the critical path (next layer's operand), the skip GEMM is not:
                             // residual first with its own commit, the skip sum runs under the residual epilogue
                             const uint64_t bw = dWrs + st * (WRS_STRIDE >> 4);
+                            const bool zp = M.zp[i] != 0;                     // z in the past-tile buffer (chunk stride 2048)
+                            const uint64_t az = zp ? apst : ax;
+                            const uint32_t kz = zp ? 4096 >> 4 : (2 * X_CHUNK) >> 4;
                             if (i < L - 1) {  // reading A8: the last block's residual conv has no effect
 #pragma unroll
                                 for (int kk = 0; kk < 4; kk++)
-                                    tc_mma_f16(dt, ax + kk * ((2 * X_CHUNK) >> 4), bw + 128 + kk * 384, idesc64, kk > 0 ? 1u : 0u);
+                                    tc_mma_f16(dt, az + kk * kz, bw + 128 + kk * 384, idesc64, kk > 0 ? 1u : 0u);
                             }
                             tc_commit(bar(B_RS_FULL + s));
                             {
@@ -338,7 +344,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                             }
 #pragma unroll
                             for (int kk = 0; kk < 4; kk++)
-                                tc_mma_f16(dskip, ax + kk * ((2 * X_CHUNK) >> 4), bw + kk * 384, idesc128, (i > 0 || kk > 0) ? 1u : 0u);
+                                tc_mma_f16(dskip, az + kk * kz, bw + kk * 384, idesc128, (i > 0 || kk > 0) ? 1u : 0u);
                         }
                         tc_commit(bar(B_SKD + s));
                         tc_commit(bar(B_WRS_FREE + st));
@@ -441,6 +447,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     if (lane == 0) TRACE(5, 10 * (warp & 7) + s, j * L + i);
                     __syncwarp();
                     tc_fence_after();
+                    const bool zp = M.zp[i] != 0;
+                    const uint32_t zstride = zp ? 2048u : (uint32_t)X_CHUNK;
+                    const uint32_t zdst = zp ? sbase + SM_PST + s * PST_BYTES + r * 16 + c0 * 2048 : xs + (64 + r) * 16 + c0 * X_CHUNK;
                     {
                         // 4 chunks of 8 channels; the TMEM loads of chunk q+1 are in flight while chunk q is gated
                         uint32_t fb[2][8], gb[2][8];
@@ -468,7 +477,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                                 float2 z = fma2(tf, tg, tf);
                                 pk[c] = pack_half2(z.x, z.y);
                             }
-                            st_shared_v4(xs + (64 + r) * 16 + (c0 + q) * X_CHUNK, pk[0], pk[1], pk[2], pk[3]);
+                            st_shared_v4(zdst + q * zstride, pk[0], pk[1], pk[2], pk[3]);
 #ifdef GWI_TC_ALTERNATE
                             if (q == GWI_TC_ALTERNATE) mbar_arrive(bar(B_HALF + s));
 #endif
@@ -489,7 +498,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
 #pragma unroll
                         for (int c = 0; c < 16; c++)
                             h[c] = add2(h[c], make_float2(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1])));
-                        mbar_wait(bar(B_SKD + s), ph);   // the skip GEMM (issued after the residual GEMM) has read z
+                        if (!zp) mbar_wait(bar(B_SKD + s), ph);   // the skip GEMM (issued after the residual GEMM) reads z from the operand rows
                         publish(i + 1, j);
                         if (lane == 0) TRACE(8, 10 * (warp & 7) + s, j * L + i);
                     } else {
@@ -796,6 +805,7 @@ gwi_status gwi_tc_pack(gwi_model* m)
         else if (M.kind[i] == 1) M.ring_off[i] = n64++;
         else M.ring_off[i] = 0, so += a.dil[i] * 128;
     }
+    for (int i = 0; i < L; i++) M.zp[i] = (M.kind[i] < 2 && M.kind[(i + 1) % L] != 2) ? 1 : 0;
     M.ring_tiles = ro > 0 ? ro : 1;
     M.n64 = n64 > 0 ? n64 : 1;
     const float* W = m->host_blob.data();
