@@ -365,3 +365,17 @@ def test_paper_scale_long_block_segment_choice(tmpdir_s, lags):
         lo = 0 if s0 == 0 else rf - 1
         got = pb[0, s0:s0 + rf + 300]
         assert np.max(np.abs(got[lo:] - want[lo:])) <= 2e-3
+
+
+@pytest.mark.parametrize("lags", [[], [4096, 12800]])
+def test_paper_scale_host_push_equals_device_push(tmpdir_s, lags):
+    """The tensor-core back ends fed through gwi_stream_push_host (pinned host chunks, side-stream copies into the
+    staging buffers: the path bench.py's month legs use) against one device push, bit for bit."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0], gwi.FP16, arch=gs.PAPER_ARCH)
+    N = 128 * 330
+    x = gs.stream_noise(41, 0, N, dtype=np.float16)
+    n0, r0, p0 = _run_stream(gms, x, [N], lags, 0.5, 16)
+    n1, r1, p1 = _run_stream(gms, x, _ragged(N, 8, 3000, 15000), lags, 0.5, 16, host=True, max_chunk=15000)
+    assert np.array_equal(p0, p1)
+    assert n0 == n1 and trig_tuples(r0) == trig_tuples(r1)
