@@ -606,19 +606,21 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
         if (lane == 0) {
             mbar_arrive_expect_tx(bar(0), W1B);
             bulk_g2s(sbase, a.w1, W1B, bar(0));
+            // stream mode: an H1 tile is read once, an L1 tile by every lag of the next max-lag output tiles
+            const uint64_t pol_once = l2_policy_evict_first(), pol_keep = l2_policy_evict_last();
             uint32_t n = 0, c = 0;
             for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x, n++) {
                 if (a.mode) {
                     const int hs = n & 1;
                     mbar_wait(bar(11 + hs), ((n >> 1) & 1) ^ 1);
                     mbar_arrive_expect_tx(bar(9 + hs), U_TILE_BYTES);
-                    bulk_g2s(sbase + OFF_U + hs * U_TILE_BYTES, stream_tile(it, 0), U_TILE_BYTES, bar(9 + hs));
+                    bulk_g2s_hint(sbase + OFF_U + hs * U_TILE_BYTES, stream_tile(it, 0), U_TILE_BYTES, bar(9 + hs), pol_once);
                     for (int k = 0; k < a.n_lags; k++, c++) {
                         const int ls = c % 3;
                         mbar_wait(l_free(ls), ((c / 3) & 1) ^ 1);
                         mbar_arrive_expect_tx(l_full(ls), U_TILE_BYTES);
-                        bulk_g2s(sbase + OFF_L + ls * U_TILE_BYTES, stream_tile(it - __ldg(a.lags + k) / TM, 1), U_TILE_BYTES,
-                                 l_full(ls));
+                        bulk_g2s_hint(sbase + OFF_L + ls * U_TILE_BYTES, stream_tile(it - __ldg(a.lags + k) / TM, 1), U_TILE_BYTES,
+                                      l_full(ls), pol_keep);
                     }
                     continue;
                 }
