@@ -12,6 +12,7 @@ rare chirping transients).
 """
 from .rng import u64, uniform01, normal
 from .modelfile import (Arch, CFG1_ARCH, PAPER_ARCH, tensor_specs, write_model, read_model,
-                        xavier_tensors, zero_tensors, make_model_file)
+                        xavier_tensors, zero_tensors, make_model_file, p16_tensors)
 from .strain import (FS, white_noise, chirp_waveform, cfg1_windows, cfg2_windows, stream_noise,
-                     coloured_whitened_noise, plateau_square_wave)
+                     coloured_whitened_noise, plateau_square_wave,
+                     CFG5_CHUNK, cfg5_injections, cfg5_chunk)

@@ -137,3 +137,27 @@ def make_model_file(path, a: Arch, seed: int, bias: str = "zero"):
     t = xavier_tensors(a, seed, bias)
     write_model(path, a, t)
     return t
+
+
+def p16_tensors(a: Arch, block=0, r=0, q=(0, 1), hid=(0, 1), gamma=8.0, past=False):
+    """Pin P16's sign pass-through model placed inside any two-branch
+    architecture: every weight and bias is zero except
+        lift      W_in[r] = 1                                   -> h[r][t] = x[t]
+        `block`   Wf[r][r] = (0,1) (or (1,0) with past=True)    -> f[r][t] = x[t] (or x[t - d_block]); g = 0
+                  Ws[q0][r] = +2, Ws[q1][r] = -2                -> u[q0] = ReLU(T), u[q1] = ReLU(-T), T = tanh(f)
+        head      W1[hid0] = (+1,-1 | +1,-1) on (q0,q1) of both branches, W1[hid1] = its negation, W2 = (gamma,-gamma)
+    so that y[t] = gamma * (T_H1[t] + T_L1[t]).  All other blocks have f = g = 0, z = 0 and contribute nothing; Wr = 0
+    keeps h = x through the stack.  Only weight placement -- none of the method's arithmetic happens here."""
+    assert a.n_branch == 2 and a.c_in == 1 and a.k == 2
+    t = zero_tensors(a)
+    for b in range(2):
+        t[f"b{b}.W_in"][r, 0] = 1.0
+        t[f"b{b}.l{block}.Wf"][r, r] = [1.0, 0.0] if past else [0.0, 1.0]
+        t[f"b{b}.l{block}.Ws"][q[0], r] = 2.0
+        t[f"b{b}.l{block}.Ws"][q[1], r] = -2.0
+        for s, qq in zip((1.0, -1.0), q):
+            t["W1"][hid[0], b * a.S + qq] = s
+            t["W1"][hid[1], b * a.S + qq] = -s
+    t["W2"][hid[0]] = gamma
+    t["W2"][hid[1]] = -gamma
+    return t

@@ -120,3 +120,38 @@ def plateau_square_wave(n, plateaus, low, dtype=np.float32):
     for s, e in plateaus:
         x[max(s, 0):min(e, n)] = 1.0
     return x.astype(dtype)
+
+
+CFG5_CHUNK = 3600 * FS  # BASELINE.json configs[4]: one-hour chunks
+
+
+def cfg5_injections(seed=5, n_chunks=744, n_inj=20, chunk=CFG5_CHUNK):
+    """The 20 seeded A26 chirps of configs[4]: [(end_global_index, tau_s, snr)] sorted by time; tau ~ U(0.2,1) s,
+    network SNR ~ U(8,20), the chirp's end uniform over the stream (whole chirp inside it)."""
+    total = n_chunks * chunk
+    out = []
+    for j in range(n_inj):
+        u = rng.uniform01(seed, 200, np.arange(3 * j, 3 * j + 3, dtype=np.uint64))
+        tau, snr = 0.2 + 0.8 * u[0], 8.0 + 12.0 * u[1]
+        n = int(round(tau * FS))
+        out.append((n + int(u[2] * (total - n)), float(tau), float(snr)))
+    return sorted(out)
+
+
+def cfg5_chunk(c, seed=5, injections=(), n=CFG5_CHUNK, chunk=CFG5_CHUNK, dtype=np.float16):
+    """configs[4] chunk c: planar [2][n] N(0,1), detector d drawn from the generator keyed (seed, stream = 16 + 2c + d,
+    counter = sample index inside the chunk) -- "seed (5, d, c)" of SURVEY.md 8(d) -- plus the parts of `injections`
+    (global indices) that fall inside [c * chunk, c * chunk + n); rounded once to `dtype`."""
+    xs = np.empty((2, n), dtype=np.float64)
+    for d in range(2):
+        xs[d] = rng.normal(seed, 16 + 2 * c + d, 0, n)
+    start = c * chunk
+    for end_g, tau, snr in injections:
+        w = chirp_waveform(tau)
+        amp = snr / np.sqrt(2.0 * np.sum(w * w))
+        s0 = end_g - len(w)
+        lo, hi = max(s0, start), min(end_g, start + n)
+        if lo < hi:
+            for d in range(2):
+                xs[d, lo - start:hi - start] += amp * w[lo - s0:hi - s0]
+    return xs.astype(dtype)

@@ -166,6 +166,9 @@ gwi_status gwi_stream_push_host(gwi_stream* s, const void* h_h1, const void* h_l
 gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, int32_t capacity, int32_t* h_count,
                              void* cuda_stream);
 int64_t gwi_stream_samples_done(const gwi_stream* s);
+/* which back end gwi_stream_create chose (parity tests assert that the kernel they mean to check is the one that ran) */
+typedef enum { GWI_BACKEND_GENERIC = 0, GWI_BACKEND_NARROW = 1, GWI_BACKEND_TENSOR = 2, GWI_BACKEND_TENSOR_SLIDES = 3 } gwi_backend;
+int gwi_stream_backend(const gwi_stream* s);
 
 /* ---- the paper's decision rule: per-model triggers + all-model coincidence (reading A34) ------
  *

@@ -13,7 +13,7 @@ EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_m
                     "gwi_infer_workspace_bytes", "gwi_infer", "gwi_carry_bytes", "gwi_triggers_workspace_bytes",
                     "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
                     "gwi_stream_tail_samples", "gwi_stream_prime", "gwi_stream_push", "gwi_stream_push_host",
-                    "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_destroy", "gwi_stream_set_rule",
+                    "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_backend", "gwi_stream_destroy", "gwi_stream_set_rule",
                     "gwi_coincidence", "gwi_sweep_workspace_bytes", "gwi_threshold_sweep", "gwi_whiten_workspace_bytes",
                     "gwi_whiten"]
 
@@ -78,6 +78,8 @@ def lib():
     L.gwi_stream_finish.argtypes = [vp, vp, C.c_int32, i32p, vp]
     L.gwi_stream_samples_done.restype = C.c_int64
     L.gwi_stream_samples_done.argtypes = [vp]
+    L.gwi_stream_backend.restype = C.c_int
+    L.gwi_stream_backend.argtypes = [vp]
     L.gwi_stream_destroy.restype = None
     L.gwi_stream_destroy.argtypes = [vp]
     L.gwi_stream_set_rule.restype = C.c_int
@@ -239,6 +241,7 @@ def new_carry(device=0):
 
 
 RULE_MEAN, RULE_PER_MODEL = 0, 1
+BACKEND_GENERIC, BACKEND_NARROW, BACKEND_TENSOR, BACKEND_TENSOR_SLIDES = 0, 1, 2, 3
 
 
 class Event(C.Structure):
@@ -282,11 +285,13 @@ class Stream:
     def tail_samples(self):
         return lib().gwi_stream_tail_samples(self._h)
 
-    def prime(self, l1_tail):
-        """l1_tail: the last .tail_samples samples of L1 (torch tensor on the host or the device)."""
+    def prime(self, l1_tail, sync=True):
+        """l1_tail: the last .tail_samples samples of L1 (torch tensor on the host or the device).  sync=False leaves the
+        call asynchronous, as the C-ABI is (the caller then keeps l1_tail alive until the stream has been synchronised)."""
         assert l1_tail.dtype == self.dtype and l1_tail.is_contiguous()
         _check(lib().gwi_stream_prime(self._h, C.c_void_p(l1_tail.data_ptr()), l1_tail.shape[-1], _stream_ptr(self.device)))
-        torch.cuda.current_stream(self.device).synchronize()   # the caller may free a host tail right away
+        if sync:
+            torch.cuda.current_stream(self.device).synchronize()   # the caller may free a host tail right away
 
     def push(self, h1, l1):
         """h1, l1: [n] tensors of the stream dtype; device tensors -> gwi_stream_push, host tensors (pin them) ->
@@ -294,6 +299,10 @@ class Stream:
         assert h1.dtype == self.dtype and l1.dtype == self.dtype and h1.is_contiguous() and l1.is_contiguous()
         f = lib().gwi_stream_push if h1.is_cuda else lib().gwi_stream_push_host
         _check(f(self._h, C.c_void_p(h1.data_ptr()), C.c_void_p(l1.data_ptr()), h1.shape[-1], _stream_ptr(self.device)))
+
+    @property
+    def backend(self):
+        return lib().gwi_stream_backend(self._h)
 
     @property
     def samples_done(self):

@@ -299,10 +299,10 @@ gwi_status tcs_block(gwi_stream* s, int n, bool last, cudaStream_t st)
 
 // appends the n samples of staging buffer xb to the pending ones and processes every whole segment (everything at the end
 // of the stream); what is left moves to the front
-gwi_status tcs_append_and_run(gwi_stream* s, int xb, int64_t n, cudaStream_t st)
+gwi_status tcs_append_and_run(gwi_stream* s, int xb, int64_t x0, int64_t n, cudaStream_t st)
 {
     const size_t rowb = (size_t)s->xcap * 2;
-    GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_acc + s->pend, (size_t)s->acc_cap * 2, s->d_x[xb], rowb, (size_t)n * 2, 2,
+    GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_acc + s->pend, (size_t)s->acc_cap * 2, (const __half*)s->d_x[xb] + x0, rowb, (size_t)n * 2, 2,
                                      cudaMemcpyDeviceToDevice, st));
     s->pend += n, s->t_recv += n;
     const bool final = s->t_recv == s->N_total;
@@ -326,6 +326,17 @@ gwi_status tcs_append_and_run(gwi_stream* s, int xb, int64_t n, cudaStream_t st)
                                              cudaMemcpyDeviceToDevice, st));
         }
         s->pend = rest;
+    }
+    return GWI_OK;
+}
+
+// a push of any size: pieces of at most `sub` samples, so that the pending samples (< one segment window + one piece) and
+// the remainder staged through d_segx stay inside their buffers whatever max_chunk is
+gwi_status tcs_push(gwi_stream* s, int xb, int64_t n, cudaStream_t st)
+{
+    for (int64_t o = 0; o < n; o += s->sub) {
+        gwi_status rc = tcs_append_and_run(s, xb, o, std::min<int64_t>(s->sub, n - o), st);
+        if (rc != GWI_OK) return rc;
     }
     return GWI_OK;
 }
@@ -469,7 +480,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
         if ((e = cudaMalloc(&s->d_lags, (size_t)nslides * 8)) != cudaSuccess) return fail(e);
         if ((e = cudaMemcpy(s->d_lags, s->lags.data(), (size_t)nslides * 8, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
         const int64_t Bmax = ((int64_t)((double)s->sub * s->segT0 / s->seg) + 2 * SEGT_MAX) / s->segT0 + 1;
-        s->acc_cap = s->sub + SEGT_MAX + s->xcap;
+        s->acc_cap = (int64_t)s->sub + SEGT_MAX + std::min<int64_t>(s->xcap, s->sub);
         if ((e = cudaMalloc(&s->d_segx, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);
         s->tcws_bytes = gwi_tc_workspace_bytes(m0, Bmax, s->segT);
         if ((e = cudaMalloc(&s->d_tcws, s->tcws_bytes)) != cudaSuccess) return fail(e);
@@ -618,6 +629,7 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
         GWI_CUDA_CHECK(cudaGetLastError());
         s->xh_cur = 0, s->hist_t_cur = 0, s->pend = 0;
         s->primed = true;
+        for (int b = 0; b < 2; b++) GWI_CUDA_CHECK(cudaEventRecord(s->ev_consumed[b], st));
         return GWI_OK;
     }
     const int c_in = s->models[0]->arch.c_in;
@@ -675,6 +687,9 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
     }
     s->hist_cur = 0;
     s->primed = true;
+    // the first gwi_stream_push_host copies into staging buffer 0 on the side stream: it must wait for the kernels above,
+    // which read the tail out of that buffer
+    for (int b = 0; b < 2; b++) GWI_CUDA_CHECK(cudaEventRecord(s->ev_consumed[b], st));
     return GWI_OK;
 }
 
@@ -693,7 +708,7 @@ extern "C" gwi_status gwi_stream_push(gwi_stream* s, const void* d_h1, const voi
     if (s->nb > 1)
         GWI_CUDA_CHECK(cudaMemcpy2DAsync((char*)s->d_x[b] + c_in * rowb, rowb, d_l1, n * elt(s), n * elt(s),
                                          (size_t)c_in * (s->nb - 1), cudaMemcpyDeviceToDevice, st));
-    rc = s->tcs ? tcs_append_and_run(s, b, n, st) : run_chunk(s, b, n, st);
+    rc = s->tcs ? tcs_push(s, b, n, st) : run_chunk(s, b, n, st);
     if (rc != GWI_OK) return rc;
     GWI_CUDA_CHECK(cudaEventRecord(s->ev_consumed[b], st));
     s->stage ^= 1;
@@ -718,7 +733,7 @@ extern "C" gwi_status gwi_stream_push_host(gwi_stream* s, const void* h_h1, cons
                                          (size_t)c_in * (s->nb - 1), cudaMemcpyHostToDevice, s->copy_stream));
     GWI_CUDA_CHECK(cudaEventRecord(s->ev_copied[b], s->copy_stream));
     GWI_CUDA_CHECK(cudaStreamWaitEvent(st, s->ev_copied[b], 0));
-    rc = s->tcs ? tcs_append_and_run(s, b, n, st) : run_chunk(s, b, n, st);
+    rc = s->tcs ? tcs_push(s, b, n, st) : run_chunk(s, b, n, st);
     if (rc != GWI_OK) return rc;
     GWI_CUDA_CHECK(cudaEventRecord(s->ev_consumed[b], st));
     s->stage ^= 1;
@@ -768,6 +783,12 @@ extern "C" gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, 
 }
 
 extern "C" int64_t gwi_stream_samples_done(const gwi_stream* s) { return s ? s->t_done : -1; }
+
+extern "C" int gwi_stream_backend(const gwi_stream* s)
+{
+    if (!s) return -1;
+    return s->tiny ? GWI_BACKEND_NARROW : s->tcb ? GWI_BACKEND_TENSOR : s->tcs ? GWI_BACKEND_TENSOR_SLIDES : GWI_BACKEND_GENERIC;
+}
 
 extern "C" gwi_status gwi_stream_set_rule(gwi_stream* s, gwi_rule rule)
 {

@@ -104,13 +104,11 @@ def test_stream_ensemble_slides_parity(tmpdir_s, prec_name, tol, bias):
     n, recs, pbar = _run_stream(gms, x, chunks, lags, 0.5, 8, max_chunk=3000)
     err = np.max(np.abs(pbar - want))
     assert err <= tol, err
-    # lists on the oracle's own mean are robust against tol?  compare only if they are (P15), else on the GPU mean
-    lo, hi = _oracle_triggers(want, 0.5 - 2 * tol, 8), _oracle_triggers(want, 0.5 + 2 * tol, 8)
     got = trig_tuples(recs)
     assert n == len(got)
-    if lo == hi:
-        assert got == lo
-    # tier T1: the list equals the oracle's clustering of the GPU's own mean, exactly, for every input
+    # tier T1: the list equals the oracle's clustering of the GPU's own mean, exactly, for every input.  (Random weights
+    # are never delta-robust at L_min = 8 -- SURVEY.md 8(c); tier T2, strain -> triggers against the oracle's own
+    # probabilities, is tests/test_gpu_t2.py.)
     assert got == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 8)
     assert got == sorted(got)
 
@@ -147,7 +145,8 @@ def test_stream_equals_stitched_windows(tmpdir_s):
 
 
 def test_stream_triggers_with_plateaus_cross_chunks(tmpdir_s):
-    """P16-style sign pass-through model: supra-threshold plateaus of known extent, cut by chunk boundaries."""
+    """Tier T1 on many runs of many lengths: random Xavier models thresholded at the median of the oracle's mean, runs cut
+    by ragged chunk boundaries, clustered by the GPU and by the oracle on the GPU's own mean."""
     import paper_2201_11133_b200 as gwi
     oms, gms = _models(tmpdir_s, [0, 1, 2, 3], gwi.FP32)
     N = 30000
@@ -379,3 +378,111 @@ def test_paper_scale_host_push_equals_device_push(tmpdir_s, lags):
     n1, r1, p1 = _run_stream(gms, x, _ragged(N, 8, 3000, 15000), lags, 0.5, 16, host=True, max_chunk=15000)
     assert np.array_equal(p0, p1)
     assert n0 == n1 and trig_tuples(r0) == trig_tuples(r1)
+
+
+def test_config4_month_recipe_hour_chunks_from_host(tmpdir_s):
+    """BASELINE.json configs[4] recipe (SURVEY.md 8(d) cfg 5): one-hour chunks, chunk c detector d
+    seeded (5, d, c), the 20 seeded A26 chirps, pushed from pinned host memory through gwi_stream_push_host.  The stream
+    is month-chunks 0, 1 and the two chunks that hold the first two injections (4 h; the oracle cannot do 744).  The mean
+    probability is compared with the oracle on the sub-spans BASELINE.md names: the start of chunk 0, the 0 -> 1 chunk
+    boundary +- 2 s, the two injection sites; the trigger list is the oracle's clustering of the GPU's mean (T1) and,
+    where the oracle's own spans allow a statement, empty as SURVEY.md 8(c) predicts for random weights."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1, 2, 3], gwi.FP16)
+    n = gs.CFG5_CHUNK
+    inj = gs.cfg5_injections()
+    assert len(inj) == 20
+    cA, cB = inj[0][0] // n, inj[1][0] // n
+    assert 1 < cA < cB
+    month_chunks = [0, 1, cA, cB]
+    N = len(month_chunks) * n
+    st = gwi.Stream(gms, N, n, 0.5, 2048, capacity=4096, want_pbar=True)
+    assert st.backend == gwi.BACKEND_NARROW
+    host = []
+    for c in month_chunks:
+        xc = torch.from_numpy(gs.cfg5_chunk(c, injections=inj))
+        host.append((xc[0].contiguous().pin_memory(), xc[1].contiguous().pin_memory()))
+        st.push(*host[-1])
+    cnt, recs = st.finish()
+    pb = st.pbar[0].cpu().numpy()
+    st.close()
+    x = np.concatenate([np.stack([h.numpy(), l.numpy()]) for h, l in host], axis=1)
+    rf = gms[0].receptive_field
+    spans = [(0, 8192), (n - 2 * 4096, n + 2 * 4096)]
+    for j, c in ((0, 2), (1, 3)):
+        loc = inj[j][0] - month_chunks[c] * n + c * n           # the chirp's end inside the 4 h stream
+        spans.append((max(loc - 6000, c * n), min(loc + 2000, (c + 1) * n)))
+        w = gs.chirp_waveform(inj[j][1])
+        assert np.abs(x[:, max(loc - len(w), c * n):loc].astype(np.float64)).max() > 0   # the chirp lies in the chunk
+    for a, b in spans:
+        span = x[:, a:b].astype(np.float64)
+        want = gwo.ensemble_mean([om.stream(span) for om in oms])
+        lo = 0 if a == 0 else rf - 1
+        assert np.max(np.abs(pb[a + lo:b] - want[lo:])) <= 2e-3, (a, b)
+        # no oracle sample of these spans stays above theta + delta for 0.5 s: no trigger can lie inside them
+        assert gwo.triggers(want[lo:], 0.5 - 2e-3, 2048)[0] == 0
+    got = trig_tuples(recs)
+    assert cnt == len(got)
+    assert got == _oracle_triggers(pb[None].astype(np.float64), float(np.float32(0.5)), 2048)
+    assert all(not (s < b and e > a) for _, s, e in got for a, b in spans)
+
+
+def test_paper_scale_slides_one_push_larger_than_the_internal_block(tmpdir_s):
+    """A single push far larger than the tensor-core back end's internal block (sub <= 2^24 samples) with time slides:
+    the push is consumed in pieces, so the pending-sample and remainder buffers cannot overflow whatever max_chunk is.
+    One 40.1 M-sample push against the same stream in 4 M-sample pushes, bit for bit."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0], gwi.FP16, arch=gs.PAPER_ARCH)
+    N = 128 * 313_500                                   # 40 128 000 samples
+    g = torch.Generator().manual_seed(13)
+    xd = torch.randn((2, N), generator=g).to(torch.float16).cuda()
+    lags = [4096]
+    outs = []
+    for chunk in (N, 1 << 22):
+        st = gwi.Stream(gms, N, chunk, 0.5, 2048, lags=lags, capacity=4096, want_pbar=True)
+        assert st.backend == gwi.BACKEND_TENSOR_SLIDES
+        st.prime(xd[1, N - st.tail_samples:].contiguous())
+        for p in range(0, N, chunk):
+            st.push(xd[0, p:p + chunk].contiguous(), xd[1, p:p + chunk].contiguous())
+        n, recs = st.finish()
+        outs.append((n, trig_tuples(recs), st.pbar.clone()))
+        st.close()
+    assert outs[0][0] == outs[1][0] and outs[0][1] == outs[1][1]
+    assert torch.equal(outs[0][2], outs[1][2])
+    pb = outs[0][2]
+    assert bool(torch.isfinite(pb).all()) and float(pb.min()) >= 0.0 and float(pb.max()) <= 1.0
+    x = xd.cpu().numpy()
+    rf = gms[0].receptive_field
+    for s0 in [(1 << 24) - 1000, N - rf - 300]:         # across the internal block edge, and the stream's end
+        span = x[:, s0:s0 + rf + 300].astype(np.float64)
+        want = oms[0].stream(span)
+        got = pb[0, s0:s0 + rf + 300].cpu().numpy()
+        assert np.max(np.abs(got[rf - 1:] - want[rf - 1:])) <= 2e-3
+
+
+@pytest.mark.parametrize("arch_name", ["cfg1", "generic"])
+def test_prime_then_host_push_without_host_sync(tmpdir_s, arch_name):
+    """C-ABI ordering: gwi_stream_prime leaves its kernels running on the caller's stream while they read the tail out
+    of staging buffer 0; the first gwi_stream_push_host copies into that buffer on the side stream and has to wait
+    for them.  No host synchronisation between the two calls; result equal to the synchronised run bit for bit."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    prec = gwi.FP16 if arch_name == "cfg1" else gwi.FP32
+    oms, gms = _models(tmpdir_s, [0, 1, 2, 3], prec)
+    dt = np.float16 if prec == gwi.FP16 else np.float32
+    N = 400_000
+    x = torch.from_numpy(gs.stream_noise(51, 0, N, dtype=dt))
+    lags = [300_000]                                    # a long tail: the prime kernels run for a while
+    res = []
+    for sync in (True, False):
+        st = gwi.Stream(gms, N, N, 0.5, 16, lags=lags, capacity=1 << 16, want_pbar=True)
+        tail = x[1, N - st.tail_samples:].contiguous().pin_memory()
+        h, l = x[0].contiguous().pin_memory(), x[1].contiguous().pin_memory()
+        st.prime(tail, sync=sync)
+        st.push(h, l)
+        n, recs = st.finish()
+        res.append((n, trig_tuples(recs), st.pbar.clone()))
+        st.close()
+    assert res[0][0] == res[1][0] and res[0][1] == res[1][1] and torch.equal(res[0][2], res[1][2])

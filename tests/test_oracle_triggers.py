@@ -179,3 +179,37 @@ def test_p16_sign_pass_through(tmpdir_s):
         for th in (0.5 - 2e-3, 0.5 + 2e-3):
             assert [(r[1], r[2]) for r in gwo.triggers(pk, th, lmin)[1]] == want
     assert len(_intersections(ph, pl, 0, N, lmin)) >= 3 and _intersections(ph, pl, 2 * fs, N, lmin) != _intersections(ph, pl, 0, N, lmin)
+
+
+# ---- peak_p / mean_p on a NON-constant run, and the fixed fp32 mean expression (values worked by hand) --------
+def test_peak_and_mean_on_non_constant_runs():
+    """p = [.1, .6, .9, .7, .2, .8, .55, .3], theta = .5, L_min = 2: runs [1,4) and [5,7).  On [1,4) the maximum (.9) is
+    neither the first (.6), the last (.7) nor the minimum (.6); mean = 2.2/3.  On [5,7): peak .8 (first), mean 1.35/2."""
+    p = np.array([.1, .6, .9, .7, .2, .8, .55, .3])
+    n, recs = gwo.triggers(p, 0.5, 2)
+    assert n == 2 and [(r[1], r[2]) for r in recs] == [(1, 4), (5, 7)]
+    assert recs[0][3] == 0.9 and abs(recs[0][4] - 2.2 / 3) < 1e-15
+    assert recs[1][3] == 0.8 and abs(recs[1][4] - 0.675) < 1e-15
+    # the peak at the last sample of a run that touches the stream end
+    n, recs = gwo.triggers(np.array([.6, .7, .95]), 0.5, 1, t0=10)
+    assert [(r[1], r[2], r[3]) for r in recs] == [(10, 13, 0.95)]
+
+
+def test_ensemble_mean_f32_is_the_fixed_order_expression():
+    """(((p0+p1)+p2)+p3)/(float)M with IEEE round-to-nearest-even adds and ONE correctly rounded division (tier T1).
+    Expected bit patterns derived by hand, t = 2^-24 (half an ulp of 1.0f):
+      (1, t, t, t): 1+t ties to even -> 1, three times; 1/4 = 0.25                          = 0x3e800000
+      (t, t, t, 1): t+t = 2t, +t = 3t (exact), 3t+1 = 1 + 1.5 ulp -> tie to even = 1+2^-22; /4   = 0x3e800002
+        (an fp64 sum rounded once, (1+3t)/4 = 0.25 + 1.5 ulp(0.25), would also give 0x3e800002 for BOTH orders)
+      (2.5, 2.5, 0) / 3: 5/3 correctly rounded                                               = 0x3fd55555
+        (5 * float(1/3), a reciprocal multiply, gives 0x3fd55556)"""
+    t = np.float32(2.0 ** -24)
+    one = np.float32(1.0)
+
+    def bits(v):
+        return int(np.asarray(v, dtype=np.float32).view(np.uint32)[0])
+
+    a = gwo.ensemble_mean_f32([np.array([v], dtype=np.float32) for v in (one, t, t, t)])
+    b = gwo.ensemble_mean_f32([np.array([v], dtype=np.float32) for v in (t, t, t, one)])
+    c = gwo.ensemble_mean_f32([np.array([v], dtype=np.float32) for v in (2.5, 2.5, 0.0)])
+    assert bits(a) == 0x3e800000 and bits(b) == 0x3e800002 and bits(c) == 0x3fd55555
