@@ -71,9 +71,6 @@ struct TcMeta {
     int D[TC_MAX_L];          // d / 128 for kind 2 (a power of two: the ring of a layer has D entries)
     int stash_off[TC_MAX_L];  // byte offset of the layer's stash inside the slot's stash area
     int ring_off[TC_MAX_L];   // kind 2: first ring entry (in tiles) of the layer; kind 1: index among the d = 64 layers
-    int zp[TC_MAX_L];         // 1: the layer's gate output z goes to the slot's past-tile buffer instead of the operand rows
-                              // (the buffer is idle: neither this layer nor the next one is kind 2), so that the residual
-                              // update may overwrite the operand rows while the skip GEMM still reads z
     int ring_tiles;           // ring entries per slot
     int n64;                  // number of d = 64 layers
 };
@@ -92,8 +89,8 @@ __device__ uint4 g_trace[19 * TRACE_CAP];
 #define TRACE(ev, slot, n)
 #endif
 
-#ifndef GWI_TC_ALTERNATE
-#define GWI_TC_ALTERNATE 1
+#if !defined(GWI_TC_ALTERNATE) && !defined(GWI_TC_ONESLOT)
+#define GWI_TC_ALTERNATE 0
 #endif
 
 struct StackArgs {
@@ -107,7 +104,13 @@ struct StackArgs {
     uint8_t* ring64;      // [gridDim.x][2][n64][2][PRE_BYTES]
     uint8_t* u;           // [nwin][n_branch][ntiles][U_TILE_BYTES]
     TcMeta meta;
+    // bf[64], bg/2[64], br[64] of every (branch, layer), passed by value: the epilogue warps read them as constant-bank
+    // operands.  Through shared memory every such load queued behind the operand reads of the SS-mode MMAs, which take
+    // all 128 B/clk the SM has: a gate running next to the other slot's GEMMs took 2950 clk instead of 1450 (measured
+    // in isolation, _work micro-benchmark)
+    float bias[2][TC_MAX_L][BIAS_FLOATS];
 };
+static_assert(sizeof(StackArgs) <= 32764, "kernel parameter space");
 
 // ---- shared memory map of k_stack ----------------------------------------------------------------------------------
 constexpr int SM_WFG = 0;                                 // 2 stages
@@ -147,7 +150,7 @@ __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
 //     G1(slot 0, n)  G2(slot 1, n-1)  G1(slot 1, n)  G2(slot 0, n)          n = (tile, layer) iteration
 // so that while one slot's 8 epilogue warps gate (MUFU-bound), the tensor pipe and the other slot's warps work on the
 // other slot.  Weights (and the layer's biases) are double-buffered and shared by the two slots.
-__global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
+__global__ void __launch_bounds__(NTHREADS, 1) k_stack(const __grid_constant__ StackArgs a)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
@@ -164,7 +167,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
         for (int i = 0; i < B_COUNT; i++) {
             uint32_t cnt = (i >= B_Z_READY && i < B_Z_READY + 2) || (i >= B_H_READY && i < B_H_READY + 2) ? 256u : 1u;
             if (i >= B_HALF && i < B_HALF + 2) cnt = 256u;
+#ifndef GWI_TC_ONESLOT
             if ((i >= B_WFG_FREE && i < B_WFG_FREE + 2) || (i >= B_WRS_FREE && i < B_WRS_FREE + 2)) cnt = 2u;   // both issuers
+#endif
             mbar_init(bar(i), cnt);
         }
         mbar_fence_init();
@@ -222,7 +227,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     // the past tiles last: their waits (GEMM2 of the previous iteration of both slots) must not hold back
                     // the weights and biases of this iteration, which the gate needs first
                     if (M.kind[i] == 2 && j >= M.D[i]) {
+#ifdef GWI_TC_ONESLOT
+                        for (int s = 0; s < 1; s++) {
+#else
                         for (int s = 0; s < 2; s++) {
+#endif
                             // the tile was stored (j - D) tiles ago by the MMA thread, which waits for the completion
                             // of its bulk stores before it issues GEMM2 of the same iteration: GEMM2 of the previous
                             // iteration of this slot being done implies the tile is in L2
@@ -305,7 +314,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                             for (int kk = 0; kk < 4; kk++, acc = 1)
                                 tc_mma_f16(dt, ax + kk * ((2 * X_CHUNK) >> 4), bw + 1024 + kk * 256, idesc128, acc);
                         }
-                        if (stored) bulk_wait_read();   // the gate overwrites these rows once it sees FG_FULL
                         tc_commit(bar(B_FG_FULL + s));
                         if (kind == 2 && past) tc_commit(bar(B_PST_FREE + s));
                         tc_commit(bar(B_WFG_FREE + st));          // one commit per slot frees the stage
@@ -319,14 +327,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                         {
                             // the residual GEMM is on the critical path (next layer's operand), the skip GEMM is not:
                             // residual first with its own commit, the skip sum runs under the residual epilogue
+                            // A = z' in tensor memory (the gate wrote it over the g columns it had drained: channels
+                            // 0-31 at columns 64..79, channels 32-63 at 96..111 of the slot's f|g accumulator)
                             const uint64_t bw = dWrs + st * (WRS_STRIDE >> 4);
-                            const bool zp = M.zp[i] != 0;                     // z in the past-tile buffer (chunk stride 2048)
-                            const uint64_t az = zp ? apst : ax;
-                            const uint32_t kz = zp ? 4096 >> 4 : (2 * X_CHUNK) >> 4;
+                            const uint32_t az = dt + 64;
                             if (i < L - 1) {  // reading A8: the last block's residual conv has no effect
 #pragma unroll
                                 for (int kk = 0; kk < 4; kk++)
-                                    tc_mma_f16(dt, az + kk * kz, bw + 128 + kk * 384, idesc64, kk > 0 ? 1u : 0u);
+                                    tc_mma_f16_ts(dt, az + 32 * (kk >> 1) + 8 * (kk & 1), bw + 128 + kk * 384, idesc64, kk > 0 ? 1u : 0u);
                             }
                             tc_commit(bar(B_RS_FULL + s));
                             {
@@ -344,7 +352,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                             }
 #pragma unroll
                             for (int kk = 0; kk < 4; kk++)
-                                tc_mma_f16(dskip, az + kk * kz, bw + kk * 384, idesc128, (i > 0 || kk > 0) ? 1u : 0u);
+                                tc_mma_f16_ts(dskip, az + 32 * (kk >> 1) + 8 * (kk & 1), bw + kk * 384, idesc128, (i > 0 || kk > 0) ? 1u : 0u);
                         }
                         tc_commit(bar(B_SKD + s));
                         tc_commit(bar(B_WRS_FREE + st));
@@ -354,13 +362,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     n_pst[s] = npst, n_pre[s] = npre;
                 };
                 if (warp == NEPI + 1) issuer(std::integral_constant<int, 0>{});
+#ifndef GWI_TC_ONESLOT
                 else issuer(std::integral_constant<int, 1>{});
+#endif
             }
             n_it += NI;
             __syncwarp();
         } else {
             // =========================== epilogue: slot s, column half wg, row r =======================================
             const int s = warp >> 3, wg = (warp >> 2) & 1;
+#ifdef GWI_TC_ONESLOT
+            if (s == 1) { n_it += NI; continue; }
+#endif
             const int r = (warp & 3) * 32 + lane;                    // row of the tile = TMEM lane
             const int ch0 = 32 * wg, c0 = 4 * wg;                     // first channel / first 16-byte chunk of this half
             const int64_t wl = 2 * pair + s;                          // window index inside this launch
@@ -398,6 +411,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                         for (int c = 0; c < 4; c++) st_shared_v4(xs + r * 16 + (c0 + c) * X_CHUNK, 0u, 0u, 0u, 0u);
                     }
                 }
+#ifdef GWI_TC_TRACE
+                if (lane == 0) TRACE(10, 10 * (warp & 7) + s, 0);
+#endif
                 tc_fence_before();
                 fence_proxy_async_smem();
                 mbar_arrive(bar(B_H_READY + s));
@@ -424,13 +440,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     const uint32_t ph = n_it & 1;
                     const int st = n_it & 1;
                     if (i == L - 1 && j + 1 < a.ntiles) xnext = load_x(j + 1);   // strain of the next tile, a whole layer early
-                    // ---- off the critical path, while GEMM1 runs: this layer's biases (streamed behind its Wrs) and the
-                    // residual bias into the fp32 master
-                    mbar_wait(bar(B_WRS_FULL + st), (n_it >> 1) & 1);
-                    const float* bl = reinterpret_cast<const float*>(smem + SM_WRS + st * WRS_STRIDE + WRS_BYTES);
+                    // ---- off the critical path, while GEMM1 runs: the residual bias into the fp32 master
+                    const float* bl = a.bias[b][i];      // constant bank (kernel parameters)
                     if (i < L - 1) {
 #pragma unroll
-                        for (int c = 0; c < 16; c++) h[c] = add2(h[c], *reinterpret_cast<const float2*>(bl + 128 + ch0 + 2 * c));
+                        for (int c = 0; c < 16; c++) h[c] = add2(h[c], make_float2(bl[128 + ch0 + 2 * c], bl[128 + ch0 + 2 * c + 1]));
                     }
                     // ---- gate: z' = tanh(f + bf) * (1 + tanh(g/2 + bg/2))
                     mbar_wait(bar(B_FG_FULL + s), ph);
@@ -447,9 +461,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                     if (lane == 0) TRACE(5, 10 * (warp & 7) + s, j * L + i);
                     __syncwarp();
                     tc_fence_after();
-                    const bool zp = M.zp[i] != 0;
-                    const uint32_t zstride = zp ? 2048u : (uint32_t)X_CHUNK;
-                    const uint32_t zdst = zp ? sbase + SM_PST + s * PST_BYTES + r * 16 + c0 * 2048 : xs + (64 + r) * 16 + c0 * X_CHUNK;
                     {
                         // 4 chunks of 8 channels; the TMEM loads of chunk q+1 are in flight while chunk q is gated
                         uint32_t fb[2][8], gb[2][8];
@@ -468,8 +479,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                             uint32_t pk[4];
 #pragma unroll
                             for (int c = 0; c < 4; c++) {
-                                float2 bf = *reinterpret_cast<const float2*>(bl + ch0 + 8 * q + 2 * c);
-                                float2 bg = *reinterpret_cast<const float2*>(bl + 64 + ch0 + 8 * q + 2 * c);
+                                float2 bf = make_float2(bl[ch0 + 8 * q + 2 * c], bl[ch0 + 8 * q + 2 * c + 1]);
+                                float2 bg = make_float2(bl[64 + ch0 + 8 * q + 2 * c], bl[64 + ch0 + 8 * q + 2 * c + 1]);
                                 float2 fa = add2(make_float2(__uint_as_float(f[2 * c]), __uint_as_float(f[2 * c + 1])), bf);
                                 float2 ga = add2(make_float2(__uint_as_float(g[2 * c]), __uint_as_float(g[2 * c + 1])), bg);
                                 float2 tf = make_float2(tanh_approx(fa.x), tanh_approx(fa.y));
@@ -477,14 +488,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                                 float2 z = fma2(tf, tg, tf);
                                 pk[c] = pack_half2(z.x, z.y);
                             }
-                            st_shared_v4(zdst + q * zstride, pk[0], pk[1], pk[2], pk[3]);
+                            // z' chunk q (8 channels = 4 packed columns) over the g columns already read: the A operand of GEMM2
+                            tmem_st4(tg0 + 4 * q, pk[0], pk[1], pk[2], pk[3]);
 #ifdef GWI_TC_ALTERNATE
                             if (q == GWI_TC_ALTERNATE) mbar_arrive(bar(B_HALF + s));
 #endif
                         }
                     }
+                    tc_wait_st();
                     tc_fence_before();
-                    fence_proxy_async_smem();
                     mbar_arrive(bar(B_Z_READY + s));
                     if (lane == 0) TRACE(6, 10 * (warp & 7) + s, j * L + i);
                     // ---- residual update (or, after the last block, the branch output)
@@ -495,10 +507,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_stack(const StackArgs a)
                         uint32_t v[32];
                         tmem_ld32(lane_t + 128 * s + ch0, v);
                         tc_wait_ld();
+                        if (lane == 0) TRACE(9, 10 * (warp & 7) + s, j * L + i);
 #pragma unroll
                         for (int c = 0; c < 16; c++)
                             h[c] = add2(h[c], make_float2(__uint_as_float(v[2 * c]), __uint_as_float(v[2 * c + 1])));
-                        if (!zp) mbar_wait(bar(B_SKD + s), ph);   // the skip GEMM (issued after the residual GEMM) reads z from the operand rows
                         publish(i + 1, j);
                         if (lane == 0) TRACE(8, 10 * (warp & 7) + s, j * L + i);
                     } else {
@@ -762,6 +774,7 @@ struct GwiTcPack {
     uint8_t *d_wfg = nullptr, *d_wrs = nullptr, *d_w1 = nullptr;
     float *d_cst = nullptr;
     float h_hc[257];        // b1[128], W2[128], b2 (passed to k_head_tc by value)
+    float h_bias[2][TC_MAX_L][BIAS_FLOATS];   // bf, bg/2, br of every (branch, layer) (passed to k_stack by value)
     TcMeta meta;
     int num_sms = 148;
 };
@@ -796,6 +809,7 @@ gwi_status gwi_tc_pack(gwi_model* m)
     TcMeta& M = p->meta;
     memset(&M, 0, sizeof(M));
     M.L = L, M.n_branch = nb;
+    memset(p->h_bias, 0, sizeof(p->h_bias));
     int so = 0, ro = 0, n64 = 0;
     for (int i = 0; i < L; i++) {
         M.dil[i] = a.dil[i];
@@ -807,7 +821,6 @@ gwi_status gwi_tc_pack(gwi_model* m)
         else if (M.kind[i] == 1) M.ring_off[i] = n64++;
         else M.ring_off[i] = 0, so += a.dil[i] * 128;
     }
-    for (int i = 0; i < L; i++) M.zp[i] = (M.kind[i] < 2 && M.kind[(i + 1) % L] != 2) ? 1 : 0;
     M.ring_tiles = ro > 0 ? ro : 1;
     M.n64 = n64 > 0 ? n64 : 1;
     const float* W = m->host_blob.data();
@@ -840,7 +853,8 @@ gwi_status gwi_tc_pack(gwi_model* m)
                 bl[64 + c] = 0.5f * W[lo.bg + c];
                 bl[128 + c] = W[lo.br + c];
             }
-            memcpy(rs + WRS_BYTES / 2, bl, sizeof(bl));   // the layer's biases travel behind its Wrs operand
+            memcpy(rs + WRS_BYTES / 2, bl, sizeof(bl));
+            memcpy(p->h_bias[b][i], bl, sizeof(bl));
             for (int q = 0; q < 128; q++) cst[b * 256 + 128 + q] += W[lo.bs + q];
         }
     }
@@ -915,6 +929,7 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
         sa.wfg = p->d_wfg, sa.wrs = p->d_wrs, sa.cst = p->d_cst, sa.strain = d_strain;
         sa.w0 = w0, sa.nwin = nwin, sa.T = T, sa.ntiles = ntiles, sa.C = nb * m->arch.c_in;
         sa.ring = ring, sa.ring64 = ring64, sa.u = u, sa.meta = p->meta;
+        memcpy(sa.bias, p->h_bias, sizeof(sa.bias));
         int64_t njobs = ((nwin + 1) / 2) * nb;
         int grid = (int)(njobs < p->num_sms ? njobs : p->num_sms);
         k_stack<<<grid, NTHREADS, SM_TOTAL, st>>>(sa);
@@ -974,6 +989,7 @@ gwi_status gwi_tc_stack(const gwi_model* m, const __half* d_strain, int64_t B, i
     sa.wfg = p->d_wfg, sa.wrs = p->d_wrs, sa.cst = p->d_cst, sa.strain = d_strain;
     sa.w0 = 0, sa.nwin = B, sa.T = T, sa.ntiles = ntiles, sa.C = nb * m->arch.c_in;
     sa.ring = ring, sa.ring64 = ring64, sa.u = u, sa.meta = p->meta;
+    memcpy(sa.bias, p->h_bias, sizeof(sa.bias));
     int64_t njobs = ((B + 1) / 2) * nb;
     int grid = (int)(njobs < p->num_sms ? njobs : p->num_sms);
     k_stack<<<grid, NTHREADS, SM_TOTAL, st>>>(sa);
