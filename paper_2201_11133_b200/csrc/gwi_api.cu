@@ -166,6 +166,7 @@ extern "C" void gwi_free_model(gwi_model* m)
     if (!m) return;
     gwi_tc_free(m);
     gwi_tiny_free(m);
+    gwi_tiny_tc_free(m);
     if (m->d_blob) cudaFree(m->d_blob);
     if (m->d_off) cudaFree(m->d_off);
     delete m;

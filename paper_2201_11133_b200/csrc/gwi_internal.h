@@ -55,6 +55,8 @@ struct GwiDevModel {
 struct GwiTcPack;
 // Packed fragments of the fused narrow-architecture stream kernel (gwi_tiny.cu); null when not covered / not FP16.
 struct GwiTinyPack;
+// Packed operands of the tcgen05 narrow-architecture stream kernel (gwi_tiny_tc.cu); null when not covered / not FP16.
+struct GwiTinyTcPack;
 
 struct gwi_model {
     GwiArch arch;
@@ -66,6 +68,7 @@ struct gwi_model {
     GwiOffsets* d_off = nullptr; // copy of `off` in device memory
     GwiTcPack* tc = nullptr;
     GwiTinyPack* tiny = nullptr;
+    GwiTinyTcPack* tinytc = nullptr;
 };
 
 // ---- generic CUDA-core path (gwi_generic.cu) ---------------------------------------------------------------
@@ -112,4 +115,10 @@ gwi_status gwi_tiny_stream(const gwi_model* m, const __half* d_x, int64_t ldx, i
                            __half* xh_next, float* d_prob, __half* d_u16, int64_t lds, cudaStream_t st);
 gwi_status gwi_tiny_heads(const gwi_model* m, const __half* d_u16, int64_t lds, int n, const int64_t* d_lags, int n_lags,
                           float* d_prob, int64_t stride_k, cudaStream_t st);
+// tcgen05 version of the same kernel (gwi_tiny_tc.cu); gwi_tiny_stream dispatches to it
+bool gwi_tiny_tc_supported(const GwiArch& a);
+gwi_status gwi_tiny_tc_pack(gwi_model* m);
+void gwi_tiny_tc_free(gwi_model* m);
+gwi_status gwi_tiny_tc_stream(const gwi_model* m, const __half* d_x, int64_t ldx, int n, int64_t t0, const __half* xh_cur,
+                              float* d_prob, __half* d_u16, int64_t lds, cudaStream_t st);
 gwi_status gwi_xhist_update(const __half* d_x, int64_t ldx, int n, int halo, const __half* xh_cur, __half* xh_next, cudaStream_t st);

@@ -53,6 +53,21 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     }
 }
 
+// The same for many waiting warps: each poll may sleep up to `hint_ns` (the hardware wakes the thread when the phase
+// completes), so that the waiters leave the issue slots to the warps that have work
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, uint32_t hint_ns)
+{
+    uint32_t spins = 0, ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity), "r"(hint_ns)
+            : "memory");
+        if (++spins > (1u << 24)) __trap();
+    }
+}
+
 // ---- bulk async copy global -> shared (1-D, multiple of 16 bytes, 16-byte aligned), completes on an mbarrier ----
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
 {

@@ -19,6 +19,7 @@
 //
 // Output: either the per-sample probability (fused head, zero lag) or, for time slides (reading A24), the branch
 // features u = ReLU(skip sum) as fp16 time-major rows, from which k_tiny_heads evaluates the head for every lag.
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -27,7 +28,8 @@
 namespace {
 
 constexpr int TW = 8;             // warps per CTA
-constexpr int ROWS = TW * 16;     // rows (time steps) per CTA tile, halo included
+constexpr int NT = 2;             // 16-row MMA tiles per warp: every weight / bias fragment load serves 32 rows
+constexpr int ROWS = TW * NT * 16;   // rows (time steps) per CTA tile, halo included
 constexpr int RS = 24;            // shared-memory row stride in halves (16 channels + 8 pad = 48 bytes)
 constexpr int PADROWS = 64;       // zero rows in front of the tile (reads at row - d of the first rows)
 constexpr int TINY_MAX_L = 8;
@@ -49,11 +51,19 @@ struct TinyArgs {
     int64_t lds;          //   (null in fused mode); row 0 = sample 0 of this chunk
 };
 
+// D (+)= A B, accumulating in place
 __device__ __forceinline__ void mma16816(float (&c)[4], const uint32_t (&a)[4], uint2 b)
 {
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b.x), "r"(b.y));
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b.x), "r"(b.y));
+}
+// D = A B + (c0, c1, c0, c1): the accumulator starts at the bias of its two columns without being initialised by moves
+__device__ __forceinline__ void mma16816_bias(float (&d)[4], const uint32_t (&a)[4], uint2 b, float c0, float c1)
+{
+    asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%11,%10,%11};"
+        : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b.x), "r"(b.y), "f"(c0), "f"(c1));
 }
 __device__ __forceinline__ uint32_t pack2(float lo, float hi)
 {
@@ -67,165 +77,216 @@ __device__ __forceinline__ float tanh_fast(float x)
     return y;
 }
 
-__global__ void __launch_bounds__(TW * 32, 3) k_tiny(const TinyArgs a)
+__global__ void __launch_bounds__(TW * 32, 2) k_tiny(const __grid_constant__ TinyArgs a)
 {
     // two operand buffers (layer parity), each PADROWS zero rows + ROWS rows of 16 halves (+ pad)
     __shared__ __align__(16) __half sm[2][(PADROWS + ROWS) * RS];
+    __shared__ uint4 sm_u[NT][2][TW * 32];                               // branch 0's head fragments, parked while branch 1 runs
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int valid = ROWS - a.halo;                                    // output rows per CTA
     const int64_t tile0 = (int64_t)blockIdx.x * valid - a.halo;          // chunk-local time of row 0
-    const int r0 = warp * 16 + g, r1 = r0 + 8;                           // this thread's two rows
-    const int64_t tl0 = tile0 + r0, tl1 = tile0 + r1;                    // chunk-local times
+    // this thread's rows: tile tl of the warp holds rows rbase + 16 tl + g and + 8
+    const int rbase = warp * (16 * NT) + g;
     // rows before the stream start are zero at every layer input (reading A4)
     const bool premask = a.t0 + tile0 < 0;                               // CTA-uniform: only the first tile of a stream
-    const bool live0 = a.t0 + tl0 >= 0, live1 = a.t0 + tl1 >= 0;
     for (int i = threadIdx.x; i < 2 * PADROWS * RS / 2; i += TW * 32) {
         int buf = i / (PADROWS * RS / 2), k = i % (PADROWS * RS / 2);
         reinterpret_cast<uint32_t*>(sm[buf])[k] = 0u;
     }
     const float* hcst = a.cst + 2 * 32;
-    uint32_t ua[2][4];                                                   // head A fragments of the current branch
-    __shared__ uint4 sm_u[2][TW * 32];                                   // branch 0's fragments, parked while branch 1 runs
+    uint32_t ua[NT][2][4];                                               // head A fragments of the current branch
 
 #pragma unroll
     for (int b = 0; b < 2; b++) {
         // ---- lift (C.1 step 1): h0[r] = W_in[r] x + b_in[r]; fp32 master in accumulator-fragment layout
-        float x0 = 0.f, x1 = 0.f;
+        float h[NT][2][4];                                               // [tile][n-tile (8 channels)][c0..c3]
         {
             const __half* xc = a.x + (int64_t)b * a.ldx;
             const __half* xp = a.xh + b * a.halo;
-            if (tl0 >= 0) { if (tl0 < a.n) x0 = __half2float(xc[tl0]); } else x0 = __half2float(xp[a.halo + tl0]);
-            if (tl1 >= 0) { if (tl1 < a.n) x1 = __half2float(xc[tl1]); } else x1 = __half2float(xp[a.halo + tl1]);
-        }
-        const float* cb = a.cst + b * 32;
-        float h[2][4];                                                   // [n-tile (8 channels)][c0..c3]
+            const float* cb = a.cst + b * 32;
+            float2 w[2], bi[2];
 #pragma unroll
-        for (int nt = 0; nt < 2; nt++) {
-            float2 w = __ldg(reinterpret_cast<const float2*>(cb + 8 * nt + 2 * t));
-            float2 bi = __ldg(reinterpret_cast<const float2*>(cb + 16 + 8 * nt + 2 * t));
-            h[nt][0] = fmaf(w.x, x0, bi.x), h[nt][1] = fmaf(w.y, x0, bi.y);
-            h[nt][2] = fmaf(w.x, x1, bi.x), h[nt][3] = fmaf(w.y, x1, bi.y);
-            if (premask) {
-                if (!live0) h[nt][0] = h[nt][1] = 0.f;
-                if (!live1) h[nt][2] = h[nt][3] = 0.f;
+            for (int nt = 0; nt < 2; nt++) {
+                w[nt] = __ldg(reinterpret_cast<const float2*>(cb + 8 * nt + 2 * t));
+                bi[nt] = __ldg(reinterpret_cast<const float2*>(cb + 16 + 8 * nt + 2 * t));
+            }
+#pragma unroll
+            for (int tl = 0; tl < NT; tl++) {
+                const int64_t tl0 = tile0 + rbase + 16 * tl, tl1 = tl0 + 8;
+                float x0 = 0.f, x1 = 0.f;
+                if (tl0 >= 0) { if (tl0 < a.n) x0 = __half2float(xc[tl0]); } else x0 = __half2float(xp[a.halo + tl0]);
+                if (tl1 >= 0) { if (tl1 < a.n) x1 = __half2float(xc[tl1]); } else x1 = __half2float(xp[a.halo + tl1]);
+#pragma unroll
+                for (int nt = 0; nt < 2; nt++) {
+                    h[tl][nt][0] = fmaf(w[nt].x, x0, bi[nt].x), h[tl][nt][1] = fmaf(w[nt].y, x0, bi[nt].y);
+                    h[tl][nt][2] = fmaf(w[nt].x, x1, bi[nt].x), h[tl][nt][3] = fmaf(w[nt].y, x1, bi[nt].y);
+                }
+                if (premask) {
+                    if (a.t0 + tl0 < 0) h[tl][0][0] = h[tl][0][1] = h[tl][1][0] = h[tl][1][1] = 0.f;
+                    if (a.t0 + tl1 < 0) h[tl][0][2] = h[tl][0][3] = h[tl][1][2] = h[tl][1][3] = 0.f;
+                }
             }
         }
-        float sk[4][4];                                                  // skip sum, 4 n-tiles of 8 channels
+        float sk[NT][4][4];                                              // skip sum, 4 n-tiles of 8 channels
 #pragma unroll
         for (int nt = 0; nt < 4; nt++) {                                 // starts at sum_i bs_i (summed on the host)
             float2 bb = __ldg(reinterpret_cast<const float2*>(a.cst + 2 * 32 + 66 + b * 32 + 8 * nt + 2 * t));
-            sk[nt][0] = bb.x, sk[nt][1] = bb.y, sk[nt][2] = bb.x, sk[nt][3] = bb.y;
+#pragma unroll
+            for (int tl = 0; tl < NT; tl++) sk[tl][nt][0] = bb.x, sk[tl][nt][1] = bb.y, sk[tl][nt][2] = bb.x, sk[tl][nt][3] = bb.y;
         }
 
-        const float* bl = a.bias + (size_t)b * a.L * 80;
+        const float* bl = a.bias + (size_t)b * a.L * 80 + 2 * t;
         const uint2* wf = a.wfg + (size_t)b * a.L * (2 * 4 * 32) + lane;
         const uint2* wr = a.wrs + (size_t)b * a.L * (6 * 32) + lane;
         for (int i = 0; i < a.L; i++, bl += 80, wf += 2 * 4 * 32, wr += 6 * 32) {
             const int d = a.dil[i];
-            __half* buf = sm[i & 1] + PADROWS * RS;
+            __half* buf = sm[i & 1] + (PADROWS + rbase) * RS + 2 * t;
             // ---- current-tap A fragment = this thread's own h values; parked in shared memory for the rows d later
-            uint32_t ac[4] = {pack2(h[0][0], h[0][1]), pack2(h[0][2], h[0][3]), pack2(h[1][0], h[1][1]), pack2(h[1][2], h[1][3])};
-            *reinterpret_cast<uint32_t*>(buf + r0 * RS + 2 * t) = ac[0];
-            *reinterpret_cast<uint32_t*>(buf + r1 * RS + 2 * t) = ac[1];
-            *reinterpret_cast<uint32_t*>(buf + r0 * RS + 8 + 2 * t) = ac[2];
-            *reinterpret_cast<uint32_t*>(buf + r1 * RS + 8 + 2 * t) = ac[3];
+            uint32_t ac[NT][4], ap[NT][4];
+#pragma unroll
+            for (int tl = 0; tl < NT; tl++) {
+                ac[tl][0] = pack2(h[tl][0][0], h[tl][0][1]), ac[tl][1] = pack2(h[tl][0][2], h[tl][0][3]);
+                ac[tl][2] = pack2(h[tl][1][0], h[tl][1][1]), ac[tl][3] = pack2(h[tl][1][2], h[tl][1][3]);
+                __half* row = buf + 16 * tl * RS;
+                *reinterpret_cast<uint32_t*>(row) = ac[tl][0];
+                *reinterpret_cast<uint32_t*>(row + 8 * RS) = ac[tl][1];
+                *reinterpret_cast<uint32_t*>(row + 8) = ac[tl][2];
+                *reinterpret_cast<uint32_t*>(row + 8 * RS + 8) = ac[tl][3];
+            }
             __syncthreads();   // one barrier per layer: the buffers alternate, so layer i+2 cannot overtake layer i readers
-            uint32_t ap[4];
-            ap[0] = *reinterpret_cast<const uint32_t*>(buf + (r0 - d) * RS + 2 * t);
-            ap[1] = *reinterpret_cast<const uint32_t*>(buf + (r1 - d) * RS + 2 * t);
-            ap[2] = *reinterpret_cast<const uint32_t*>(buf + (r0 - d) * RS + 8 + 2 * t);
-            ap[3] = *reinterpret_cast<const uint32_t*>(buf + (r1 - d) * RS + 8 + 2 * t);
+#pragma unroll
+            for (int tl = 0; tl < NT; tl++) {
+                const __half* row = buf + (16 * tl - d) * RS;
+                ap[tl][0] = *reinterpret_cast<const uint32_t*>(row);
+                ap[tl][1] = *reinterpret_cast<const uint32_t*>(row + 8 * RS);
+                ap[tl][2] = *reinterpret_cast<const uint32_t*>(row + 8);
+                ap[tl][3] = *reinterpret_cast<const uint32_t*>(row + 8 * RS + 8);
+            }
             // ---- f | g/2 = [h(t-d) | h(t)] . W^T + bias                                      (C.1 step 2)
-            float fg[4][4];
+            float fg[NT][4][4];
 #pragma unroll
             for (int nt = 0; nt < 4; nt++) {
-                float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 8 * nt + 2 * t));
-                fg[nt][0] = bb.x, fg[nt][1] = bb.y, fg[nt][2] = bb.x, fg[nt][3] = bb.y;
-                mma16816(fg[nt], ap, __ldg(wf + (0 * 4 + nt) * 32));
-                mma16816(fg[nt], ac, __ldg(wf + (1 * 4 + nt) * 32));
+                const float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 8 * nt));
+                const uint2 w0 = __ldg(wf + (0 * 4 + nt) * 32), w1 = __ldg(wf + (1 * 4 + nt) * 32);
+#pragma unroll
+                for (int tl = 0; tl < NT; tl++) {
+                    mma16816_bias(fg[tl][nt], ap[tl], w0, bb.x, bb.y);
+                    mma16816(fg[tl][nt], ac[tl], w1);
+                }
             }
             // ---- z' = tanh(f) (1 + tanh(g/2)) = 2 tanh(f) sigmoid(g); the 2 is folded into Wr/2, Ws/2
-            uint32_t az[4];
-            {
+            uint32_t az[NT][4];
+#pragma unroll
+            for (int tl = 0; tl < NT; tl++) {
                 float z[2][4];
 #pragma unroll
                 for (int nt = 0; nt < 2; nt++)
 #pragma unroll
                     for (int c = 0; c < 4; c++) {
-                        float tf = tanh_fast(fg[nt][c]), tg = tanh_fast(fg[nt + 2][c]);
+                        float tf = tanh_fast(fg[tl][nt][c]), tg = tanh_fast(fg[tl][nt + 2][c]);
                         z[nt][c] = fmaf(tf, tg, tf);
                     }
-                az[0] = pack2(z[0][0], z[0][1]), az[1] = pack2(z[0][2], z[0][3]);
-                az[2] = pack2(z[1][0], z[1][1]), az[3] = pack2(z[1][2], z[1][3]);
+                az[tl][0] = pack2(z[0][0], z[0][1]), az[tl][1] = pack2(z[0][2], z[0][3]);
+                az[tl][2] = pack2(z[1][0], z[1][1]), az[tl][3] = pack2(z[1][2], z[1][3]);
             }
-            // ---- res | skip = z' . [Wr/2 | Ws/2]^T
+            // ---- h += br + z' . (Wr/2)^T ;  skip += z' . (Ws/2)^T
             if (i < a.L - 1) {                                           // reading A8: the last residual conv is dead
 #pragma unroll
                 for (int nt = 0; nt < 2; nt++) {
-                    float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 32 + 8 * nt + 2 * t));
-                    float rr[4] = {bb.x, bb.y, bb.x, bb.y};
-                    mma16816(rr, az, __ldg(wr + nt * 32));
-                    h[nt][0] += rr[0], h[nt][1] += rr[1], h[nt][2] += rr[2], h[nt][3] += rr[3];
-                    if (premask) {
-                        if (!live0) h[nt][0] = h[nt][1] = 0.f;
-                        if (!live1) h[nt][2] = h[nt][3] = 0.f;
+                    const float2 bb = __ldg(reinterpret_cast<const float2*>(bl + 32 + 8 * nt));
+                    const uint2 w = __ldg(wr + nt * 32);
+#pragma unroll
+                    for (int tl = 0; tl < NT; tl++) {
+                        float rr[4];
+                        mma16816_bias(rr, az[tl], w, bb.x, bb.y);
+                        h[tl][nt][0] += rr[0], h[tl][nt][1] += rr[1], h[tl][nt][2] += rr[2], h[tl][nt][3] += rr[3];
+                    }
+                }
+                if (premask) {
+#pragma unroll
+                    for (int tl = 0; tl < NT; tl++) {
+                        const int64_t tg0 = a.t0 + tile0 + rbase + 16 * tl;
+                        if (tg0 < 0) h[tl][0][0] = h[tl][0][1] = h[tl][1][0] = h[tl][1][1] = 0.f;
+                        if (tg0 + 8 < 0) h[tl][0][2] = h[tl][0][3] = h[tl][1][2] = h[tl][1][3] = 0.f;
                     }
                 }
             }
 #pragma unroll
             for (int nt = 0; nt < 4; nt++) {
-                mma16816(sk[nt], az, __ldg(wr + (2 + nt) * 32));
+                const uint2 w = __ldg(wr + (2 + nt) * 32);
+#pragma unroll
+                for (int tl = 0; tl < NT; tl++) mma16816(sk[tl][nt], az[tl], w);
             }
         }
-        if (a.u16) {
-            // ---- time-slide mode: u_b = ReLU(skip sum) in fp16, time-major, for the per-lag heads (k_tiny_heads)
-            __half* up = a.u16 + (size_t)b * a.lds * 32;
 #pragma unroll
-            for (int nt = 0; nt < 4; nt++) {
-                const int q = 8 * nt + 2 * t;
-                if (r0 >= a.halo && tl0 < a.n)
-                    *reinterpret_cast<uint32_t*>(up + tl0 * 32 + q) = pack2(fmaxf(sk[nt][0], 0.f), fmaxf(sk[nt][1], 0.f));
-                if (r1 >= a.halo && tl1 < a.n)
-                    *reinterpret_cast<uint32_t*>(up + tl1 * 32 + q) = pack2(fmaxf(sk[nt][2], 0.f), fmaxf(sk[nt][3], 0.f));
-            }
-        } else {
-            // ---- u_b = ReLU(skip sum) as the A fragments of the head                        (C.1 steps 3, 4)
+        for (int tl = 0; tl < NT; tl++) {
+            const int r0 = rbase + 16 * tl, r1 = r0 + 8;
+            const int64_t tl0 = tile0 + r0, tl1 = tl0 + 8;
+            if (a.u16) {
+                // ---- time-slide mode: u_b = ReLU(skip sum) in fp16, time-major, for the per-lag heads (k_tiny_heads)
+                __half* up = a.u16 + (size_t)b * a.lds * 32;
 #pragma unroll
-            for (int ks = 0; ks < 2; ks++) {
-                ua[ks][0] = pack2(fmaxf(sk[2 * ks][0], 0.f), fmaxf(sk[2 * ks][1], 0.f));
-                ua[ks][1] = pack2(fmaxf(sk[2 * ks][2], 0.f), fmaxf(sk[2 * ks][3], 0.f));
-                ua[ks][2] = pack2(fmaxf(sk[2 * ks + 1][0], 0.f), fmaxf(sk[2 * ks + 1][1], 0.f));
-                ua[ks][3] = pack2(fmaxf(sk[2 * ks + 1][2], 0.f), fmaxf(sk[2 * ks + 1][3], 0.f));
-                if (b == 0) sm_u[ks][threadIdx.x] = make_uint4(ua[ks][0], ua[ks][1], ua[ks][2], ua[ks][3]);
+                for (int nt = 0; nt < 4; nt++) {
+                    const int q = 8 * nt + 2 * t;
+                    if (r0 >= a.halo && tl0 < a.n)
+                        *reinterpret_cast<uint32_t*>(up + tl0 * 32 + q) = pack2(fmaxf(sk[tl][nt][0], 0.f), fmaxf(sk[tl][nt][1], 0.f));
+                    if (r1 >= a.halo && tl1 < a.n)
+                        *reinterpret_cast<uint32_t*>(up + tl1 * 32 + q) = pack2(fmaxf(sk[tl][nt][2], 0.f), fmaxf(sk[tl][nt][3], 0.f));
+                }
+            } else {
+                // ---- u_b = ReLU(skip sum) as the A fragments of the head                        (C.1 steps 3, 4)
+#pragma unroll
+                for (int ks = 0; ks < 2; ks++) {
+                    ua[tl][ks][0] = pack2(fmaxf(sk[tl][2 * ks][0], 0.f), fmaxf(sk[tl][2 * ks][1], 0.f));
+                    ua[tl][ks][1] = pack2(fmaxf(sk[tl][2 * ks][2], 0.f), fmaxf(sk[tl][2 * ks][3], 0.f));
+                    ua[tl][ks][2] = pack2(fmaxf(sk[tl][2 * ks + 1][0], 0.f), fmaxf(sk[tl][2 * ks + 1][1], 0.f));
+                    ua[tl][ks][3] = pack2(fmaxf(sk[tl][2 * ks + 1][2], 0.f), fmaxf(sk[tl][2 * ks + 1][3], 0.f));
+                    if (b == 0) sm_u[tl][ks][threadIdx.x] = make_uint4(ua[tl][ks][0], ua[tl][ks][1], ua[tl][ks][2], ua[tl][ks][3]);
+                }
             }
         }
         __syncthreads();   // the next branch starts again with buffer 0
     }
     if (a.u16) return;
     // ---- head: v = ReLU(W1 [u_H; u_L] + b1), y = W2 . v + b2, p = sigmoid(y)                   (C.1 step 5)
-    float y0 = 0.f, y1 = 0.f;
+    float y[NT][2];
+#pragma unroll
+    for (int tl = 0; tl < NT; tl++) y[tl][0] = y[tl][1] = 0.f;
 #pragma unroll
     for (int nt = 0; nt < 4; nt++) {
-        float2 bb = __ldg(reinterpret_cast<const float2*>(hcst + 8 * nt + 2 * t));
-        float v[4] = {bb.x, bb.y, bb.x, bb.y};
+        const float2 bb = __ldg(reinterpret_cast<const float2*>(hcst + 8 * nt + 2 * t));
+        const float2 w2 = __ldg(reinterpret_cast<const float2*>(hcst + 32 + 8 * nt + 2 * t));
+        uint2 w[4];
 #pragma unroll
-        for (int ks = 0; ks < 2; ks++) {                                 // H1 half (parked), then L1 half
-            uint4 p = sm_u[ks][threadIdx.x];
-            uint32_t ah[4] = {p.x, p.y, p.z, p.w};
-            mma16816(v, ah, __ldg(a.w1 + (ks * 4 + nt) * 32 + lane));
+        for (int ks = 0; ks < 4; ks++) w[ks] = __ldg(a.w1 + (ks * 4 + nt) * 32 + lane);
+#pragma unroll
+        for (int tl = 0; tl < NT; tl++) {
+            float v[4];
+#pragma unroll
+            for (int ks = 0; ks < 2; ks++) {                             // H1 half (parked), then L1 half
+                uint4 p = sm_u[tl][ks][threadIdx.x];
+                uint32_t ah[4] = {p.x, p.y, p.z, p.w};
+                if (ks == 0) mma16816_bias(v, ah, w[0], bb.x, bb.y);
+                else mma16816(v, ah, w[1]);
+            }
+#pragma unroll
+            for (int ks = 0; ks < 2; ks++) mma16816(v, ua[tl][ks], w[2 + ks]);
+            y[tl][0] = fmaf(w2.x, fmaxf(v[0], 0.f), y[tl][0]), y[tl][0] = fmaf(w2.y, fmaxf(v[1], 0.f), y[tl][0]);
+            y[tl][1] = fmaf(w2.x, fmaxf(v[2], 0.f), y[tl][1]), y[tl][1] = fmaf(w2.y, fmaxf(v[3], 0.f), y[tl][1]);
         }
-#pragma unroll
-        for (int ks = 0; ks < 2; ks++) mma16816(v, ua[ks], __ldg(a.w1 + ((2 + ks) * 4 + nt) * 32 + lane));
-        float2 w2 = __ldg(reinterpret_cast<const float2*>(hcst + 32 + 8 * nt + 2 * t));
-        y0 = fmaf(w2.x, fmaxf(v[0], 0.f), y0), y0 = fmaf(w2.y, fmaxf(v[1], 0.f), y0);
-        y1 = fmaf(w2.x, fmaxf(v[2], 0.f), y1), y1 = fmaf(w2.y, fmaxf(v[3], 0.f), y1);
     }
-    y0 += __shfl_xor_sync(0xffffffffu, y0, 1), y1 += __shfl_xor_sync(0xffffffffu, y1, 1);
-    y0 += __shfl_xor_sync(0xffffffffu, y0, 2), y1 += __shfl_xor_sync(0xffffffffu, y1, 2);
-    if (t == 0) {
-        const float b2 = __ldg(hcst + 64);
-        if (r0 >= a.halo && tl0 < a.n) a.prob[tl0] = 1.0f / (1.0f + __expf(-(y0 + b2)));
-        if (r1 >= a.halo && tl1 < a.n) a.prob[tl1] = 1.0f / (1.0f + __expf(-(y1 + b2)));
+    const float b2 = __ldg(hcst + 64);
+#pragma unroll
+    for (int tl = 0; tl < NT; tl++) {
+        float y0 = y[tl][0], y1 = y[tl][1];
+        y0 += __shfl_xor_sync(0xffffffffu, y0, 1), y1 += __shfl_xor_sync(0xffffffffu, y1, 1);
+        y0 += __shfl_xor_sync(0xffffffffu, y0, 2), y1 += __shfl_xor_sync(0xffffffffu, y1, 2);
+        if (t == 0) {
+            const int r0 = rbase + 16 * tl, r1 = r0 + 8;
+            const int64_t tl0 = tile0 + r0, tl1 = tl0 + 8;
+            if (r0 >= a.halo && tl0 < a.n) a.prob[tl0] = 1.0f / (1.0f + __expf(-(y0 + b2)));
+            if (r1 >= a.halo && tl1 < a.n) a.prob[tl1] = 1.0f / (1.0f + __expf(-(y1 + b2)));
+        }
     }
 }
 
@@ -347,6 +408,7 @@ struct GwiTinyPack {
     uint4* d_w1t = nullptr;
     float *d_bias = nullptr, *d_cst = nullptr;
     int halo = 16;
+    bool force_mma_sync = false;
 };
 
 bool gwi_tiny_supported(const GwiArch& a)
@@ -434,6 +496,9 @@ gwi_status gwi_tiny_pack(gwi_model* m)
     GWI_CUDA_CHECK(up((void**)&p->d_w1t, w1t.data(), w1t.size() * 16));
     GWI_CUDA_CHECK(up((void**)&p->d_bias, bias.data(), bias.size() * 4));
     GWI_CUDA_CHECK(up((void**)&p->d_cst, cst.data(), cst.size() * 4));
+    const char* env = getenv("GWI_TINY_MMASYNC");
+    p->force_mma_sync = env && env[0] == '1';
+    if (gwi_tiny_tc_supported(a)) return gwi_tiny_tc_pack(m);
     return GWI_OK;
 }
 
@@ -453,6 +518,17 @@ gwi_status gwi_tiny_stream(const gwi_model* m, const __half* d_x, int64_t ldx, i
                            __half* xh_next, float* d_prob, __half* d_u16, int64_t lds, cudaStream_t st)
 {
     const GwiTinyPack* p = m->tiny;
+    if (m->tinytc && !p->force_mma_sync) {
+        // the tcgen05 kernel (gwi_tiny_tc.cu); the warp-MMA kernel below stays as the A/B reference (GWI_TINY_MMASYNC=1)
+        gwi_status rc = gwi_tiny_tc_stream(m, d_x, ldx, n, t0, xh_cur, d_prob, d_u16, lds, st);
+        if (rc != GWI_OK) return rc;
+        if (xh_next) {
+            k_tiny_xhist<<<(2 * p->halo + 127) / 128, 128, 0, st>>>(d_x, ldx, n, p->halo, xh_cur, xh_next);
+            gwi_count_launch(1);
+            GWI_CUDA_CHECK(cudaGetLastError());
+        }
+        return GWI_OK;
+    }
     TinyArgs a;
     a.wfg = p->d_wfg, a.wrs = p->d_wrs, a.w1 = p->d_w1, a.bias = p->d_bias, a.cst = p->d_cst;
     a.x = d_x, a.xh = xh_cur, a.ldx = ldx, a.t0 = t0, a.n = n, a.L = m->arch.L, a.halo = p->halo;
