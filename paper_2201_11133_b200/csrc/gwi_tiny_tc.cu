@@ -24,10 +24,16 @@
 // independent work hide the ~400-clock issue -> complete -> wake latency of each tiny GEMM.  The weights of the model
 // (52 KB with the bias steps) stay in shared memory for the whole launch.
 //
-// Overlap reuse as in gwi_tiny.cu: the first `halo` rows of a tile are recomputed from the input (the carried last
-// `halo` samples of the previous chunk), so nothing else is carried; rows at global time t < 0 are forced to zero at
-// every layer input (reading A4).  Every output sample is a fixed-order computation that does not depend on the tile
-// it falls in, so chunked == unchunked bit for bit (reading A17).
+// Overlap reuse: a slot works through a contiguous span of tiles; the last SR = 16 operand rows of every (branch, block)
+// are kept in a shared-memory stash and put in front of the next tile's operand rows (all d <= 16), so a tile is 128
+// output samples.  A span starts with one warm-up tile (the 128 samples before it, nothing stored) that fills the
+// stash; before a chunk it is fed from the carried last `halo` input samples of the previous chunk, which is all the
+// stashed rows depend on (receptive field <= halo + 1).  With a dilation > 16 the kernel falls back to recomputing a
+// halo of `halo` rows per tile, as gwi_tiny.cu does.  Rows at global time t < 0 are forced to zero at every layer input
+// (reading A4).  Every output sample is a fixed-order computation that does not depend on the tile it falls in, so
+// chunked == unchunked bit for bit (reading A17).
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -50,6 +56,8 @@ constexpr int WFG_L = 32 * 48 * 2;              // per (branch, layer): N = 32 (
 constexpr int WRS_L = 48 * 32 * 2;              // N = 48 (res | skip) x K = 32 (z' | bias step: br, bs)
 constexpr int W1_B = 32 * 80 * 2;               // N = 32 x K = 80 ([u_H | u_L] | bias step: b1)
 constexpr int ONES_B = 2 * 128 * 16;            // A operand of the bias steps: 128 rows x K = 16, element (r, 0) = 1
+constexpr int SR = 16;                          // stashed operand rows per (branch, block)
+constexpr int STASH_SLOT = 2 * TT_MAX_L * 2 * SR * 16;   // [branch][block][chunk][SR rows] x 16 B = 8 KB
 constexpr int TCOLS = 80;                       // TMEM columns per slot: f 0-15, g 16-31 (z' over 16-23), h 32-47, skip 48-79
 
 struct TtArgs {
@@ -58,6 +66,7 @@ struct TtArgs {
     const __half* xh;     // [2][halo] last halo samples of the previous chunk (zeros at the stream start)
     int64_t ldx, t0;      // t0 = global index of sample 0 of this chunk
     int n, L, halo, ntiles;
+    int stash;            // 1: 128-sample tiles with stashed operand rows, 0: tiles of 128 - halo samples with recomputed halo
     int dil[TT_MAX_L];
     float* prob;          // fused head: [n] probabilities (null in time-slide mode)
     __half* u16;          // time-slide mode: [2][lds][32] branch features, fp16, time-major; row 0 = sample 0 of the chunk
@@ -82,15 +91,38 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8])
                  : "memory");
 }
 
+#ifdef GWI_TT_TRACE
+__device__ unsigned long long g_tt_trace[8192];
+#define TT_TRACE(code)                                                                          \
+    do {                                                                                        \
+        if (blockIdx.x == 0 && slot == 0 && q == TT_TRACE_Q && lane == 0 && tt_k < 8190) g_tt_trace[tt_k++] = ((unsigned long long)(code) << 48) | (clock64() & 0xffffffffffffull); \
+    } while (0)
+#ifndef TT_TRACE_Q
+#define TT_TRACE_Q 0
+#endif
+#else
+#define TT_TRACE(code)
+#endif
+
+#ifndef GWI_TT_SLEEP_NS
+#define GWI_TT_SLEEP_NS 4000
+#endif
+
+// LT = compile-time number of blocks (the layer loop is unrolled, descriptor offsets become constants), 0 = any (a.L)
+template <int LT>
 __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant__ TtArgs a)
 {
     extern __shared__ __align__(1024) uint8_t smem[];
-    const int L = a.L;
+    const int L = LT ? LT : a.L;
     const int OFF_WRS = 2 * L * WFG_L, OFF_W1 = OFF_WRS + 2 * L * WRS_L, OFF_ONES = OFF_W1 + W1_B,
               OFF_X = (OFF_ONES + ONES_B + 1023) & ~1023;
-    const int OFF_BAR = OFF_X + NSLOT * X_SLOT;
+    const int OFF_STASH = OFF_X + NSLOT * X_SLOT;
+    const int OFF_BAR = OFF_STASH + NSLOT * STASH_SLOT;
     const uint32_t sbase = smem_u32(smem);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // warp index through a broadcast shuffle: the compiler then knows that everything derived from it (slot, TMEM and
+    // shared-memory addresses, MMA descriptors) is warp-uniform and keeps it in uniform registers, which is what the
+    // single-lane tcgen05.mma issue wants (no per-MMA vector -> uniform moves)
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     const int slot = warp >> 2, q = warp & 3;
     const int r = q * 32 + lane;                                  // row of the tile = TMEM lane
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * NSLOT);
@@ -103,7 +135,7 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
         uint4* on = reinterpret_cast<uint4*>(smem + OFF_ONES);
         for (int i = threadIdx.x; i < ONES_B / 16; i += TT_THREADS) on[i] = make_uint4(i < 128 ? 0x3C00u : 0u, 0, 0, 0);   // half(1.0) at k = 0
         uint4* zx = reinterpret_cast<uint4*>(smem + OFF_X);
-        for (int i = threadIdx.x; i < NSLOT * X_SLOT / 16; i += TT_THREADS) zx[i] = make_uint4(0, 0, 0, 0);
+        for (int i = threadIdx.x; i < NSLOT * (X_SLOT + STASH_SLOT) / 16; i += TT_THREADS) zx[i] = make_uint4(0, 0, 0, 0);
         if (threadIdx.x == 0) {
             for (int i = 0; i < NSLOT; i++) mbar_init(sbase + OFF_BAR + 8 * i, 1);
             mbar_fence_init();
@@ -114,7 +146,7 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem = *tmem_slot;
+    const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);
     const uint32_t tcol = tmem + TCOLS * slot;                    // the slot's columns (lane field 0: MMA operands)
     const uint32_t tlane = tcol + ((uint32_t)(q * 32) << 16);     // this warp's lane quadrant (tcgen05.ld / st)
     const uint32_t mbar = sbase + OFF_BAR + 8 * slot;
@@ -126,28 +158,61 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
     const uint64_t dX = make_sdesc(xs + PADR * 16, X_CH, 128);
     const uint64_t dWfg = make_sdesc(sbase, 32 * 16, 128), dWrs = make_sdesc(sbase + OFF_WRS, 48 * 16, 128),
                    dW1 = make_sdesc(sbase + OFF_W1, 32 * 16, 128), dOnes = make_sdesc(sbase + OFF_ONES, 128 * 16, 128);
-    const int valid = 128 - a.halo;
+    const int valid = a.stash ? 128 : 128 - a.halo;
+    // stash mode: rows 128 - SR .. 127 exchange their operand row with the stash of (branch, block): the row kept from the
+    // previous tile goes in front of the tile (rows -SR .. -1 of the operand buffer), the new one is kept for the next tile
+    const bool tail = a.stash && r >= 128 - SR;
+    const uint32_t stash0 = sbase + OFF_STASH + slot * STASH_SLOT + (r - (128 - SR)) * 16;
+    const uint32_t xpre = xs + (PADR - SR + (r - (128 - SR))) * 16;
+    auto put_operand = [&](int bi, const uint32_t (&pk)[8]) {
+        st_shared_v4(xrow, pk[0], pk[1], pk[2], pk[3]);
+        st_shared_v4(xrow + X_CH, pk[4], pk[5], pk[6], pk[7]);
+        if (tail) {
+            const uint32_t sa = stash0 + bi * (2 * SR * 16);
+            const uint4 o0 = ld_shared_v4(sa), o1 = ld_shared_v4(sa + SR * 16);
+            st_shared_v4(xpre, o0.x, o0.y, o0.z, o0.w);
+            st_shared_v4(xpre + X_CH, o1.x, o1.y, o1.z, o1.w);
+            st_shared_v4(sa, pk[0], pk[1], pk[2], pk[3]);
+            st_shared_v4(sa + SR * 16, pk[4], pk[5], pk[6], pk[7]);
+        }
+    };
 
     // the leader's elected lane issues `f` (the slot's MMAs) and commits; everybody waits for the completion
+#ifdef GWI_TT_TRACE
+    int tt_k = 0;
+#endif
     auto mma_round = [&](auto&& f) {
+        TT_TRACE(1);
         named_bar(1 + slot, 128);
+        TT_TRACE(2);
         if (leader) {
             if (elect_one()) {
+                TT_TRACE(11);
                 tc_fence_after();
+                TT_TRACE(12);
                 f();
+                TT_TRACE(13);
                 tc_commit(mbar);
+                TT_TRACE(14);
             }
             __syncwarp();
         }
-        mbar_wait_sleep(mbar, ph, 4000);
+        TT_TRACE(3);
+        mbar_wait_sleep(mbar, ph, GWI_TT_SLEEP_NS);
         ph ^= 1;
         tc_fence_after();
+        TT_TRACE(4);
     };
 
-    for (int tile = blockIdx.x * NSLOT + slot; tile < a.ntiles; tile += gridDim.x * NSLOT) {
-        const int64_t tl = (int64_t)tile * valid - a.halo + r;    // chunk-local time of this thread's row
+    // halo mode: tiles blockIdx * NSLOT + slot, + gridDim * NSLOT, ...; stash mode: the slot's span [k0, k1) of the tiles,
+    // preceded by the warm-up tile k0 - 1
+    const int64_t gs = (int64_t)blockIdx.x * NSLOT + slot, ns = (int64_t)gridDim.x * NSLOT;
+    const int k0 = a.stash ? (int)(gs * a.ntiles / ns) : (int)gs, k1 = a.stash ? (int)((gs + 1) * a.ntiles / ns) : a.ntiles;
+    const int kstep = a.stash ? 1 : (int)ns;
+    for (int tile = (a.stash && k0 < k1) ? k0 - 1 : k0; tile < k1; tile += kstep) {
+        const int64_t tl = (int64_t)tile * valid - (a.stash ? 0 : a.halo) + r;    // chunk-local time of this thread's row
         const bool dead = a.t0 + tl < 0;                          // before the stream start: zero at every layer input (A4)
-        const bool store = r >= a.halo && tl < a.n;
+        const bool store = (a.stash ? tile >= k0 : r >= a.halo) && tl >= 0 && tl < a.n;
         uint32_t uH[16];                                          // u of branch 0 (fp16 pairs), parked while branch 1 runs
 #pragma unroll 1
         for (int b = 0; b < 2; b++) {
@@ -156,7 +221,7 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
                 float x = 0.f;
                 if (tl >= 0) {
                     if (tl < a.n) x = __half2float(a.x[(int64_t)b * a.ldx + tl]);
-                } else {
+                } else if (tl >= -a.halo) {
                     x = __half2float(a.xh[b * a.halo + a.halo + tl]);
                 }
                 uint32_t hv[16], pk[8];
@@ -170,14 +235,13 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
                 for (int c = 0; c < 16; c++) sv[c] = 0u;
                 tmem_st16(tlane + 48, sv);                        // skip sum starts at 0; the bs_i arrive with GEMM2's bias step
                 tmem_st16(tlane + 64, sv);
-                st_shared_v4(xrow, pk[0], pk[1], pk[2], pk[3]);
-                st_shared_v4(xrow + X_CH, pk[4], pk[5], pk[6], pk[7]);
+                put_operand(b * TT_MAX_L, pk);
                 tc_wait_st();
                 fence_proxy_async_smem();
                 tc_fence_before();
             }
-#pragma unroll 1
-            for (int i = 0; i < L; i++) {
+#pragma unroll
+            for (int i = 0; i < (LT ? LT : L); i++) {
                 const int d = a.dil[i];
                 // ---- GEMM1: f | g/2 = [h(t-d) | h(t)] . Wfg^T                                  (C.1 step 2)
                 mma_round([&] {
@@ -192,15 +256,23 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
                     tmem_ld16(tlane, f);
                     tmem_ld16(tlane + 16, g);
                     tc_wait_ld();
+                    TT_TRACE(5);
 #pragma unroll
                     for (int c = 0; c < 8; c++) {
+#ifdef GWI_TT_NOMUFU   // diagnostic only: the chain without the MUFU work
+                        const float t0 = __uint_as_float(f[2 * c]) * 0.5f, t1 = __uint_as_float(f[2 * c + 1]) * 0.5f;
+                        const float s0 = __uint_as_float(g[2 * c]) * 0.5f, s1 = __uint_as_float(g[2 * c + 1]) * 0.5f;
+#else
                         const float t0 = tanh_approx(__uint_as_float(f[2 * c])), t1 = tanh_approx(__uint_as_float(f[2 * c + 1]));
                         const float s0 = tanh_approx(__uint_as_float(g[2 * c])), s1 = tanh_approx(__uint_as_float(g[2 * c + 1]));
+#endif
                         z[c] = pack_half2(fmaf(t0, s0, t0), fmaf(t1, s1, t1));
                     }
+                    TT_TRACE(6);
                     tmem_st8(tlane + 16, z);
                     tc_wait_st();
                     tc_fence_before();
+                    TT_TRACE(7);
                 }
                 // ---- GEMM2: [h | skip] += z' . [Wr/2 | Ws/2]^T  (the last block's residual conv is dead, reading A8: its
                 // contribution lands in h columns nobody reads again)
@@ -215,11 +287,13 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
                     tmem_ld16(tlane + 32, hv);
                     tc_wait_ld();
 #pragma unroll
+                    TT_TRACE(8);
                     for (int c = 0; c < 8; c++) pk[c] = dead ? 0u : pack_half2(__uint_as_float(hv[2 * c]), __uint_as_float(hv[2 * c + 1]));
-                    st_shared_v4(xrow, pk[0], pk[1], pk[2], pk[3]);
-                    st_shared_v4(xrow + X_CH, pk[4], pk[5], pk[6], pk[7]);
+                    put_operand(b * TT_MAX_L + i + 1, pk);
+                    TT_TRACE(9);
                     fence_proxy_async_smem();
                     tc_fence_before();
+                    TT_TRACE(10);
                 }
             }
             // ---- u_b = ReLU(skip sum)                                                         (C.1 step 3)
@@ -287,7 +361,7 @@ inline uint16_t h16(float v)
 struct GwiTinyTcPack {
     uint8_t* d_w = nullptr;
     size_t w_bytes = 0;
-    int smem = 0, num_sms = 148, halo = 16;
+    int smem = 0, num_sms = 148, halo = 16, stash = 0;
     float lift[2][32], head[33];
 };
 
@@ -314,6 +388,9 @@ gwi_status gwi_tiny_tc_pack(gwi_model* m)
     for (int i = 0; i < L; i++) sum += a.dil[i];
     p->halo = ((sum + 15) / 16) * 16;
     if (p->halo < 16) p->halo = 16;
+    p->stash = 1;
+    for (int i = 0; i < L; i++)
+        if (a.dil[i] > SR) p->stash = 0;
     const float* W = m->host_blob.data();
     const size_t off_wrs = (size_t)2 * L * WFG_L, off_w1 = off_wrs + (size_t)2 * L * WRS_L;
     p->w_bytes = off_w1 + W1_B;
@@ -352,11 +429,12 @@ gwi_status gwi_tiny_tc_pack(gwi_model* m)
     p->head[32] = W[m->off.b2];
     GWI_CUDA_CHECK(cudaMalloc((void**)&p->d_w, p->w_bytes));
     GWI_CUDA_CHECK(cudaMemcpy(p->d_w, w.data(), p->w_bytes, cudaMemcpyHostToDevice));
-    p->smem = (int)(((off_w1 + W1_B + ONES_B + 1023) & ~(size_t)1023) + NSLOT * X_SLOT + 8 * NSLOT + 16);
+    p->smem = (int)(((off_w1 + W1_B + ONES_B + 1023) & ~(size_t)1023) + NSLOT * (X_SLOT + STASH_SLOT) + 8 * NSLOT + 16);
     cudaDeviceProp prop;
     GWI_CUDA_CHECK(cudaGetDeviceProperties(&prop, m->device));
     p->num_sms = prop.multiProcessorCount;
-    GWI_CUDA_CHECK(cudaFuncSetAttribute(k_tiny_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem));
+    GWI_CUDA_CHECK(cudaFuncSetAttribute(k_tiny_tc<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem));
+    GWI_CUDA_CHECK(cudaFuncSetAttribute(k_tiny_tc<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem));
     return GWI_OK;
 }
 
@@ -378,15 +456,28 @@ gwi_status gwi_tiny_tc_stream(const gwi_model* m, const __half* d_x, int64_t ldx
     const GwiTinyTcPack* p = m->tinytc;
     TtArgs a;
     a.w = p->d_w, a.x = d_x, a.xh = xh_cur, a.ldx = ldx, a.t0 = t0, a.n = n, a.L = m->arch.L, a.halo = p->halo;
-    const int valid = 128 - p->halo;
+    a.stash = p->stash;
+    const int valid = a.stash ? 128 : 128 - p->halo;
     a.ntiles = (n + valid - 1) / valid;
     for (int i = 0; i < TT_MAX_L; i++) a.dil[i] = i < m->arch.L ? m->arch.dil[i] : 0;
     a.prob = d_prob, a.u16 = d_prob ? nullptr : d_u16, a.lds = lds;
     memcpy(a.lift, p->lift, sizeof(a.lift)), memcpy(a.head, p->head, sizeof(a.head));
     const int slots = (a.ntiles + NSLOT - 1) / NSLOT;
     const int grid = slots < p->num_sms ? slots : p->num_sms;
-    k_tiny_tc<<<grid, TT_THREADS, p->smem, st>>>(a);
+    if (a.L == 4) k_tiny_tc<4><<<grid, TT_THREADS, p->smem, st>>>(a);
+    else k_tiny_tc<0><<<grid, TT_THREADS, p->smem, st>>>(a);
     gwi_count_launch(1);
     GWI_CUDA_CHECK(cudaGetLastError());
+#ifdef GWI_TT_TRACE
+    if (const char* tp = getenv("GWI_TT_TRACE_FILE")) {
+        cudaStreamSynchronize(st);
+        std::vector<unsigned long long> ev(8192);
+        cudaMemcpyFromSymbol(ev.data(), g_tt_trace, ev.size() * 8);
+        if (FILE* f = fopen(tp, "w")) {
+            for (auto e : ev) fprintf(f, "%llu %llu\n", e >> 48, e & 0xffffffffffffull);
+            fclose(f);
+        }
+    }
+#endif
     return GWI_OK;
 }
