@@ -104,6 +104,12 @@ __device__ unsigned long long g_tt_trace[8192];
 #define TT_TRACE(code)
 #endif
 
+#ifndef GWI_TT_ARRIVE
+#define GWI_TT_ARRIVE 1
+#endif
+#ifndef GWI_TT_SPIN
+#define GWI_TT_SPIN 0
+#endif
 #ifndef GWI_TT_SLEEP_NS
 #define GWI_TT_SLEEP_NS 4000
 #endif
@@ -183,7 +189,12 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
 #endif
     auto mma_round = [&](auto&& f) {
         TT_TRACE(1);
+#if GWI_TT_ARRIVE
+        if (leader) named_bar(1 + slot, 128);
+        else asm volatile("bar.arrive %0, %1;" ::"r"(1 + slot), "r"(128) : "memory");
+#else
         named_bar(1 + slot, 128);
+#endif
         TT_TRACE(2);
         if (leader) {
             if (elect_one()) {
@@ -198,7 +209,15 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
             __syncwarp();
         }
         TT_TRACE(3);
+#if GWI_TT_SPIN
+        {
+            uint32_t spins = 0;
+            while (!mbar_test(mbar, ph))
+                if (++spins > (1u << 26)) __trap();
+        }
+#else
         mbar_wait_sleep(mbar, ph, GWI_TT_SLEEP_NS);
+#endif
         ph ^= 1;
         tc_fence_after();
         TT_TRACE(4);
