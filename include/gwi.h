@@ -53,6 +53,8 @@ typedef enum { GWI_FP32 = 0, GWI_FP16 = 1 } gwi_precision;
  * estimate.  model_mask bit j: model j alone exceeded the threshold somewhere in the run.
  * Exactly compared with the oracle: slide, start, end.  peak_p / mean_p are fp32 statistics of the mean
  * probability over the run. */
+#define GWI_EDGE_LEFT (1 << 30)  /* time-shard mode only: the run starts at the shard's first sample */
+#define GWI_EDGE_RIGHT (1 << 29) /* time-shard mode only: the run ends at the shard's last sample    */
 typedef struct {
     int32_t slide;
     int32_t model_mask;
@@ -166,6 +168,21 @@ gwi_status gwi_stream_push_host(gwi_stream* s, const void* h_h1, const void* h_l
 gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, int32_t capacity, int32_t* h_count,
                              void* cuda_stream);
 int64_t gwi_stream_samples_done(const gwi_stream* s);
+/* ---- time shards (one rank per GPU, the data sharded across ranks) -------------------------
+ * A rank that owns the global samples [t_first, t_first + n) of a longer stream creates its handle with
+ * n_total = warmup + n and pushes the `warmup` samples that precede its span (R_f - 1 of them make every kept output
+ * exact, pin P8; 0 for the rank that owns t = 0) followed by its own samples.  gwi_stream_set_shard (before the first
+ * push and before gwi_stream_prime) makes the handle
+ *   - discard the outputs of the first `warmup` pushed samples (d_pbar, if given, is then [1 + n_lags][n_total - warmup]),
+ *   - report global sample indices (t_first = index of the first kept sample),
+ *   - emit a run that touches the shard's first or last sample whatever its length, flagged GWI_EDGE_LEFT / GWI_EDGE_RIGHT
+ *     in model_mask: it may continue in the neighbouring shard; the caller joins such runs across ranks and applies
+ *     min_len to the joined run (paper_2201_11133_b200/shard.py: merge_edge_records).
+ * Time slides: the caller primes the handle with the L1 samples that precede its first PUSHED sample in the GLOBAL stream
+ * (circularly), i.e. the global samples [t_first - warmup - tail, t_first - warmup) mod the global length, so that
+ * every slide sees L1[(t - lag) mod N_global].  No collective is involved; the only exchange is the record gather.
+ * Errors: GWI_ERR_ARG (after the first push, warmup < 0 or >= n_total). */
+gwi_status gwi_stream_set_shard(gwi_stream* s, int64_t t_first, int64_t warmup);
 /* which back end gwi_stream_create chose (parity tests assert that the kernel they mean to check is the one that ran) */
 typedef enum { GWI_BACKEND_GENERIC = 0, GWI_BACKEND_NARROW = 1, GWI_BACKEND_TENSOR = 2, GWI_BACKEND_TENSOR_SLIDES = 3 } gwi_backend;
 int gwi_stream_backend(const gwi_stream* s);

@@ -13,7 +13,7 @@ EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_m
                     "gwi_infer_workspace_bytes", "gwi_infer", "gwi_carry_bytes", "gwi_triggers_workspace_bytes",
                     "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
                     "gwi_stream_tail_samples", "gwi_stream_prime", "gwi_stream_push", "gwi_stream_push_host",
-                    "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_backend", "gwi_stream_destroy", "gwi_stream_set_rule",
+                    "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_backend", "gwi_stream_set_shard", "gwi_stream_destroy", "gwi_stream_set_rule",
                     "gwi_coincidence", "gwi_sweep_workspace_bytes", "gwi_threshold_sweep", "gwi_whiten_workspace_bytes",
                     "gwi_whiten"]
 
@@ -78,6 +78,8 @@ def lib():
     L.gwi_stream_finish.argtypes = [vp, vp, C.c_int32, i32p, vp]
     L.gwi_stream_samples_done.restype = C.c_int64
     L.gwi_stream_samples_done.argtypes = [vp]
+    L.gwi_stream_set_shard.restype = C.c_int
+    L.gwi_stream_set_shard.argtypes = [vp, C.c_int64, C.c_int64]
     L.gwi_stream_backend.restype = C.c_int
     L.gwi_stream_backend.argtypes = [vp]
     L.gwi_stream_destroy.restype = None
@@ -241,6 +243,7 @@ def new_carry(device=0):
 
 
 RULE_MEAN, RULE_PER_MODEL = 0, 1
+EDGE_LEFT, EDGE_RIGHT = 1 << 30, 1 << 29
 BACKEND_GENERIC, BACKEND_NARROW, BACKEND_TENSOR, BACKEND_TENSOR_SLIDES = 0, 1, 2, 3
 
 
@@ -265,12 +268,15 @@ class Stream:
     tensor in .pbar) for parity tests."""
 
     def __init__(self, models, n_total, max_chunk, threshold=0.5, min_len=2048, lags=(), capacity=4096, want_pbar=False,
-                 rule=RULE_MEAN):
+                 rule=RULE_MEAN, shard=None):
+        """shard = (t_first, warmup): time-shard mode (gwi_stream_set_shard); n_total then counts the warm-up samples too
+        and .pbar covers the kept samples only."""
         self.models = list(models)
         self.device = torch.device("cuda", self.models[0].device)
         self.dtype = torch.float16 if self.models[0].precision == FP16 else torch.float32
         self.capacity = int(capacity)
-        shape = (1 + len(lags), int(n_total)) if rule == RULE_MEAN else (1 + len(lags), len(self.models), int(n_total))
+        n_kept = int(n_total) - (int(shard[1]) if shard else 0)
+        shape = (1 + len(lags), n_kept) if rule == RULE_MEAN else (1 + len(lags), len(self.models), n_kept)
         self.pbar = torch.zeros(shape, dtype=torch.float32, device=self.device) if want_pbar else None
         mp = (C.c_void_p * len(self.models))(*[m._h for m in self.models])
         lg = (C.c_int64 * max(len(lags), 1))(*[int(v) for v in lags])
@@ -280,6 +286,8 @@ class Stream:
                                        C.c_void_p(self.pbar.data_ptr()) if want_pbar else None, C.byref(self._h)))
         if rule != RULE_MEAN:
             _check(lib().gwi_stream_set_rule(self._h, int(rule)))
+        if shard is not None:
+            _check(lib().gwi_stream_set_shard(self._h, int(shard[0]), int(shard[1])))
 
     @property
     def tail_samples(self):

@@ -96,7 +96,7 @@ gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, 
 gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0, float threshold,
                         int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry, gwi_trigger* d_triggers,
                         int32_t capacity, int32_t* d_count, int append, float* d_pbar, void* d_workspace,
-                        size_t workspace_bytes, cudaStream_t st);
+                        size_t workspace_bytes, cudaStream_t st, int64_t shard_begin = -1, int64_t shard_end = -1);
 
 // ---- tcgen05 path (gwi_tc.cu) -------------------------------------------------------------------------------
 bool gwi_tc_supported(const GwiArch& a);

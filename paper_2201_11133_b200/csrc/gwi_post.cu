@@ -117,8 +117,12 @@ __device__ int64_t find_end(const uint32_t* __restrict__ bits, const uint8_t* __
     return N;
 }
 
+// shard_begin / shard_end (time-shard mode of the stream driver; -1 = off): global index of the shard's
+// first sample / one past its last.  A run that touches either is emitted whatever its length (it may continue in the
+// neighbouring shard; the host merges and applies L_min afterwards) and is flagged in model_mask by k_stats.
 __global__ void k_head_run(const uint32_t* __restrict__ bits, const uint8_t* __restrict__ flags, int64_t NW, int64_t N,
-                           int64_t t0, int64_t Lmin, int last_chunk, const Carry* __restrict__ carry, Header* hd)
+                           int64_t t0, int64_t Lmin, int last_chunk, const Carry* __restrict__ carry, Header* hd,
+                           int64_t shard_begin, int64_t shard_end)
 {
     if (threadIdx.x != 0) return;
     Carry c;
@@ -131,7 +135,7 @@ __global__ void k_head_run(const uint32_t* __restrict__ bits, const uint8_t* __r
         if (e0 < N || last_chunk) {
             hd->head_closed = 1;
             hd->head_end = e0;
-            hd->head_emit = (t0 + e0 - c.start >= Lmin) ? 1 : 0;
+            hd->head_emit = (t0 + e0 - c.start >= Lmin || c.start == shard_begin || t0 + e0 == shard_end) ? 1 : 0;
         } else {
             hd->out_open = 1;
             hd->out_start = c.start;
@@ -143,7 +147,8 @@ __global__ void k_head_run(const uint32_t* __restrict__ bits, const uint8_t* __r
 template <int MODE>
 __global__ void k_runs(const uint32_t* __restrict__ bits, const uint8_t* __restrict__ flags, int64_t NW, int64_t N,
                        int64_t t0, int64_t Lmin, int last_chunk, int slide, Header* hd, uint32_t* __restrict__ blkcnt,
-                       const uint32_t* __restrict__ blkoff, gwi_trigger* __restrict__ out, int capacity)
+                       const uint32_t* __restrict__ blkoff, gwi_trigger* __restrict__ out, int capacity,
+                       int64_t shard_begin, int64_t shard_end)
 {
     __shared__ uint32_t wsum[RT / 32];
     const int64_t i = (int64_t)blockIdx.x * RT + threadIdx.x;
@@ -160,7 +165,7 @@ __global__ void k_runs(const uint32_t* __restrict__ bits, const uint8_t* __restr
             int64_t g = i * 32 + s;
             int64_t e = find_end(bits, flags, NW, N, g);
             if (e < N || last_chunk) {
-                if (e - g >= Lmin) {
+                if (e - g >= Lmin || t0 + g == shard_begin || t0 + e == shard_end) {
                     if (MODE == 1) rs[cnt] = g, re[cnt] = e;
                     cnt++;
                 }
@@ -277,7 +282,7 @@ __device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t 
 }
 
 __global__ void k_stats(Ptrs P, int M, float theta, int64_t N, int64_t t0, const Header* __restrict__ hd,
-                        gwi_trigger* __restrict__ out, int capacity, Carry* carry)
+                        gwi_trigger* __restrict__ out, int capacity, Carry* carry, int64_t shard_begin, int64_t shard_end)
 {
     const int nrec = min(hd->total, capacity);
     if ((int)blockIdx.x == (int)gridDim.x - 1) {   // last CTA: write the outgoing carry
@@ -304,7 +309,7 @@ __global__ void k_stats(Ptrs P, int M, float theta, int64_t N, int64_t t0, const
         if (threadIdx.x == 0) {
             out[r].peak_p = pk;
             out[r].mean_p = (float)(sm / (double)(e - s));
-            out[r].model_mask = mk;
+            out[r].model_mask = mk | (s == shard_begin ? GWI_EDGE_LEFT : 0) | (e == shard_end ? GWI_EDGE_RIGHT : 0);
         }
     }
 }
@@ -341,14 +346,14 @@ extern "C" gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t 
                                             float* d_pbar, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
 {
     return gwi_post_run(d_prob, n_models, N, t0, threshold, min_len, slide_id, last_chunk, d_carry, d_triggers, capacity,
-                        d_count, 0, d_pbar, d_workspace, workspace_bytes, (cudaStream_t)cuda_stream);
+                        d_count, 0, d_pbar, d_workspace, workspace_bytes, (cudaStream_t)cuda_stream, -1, -1);
 }
 
 // append != 0: *d_count holds the number of records already in d_triggers; the new ones go behind them.
 gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0, float threshold,
                         int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry, gwi_trigger* d_triggers,
                         int32_t capacity, int32_t* d_count, int append, float* d_pbar, void* d_workspace,
-                        size_t workspace_bytes, cudaStream_t st)
+                        size_t workspace_bytes, cudaStream_t st, int64_t shard_begin, int64_t shard_end)
 {
     if (!d_prob || n_models < 1 || n_models > GWI_MAX_MODELS || N < 1 || capacity < 0 || !d_count || !d_workspace ||
         (capacity > 0 && !d_triggers) || ((uintptr_t)d_workspace & 255)) {
@@ -392,14 +397,14 @@ gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N,
     if (vec) k_mask<true><<<grid, 256, 0, st>>>(P, n_models, N, threshold, bits, L.NW, d_pbar);
     else k_mask<false><<<grid, 256, 0, st>>>(P, n_models, N, threshold, bits, L.NW, d_pbar);
     k_blkflags<<<(unsigned)L.NB, WB, 0, st>>>(bits, L.NW, flags);
-    k_head_run<<<1, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd);
+    k_head_run<<<1, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd, shard_begin, shard_end);
     k_runs<0><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
-                                             d_triggers, capacity);
+                                             d_triggers, capacity, shard_begin, shard_end);
     k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append);
     k_runs<1><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
-                                             d_triggers, capacity);
+                                             d_triggers, capacity, shard_begin, shard_end);
     int sgrid = capacity < 1024 ? capacity + 1 : 1025;
-    k_stats<<<sgrid, 256, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry);
+    k_stats<<<sgrid, 256, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry, shard_begin, shard_end);
     gwi_count_launch(7);
     GWI_CUDA_CHECK(cudaGetLastError());
     return GWI_OK;

@@ -59,6 +59,10 @@ struct gwi_stream {
     std::vector<__half*> d_u16;             // time slides: per model [2][lds][32] fp16 branch features, time-major
     int64_t* d_lags = nullptr;              // device copy of the lag list
     int rule = 0;                           // GWI_RULE_MEAN / GWI_RULE_PER_MODEL
+    // time-shard mode (gwi_stream_set_shard): the first `warm` pushed samples are warm-up, the first kept sample has the
+    // global index t_first
+    bool shard = false;
+    int64_t warm = 0, t_first = 0;
     void* d_carry_pm = nullptr;             // per-model rule: [n_slides][M] carry blocks
     // tensor-core back end (paper-scale models, FP16 mode, zero lag only)
     bool tcb = false;
@@ -226,16 +230,25 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
 gwi_status post_block(gwi_stream* s, int n, bool last, cudaStream_t st)
 {
     const int nslides = (int)s->lags.size();
+    // time-shard mode: warm-up samples produce no output; times are global
+    const int64_t skip = s->t_done < s->warm ? std::min<int64_t>(n, s->warm - s->t_done) : 0;
+    if (skip == n) {
+        s->t_done += n;
+        return GWI_OK;
+    }
+    const int64_t nn = n - skip, kept = s->t_done + skip - s->warm;   // kept = index of the block's first kept sample
+    const int64_t t0 = s->t_first + kept, Nk = s->N_total - s->warm;
+    const int64_t sb = s->shard ? s->t_first : -1, se = s->shard ? s->t_first + Nk : -1;
     if (s->rule == GWI_RULE_PER_MODEL) {
         // the paper's rule: every model thresholded and clustered on its own; slide k and model m are
         // packed into the record's slide field (k | m << 20) and unpacked at finish
         for (int k = 0; k < nslides; k++)
             for (int m = 0; m < s->M; m++) {
-                const float* ptr1[1] = {s->d_prob + ((size_t)k * s->M + m) * s->sub};
-                float* pb = s->d_pbar ? s->d_pbar + ((size_t)k * s->M + m) * s->N_total + s->t_done : nullptr;
-                gwi_status rc = gwi_post_run(ptr1, 1, n, s->t_done, s->theta, s->min_len, k | (m << 20), last ? 1 : 0,
+                const float* ptr1[1] = {s->d_prob + ((size_t)k * s->M + m) * s->sub + skip};
+                float* pb = s->d_pbar ? s->d_pbar + ((size_t)k * s->M + m) * Nk + kept : nullptr;
+                gwi_status rc = gwi_post_run(ptr1, 1, nn, t0, s->theta, s->min_len, k | (m << 20), last ? 1 : 0,
                                              (char*)s->d_carry_pm + ((size_t)k * s->M + m) * gwi_carry_bytes(), s->d_trig, s->cap,
-                                             s->d_count, 1, pb, s->d_post_ws, s->post_ws_bytes, st);
+                                             s->d_count, 1, pb, s->d_post_ws, s->post_ws_bytes, st, sb, se);
                 if (rc != GWI_OK) return rc;
             }
         s->t_done += n;
@@ -243,11 +256,11 @@ gwi_status post_block(gwi_stream* s, int n, bool last, cudaStream_t st)
     }
     for (int k = 0; k < nslides; k++) {
         const float* ptrs[GWI_MAX_MODELS];
-        for (int m = 0; m < s->M; m++) ptrs[m] = s->d_prob + ((size_t)k * s->M + m) * s->sub;
-        float* pb = s->d_pbar ? s->d_pbar + (size_t)k * s->N_total + s->t_done : nullptr;
-        gwi_status rc = gwi_post_run(ptrs, s->M, n, s->t_done, s->theta, s->min_len, k, last ? 1 : 0,
+        for (int m = 0; m < s->M; m++) ptrs[m] = s->d_prob + ((size_t)k * s->M + m) * s->sub + skip;
+        float* pb = s->d_pbar ? s->d_pbar + (size_t)k * Nk + kept : nullptr;
+        gwi_status rc = gwi_post_run(ptrs, s->M, nn, t0, s->theta, s->min_len, k, last ? 1 : 0,
                                      (char*)s->d_carry + (size_t)k * gwi_carry_bytes(), s->d_trig, s->cap, s->d_count, 1, pb,
-                                     s->d_post_ws, s->post_ws_bytes, st);
+                                     s->d_post_ws, s->post_ws_bytes, st, sb, se);
         if (rc != GWI_OK) return rc;
     }
     s->t_done += n;
@@ -764,7 +777,7 @@ extern "C" gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, 
     }
     if (s->rule == GWI_RULE_PER_MODEL)
         for (auto& r : recs) {
-            r.model_mask = 1 << (r.slide >> 20);
+            r.model_mask = (1 << (r.slide >> 20)) | (r.model_mask & (GWI_EDGE_LEFT | GWI_EDGE_RIGHT));
             r.slide &= (1 << 20) - 1;
         }
     // records arrive grouped by sub-chunk; the list is sorted by (slide, start)
@@ -783,6 +796,16 @@ extern "C" gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, 
 }
 
 extern "C" int64_t gwi_stream_samples_done(const gwi_stream* s) { return s ? s->t_done : -1; }
+
+extern "C" gwi_status gwi_stream_set_shard(gwi_stream* s, int64_t t_first, int64_t warmup)
+{
+    if (!s || warmup < 0 || warmup >= s->N_total || t_first < 0 || s->t_done != 0 || s->t_recv != 0 || s->primed) {
+        gwi_set_error("gwi_stream_set_shard: bad argument (before the first push and before gwi_stream_prime; 0 <= warmup < n_total)");
+        return GWI_ERR_ARG;
+    }
+    s->shard = true, s->warm = warmup, s->t_first = t_first;
+    return GWI_OK;
+}
 
 extern "C" int gwi_stream_backend(const gwi_stream* s)
 {

@@ -75,3 +75,41 @@ def gather_objects(obj, dist=None):
     out = [None] * dist.get_world_size()
     dist.all_gather_object(out, obj)
     return out
+
+
+# ---- time shards through gwi_stream_* (include/gwi.h: gwi_stream_set_shard) --------------------------------------------
+EDGE_LEFT, EDGE_RIGHT = 1 << 30, 1 << 29      # model_mask flags of a record that touches its shard's first / last sample
+
+
+def shard_stream_args(n_global: int, start: int, end: int, receptive_field: int, max_lag: int = 0, align: int = 1):
+    """What rank r, owner of the global samples [start, end), hands to gwi_stream_*:
+    n_total (= warm-up + own samples), the shard tuple (t_first, warmup) of binding.Stream, the global index of its
+    first pushed sample, and the global indices (circular) of the L1 samples it primes the slides with.  The warm-up is
+    R_f - 1 samples rounded up to `align` (128 for the tensor-core slide back end), 0 for the owner of t = 0."""
+    warm = 0 if start == 0 else -(-(receptive_field - 1) // align) * align
+    warm = min(warm, start)
+    first_pushed = start - warm
+    n_total = end - first_pushed
+    n_tail = min(n_total, max_lag + receptive_field - 1) if max_lag > 0 else 0
+    tail_idx = [(first_pushed - n_tail + i) % n_global for i in range(n_tail)] if n_tail else []
+    return {"n_total": n_total, "shard": (start, warm), "first_pushed": first_pushed, "tail_indices": tail_idx}
+
+
+def merge_edge_records(records, min_len: int):
+    """records: (slide, start, end, peak_p, mean_p, model_mask) of ALL shards, any order, as the shard-mode streams report
+    them: runs >= min_len plus every run that touches a shard edge (flagged in model_mask).  A run flagged EDGE_RIGHT that
+    ends where a run of the same slide flagged EDGE_LEFT starts is one run of the whole stream (chains over several shards
+    join one after the other).  Returns the joined runs of length >= min_len sorted by (slide, start): the list the
+    unsharded stream gives.  peak = max, mean = length-weighted, mask = OR of the parts (flags cleared)."""
+    flags = EDGE_LEFT | EDGE_RIGHT
+    out = []
+    for slide, s, e, pk, mn, mask in sorted(records, key=lambda r: (r[0], r[1])):
+        if out and out[-1][0] == slide and out[-1][2] == s and (out[-1][5] & EDGE_RIGHT) and (mask & EDGE_LEFT):
+            p = out[-1]
+            ln0, ln1 = p[2] - p[1], e - s
+            p[2], p[3] = e, max(p[3], pk)
+            p[4] = (p[4] * ln0 + mn * ln1) / (ln0 + ln1)
+            p[5] = (p[5] & ~EDGE_RIGHT) | (mask & ~EDGE_LEFT)
+        else:
+            out.append([slide, s, e, pk, mn, mask])
+    return [(r[0], r[1], r[2], r[3], r[4], r[5] & ~flags) for r in out if r[2] - r[1] >= min_len]

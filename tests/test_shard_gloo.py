@@ -92,3 +92,22 @@ def test_world_size_2_gloo():
     assert got[0][1] == (0, 512) and got[1][1] == (512, 1024)
     assert got[0][2] == got[1][2] == 11.0
     assert got[0][3] == got[1][3] == [(9000, 11500)]
+
+
+def test_shard_stream_args_and_edge_merge():
+    a = shard.shard_stream_args(1000, 0, 400, receptive_field=16, max_lag=100)
+    assert a["shard"] == (0, 0) and a["n_total"] == 400 and a["tail_indices"][0] == 1000 - 115 and a["tail_indices"][-1] == 999
+    b = shard.shard_stream_args(1000, 400, 1000, receptive_field=16, max_lag=100)
+    assert b["shard"] == (400, 15) and b["first_pushed"] == 385 and b["n_total"] == 615
+    assert b["tail_indices"] == list(range(385 - 115, 385))
+    c = shard.shard_stream_args(128 * 100, 128 * 50, 128 * 100, receptive_field=2047, max_lag=4096, align=128)
+    assert c["shard"] == (6400, 2048) and c["n_total"] % 128 == 0
+    L, R = shard.EDGE_LEFT, shard.EDGE_RIGHT
+    recs = [(0, 390, 400, 0.9, 0.8, 1 | R), (0, 400, 450, 0.7, 0.6, 2 | L),          # joined: 60 samples
+            (0, 100, 130, 0.9, 0.9, 3),                                              # an inner run, long enough
+            (0, 0, 5, 0.9, 0.9, 1 | L),                                              # touches the stream start, too short
+            (1, 395, 400, 0.9, 0.9, 1 | R), (1, 400, 600, 0.8, 0.8, 1 | L | R), (1, 600, 610, 0.6, 0.6, 4 | L),   # three shards
+            (2, 390, 400, 0.9, 0.9, 1 | R), (2, 401, 450, 0.9, 0.9, 1)]              # not adjacent: not joined
+    got = shard.merge_edge_records(recs, 30)
+    assert [(r[0], r[1], r[2], r[5]) for r in got] == [(0, 100, 130, 3), (0, 390, 450, 3), (1, 395, 610, 5), (2, 401, 450, 1)]
+    assert abs(got[1][4] - (0.8 * 10 + 0.6 * 50) / 60) < 1e-12 and got[1][3] == 0.9
