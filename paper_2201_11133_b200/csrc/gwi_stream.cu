@@ -25,7 +25,9 @@ struct gwi_stream {
     std::vector<const gwi_model*> models;
     int M = 0, device = 0;
     bool half_in = false;
-    std::vector<int64_t> lags;     // lags[0] = 0 (zero lag), then the caller's lags in samples
+    std::vector<int64_t> lags;     // lags[0] = 0 (zero lag), then the lags in samples as the heads use them: the caller's
+                                   // lags mod n_total (circular slides, reading A24), the caller's own in shard mode
+    std::vector<int64_t> lags_in;  // the caller's lags (lags_in[0] = 0)
     int64_t maxlag = 0, N_total = 0, min_len = 0, t_done = 0;
     float theta = 0.5f;
     int cap = 0, sub = 0;          // record capacity; internal sub-chunk length (samples)
@@ -191,7 +193,10 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
             // per-lag heads follow below
             __half* xh_next = (m == 0) ? s->d_xh[s->xh_cur ^ 1] : nullptr;
             __half* u0 = nslides > 1 ? s->d_u16[m] + (size_t)s->maxlag * 32 : nullptr;
-            rc = gwi_tiny_stream(gm, (const __half*)x, s->xcap, n, s->t_done, s->d_xh[s->xh_cur], xh_next,
+            // global time of the chunk (rows before the stream start are zero at every layer input, reading A4); a time
+            // shard that does not own t = 0 has no such rows
+            rc = gwi_tiny_stream(gm, (const __half*)x, s->xcap, n, (s->shard && s->warm > 0 ? (int64_t)1 << 40 : 0) + s->t_done,
+                                 s->d_xh[s->xh_cur], xh_next,
                                  nslides == 1 ? s->d_prob + (size_t)m * s->sub : nullptr, u0, s->lds, st);
             if (rc != GWI_OK) return rc;
             if (nslides == 1) continue;
@@ -283,7 +288,7 @@ gwi_status run_chunk(gwi_stream* s, int xb, int64_t n, cudaStream_t st)
 gwi_status tcs_block(gwi_stream* s, int n, bool last, cudaStream_t st)
 {
     const int nslides = (int)s->lags.size();
-    const int B = (n + s->seg - 1) / s->seg, start = s->t_done == 0 ? 1 : 0;
+    const int B = (n + s->seg - 1) / s->seg, start = (s->t_done == 0 && !(s->shard && s->warm > 0)) ? 1 : 0;
     const int ntiles = s->segT / 128, seg_tiles = s->seg / 128, warm_tiles = s->segH / 128;
     const int64_t nq = (n + 127) / 128, total = (int64_t)B * s->segT;
     k_seg_gather<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(s->d_acc, s->acc_cap, s->d_xh[s->xh_cur], n, s->seg, s->segH, s->segT,
@@ -408,9 +413,10 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     s->models.assign(models, models + n_models);
     s->M = n_models, s->device = m0->device, s->half_in = (m0->prec == GWI_FP16);
     s->lags.push_back(0);
+    s->lags_in.push_back(0);
     for (int i = 0; i < n_lags; i++) {
-        if (lags[i] < 1 || lags[i] >= n_total) {
-            gwi_set_error("gwi_stream_create: lag %lld outside [1, n_total)", (long long)lags[i]);
+        if (lags[i] < 1) {
+            gwi_set_error("gwi_stream_create: lag %lld < 1", (long long)lags[i]);
             delete s;
             return GWI_ERR_ARG;
         }
@@ -419,7 +425,10 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
             delete s;
             return GWI_ERR_UNSUPPORTED;
         }
-        s->lags.push_back(lags[i]);
+        // the slides are circular over the stream: a lag >= n_total wraps (a multiple of n_total is the zero lag again).  The
+        // ring of L1 features is sized by the largest lag as given, which is what a time shard needs (gwi_stream_set_shard)
+        s->lags.push_back(lags[i] % n_total);
+        s->lags_in.push_back(lags[i]);
         s->maxlag = std::max(s->maxlag, lags[i]);
     }
     s->N_total = n_total, s->min_len = min_len, s->theta = threshold, s->cap = capacity, s->d_pbar = d_pbar;
@@ -450,7 +459,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
         s->halo = s->segH;
         s->Rt = (int)(s->maxlag / 128);
     }
-    s->xcap = std::max<int64_t>(std::min(max_chunk, n_total), std::min<int64_t>(n_total, s->maxlag + s->Rf - 1));
+    s->xcap = std::max<int64_t>(std::min(max_chunk, n_total), s->maxlag > 0 ? s->maxlag + s->Rf - 1 : 0);   // chunks and the primed tail
     // sub-chunk: bounds the activation workspace (2R floats per branch-sample) to ~2 GiB
     int64_t per = (int64_t)s->nb * 2 * s->R * 4;
     int64_t sub = std::max<int64_t>(4096, (2LL << 30) / per);
@@ -603,7 +612,9 @@ extern "C" void gwi_stream_destroy(gwi_stream* s)
 extern "C" int64_t gwi_stream_tail_samples(const gwi_stream* s)
 {
     if (!s || s->maxlag == 0) return 0;
-    return std::min<int64_t>(s->N_total, s->maxlag + s->Rf - 1);
+    // shard mode: the L1 samples that precede the first pushed sample in the global stream, as many as the largest lag
+    // reaches back; otherwise the stream's own tail (at most the whole stream)
+    return s->shard ? s->maxlag + s->Rf - 1 : std::min<int64_t>(s->N_total, s->maxlag + s->Rf - 1);
 }
 
 extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64_t n_tail, void* cuda_stream)
@@ -614,6 +625,11 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     GWI_CUDA_CHECK(cudaSetDevice(s->device));
+    if (s->tcs && s->shard && s->t_first - s->warm > 0 && n_tail > s->t_first - s->warm) {
+        gwi_set_error("gwi_stream_prime: a time shard whose L1 prefix wraps around the global stream start is not supported by the "
+                      "tensor-core slide back end (make the first shard longer than max lag + 2 R_f)");
+        return GWI_ERR_UNSUPPORTED;
+    }
     if (s->tcs) {
         // tail = L1[N - maxlag - (R_f - 1), N): the first R_f - 1 samples are the warm-up of the history tiles (the segment
         // warm-up is R_f - 1 rounded up to whole tiles, the front of it stays zero and is never looked at by an output)
@@ -639,6 +655,8 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
         }
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * H * 2, st));
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * H * 2, st));
+        if (s->shard && s->warm > 0 && n_tail >= H)   // time shard: the L1 warm-up of the first segment is the tail's end (see below)
+            GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_xh[0] + H, (const __half*)l1_tail + (n_tail - H), (size_t)H * 2, cudaMemcpyDefault, st));
         GWI_CUDA_CHECK(cudaGetLastError());
         s->xh_cur = 0, s->hist_t_cur = 0, s->pend = 0;
         s->primed = true;
@@ -651,6 +669,12 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
                                      n_tail * elt(s), n_tail * elt(s), (size_t)c_in * (s->nb - 1), cudaMemcpyDefault, st));
     // features of the tail: zero history is exact for the last maxlag samples because either the tail starts at t = 0
     // or it starts R_f - 1 samples before them
+    const bool keepL = s->shard && s->warm > 0;
+    int tiny_xc = 0;
+    // shard mode: the tail is the global samples [first_pushed - n_tail, first_pushed) taken circularly; position of the
+    // global t = 0 inside it (0: no wrap inside the tail)
+    const int64_t first_pushed = s->t_first - s->warm;
+    const int64_t wrap_at = (s->shard && n_tail > first_pushed && first_pushed > 0) ? n_tail - first_pushed : 0;
     for (int m = 0; m < s->M; m++) {
         if (!s->tiny)
             GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
@@ -659,15 +683,32 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
             GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * s->halo * 2, st));
         }
         int xc = 0;
-        for (int64_t o = 0; o < n_tail; o += s->sub) {
-            int nn = (int)std::min<int64_t>(s->sub, n_tail - o);
+        for (int64_t o = 0; o < n_tail;) {
+            // a shard's tail may wrap around the global stream (.. N-1, 0, 1 ..): the part from global t = 0 on starts
+            // from zero history again, as the stream itself does (reading A4), so that the features are the ones the
+            // unsharded pass has
+            const bool at_wrap = wrap_at > 0 && o == wrap_at;
+            if (at_wrap) {
+                if (s->tiny) {
+                    GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * s->halo * 2, st));
+                    GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * s->halo * 2, st));
+                } else {
+                    GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
+                }
+            }
+            const int64_t lim = (wrap_at > 0 && o < wrap_at) ? wrap_at : n_tail;
+            int nn = (int)std::min<int64_t>(s->sub, lim - o);
+            const int64_t tail_t0 = !s->shard ? s->N_total - n_tail + o : (wrap_at > 0 && o >= wrap_at) ? o - wrap_at : ((int64_t)1 << 40) + o;
             gwi_status rc;
             if (s->tiny) {
                 // both branches are evaluated; the H1 rows of the staging buffer hold nothing meaningful here and the
                 // H1 skip rows they produce are overwritten by the first real chunk
-                rc = gwi_tiny_stream(s->models[m], (const __half*)s->d_x[0] + o, s->xcap, nn, s->N_total - n_tail + o,
+                // global time of the tail's first sample: the stream's own tail, or (shard mode) samples somewhere inside
+                // the global stream -- never the stream start, so no row is masked as "before t = 0"
+                rc = gwi_tiny_stream(s->models[m], (const __half*)s->d_x[0] + o, s->xcap, nn, tail_t0,
                                      s->d_xh[xc], s->d_xh[xc ^ 1], nullptr, s->d_u16[m] + (size_t)s->maxlag * 32, s->lds, st);
                 xc ^= 1;
+                o += nn;
                 if (rc != GWI_OK) return rc;
                 __half* base16 = s->d_u16[m] + (size_t)s->lds * 32;
                 GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_tmp, base16 + (size_t)nn * 32, (size_t)s->maxlag * 64, cudaMemcpyDeviceToDevice, st));
@@ -687,16 +728,30 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
                                              cudaMemcpyDeviceToDevice, st));
             // history ping-pong inside the tail pass
             std::swap(s->d_hist[0][m], s->d_hist[1][m]);
+            o += nn;
         }
-        // the real pass starts from zero history again
-        if (s->tiny) continue;
+        // the real pass starts from zero history again -- except for the L1 branch of a time shard that does not start at
+        // t = 0: its tail ends where the first pushed sample begins, so the L1 state carries over and the L1 features of
+        // the warm-up samples, which the slides read max-lag later, are exact (the H1 branch starts from zero: its
+        // warm-up outputs are discarded)
+        if (s->tiny) {
+            tiny_xc = xc;
+            continue;
+        }
+        if (keepL) continue;
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[0][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_hist[1][m], 0, (size_t)std::max<int64_t>(1, gwi_generic_hist_floats(s->models[m])) * 4, st));
     }
     if (s->tiny) {
-        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * s->halo * 2, st));
-        GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * s->halo * 2, st));
-        s->xh_cur = 0;
+        if (keepL) {
+            // carried input samples: L1 = the tail's last `halo` samples, H1 = zero
+            GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[tiny_xc], 0, (size_t)s->halo * 2, st));
+            s->xh_cur = tiny_xc;
+        } else {
+            GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[0], 0, (size_t)2 * s->halo * 2, st));
+            GWI_CUDA_CHECK(cudaMemsetAsync(s->d_xh[1], 0, (size_t)2 * s->halo * 2, st));
+            s->xh_cur = 0;
+        }
     }
     s->hist_cur = 0;
     s->primed = true;
@@ -804,6 +859,11 @@ extern "C" gwi_status gwi_stream_set_shard(gwi_stream* s, int64_t t_first, int64
         return GWI_ERR_ARG;
     }
     s->shard = true, s->warm = warmup, s->t_first = t_first;
+    s->lags = s->lags_in;      // no wrap inside a shard: the primed L1 prefix is the global stream's
+    if (s->d_lags) {
+        GWI_CUDA_CHECK(cudaSetDevice(s->device));
+        GWI_CUDA_CHECK(cudaMemcpy(s->d_lags, s->lags.data(), s->lags.size() * 8, cudaMemcpyHostToDevice));
+    }
     return GWI_OK;
 }
 

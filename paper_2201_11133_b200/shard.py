@@ -90,7 +90,7 @@ def shard_stream_args(n_global: int, start: int, end: int, receptive_field: int,
     warm = min(warm, start)
     first_pushed = start - warm
     n_total = end - first_pushed
-    n_tail = min(n_total, max_lag + receptive_field - 1) if max_lag > 0 else 0
+    n_tail = max_lag + receptive_field - 1 if max_lag > 0 else 0     # gwi_stream_tail_samples() in shard mode
     tail_idx = [(first_pushed - n_tail + i) % n_global for i in range(n_tail)] if n_tail else []
     return {"n_total": n_total, "shard": (start, warm), "first_pushed": first_pushed, "tail_indices": tail_idx}
 

@@ -179,8 +179,8 @@ def test_stream_argument_errors(tmpdir_s):
         st.push(x, x)
     n, recs = st.finish()
     assert n == len(recs)
-    with pytest.raises(gwi.GwiError):
-        gwi.Stream(gms, 1000, 500, lags=[1000])
+    with pytest.raises(gwi.GwiError):      # a lag must be >= 1 (lags >= n_total wrap: test_stream_degenerate_sizes)
+        gwi.Stream(gms, 1000, 500, lags=[0])
 
 
 def test_full_hour_sampled_against_oracle(tmpdir_s):
@@ -212,7 +212,8 @@ def test_full_hour_sampled_against_oracle(tmpdir_s):
 @pytest.mark.parametrize("prec_name,tol", [("FP16", 2e-3), ("FP32", 1e-5)])
 @pytest.mark.parametrize("N,chunks,lags", [(1, [1], []), (5, [1, 1, 1, 1, 1], [3]), (17, [16, 1], [16]),
                                            (113, [112, 1], []), (225, [1, 111, 113], [1, 224]),
-                                           (4096, [4096], [4095])])
+                                           (4096, [4096], [4095]),
+                                           (300, [100, 200], [307, 600, 1203])])      # lags >= N wrap (k fs >= N)
 def test_stream_degenerate_sizes(tmpdir_s, prec_name, tol, N, chunks, lags):
     """Streams shorter than the receptive field / the kernel halo / one tile, one-sample chunks, lags next to N."""
     import paper_2201_11133_b200 as gwi
