@@ -7,10 +7,13 @@ with 10 % of windows carrying a chirp.  One "step" = one pass of the whole hot p
 gwi_infer (lift, 40 block-layers, head) -> gwi_ensemble_triggers (mean, threshold 0.5, runs >= 2048) -> trigger count.
 1 window = 1 s of two-detector strain, so value = windows / s.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--windows B] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--windows B] [--impl reference] [--scaling weak|strong]
 
-Multi-GPU: weak scaling, every rank runs the same per-GPU batch (the path shards over windows; no collective on the
-data path); value = all ranks' windows / max-over-ranks time.
+Multi-GPU (one process per GPU; with --gpus N > 1 and no launcher the ranks are started here through
+torch.distributed.run): --scaling weak (default): every rank runs the same per-GPU batch (the path shards over windows;
+no collective on the data path), value = all ranks' windows / max-over-ranks time.  --scaling strong: the configs[4]
+stream (--stream-chunks one-hour chunks) is time-sharded over the ranks (gwi_stream_set_shard), the shard-edge runs are
+gathered and joined on rank 0; value = stream seconds / max-over-ranks wall time.
 """
 import argparse
 import json
@@ -40,6 +43,32 @@ def peaks():
         d = json.load(open(p))
         return d, "measured"
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+PROFILE_CSV = os.path.join("profiles", "r2_k_stack_raw.csv")   # `ncu -i ... --page raw --csv` of the committed capture
+
+
+def profile_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum of k_stack per launch, read from the committed ncu capture
+    (profiles/r2_k_stack.md names the command).  None if the file is missing."""
+    import csv
+    path = os.path.join(ROOT, PROFILE_CSV)
+    if not os.path.exists(path):
+        return None
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    rows = list(csv.reader(open(path)))
+    hdr, units = rows[0], rows[1]
+    best = None
+    for r in rows[2:]:
+        name = r[hdr.index("Kernel Name")] if "Kernel Name" in hdr else ""
+        if "k_stack" not in name:
+            continue
+        tot = 0.0
+        for col in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            i = hdr.index(col)
+            tot += float(r[i].replace(",", "")) * scale.get(units[i], 1.0)
+        best = tot if best is None else max(best, tot)
+    return best
 
 
 class ClockSampler(threading.Thread):
@@ -131,22 +160,44 @@ def stream_bench(dev, work, rank, n_chunks=744, paper_month=False):
                                    "tflops_algorithmic": gs.PAPER_ARCH.flops_per_timestep() * N1 * 4 / (ms * 1e-3) / 1e12}
         # the same with 32 one-second time slides (paper-scale background estimation)
         lags = [gs.FS * k for k in range(1, 33)]
-        times = []
-        for rep in range(2):
-            st = gwi.Stream(pm, N1, N1, THETA, LMIN, lags=lags, capacity=4096)
-            st.prime(xd[1, N1 - st.tail_samples:].contiguous())
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            st.push(xd[0], xd[1])
-            e1.record()
-            n, _ = st.finish()
-            times.append(e0.elapsed_time(e1))
-            st.close()
-        ms = float(times[-1])
-        out["hour_paper_scale_32_slides"] = {"workload": "4 paper-scale models, 1 h stream, zero lag + 32 circular lags of k x 1 s, FP16",
-                                             "ms": ms, "strain_seconds_per_s": 3600 / (ms * 1e-3),
-                                             "slid_strain_seconds_per_s": 33 * 3600 / (ms * 1e-3), "triggers": n}
+        for nl in (32, 60):
+            # 60 one-second lags = the paper's 5 yr of time-slid background per month of data
+            lg = [gs.FS * k for k in range(1, nl + 1)]
+            times = []
+            for rep in range(2):
+                st = gwi.Stream(pm, N1, N1, THETA, LMIN, lags=lg, capacity=4096)
+                tail = xd[1, N1 - st.tail_samples:].contiguous()
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                st.prime(tail, sync=False)                       # the priming pass is part of the timed region
+                st.push(xd[0], xd[1])
+                e1.record()
+                n, _ = st.finish()
+                times.append(e0.elapsed_time(e1))
+                st.close()
+            ms = float(times[-1])
+            out[f"hour_paper_scale_{nl}_slides"] = {"workload": f"4 paper-scale models, 1 h stream, zero lag + {nl} circular lags of k x 1 s, FP16 "
+                                                                "(priming pass included)",
+                                                    "ms": ms, "strain_seconds_per_s": 3600 / (ms * 1e-3),
+                                                    "slid_strain_seconds_per_s": (nl + 1) * 3600 / (ms * 1e-3), "triggers": n}
+        # NEXT-2 scaled to the default run: 24 one-hour chunks from pinned host memory through the 4 x paper-scale ensemble
+        # (the whole month, 744 chunks, is --paper-month: about 2.5 minutes without slides)
+        nh = min(24, n_chunks)
+        st = gwi.Stream(pm, nh * N1, N1, THETA, LMIN, capacity=65536)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for c in range(nh):
+            h = host[c & 1]
+            st.push(h[0], h[1])
+        n, _ = st.finish()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        st.close()
+        out["day_paper_scale"] = {"workload": f"{nh} one-hour chunks from pinned host memory (H2D on the side stream inside the timed region), "
+                                              "4 paper-scale models, zero lag, FP16; the month (744 chunks) is this x 31 (--paper-month runs it)",
+                                  "wall_s": dt, "strain_seconds_per_s": nh * 3600 / dt, "triggers": n,
+                                  "tflops_algorithmic": gs.PAPER_ARCH.flops_per_timestep() * N1 * nh * 4 / dt / 1e12}
         if paper_month:
             # the month through the 4 x paper-scale ensemble, streamed from pinned host memory
             for name, lg in (("month_paper_scale", []), ("month_paper_scale_32_slides", lags)):
@@ -175,10 +226,11 @@ def stream_bench(dev, work, rank, n_chunks=744, paper_month=False):
         xc = torch.from_numpy(np.stack([gs.coloured_whitened_noise(2 + d, d, N1, seg_len=N1) for d in range(2)])).to(dev)
         lags = [gs.FS * k for k in range(1, 33)]
         st = gwi.Stream(models, n_hours * N1, N1, THETA, LMIN, lags=lags, capacity=65536)
-        st.prime(xc[1, N1 - st.tail_samples:].contiguous())
+        tail = xc[1, N1 - st.tail_samples:].contiguous()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
+        st.prime(tail, sync=False)                               # the priming pass is part of the timed region
         for c in range(n_hours):
             st.push(xc[0], xc[1])
         e1.record()
@@ -250,6 +302,71 @@ def stream_bench(dev, work, rank, n_chunks=744, paper_month=False):
     return out
 
 
+def strong_bench(args, dev, work, rank, world):
+    """--scaling strong: BASELINE.json configs[4] time-sharded over the ranks: the
+    stream of --stream-chunks one-hour chunks is cut into `world` contiguous spans; rank r runs its span through its own
+    gwi_stream handle in shard mode (R_f - 1 warm-up samples in front, chunks pushed from pinned host memory), the
+    records that touch a span edge are gathered and joined on rank 0.  No collective on the data path.  Time = max over
+    ranks of the wall time from the first push to the records on the host."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    from paper_2201_11133_b200 import shard
+    N1 = 3600 * gs.FS
+    models = []
+    for sd in range(4):
+        pth = os.path.join(work, f"bench_cfg1_seed{sd}_r{rank}.gwim")
+        gs.make_model_file(pth, gs.CFG1_ARCH, seed=sd)
+        models.append(gwi.load_model(pth, gwi.FP16, dev.index))
+    host = [torch.from_numpy(gs.stream_noise(1, c * N1, N1)).pin_memory() for c in range(2)]
+    n_chunks = args.stream_chunks
+    c0, c1 = shard.plan_windows(n_chunks, world)[rank]
+    rf = models[0].receptive_field
+    a = shard.shard_stream_args(n_chunks * N1, c0 * N1, c1 * N1, rf)
+    warm = a["shard"][1]
+
+    def run():
+        st = gwi.Stream(models, a["n_total"], N1, THETA, LMIN, capacity=65536, shard=a["shard"])
+        torch.cuda.synchronize()
+        if world > 1:
+            torch.distributed.barrier()
+        t0 = time.perf_counter()
+        if warm:
+            prev = host[(c0 - 1) & 1]
+            st.push(prev[0, N1 - warm:].contiguous().pin_memory(), prev[1, N1 - warm:].contiguous().pin_memory())
+        for c in range(c0, c1):
+            h = host[c & 1]
+            st.push(h[0], h[1])
+        n, recs = st.finish()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        st.close()
+        return dt, [(r.slide, r.start, r.end, r.peak_p, r.mean_p, r.model_mask) for r in recs]
+
+    run() if c1 - c0 <= 4 else None                                # warm-up pass only when it is cheap
+    dt, recs = run()
+    if world > 1:
+        import torch.distributed as dist
+        tt = torch.tensor([dt], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dt = float(tt.item())
+        allrecs = [r for part in shard.gather_objects(recs, dist) for r in part]
+    else:
+        allrecs = recs
+    if rank != 0:
+        return
+    merged = shard.merge_edge_records(allrecs, LMIN)
+    line = {"metric": METRIC, "value": n_chunks * 3600 / dt, "unit": UNIT, "n_gpus": world, "steps": 1, "warmup": 0,
+            "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f16",
+            "data": "synthetic",
+            "config": {"workload": f"configs[4] time-sharded: {n_chunks} one-hour chunks x 4096 Hz x 2 detectors FP16 from pinned host "
+                                   "memory, 4-model ensemble (config-1 arch) + trigger clustering; contiguous spans per rank with "
+                                   f"{rf - 1} warm-up samples, shard-edge runs joined on rank 0",
+                       "chunks_per_rank": [c1_ - c0_ for c0_, c1_ in shard.plan_windows(n_chunks, world)],
+                       "l2": "every chunk (59 MB) is streamed from host memory", "parallelism": f"time shards x{world} (strong)"},
+            "triggers": len(merged)}
+    print(json.dumps(line), flush=True)
+
+
 def oracle_sample(model_path, x16, n_windows):
     """Times the oracle as it stands on the host cores over `n_windows` windows of the workload."""
     from oracle import gwo
@@ -297,10 +414,21 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stream", action="store_true", help="skip the extra streaming-ensemble measurements")
     ap.add_argument("--stream-chunks", type=int, default=744, help="one-hour chunks of the month-long stream leg")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak: every rank runs the configs[1] batch (headline); strong: the configs[4] stream time-sharded over the ranks")
     ap.add_argument("--paper-month", action="store_true",
                     help="also stream the month through the 4 x paper-scale ensemble, without and with 32 slides (about 7 minutes)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started without a launcher: start the N ranks here (one process per GPU, NCCL over NVLink for the plumbing)
+        import socket
+        sk = socket.socket()
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+        sk.close()
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
 
     work = os.path.join(ROOT, "gpurun_out") if os.access(ROOT, os.W_OK) else "/tmp"
     os.makedirs(work, exist_ok=True)
@@ -325,6 +453,11 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
+    if args.scaling == "strong":
+        strong_bench(args, dev, work, rank, world)
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     # ---- inputs: NROT different seeded batches so that the rotating working set exceeds L2 -------------------
     x_host = []
@@ -436,13 +569,18 @@ def main():
     ms_per_step = total_ms / args.steps
     value = world * B * args.steps / (total_ms * 1e-3)
     tflops = flops_per_step / (infer_ms * 1e-3) / 1e12
-    peak_tf = pk.get("bf16_tflops_sustained", pk["bf16_tflops"])
+    # the timed region is a fraction of a second at near-maximum clocks: the burst figure is the denominator;
+    # the sustained and the nominal ones are reported beside it
+    peak_tf = pk["bf16_tflops"]
+    traffic = profile_traffic()
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
         "data": "synthetic",
-        "config": {"workload": "configs[1]: paper-scale single model (2x20 blocks, R64/S128, k2), FP16 operands / FP32 "
-                               "accumulate, batch of windows x 4096 x 2, then mean/threshold/cluster",
+        "config": {"workload": "configs[1]: paper-scale SINGLE model (2x20 blocks, R64/S128, k2), FP16 operands / FP32 "
+                               "accumulate, batch of windows x 4096 x 2, then mean/threshold/cluster; `value` is this model's "
+                               "windows/s (1 window = 1 strain-second); the 4-model ensemble strain-seconds/s of configs[2]-[4] "
+                               "are in `stream`",
                    "windows_per_gpu": B, "T": T, "threshold": THETA, "min_len": LMIN,
                    "l2": f"rotating {NROT} input+output buffer pairs ({NROT * B * T * 8 / 1e6:.0f} MB) > 126 MB L2",
                    "tensor_core_kernel": bool(model.uses_tensor_cores), "parallelism": f"replicas x{world} (weak)"},
@@ -453,10 +591,13 @@ def main():
                        "step i (two device buffers); count + records read back every step"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "tensor", "achieved": tflops, "peak": peak_tf, "unit": "TFLOP/s", "frac": tflops / peak_tf,
-                     "traffic": 5.25e9, "traffic_note": "dram__bytes_read+write of k_stack per launch, ncu --set full, "
-                     "profiles/r1_v5_k_stack_dram.md (u tiles 2.15 GB + history-ring tiles evicted from L2)", "peak_kind": f"bf16 cuBLAS sustained, {pk_kind}; fp16 = same tensor rate",
-                     "kernel": "gwi_infer (all launches of one call)", "flops_per_launch": flops_per_step,
-                     "infer_ms": infer_ms, "frac_of_nominal_2250": tflops / 2250.0},
+                     "traffic": traffic, "traffic_note": f"dram__bytes_read.sum + dram__bytes_write.sum of k_stack per launch, read from {PROFILE_CSV} "
+                     "(ncu --set full capture of this command, profiles/r2_k_stack.md)",
+                     "peak_kind": f"bf16 cuBLAS burst (best of 10), {pk_kind}; fp16 = same tensor rate",
+                     "frac_of_sustained": tflops / pk.get("bf16_tflops_sustained", peak_tf),
+                     "peak_sustained": pk.get("bf16_tflops_sustained"), "frac_of_nominal_2250": tflops / 2250.0,
+                     "kernel": "gwi_infer (k_stack + k_head_tc of one call)", "flops_per_launch": flops_per_step,
+                     "infer_ms": infer_ms},
     }
     if stream_extra is not None:
         line["stream"] = stream_extra

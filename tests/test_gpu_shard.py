@@ -134,3 +134,56 @@ def test_time_shards_paper_scale_tensor_core(tmpdir_s, lags):
     got = shard.merge_edge_records(recs, 5)
     assert [(r[0], r[1], r[2]) for r in got] == [(r[0], r[1], r[2]) for r in ref] and len(ref) > 100
     assert np.array_equal(pb, pb_ref)
+
+
+def _rank_worker(rank, world, port, tmp, q):
+    """One process per rank (both on cuda:0, as the single-GPU box allows: the ranks' kernels do not wait on one
+    another): its span through the library in shard mode, gloo gather of the records, join on every rank."""
+    import torch
+    import torch.distributed as dist
+    import paper_2201_11133_b200 as gwi
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        arch = gs.CFG1_ARCH
+        path = os.path.join(tmp, f"rank{rank}.gwim")
+        gs.write_model(path, arch, gs.p16_tensors(arch, block=2, r=7, q=(3, 4), hid=(5, 6)))
+        gm = gwi.load_model(path, gwi.FP16, 0)
+        N, kstar = 40 * FS, 5
+        ph, pl = _instance(N, kstar, N // 2)
+        x = torch.from_numpy(np.stack([gs.plateau_square_wave(N, ph, -2, np.float16), gs.plateau_square_wave(N, pl, -3, np.float16)]))
+        lags = [FS, kstar * FS]
+        sh = shard.plan_time(N, world, gm.receptive_field, max(lags))[rank]
+        a = shard.shard_stream_args(N, sh.start, sh.end, gm.receptive_field, max(lags))
+        st = gwi.Stream([gm], a["n_total"], 50000, 0.5, LMIN, lags=lags, capacity=4096, shard=a["shard"])
+        st.prime(x[1, torch.tensor(a["tail_indices"])].contiguous())
+        for p in range(a["first_pushed"], sh.end, 50000):
+            e = min(p + 50000, sh.end)
+            st.push(x[0, p:e].contiguous().cuda(), x[1, p:e].contiguous().cuda())
+        n, recs = st.finish()
+        st.close()
+        mine = [(r.slide, r.start, r.end, r.peak_p, r.mean_p, r.model_mask) for r in recs]
+        allr = [r for part in shard.gather_objects(mine, dist) for r in part]
+        got = [(r[0], r[1], r[2]) for r in shard.merge_edge_records(allr, LMIN)]
+        q.put((rank, got, got == _hand_lists(ph, pl, lags, N)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_processes_time_sharded_stream(tmpdir_s):
+    import socket
+    import torch.multiprocessing as mp
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    ps = [ctx.Process(target=_rank_worker, args=(r, 2, port, str(tmpdir_s), q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    got = sorted(q.get(timeout=300) for _ in ps)
+    for p in ps:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert got[0][2] and got[1][2] and got[0][1] == got[1][1] and len(got[0][1]) >= 6
