@@ -22,6 +22,11 @@ class Trigger(C.Structure):
                 ("peak_p", C.c_double), ("mean_p", C.c_double)]
 
 
+class Peak(C.Structure):
+    _fields_ = [("index", C.c_int64), ("height", C.c_double), ("prominence", C.c_double), ("width", C.c_double),
+                ("left_ip", C.c_double), ("right_ip", C.c_double)]
+
+
 class Event(C.Structure):
     _fields_ = [("t_first", C.c_int64), ("t_last", C.c_int64), ("n_triggers", C.c_int32), ("slide", C.c_int32)]
 
@@ -61,6 +66,8 @@ def lib():
         L.gwo_coincidence.restype = C.c_long
         L.gwo_coincidence.argtypes = [C.POINTER(C.POINTER(C.c_long)), C.POINTER(C.c_int), C.c_int, C.c_long, C.c_int,
                                       C.POINTER(Event), C.c_long]
+        L.gwo_find_peaks.restype = C.c_long
+        L.gwo_find_peaks.argtypes = [_dp, C.c_long, C.c_double, C.c_double, C.POINTER(Peak), C.c_long]
         L.gwo_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -207,3 +214,12 @@ def coincidence(ends, window, slide=0, cap=1 << 14):
     out = (Event * cap)()
     k = lib().gwo_coincidence(ptrs, n, M, int(window), int(slide), out, cap)
     return [(o.t_first, o.t_last, o.n_triggers) for o in out[:min(k, cap)]]
+
+
+def find_peaks(x, height, width, cap=1 << 16):
+    """SciPy's find_peaks(x, height=height, width=width) restated -> (count, [(index, height,
+    prominence, width, left_ip, right_ip)])."""
+    x, xp = _d(x)
+    out = (Peak * cap)()
+    n = lib().gwo_find_peaks(xp, x.shape[0], float(height), float(width), out, cap)
+    return n, [(o.index, o.height, o.prominence, o.width, o.left_ip, o.right_ip) for o in out[:min(n, cap)]]

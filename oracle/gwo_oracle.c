@@ -399,3 +399,67 @@ int gwo_num_threads(void)
     return 1;
 #endif
 }
+
+/* ---- the paper's post-processing rule as stated: SciPy's find_peaks with a height and a width condition ------------
+ * PAPER.md:53 ("post-processed it with the find_peaks algorithm, a SciPy's off-the-shelve tool"), PAPER.md:102 ("uses the
+ * find_peaks algorithm to identity peaks whose width is at least 0.5 seconds long ... height in our find_peaks
+ * algorithms").  find_peaks(x, height=h, width=w) is a public, fully defined procedure; it is restated here step by
+ * step (SciPy reference guide, scipy.signal.find_peaks / peak_prominences / peak_widths, default wlen = None and
+ * rel_height = 0.5):
+ *  1. local maxima: i is a peak iff x[i-1] < x[i] and x[i] > x[i+1]; a flat top x[i] = ... = x[j] with x[i-1] < x[i] and
+ *     x[j] > x[j+1] counts once, at floor((i + j) / 2); the first and the last sample are never peaks (a flat top that
+ *     reaches either end of the array is not one).
+ *  2. height: keep peaks with x[p] >= h.
+ *  3. prominence of p: walk left from p while x[i] <= x[p] (stop at the array start), left_min = smallest value met;
+ *     likewise to the right; prominence = x[p] - max(left_min, right_min).
+ *  4. width of p at rel_height 0.5: level = x[p] - prominence / 2; walk left from p while level < x[i] (not past the
+ *     position of left_min), the crossing is interpolated linearly between that sample and the one after it; likewise
+ *     to the right; width = right crossing - left crossing (in samples).
+ *  5. keep peaks with width >= w.  Output sorted by position.
+ * TEST INFRASTRUCTURE like everything in this file; pinned against scipy.signal.find_peaks in tests/test_oracle_peaks.py. */
+typedef struct { int64_t index; double height, prominence, width, left_ip, right_ip; } gwo_peak;
+
+long gwo_find_peaks(const double *x, long N, double hmin, double wmin, gwo_peak *out, long cap)
+{
+    long count = 0;
+    long i = 1;
+    while (i < N - 1) {
+        if (x[i - 1] < x[i]) {
+            long j = i;                                   /* end of the flat top that starts at i */
+            while (j < N - 1 && x[j + 1] == x[i]) j++;
+            if (j < N - 1 && x[j + 1] < x[i]) {
+                long p = (i + j) / 2;
+                if (x[p] >= hmin) {
+                    /* step 3 */
+                    double lmin = x[p], rmin = x[p];
+                    long lb = p, rb = p;
+                    for (long k = p; k >= 0 && x[k] <= x[p]; k--) if (x[k] < lmin) { lmin = x[k]; lb = k; }
+                    for (long k = p; k < N && x[k] <= x[p]; k++) if (x[k] < rmin) { rmin = x[k]; rb = k; }
+                    double prom = x[p] - (lmin > rmin ? lmin : rmin);
+                    /* step 4 */
+                    double level = x[p] - prom * 0.5;
+                    long k = p;
+                    while (lb < k && level < x[k]) k--;
+                    double lip = (double)k;
+                    if (x[k] < level) lip += (level - x[k]) / (x[k + 1] - x[k]);
+                    k = p;
+                    while (k < rb && level < x[k]) k++;
+                    double rip = (double)k;
+                    if (x[k] < level) rip -= (level - x[k]) / (x[k - 1] - x[k]);
+                    double width = rip - lip;
+                    if (width >= wmin) {
+                        if (count < cap) {
+                            out[count].index = p; out[count].height = x[p]; out[count].prominence = prom;
+                            out[count].width = width; out[count].left_ip = lip; out[count].right_ip = rip;
+                        }
+                        count++;
+                    }
+                }
+            }
+            i = j + 1;
+        } else {
+            i++;
+        }
+    }
+    return count;
+}
