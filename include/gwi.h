@@ -226,6 +226,32 @@ gwi_status gwi_threshold_sweep(const float* const* d_prob, int32_t n_models, int
                                int32_t n_thresholds, int64_t min_len, int64_t* d_counts, void* d_workspace,
                                size_t workspace_bytes, void* cuda_stream);
 
+/* ---- the paper's peak rule: SciPy find_peaks(height, width) on one model's probabilities (NEXT-1) ------
+ * "post-processed it with the find_peaks algorithm, a SciPy's off-the-shelve tool"; "peaks whose width is at
+ * least 0.5 seconds long ... height in our find_peaks algorithms".  On the device array d_x[N] (one model's
+ * per-timestep probabilities of a whole segment; the search for a peak's prominence is not local, so there is no chunk
+ * carry) the call finds, exactly as scipy.signal.find_peaks(x, height=height, width=min_width) does:
+ *   local maxima (a flat top counts once, at the floor of its middle; the first and last sample never),  x[p] >= height,
+ *   prominence = x[p] - max(lowest sample between p and the nearest higher sample on the left, same on the right),
+ *   width between the linearly interpolated crossings of x[p] - prominence / 2,  width >= min_width (in samples).
+ * d_peaks: DEVICE [capacity], sorted by index; *d_count (DEVICE) = number of peaks found; if it exceeds capacity the
+ * records are not valid (the call is asynchronous and returns GWI_OK; compare after synchronising).
+ * d_workspace: DEVICE, >= gwi_find_peaks_workspace_bytes(N, capacity), 256 B aligned.  Peak positions, prominences and
+ * widths equal the fp64 oracle's on the same fp32 samples (decisions are taken in fp64 on exact differences).
+ * A peak's position is the model's trigger time for gwi_coincidence (pass index as `end`).
+ * Errors: GWI_ERR_ARG, GWI_ERR_NOMEM, GWI_ERR_CUDA. */
+typedef struct {
+    int64_t index;
+    float height;
+    float prominence;
+    double width;
+    double left_ip;
+    double right_ip;
+} gwi_peak;
+size_t gwi_find_peaks_workspace_bytes(int64_t N, int32_t capacity);
+gwi_status gwi_find_peaks(const float* d_x, int64_t N, float height, double min_width, gwi_peak* d_peaks, int32_t capacity,
+                          int32_t* d_count, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---- whitening front end (reading A35) ----------------------------------------
  * One segment of n raw strain samples of one detector -> whitened, unit-variance samples (what gwi_infer / gwi_stream_*
  * take as input): Welch estimate of the segment's own PSD (frames of nper samples every nper/2, symmetric Hann window,

@@ -14,7 +14,7 @@ EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_m
                     "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
                     "gwi_stream_tail_samples", "gwi_stream_prime", "gwi_stream_push", "gwi_stream_push_host",
                     "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_backend", "gwi_stream_set_shard", "gwi_stream_destroy", "gwi_stream_set_rule",
-                    "gwi_coincidence", "gwi_sweep_workspace_bytes", "gwi_threshold_sweep", "gwi_whiten_workspace_bytes",
+                    "gwi_coincidence", "gwi_find_peaks_workspace_bytes", "gwi_find_peaks", "gwi_sweep_workspace_bytes", "gwi_threshold_sweep", "gwi_whiten_workspace_bytes",
                     "gwi_whiten"]
 
 
@@ -88,6 +88,10 @@ def lib():
     L.gwi_stream_set_rule.argtypes = [vp, C.c_int]
     L.gwi_coincidence.restype = C.c_int
     L.gwi_coincidence.argtypes = [vp, C.c_int32, C.c_int32, C.c_int64, vp, C.c_int32, i32p]
+    L.gwi_find_peaks_workspace_bytes.restype = C.c_size_t
+    L.gwi_find_peaks_workspace_bytes.argtypes = [C.c_int64, C.c_int32]
+    L.gwi_find_peaks.restype = C.c_int
+    L.gwi_find_peaks.argtypes = [vp, C.c_int64, C.c_float, C.c_double, vp, C.c_int32, vp, vp, C.c_size_t, vp]
     L.gwi_sweep_workspace_bytes.restype = C.c_size_t
     L.gwi_sweep_workspace_bytes.argtypes = [C.c_int32]
     L.gwi_threshold_sweep.restype = C.c_int
@@ -225,6 +229,30 @@ def threshold_sweep(probs, thresholds, min_len):
     _check(lib().gwi_threshold_sweep(ptrs, len(probs), N, C.c_void_p(th.data_ptr()), K, int(min_len),
                                      C.c_void_p(counts.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(dev)))
     return counts
+
+
+class Peak(C.Structure):
+    _fields_ = [("index", C.c_int64), ("height", C.c_float), ("prominence", C.c_float), ("width", C.c_double),
+                ("left_ip", C.c_double), ("right_ip", C.c_double)]
+
+
+def find_peaks(x, height, min_width, capacity=65536):
+    """gwi_find_peaks on a [N] float32 device tensor -> (count, [Peak...]) sorted by index; raises GwiError(GWI_ERR_CAPACITY)
+    when count > capacity."""
+    if not x.is_cuda or x.dtype != torch.float32:
+        raise GwiError(1, "x must be a float32 CUDA tensor (no CPU fallback)")
+    x = x.contiguous()
+    N = x.numel()
+    out = torch.zeros(max(capacity, 1) * C.sizeof(Peak), dtype=torch.uint8, device=x.device)
+    cnt = torch.zeros(1, dtype=torch.int32, device=x.device)
+    ws = torch.empty(max(lib().gwi_find_peaks_workspace_bytes(N, int(capacity)), 256), dtype=torch.uint8, device=x.device)
+    _check(lib().gwi_find_peaks(C.c_void_p(x.data_ptr()), N, float(height), float(min_width), C.c_void_p(out.data_ptr()),
+                                int(capacity), C.c_void_p(cnt.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(x.device)))
+    n = int(cnt.item())
+    if n > capacity:
+        raise GwiError(7, f"{n} peaks > capacity {capacity}")
+    raw = out.cpu().numpy().tobytes()
+    return n, [Peak.from_buffer_copy(raw, i * C.sizeof(Peak)) for i in range(n)]
 
 
 def whiten(raw, nper, half=True):

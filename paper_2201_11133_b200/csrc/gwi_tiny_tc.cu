@@ -305,8 +305,8 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
                     uint32_t hv[16], pk[8];
                     tmem_ld16(tlane + 32, hv);
                     tc_wait_ld();
-#pragma unroll
                     TT_TRACE(8);
+#pragma unroll
                     for (int c = 0; c < 8; c++) pk[c] = dead ? 0u : pack_half2(__uint_as_float(hv[2 * c]), __uint_as_float(hv[2 * c + 1]));
                     put_operand(b * TT_MAX_L + i + 1, pk);
                     TT_TRACE(9);
