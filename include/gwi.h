@@ -260,7 +260,8 @@ gwi_status gwi_find_peaks(const float* d_x, int64_t N, float height, double min_
  * d_raw: DEVICE [n] float (not modified).  d_out: DEVICE [n], float, or __half when out_is_half != 0 (may not alias
  * d_raw).  n, nper even, 4 <= nper <= n <= 2^30.  d_workspace: DEVICE, >= gwi_whiten_workspace_bytes(n, nper), 256 B
  * aligned.  The FFTs are cuFFT transforms; the library is loaded on first use (GWI_ERR_UNSUPPORTED if it cannot be).
- * The call enqueues on cuda_stream and waits for it before returning (the FFT plans are released).
+ * The call enqueues on cuda_stream and returns; the FFT plans are cached per (device, n, nper, stream) for the life of the
+ * process, so successive segments of one length re-use them.
  * Errors: GWI_ERR_ARG, GWI_ERR_NOMEM, GWI_ERR_UNSUPPORTED, GWI_ERR_CUDA. */
 size_t gwi_whiten_workspace_bytes(int64_t n, int32_t nper);
 gwi_status gwi_whiten(const float* d_raw, int64_t n, int32_t nper, void* d_out, int out_is_half, void* d_workspace,

@@ -17,8 +17,9 @@
 //           warps gate the other.  Output: u = ReLU(sum of skips) per branch, fp16, tile-major in the workspace.
 //  k_head   [128 x 128] = [u_H | u_L] . W1^T on tcgen05, then ReLU, dot with W2, sigmoid (C.1 steps 4-5).
 //
-// Roles in k_stack (320 threads): warps 0-3 epilogue of slot 0, warps 4-7 epilogue of slot 1 (warp % 4 = TMEM lane
-// quadrant), warp 8 lane 0 = bulk-copy producer (weights, ring tiles), warp 9 lane 0 = MMA issuer.
+// Roles in k_stack (608 threads): warps 0-7 epilogue of slot 0, warps 8-15 of slot 1 (warp % 4 = TMEM lane quadrant,
+// (warp / 4) % 2 = channel half), warp 16 lane 0 = bulk-copy producer (weights, ring tiles), warps 17 / 18: one elected
+// lane each = MMA issuer of slot 0 / 1.
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>

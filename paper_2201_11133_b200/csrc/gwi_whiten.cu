@@ -13,6 +13,11 @@
 #include <cufft.h>
 #include <dlfcn.h>
 
+#include <array>
+#include <map>
+#include <mutex>
+#include <tuple>
+
 #include "gwi_internal.h"
 
 namespace {
@@ -182,18 +187,38 @@ extern "C" gwi_status gwi_whiten(const float* d_raw, int64_t n, int32_t nper, vo
     float* y = (float*)(ws + L.y);
     double* stats = (double*)(ws + L.stats);
     const int K = L.K, nf = nper / 2 + 1;
+    // The three plans (and the work areas they own) are cached per (device, n, nper, stream) for the life of the process,
+    // so the call only enqueues work and returns: segment after segment of the same length re-uses them.
+    int device = 0;
+    GWI_CUDA_CHECK(cudaGetDevice(&device));
     cufftHandle pf = 0, pr = 0, pi = 0;
+    {
+        static std::mutex mu;
+        static std::map<std::tuple<int, int64_t, int, void*>, std::array<cufftHandle, 3>> cache;
+        std::lock_guard<std::mutex> lock(mu);
+        auto key = std::make_tuple(device, n, (int)nper, cuda_stream);
+        auto it = cache.find(key);
+        if (it == cache.end()) {
+            auto fail = [&](const char* what) {
+                if (pf) fft.Destroy(pf);
+                if (pr) fft.Destroy(pr);
+                if (pi) fft.Destroy(pi);
+                gwi_set_error("gwi_whiten: cuFFT %s failed", what);
+                return GWI_ERR_CUDA;
+            };
+            if (fft.Plan1d(&pf, nper, CUFFT_R2C, K) != CUFFT_SUCCESS) return fail("plan (frames)");
+            if (fft.Plan1d(&pr, (int)n, CUFFT_R2C, 1) != CUFFT_SUCCESS) return fail("plan (forward)");
+            if (fft.Plan1d(&pi, (int)n, CUFFT_C2R, 1) != CUFFT_SUCCESS) return fail("plan (inverse)");
+            fft.SetStream(pf, st), fft.SetStream(pr, st), fft.SetStream(pi, st);
+            cache[key] = {pf, pr, pi};
+        } else {
+            pf = it->second[0], pr = it->second[1], pi = it->second[2];
+        }
+    }
     auto fail = [&](const char* what) {
-        if (pf) fft.Destroy(pf);
-        if (pr) fft.Destroy(pr);
-        if (pi) fft.Destroy(pi);
         gwi_set_error("gwi_whiten: cuFFT %s failed", what);
         return GWI_ERR_CUDA;
     };
-    if (fft.Plan1d(&pf, nper, CUFFT_R2C, K) != CUFFT_SUCCESS) return fail("plan (frames)");
-    if (fft.Plan1d(&pr, (int)n, CUFFT_R2C, 1) != CUFFT_SUCCESS) return fail("plan (forward)");
-    if (fft.Plan1d(&pi, (int)n, CUFFT_C2R, 1) != CUFFT_SUCCESS) return fail("plan (inverse)");
-    fft.SetStream(pf, st), fft.SetStream(pr, st), fft.SetStream(pi, st);
     const int64_t nfr = (int64_t)K * nper;
     cudaMemsetAsync(stats, 0, 32, st);
     k_stats_y<<<592, 256, 0, st>>>(d_raw, n, stats + 2);          // stats[2..3]: sum and sum of squares of the raw input
@@ -209,9 +234,6 @@ extern "C" gwi_status gwi_whiten(const float* d_raw, int64_t n, int32_t nper, vo
     else k_scale_out<float><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(y, n, stats, (float*)d_out);
     gwi_count_launch(6);
     cudaError_t e = cudaGetLastError();
-    // the plans own work areas that the enqueued transforms use: release them once the stream has drained
-    cudaStreamSynchronize(st);
-    fft.Destroy(pf), fft.Destroy(pr), fft.Destroy(pi);
     if (e != cudaSuccess) {
         gwi_set_error("gwi_whiten: %s", cudaGetErrorString(e));
         return GWI_ERR_CUDA;
