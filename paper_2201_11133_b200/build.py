@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgwi.so")
-SOURCES = ["gwi_api.cu", "gwi_generic.cu", "gwi_post.cu", "gwi_tc.cu", "gwi_stream.cu", "gwi_tiny.cu", "gwi_tiny_tc.cu", "gwi_sweep.cu", "gwi_whiten.cu", "gwi_peaks.cu"]
+SOURCES = ["gwi_api.cu", "gwi_generic.cu", "gwi_post.cu", "gwi_tc.cu", "gwi_stream.cu", "gwi_tiny.cu", "gwi_tiny_tc.cu", "gwi_sweep.cu", "gwi_whiten.cu", "gwi_peaks.cu", "gwi_heads.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "--fmad=true", "-Xptxas", "-v"]
 

@@ -98,6 +98,16 @@ gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N,
                         int32_t capacity, int32_t* d_count, int append, float* d_pbar, void* d_workspace,
                         size_t workspace_bytes, cudaStream_t st, int64_t shard_begin = -1, int64_t shard_end = -1);
 
+gwi_status gwi_post_run_bits(const uint32_t* d_bits, const float* d_pbar, const uint8_t* d_mm, int64_t N, int64_t t0, float threshold,
+                             int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry, gwi_trigger* d_triggers,
+                             int32_t capacity, int32_t* d_count, int append, void* d_workspace, size_t workspace_bytes,
+                             cudaStream_t st, int64_t shard_begin = -1, int64_t shard_end = -1);
+// fused time-slide heads of the narrow architecture (gwi_heads.cu): all lags, all models, mean, threshold
+gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* const* d_v, int64_t lds, int n, const int64_t* d_lags,
+                           int n_lags, const int64_t* h_lags, float theta, uint32_t* d_bits, int64_t bits_stride, float* d_pbar,
+                           uint8_t* d_mm, int64_t row_stride, float* d_prob, cudaStream_t st);
+bool gwi_tiny_writes_v(const gwi_model* m);
+
 // ---- tcgen05 path (gwi_tc.cu) -------------------------------------------------------------------------------
 bool gwi_tc_supported(const GwiArch& a);
 gwi_status gwi_tc_pack(gwi_model* m);

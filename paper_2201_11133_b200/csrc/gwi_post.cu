@@ -253,7 +253,10 @@ __global__ void k_scan(const uint32_t* __restrict__ blkcnt, uint32_t* __restrict
 }
 
 // statistics of pbar over local [a,b): peak, sum (double), per-model mask.  256 threads cooperate.
-__device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t b, float& peak, double& sum, int& mask)
+// mm (fused time-slide heads, gwi_heads.cu): one byte per sample with the models that exceeded the threshold on their own;
+// P then holds the mean itself (M = 1)
+__device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t b, float& peak, double& sum, int& mask,
+                          const uint8_t* __restrict__ mm)
 {
     __shared__ float s_peak[256];
     __shared__ double s_sum[256];
@@ -265,7 +268,9 @@ __device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t 
         float v = ens_mean(P, M, i);
         pk = fmaxf(pk, v);
         sm += (double)v;
-        for (int j = 0; j < M; j++) mk |= (P.p[j][i] > theta) << j;
+        if (mm) mk |= mm[i];
+        else
+            for (int j = 0; j < M; j++) mk |= (P.p[j][i] > theta) << j;
     }
     s_peak[threadIdx.x] = pk, s_sum[threadIdx.x] = sm, s_mask[threadIdx.x] = mk;
     __syncthreads();
@@ -282,7 +287,8 @@ __device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t 
 }
 
 __global__ void k_stats(Ptrs P, int M, float theta, int64_t N, int64_t t0, const Header* __restrict__ hd,
-                        gwi_trigger* __restrict__ out, int capacity, Carry* carry, int64_t shard_begin, int64_t shard_end)
+                        gwi_trigger* __restrict__ out, int capacity, Carry* carry, int64_t shard_begin, int64_t shard_end,
+                        const uint8_t* __restrict__ mm)
 {
     const int nrec = min(hd->total, capacity);
     if ((int)blockIdx.x == (int)gridDim.x - 1) {   // last CTA: write the outgoing carry
@@ -292,7 +298,7 @@ __global__ void k_stats(Ptrs P, int M, float theta, int64_t N, int64_t t0, const
         if (c.open) {
             int64_t a = c.start > t0 ? c.start - t0 : 0;
             float pk; double sm; int mk;
-            run_stats(P, M, theta, a, N, pk, sm, mk);
+            run_stats(P, M, theta, a, N, pk, sm, mk, mm);
             if (c.start < t0) pk = fmaxf(pk, hd->in.peak), sm += hd->in.sum, mk |= hd->in.mask;
             c.peak = pk, c.sum = sm, c.mask = mk;
         }
@@ -304,7 +310,7 @@ __global__ void k_stats(Ptrs P, int M, float theta, int64_t N, int64_t t0, const
         int64_t s = out[r].start, e = out[r].end;
         int64_t a = s > t0 ? s - t0 : 0;
         float pk; double sm; int mk;
-        run_stats(P, M, theta, a, e - t0, pk, sm, mk);
+        run_stats(P, M, theta, a, e - t0, pk, sm, mk, mm);
         if (s < t0) pk = fmaxf(pk, hd->in.peak), sm += hd->in.sum, mk |= hd->in.mask;
         if (threadIdx.x == 0) {
             out[r].peak_p = pk;
@@ -350,6 +356,50 @@ extern "C" gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t 
 }
 
 // append != 0: *d_count holds the number of records already in d_triggers; the new ones go behind them.
+static gwi_status post_from_bits(const Ptrs& P, int n_models, const uint8_t* d_mm, const uint32_t* bits, int64_t N, int64_t t0,
+                                 float threshold, int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry,
+                                 gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count, int append, char* ws, const Layout& L,
+                                 cudaStream_t st, int64_t shard_begin, int64_t shard_end)
+{
+    Header* hd = (Header*)(ws + L.hdr);
+    uint8_t* flags = (uint8_t*)(ws + L.flags);
+    uint32_t* cnt = (uint32_t*)(ws + L.cnt);
+    uint32_t* off = (uint32_t*)(ws + L.off);
+    k_blkflags<<<(unsigned)L.NB, WB, 0, st>>>(bits, L.NW, flags);
+    k_head_run<<<1, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd, shard_begin, shard_end);
+    k_runs<0><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
+                                             d_triggers, capacity, shard_begin, shard_end);
+    k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append);
+    k_runs<1><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
+                                             d_triggers, capacity, shard_begin, shard_end);
+    int sgrid = capacity < 1024 ? capacity + 1 : 1025;
+    k_stats<<<sgrid, 256, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry, shard_begin, shard_end, d_mm);
+    gwi_count_launch(6);
+    GWI_CUDA_CHECK(cudaGetLastError());
+    return GWI_OK;
+}
+
+// Clustering of one slide from a bit mask that the fused heads kernel (gwi_heads.cu) has written: d_bits = words of the
+// mask (bit i of word w = sample 32 w + i, bits past N zero), d_pbar = the mean probability (run statistics), d_mm = the
+// per-sample model bytes.  Same carry / append / shard semantics as gwi_post_run.
+gwi_status gwi_post_run_bits(const uint32_t* d_bits, const float* d_pbar, const uint8_t* d_mm, int64_t N, int64_t t0, float threshold,
+                             int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry, gwi_trigger* d_triggers,
+                             int32_t capacity, int32_t* d_count, int append, void* d_workspace, size_t workspace_bytes,
+                             cudaStream_t st, int64_t shard_begin, int64_t shard_end)
+{
+    Layout L = layout(N);
+    if (workspace_bytes < L.total || !d_bits || !d_pbar) {
+        gwi_set_error("gwi_post_run_bits: bad argument / workspace");
+        return GWI_ERR_ARG;
+    }
+    Ptrs P;
+    P.p[0] = d_pbar;
+    for (int j = 1; j < GWI_MAX_MODELS; j++) P.p[j] = nullptr;
+    if (!d_carry) last_chunk = 1;
+    return post_from_bits(P, 1, d_mm, d_bits, N, t0, threshold, min_len, slide_id, last_chunk, d_carry, d_triggers, capacity, d_count,
+                          append, (char*)d_workspace, L, st, shard_begin, shard_end);
+}
+
 gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0, float threshold,
                         int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry, gwi_trigger* d_triggers,
                         int32_t capacity, int32_t* d_count, int append, float* d_pbar, void* d_workspace,
@@ -384,11 +434,7 @@ gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N,
     }
     if (!d_carry) last_chunk = 1;   // a chunk without carry is a whole stream
     char* ws = (char*)d_workspace;
-    Header* hd = (Header*)(ws + L.hdr);
     uint32_t* bits = (uint32_t*)(ws + L.bits);
-    uint8_t* flags = (uint8_t*)(ws + L.flags);
-    uint32_t* cnt = (uint32_t*)(ws + L.cnt);
-    uint32_t* off = (uint32_t*)(ws + L.off);
     // one warp handles 128 samples per iteration; 148 SMs x 8 CTAs of 256 threads
     int64_t warps_needed = (L.NW * 32 + 127) / 128;
     int grid = (int)((warps_needed + 7) / 8);
@@ -396,16 +442,7 @@ gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N,
     if (grid < 1) grid = 1;
     if (vec) k_mask<true><<<grid, 256, 0, st>>>(P, n_models, N, threshold, bits, L.NW, d_pbar);
     else k_mask<false><<<grid, 256, 0, st>>>(P, n_models, N, threshold, bits, L.NW, d_pbar);
-    k_blkflags<<<(unsigned)L.NB, WB, 0, st>>>(bits, L.NW, flags);
-    k_head_run<<<1, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd, shard_begin, shard_end);
-    k_runs<0><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
-                                             d_triggers, capacity, shard_begin, shard_end);
-    k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append);
-    k_runs<1><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
-                                             d_triggers, capacity, shard_begin, shard_end);
-    int sgrid = capacity < 1024 ? capacity + 1 : 1025;
-    k_stats<<<sgrid, 256, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry, shard_begin, shard_end);
-    gwi_count_launch(7);
-    GWI_CUDA_CHECK(cudaGetLastError());
-    return GWI_OK;
+    gwi_count_launch(1);
+    return post_from_bits(P, n_models, nullptr, bits, N, t0, threshold, min_len, slide_id, last_chunk, d_carry, d_triggers, capacity,
+                          d_count, append, ws, L, st, shard_begin, shard_end);
 }

@@ -61,6 +61,12 @@ struct gwi_stream {
     std::vector<__half*> d_u16;             // time slides: per model [2][lds][32] fp16 branch features, time-major
     int64_t* d_lags = nullptr;              // device copy of the lag list
     int rule = 0;                           // GWI_RULE_MEAN / GWI_RULE_PER_MODEL
+    // fused time-slide heads of the narrow architecture (gwi_heads.cu): per slide a bit mask, the mean and the model bytes
+    bool fused = false;
+    uint32_t* d_fbits = nullptr;
+    float* d_fpbar = nullptr;
+    uint8_t* d_fmm = nullptr;
+    int64_t fbits_stride = 0;
     // time-shard mode (gwi_stream_set_shard): the first `warm` pushed samples are warm-up, the first kept sample has the
     // global index t_first
     bool shard = false;
@@ -199,9 +205,10 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
                                  s->d_xh[s->xh_cur], xh_next,
                                  nslides == 1 ? s->d_prob + (size_t)m * s->sub : nullptr, u0, s->lds, st);
             if (rc != GWI_OK) return rc;
-            if (nslides == 1) continue;
+            if (nslides == 1 || s->fused) continue;
             rc = gwi_tiny_heads(gm, u0, s->lds, n, s->d_lags, nslides, s->d_prob + (size_t)m * s->sub, (int64_t)s->M * s->sub, st);
             if (rc != GWI_OK) return rc;
+            if (s->fused) continue;   // (shifted after the fused heads launch below)
             // ring shift: the last maxlag rows of the L1 features move to the front
             __half* base = s->d_u16[m] + (size_t)s->lds * 32;
             GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_tmp, base + (size_t)n * 32, (size_t)s->maxlag * 64, cudaMemcpyDeviceToDevice, st));
@@ -224,6 +231,24 @@ gwi_status run_sub(gwi_stream* s, int xb, int64_t x0, int n, bool last, cudaStre
                                              cudaMemcpyDeviceToDevice, st));
             GWI_CUDA_CHECK(cudaMemcpy2DAsync(base, s->lds * 4, s->d_tmp, s->maxlag * 4, s->maxlag * 4, rows,
                                              cudaMemcpyDeviceToDevice, st));
+        }
+    }
+    if (s->fused) {
+        // every lag, every model, mean and threshold in one launch on the kept samples of the block (a time shard's
+        // warm-up samples produce no output); the rings shift afterwards
+        const int64_t skip = (s->rule == GWI_RULE_PER_MODEL) ? 0 : (s->t_done < s->warm ? std::min<int64_t>(n, s->warm - s->t_done) : 0);
+        if (skip < n) {
+            const __half* vp[GWI_MAX_MODELS];
+            for (int m = 0; m < s->M; m++) vp[m] = s->d_u16[m] + (size_t)(s->maxlag + skip) * 32;
+            const bool pm = s->rule == GWI_RULE_PER_MODEL;
+            gwi_status rc = gwi_heads_fused(s->models.data(), s->M, vp, s->lds, (int)(n - skip), s->d_lags, nslides, s->lags.data(), s->theta,
+                                            s->d_fbits, s->fbits_stride, s->d_fpbar, s->d_fmm, s->sub, pm ? s->d_prob : nullptr, st);
+            if (rc != GWI_OK) return rc;
+        }
+        for (int m = 0; m < s->M; m++) {
+            __half* base = s->d_u16[m] + (size_t)s->lds * 32;
+            GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_tmp, base + (size_t)n * 32, (size_t)s->maxlag * 64, cudaMemcpyDeviceToDevice, st));
+            GWI_CUDA_CHECK(cudaMemcpyAsync(base, s->d_tmp, (size_t)s->maxlag * 64, cudaMemcpyDeviceToDevice, st));
         }
     }
     s->hist_cur ^= 1;
@@ -256,6 +281,21 @@ gwi_status post_block(gwi_stream* s, int n, bool last, cudaStream_t st)
                                              s->d_count, 1, pb, s->d_post_ws, s->post_ws_bytes, st, sb, se);
                 if (rc != GWI_OK) return rc;
             }
+        s->t_done += n;
+        return GWI_OK;
+    }
+    if (s->fused) {
+        // the fused heads kernel has written mask, mean and model bytes of the kept samples, starting at index 0
+        for (int k = 0; k < nslides; k++) {
+            gwi_status rc = gwi_post_run_bits(s->d_fbits + (size_t)k * s->fbits_stride, s->d_fpbar + (size_t)k * s->sub,
+                                              s->d_fmm + (size_t)k * s->sub, nn, t0, s->theta, s->min_len, k, last ? 1 : 0,
+                                              (char*)s->d_carry + (size_t)k * gwi_carry_bytes(), s->d_trig, s->cap, s->d_count, 1,
+                                              s->d_post_ws, s->post_ws_bytes, st, sb, se);
+            if (rc != GWI_OK) return rc;
+            if (s->d_pbar)
+                GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_pbar + (size_t)k * Nk + kept, s->d_fpbar + (size_t)k * s->sub, (size_t)nn * 4,
+                                               cudaMemcpyDeviceToDevice, st));
+        }
         s->t_done += n;
         return GWI_OK;
     }
@@ -534,8 +574,18 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
             if ((e = cudaMemset(s->d_hist[b][m], 0, histb)) != cudaSuccess) return fail(e);   // zero history == A4 padding
         }
     }
+    s->fused = s->tiny && nslides > 1 && s->M <= 8;
+    for (int i = 0; i < n_models; i++) s->fused = s->fused && gwi_tiny_writes_v(models[i]);
+    if (s->fused) {
+        s->fbits_stride = (s->sub + 31) / 32 + 8;
+        if ((e = cudaMalloc(&s->d_fbits, (size_t)nslides * s->fbits_stride * 4)) != cudaSuccess) return fail(e);
+        if ((e = cudaMemset(s->d_fbits, 0, (size_t)nslides * s->fbits_stride * 4)) != cudaSuccess) return fail(e);
+        if ((e = cudaMalloc(&s->d_fpbar, (size_t)nslides * s->sub * 4)) != cudaSuccess) return fail(e);
+        if ((e = cudaMalloc(&s->d_fmm, (size_t)nslides * s->sub)) != cudaSuccess) return fail(e);
+    }
     if (s->maxlag > 0 && !s->tcs && (e = cudaMalloc(&s->d_tmp, (size_t)(s->nb - 1) * s->S * s->maxlag * 4)) != cudaSuccess) return fail(e);
-    if ((e = cudaMalloc(&s->d_prob, (size_t)nslides * s->M * s->sub * 4)) != cudaSuccess) return fail(e);
+    // (the fused slide path keeps no per-model probabilities; the per-model rule allocates them in gwi_stream_set_rule)
+    if (!s->fused && (e = cudaMalloc(&s->d_prob, (size_t)nslides * s->M * s->sub * 4)) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_carry, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
     if ((e = cudaMemset(s->d_carry, 0, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_carry_pm, (size_t)nslides * s->M * gwi_carry_bytes())) != cudaSuccess) return fail(e);
@@ -600,6 +650,9 @@ extern "C" void gwi_stream_destroy(gwi_stream* s)
     if (s->d_hB) cudaFree(s->d_hB);
     if (s->d_tmp) cudaFree(s->d_tmp);
     if (s->d_prob) cudaFree(s->d_prob);
+    if (s->d_fbits) cudaFree(s->d_fbits);
+    if (s->d_fpbar) cudaFree(s->d_fpbar);
+    if (s->d_fmm) cudaFree(s->d_fmm);
     if (s->d_carry) cudaFree(s->d_carry);
     if (s->d_carry_pm) cudaFree(s->d_carry_pm);
     if (s->d_post_ws) cudaFree(s->d_post_ws);
@@ -880,6 +933,14 @@ extern "C" gwi_status gwi_stream_set_rule(gwi_stream* s, gwi_rule rule)
         return GWI_ERR_ARG;
     }
     s->rule = (int)rule;
+    if (rule == GWI_RULE_PER_MODEL && s->fused && !s->d_prob) {
+        GWI_CUDA_CHECK(cudaSetDevice(s->device));
+        if (cudaMalloc(&s->d_prob, s->lags.size() * s->M * (size_t)s->sub * 4) != cudaSuccess) {
+            cudaGetLastError();
+            gwi_set_error("gwi_stream_set_rule: out of device memory for the per-model probabilities");
+            return GWI_ERR_NOMEM;
+        }
+    }
     return GWI_OK;
 }
 

@@ -424,6 +424,10 @@ bool gwi_tiny_supported(const GwiArch& a)
 
 int gwi_tiny_halo(const gwi_model* m) { return m->tiny ? m->tiny->halo : 0; }
 
+// true: gwi_tiny_stream in time-slide mode writes the half-head pre-activations v (tcgen05 kernel) for gwi_heads_fused;
+// false: it writes the branch features u for gwi_tiny_heads (warp-MMA reference kernel)
+bool gwi_tiny_writes_v(const gwi_model* m) { return m->tiny && m->tinytc && !m->tiny->force_mma_sync; }
+
 gwi_status gwi_tiny_pack(gwi_model* m)
 {
     const GwiArch& a = m->arch;

@@ -69,7 +69,7 @@ struct TtArgs {
     int stash;            // 1: 128-sample tiles with stashed operand rows, 0: tiles of 128 - halo samples with recomputed halo
     int dil[TT_MAX_L];
     float* prob;          // fused head: [n] probabilities (null in time-slide mode)
-    __half* u16;          // time-slide mode: [2][lds][32] branch features, fp16, time-major; row 0 = sample 0 of the chunk
+    __half* u16;          // time-slide mode: [2][lds][32] half-head pre-activations v_b = W1_b u_b (+ b1), fp16, time-major; row 0 = sample 0
     int64_t lds;
     // constant-bank operands
     float lift[2][32];            // W_in[16], b_in[16]
@@ -326,11 +326,30 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
                     u[c] = pack_half2(fmaxf(__uint_as_float(sv[2 * c]), 0.f), fmaxf(__uint_as_float(sv[2 * c + 1]), 0.f));
             }
             if (a.u16) {
+                // ---- time-slide mode: the branch's half of the head's first layer, v_b = W1[:, 32 b : 32 b + 32] u_b (+ b1 for
+                // b = 0).  W1 [u_H; u_L] + b1 = v_H[t] + v_L[t - lag] by linearity, so the per-lag work that follows
+                // (gwi_heads.cu) is element-wise: no contraction per (sample, lag).
+                tmem_st16(tlane + 32, u);
+                tc_wait_st();
+                tc_fence_before();
+                mma_round([&] {
+                    tc_mma_f16_ts(tcol, tcol + 32, dW1 + (uint64_t)(2 * b * 64), idesc32, 0u);
+                    tc_mma_f16_ts(tcol, tcol + 40, dW1 + (uint64_t)((2 * b + 1) * 64), idesc32, 1u);
+                    if (b == 0) tc_mma_f16(tcol, dOnes, dW1 + (uint64_t)(4 * 64), idesc32, 1u);
+                });
+                uint32_t v[32];
+                tmem_ld32(tlane, v);
+                tc_wait_ld();
                 if (store) {
                     uint4* up = reinterpret_cast<uint4*>(a.u16 + ((size_t)b * a.lds + tl) * 32);
 #pragma unroll
-                    for (int c = 0; c < 4; c++) up[c] = make_uint4(u[4 * c], u[4 * c + 1], u[4 * c + 2], u[4 * c + 3]);
+                    for (int c = 0; c < 4; c++)
+                        up[c] = make_uint4(pack_half2(__uint_as_float(v[8 * c]), __uint_as_float(v[8 * c + 1])),
+                                           pack_half2(__uint_as_float(v[8 * c + 2]), __uint_as_float(v[8 * c + 3])),
+                                           pack_half2(__uint_as_float(v[8 * c + 4]), __uint_as_float(v[8 * c + 5])),
+                                           pack_half2(__uint_as_float(v[8 * c + 6]), __uint_as_float(v[8 * c + 7])));
                 }
+                tc_fence_before();
             } else if (b == 0) {
 #pragma unroll
                 for (int c = 0; c < 16; c++) uH[c] = u[c];
