@@ -57,6 +57,13 @@ __device__ __forceinline__ uint32_t mul2h(uint32_t a, uint32_t b)
     asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
     return d;
 }
+// sigmoid(y) = 0.5 + 0.5 tanh(y / 2): one MUFU op (tanh.approx.f32, relative error 2^-11: 2.5e-4 absolute at most on p)
+__device__ __forceinline__ float sigmoid_fast(float y)
+{
+    float t;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(0.5f * y));
+    return fmaf(0.5f, t, 0.5f);
+}
 __device__ __forceinline__ float2 h2f2(uint32_t a)
 {
     __half2 h = *reinterpret_cast<__half2*>(&a);
@@ -97,7 +104,7 @@ __global__ void __launch_bounds__(256) k_heads_fused(const __grid_constant__ Hea
 #pragma unroll
             for (int c = 0; c < 4; c++) h[c] = __ldg(vH + c), l[c] = __ldg(vL + c);
             const float y = head_y(h, l, a.w2[m], a.b2[m]);
-            const float p = __fdividef(1.0f, 1.0f + __expf(-y));
+            const float p = sigmoid_fast(y);
             if (a.prob) {
                 if (live) a.prob[((size_t)k * a.M + m) * a.row_stride + t] = p;
             } else {
@@ -160,6 +167,7 @@ __global__ void __launch_bounds__(COMB_THREADS, 2) k_heads_comb(const __grid_con
     for (int q = 0; q < CKH; q++) sum[q] = 0.f;
 #pragma unroll
     for (int q = 0; q < (CKH + 3) / 4; q++) mk[q] = 0u;
+    for (int e = tid; e < a.M * 16; e += COMB_THREADS) reinterpret_cast<uint32_t*>(smem + 2 * stage_bytes)[e] = a.w2[e >> 4][e & 15];
     stage_load(0, 0);
     for (int m = 0; m < a.M; m++) {
         if (m + 1 < a.M) {
@@ -175,22 +183,31 @@ __global__ void __launch_bounds__(COMB_THREADS, 2) k_heads_comb(const __grid_con
 #pragma unroll
             for (int cc = 0; cc < 4; cc++) h[cc] = __ldg(vH + cc);
         }
-        const uint32_t st0 = sbase + (m & 1) * stage_bytes + row * 16;
+        // W2 of this model as broadcast shared-memory loads; the address of the thread's row in the block of lag k = 2 q + kh
+        // is sa0 - 2048 q (immediate offsets once the q loop is unrolled).  Lags past the list (k >= K, one of 34 at most)
+        // are evaluated on block 0 and dropped at the end: no branch in the loop.
+        const uint32_t sw = sbase + 2 * stage_bytes + m * 64;
+        const uint32_t sa0 = sbase + (m & 1) * stage_bytes + row * 16 + (uint32_t)(j - kh + K - 1) * 1024;
         const float b2 = a.b2[m];
 #pragma unroll
         for (int q = 0; q < CKH; q++) {
-            const int k = 2 * q + kh;
-            if (k < K) {
-                const uint32_t sa = st0 + (uint32_t)(j - k + K - 1) * 1024;
-                uint4 l[4];
+            const uint32_t sa = (2 * q + kh < K) ? sa0 - 2048u * q : sbase + (m & 1) * stage_bytes + row * 16;
+            float y = b2;
 #pragma unroll
-                for (int cc = 0; cc < 4; cc++)
-                    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(l[cc].x), "=r"(l[cc].y), "=r"(l[cc].z), "=r"(l[cc].w) : "r"(sa + cc * 256));
-                const float y = head_y(h, l, a.w2[m], b2);
-                const float p = __fdividef(1.0f, 1.0f + __expf(-y));
-                sum[q] = m == 0 ? p : __fadd_rn(sum[q], p);
-                mk[q >> 2] |= (uint32_t)(p > a.theta) << (8 * (q & 3) + m);
+            for (int cc = 0; cc < 4; cc++) {
+                uint4 l, w;
+                asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(l.x), "=r"(l.y), "=r"(l.z), "=r"(l.w) : "r"(sa + cc * 256));
+                asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(sw + cc * 16));
+                uint32_t acc = mul2h(add_relu2(l.x, h[cc].x), w.x);
+                acc = fma2h(add_relu2(l.y, h[cc].y), w.y, acc);
+                acc = fma2h(add_relu2(l.z, h[cc].z), w.z, acc);
+                acc = fma2h(add_relu2(l.w, h[cc].w), w.w, acc);
+                const float2 f = h2f2(acc);
+                y += f.x + f.y;
             }
+            const float p = sigmoid_fast(y);
+            sum[q] = __fadd_rn(sum[q], p);                               // 0 + p0 = p0 exactly: the T1 expression
+            if (p > a.theta) mk[q >> 2] |= 1u << (8 * (q & 3) + m);
         }
         __syncthreads();                                                // the stage is refilled two models later
     }
@@ -249,10 +266,10 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
     }
     if (comb) {
         const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
-        const size_t smem = (size_t)2 * (CJ + n_lags - 1) * 1024;
+        const size_t smem = (size_t)2 * (CJ + n_lags - 1) * 1024 + HF_MAX_M * 64;
         static bool attr = false;
         if (!attr) {
-            GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_comb, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (CJ + CK_MAX - 1) * 1024));
+            GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_comb, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (CJ + CK_MAX - 1) * 1024 + HF_MAX_M * 64));
             attr = true;
         }
         k_heads_comb<<<(unsigned)(groups * (G / 16)), COMB_THREADS, smem, st>>>(a, n_lags, G);
