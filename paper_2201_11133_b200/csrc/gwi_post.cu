@@ -151,6 +151,7 @@ __global__ void k_runs(const uint32_t* __restrict__ bits, const uint8_t* __restr
                        int64_t shard_begin, int64_t shard_end)
 {
     __shared__ uint32_t wsum[RT / 32];
+    if (MODE == 1 && blkcnt[blockIdx.x] == 0) return;   // the counting pass found no qualifying run in this CTA's words
     const int64_t i = (int64_t)blockIdx.x * RT + threadIdx.x;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     uint32_t cnt = 0;
@@ -372,7 +373,7 @@ static gwi_status post_from_bits(const Ptrs& P, int n_models, const uint8_t* d_m
     k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append);
     k_runs<1><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
                                              d_triggers, capacity, shard_begin, shard_end);
-    int sgrid = capacity < 1024 ? capacity + 1 : 1025;
+    int sgrid = capacity < 128 ? capacity + 1 : 129;   // records are few: 128 CTAs loop over them, the last one writes the carry
     k_stats<<<sgrid, 256, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry, shard_begin, shard_end, d_mm);
     gwi_count_launch(6);
     GWI_CUDA_CHECK(cudaGetLastError());
