@@ -131,13 +131,16 @@ gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t n_models, i
  *   carried across chunk boundaries; records sorted by (slide, start).  Pushing the stream in chunks of any sizes
  *   gives bit-identical results to pushing it whole (reading A17).
  *
- * Back ends (chosen at create, same results contract): FP16-mode ensembles of the narrow config-1 architecture run on a
- * fused kernel; FP16-mode paper-scale models run on the tcgen05 kernel over segments with recomputed warm-up (with
- * slides when the lags and n_total are multiples of 128 samples and n_total >= max lag + R_f - 1); everything else
- * (FP32 mode, other architectures) runs on the generic kernels.
+ * Back ends (chosen at create, same results contract; gwi_stream_backend tells which): FP16-mode ensembles of the narrow
+ * config-1 architecture run on a fused tcgen05 kernel (with slides: the head's first layer is split by linearity into
+ * per-sample halves, and every (sample, lag, model) is evaluated element-wise, fused with the mean and the threshold -- no
+ * per-lag probability array exists unless d_pbar or the per-model rule asks for one); FP16-mode paper-scale models run on
+ * the tcgen05 kernel over segments with recomputed warm-up (with slides when the lags and n_total are multiples of 128
+ * samples and n_total >= max lag + R_f - 1); everything else (FP32 mode, other architectures) runs on the generic kernels.
  *
  * gwi_stream_create   models: HOST array of n_models loaded models sharing device, precision and architecture
- *                     (1..16).  lags: HOST array of n_lags lags in SAMPLES, each in [1, n_total) (n_lags = 0: zero lag
+ *                     (1..16).  lags: HOST array of n_lags lags in SAMPLES, each >= 1; a lag >= n_total wraps (lag mod n_total: the slides are
+ *                     circular, so a multiple of n_total is the zero lag again) (n_lags = 0: zero lag
  *                     only; slides need a two-branch model).  max_chunk: largest n a push will carry.  capacity:
  *                     records the stream can hold.  d_pbar: NULL, or a DEVICE array [1 + n_lags][n_total] float that
  *                     receives pbar_j (for parity tests; ~4 B x n_total per slide).  The handle owns all its device

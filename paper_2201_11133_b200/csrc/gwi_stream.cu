@@ -11,10 +11,12 @@
 //   a-8..a-10  per slide: ensemble mean, strict threshold, run clustering with the run carried across chunks
 //   a-11 trigger records copied to the host at finish, sorted by (slide, start)
 //
-// Two back ends: the fused narrow-architecture kernel (gwi_tiny.cu; FP16 mode, config-1 widths: the ensembles of
-// BASELINE.json configs 3-5), and the generic CUDA-core kernels (gwi_generic.cu) for every other architecture and for
-// FP32 mode.  In both, each output sample is an independent fixed-order computation, which is what makes
-// chunked == unchunked exact.
+// Back ends (gwi_stream_backend): the fused narrow-architecture kernel (gwi_tiny_tc.cu; FP16 mode, config-1 widths: the
+// ensembles of BASELINE.json configs 3-5; with slides followed by the fused element-wise heads of gwi_heads.cu), the
+// tcgen05 kernel for paper-scale models over segments with recomputed warm-up (gwi_tc.cu; zero lag, or with slides on the
+// 128-sample tile grid), and the generic CUDA-core kernels (gwi_generic.cu) for every other architecture and for FP32
+// mode.  In all of them each output sample is an independent fixed-order computation, which is what makes
+// chunked == unchunked exact.  Time-shard mode (gwi_stream_set_shard) runs one rank's span of a longer stream.
 #include <algorithm>
 #include <new>
 #include <vector>
