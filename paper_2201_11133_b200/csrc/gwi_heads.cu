@@ -23,7 +23,7 @@ namespace {
 constexpr int HF_MAX_M = 8;
 
 struct HeadsFusedArgs {
-    const __half* v[HF_MAX_M];   // per model: row 0 of this chunk inside its [2][lds][32] fp16 buffer (v_H rows, then v_L rows)
+    const __half* v[HF_MAX_M];   // per model: row 0 of this chunk inside its [2][lds][CH] fp16 buffer (v_H rows, then v_L rows)
     int64_t lds;
     int n, M, n_lags;
     const int64_t* lags;         // device, lags[0] = 0
@@ -34,7 +34,7 @@ struct HeadsFusedArgs {
     uint8_t* mm;                 // [n_lags][row_stride]: bit j = model j alone above the threshold
     int64_t row_stride;
     float* prob;                 // per-model rule: [n_lags][M][row_stride] probabilities instead of the three above (else null)
-    uint32_t w2[HF_MAX_M][16];   // W2 as half2 pairs (channels 2c, 2c + 1)
+    uint32_t w2[HF_MAX_M][64];   // W2 as half2 pairs (channels 2c, 2c + 1), CH / 2 of them used
     float b2[HF_MAX_M];
 };
 
@@ -70,24 +70,31 @@ __device__ __forceinline__ float2 h2f2(uint32_t a)
     return __half22float2(h);
 }
 
-// y = b2 + W2 . relu(vh + vl): four half2 accumulators of four products each, combined in fp32
-__device__ __forceinline__ float head_y(const uint4 (&vh)[4], const uint4 (&vl)[4], const uint32_t (&w2)[16], float b2)
+__device__ __forceinline__ uint4 lds128(uint32_t addr)
 {
-    float y = b2;
-#pragma unroll
-    for (int c = 0; c < 4; c++) {
-        uint32_t acc = mul2h(add_relu2(vl[c].x, vh[c].x), w2[4 * c]);
-        acc = fma2h(add_relu2(vl[c].y, vh[c].y), w2[4 * c + 1], acc);
-        acc = fma2h(add_relu2(vl[c].z, vh[c].z), w2[4 * c + 2], acc);
-        acc = fma2h(add_relu2(vl[c].w, vh[c].w), w2[4 * c + 3], acc);
-        const float2 f = h2f2(acc);
-        y += f.x + f.y;
-    }
-    return y;
+    uint4 v;
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+// contribution of 8 channels (one 16-byte chunk of v_H, v_L and W2) to y: one half2 accumulator of four products, to fp32
+__device__ __forceinline__ float chunk_y(uint4 h, uint4 l, uint4 w)
+{
+    uint32_t acc = mul2h(add_relu2(l.x, h.x), w.x);
+    acc = fma2h(add_relu2(l.y, h.y), w.y, acc);
+    acc = fma2h(add_relu2(l.z, h.z), w.z, acc);
+    acc = fma2h(add_relu2(l.w, h.w), w.w, acc);
+    const float2 f = h2f2(acc);
+    return f.x + f.y;
 }
 
+// ---- any lag list: one thread per sample, the lagged row of every evaluation comes from global memory / L2 ---------------
+template <int CH>
 __global__ void __launch_bounds__(256) k_heads_fused(const __grid_constant__ HeadsFusedArgs a)
 {
+    constexpr int CHC = CH / 8;                                          // 16-byte chunks per row
+    __shared__ uint4 sw[HF_MAX_M * CHC];
+    for (int e = threadIdx.x; e < a.M * CHC * 4; e += 256) reinterpret_cast<uint32_t*>(sw)[e] = a.w2[e / (CHC * 4)][e % (CHC * 4)];
+    __syncthreads();
     const int64_t t = (int64_t)blockIdx.x * 256 + threadIdx.x;
     const bool live = t < a.n;
     const int64_t tc = live ? t : a.n - 1;                            // clamp the loads of the ragged tail
@@ -98,17 +105,16 @@ __global__ void __launch_bounds__(256) k_heads_fused(const __grid_constant__ Hea
         float s = 0.f;
         uint32_t mk = 0;
         for (int m = 0; m < a.M; m++) {
-            const uint4* vH = reinterpret_cast<const uint4*>(a.v[m]) + tc * 4;
-            const uint4* vL = reinterpret_cast<const uint4*>(a.v[m] + a.lds * 32) + (tc - lag) * 4;
-            uint4 h[4], l[4];
-#pragma unroll
-            for (int c = 0; c < 4; c++) h[c] = __ldg(vH + c), l[c] = __ldg(vL + c);
-            const float y = head_y(h, l, a.w2[m], a.b2[m]);
+            const uint4* vH = reinterpret_cast<const uint4*>(a.v[m]) + tc * CHC;
+            const uint4* vL = reinterpret_cast<const uint4*>(a.v[m] + a.lds * CH) + (tc - lag) * CHC;
+            float y = a.b2[m];
+#pragma unroll 4
+            for (int c = 0; c < CHC; c++) y += chunk_y(__ldg(vH + c), __ldg(vL + c), sw[m * CHC + c]);
             const float p = sigmoid_fast(y);
             if (a.prob) {
                 if (live) a.prob[((size_t)k * a.M + m) * a.row_stride + t] = p;
             } else {
-                s = m == 0 ? p : __fadd_rn(s, p);
+                s = __fadd_rn(s, p);                                  // 0 + p0 = p0 exactly: the T1 expression
                 mk |= (uint32_t)(p > a.theta) << m;
             }
         }
@@ -124,104 +130,103 @@ __global__ void __launch_bounds__(256) k_heads_fused(const __grid_constant__ Hea
 }
 
 // ---- regular lag lists (lag_k = k G, BASELINE.json configs[3]: k x 1 s): the "comb" schedule ------------------------------
-// A lagged L1 row s is used by every (t, k) with t - k G = s.  A CTA therefore takes a comb of CJ blocks of 16 samples G
-// apart, t = (c CJ + j) G + 16 r + [0, 16), j < CJ: for all K lags it needs only the CJ + K - 1 blocks of v_L rows at
-// (c CJ + i) G + 16 r, -K < i < CJ, which it stages in shared memory once per model (double-buffered over the models, the
-// next model's blocks arrive by cp.async while this one is evaluated): 48 KB feed 8448 evaluations, 8 x fewer bytes from L2
-// than one row per evaluation.  512 threads = 16 rows x CJ blocks x 2 interleaved halves of the lag list; a thread keeps
-// the running sums of its <= 17 lags in registers across the models (fixed order m = 0, 1, ...: the T1 expression).
-constexpr int CJ = 16, CK_MAX = 34, CKH = CK_MAX / 2;
-constexpr int COMB_THREADS = 512;
+// A lagged L1 row s is used by every (t, k) with t - k G = s.  A CTA therefore takes a comb of CJ blocks of T samples G
+// apart, t = (c CJ + j) G + T r + [0, T), j < CJ: for all K lags it needs only the CJ + K - 1 blocks of v_L rows at
+// (c CJ + i) G + T r, -K < i < CJ, which it stages in shared memory once per model: with T = 16 rows of 32 channels, 48 KB
+// feed 8448 evaluations, 8 x fewer bytes from L2 than one row per evaluation (double-buffered over the models: the next
+// model's blocks arrive by cp.async while this one is evaluated); with T = 8 rows of 128 channels (paper-scale models,
+// up to 64 slides) CJ = 8 and one 136 KB stage.  Threads = T rows x CJ blocks x NG interleaved groups of the lag list; a thread
+// keeps the running sums of its <= KQ lags in registers across the models (fixed order m = 0, 1, ...: the T1 expression).
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src)
 {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
 
-__global__ void __launch_bounds__(COMB_THREADS, 2) k_heads_comb(const __grid_constant__ HeadsFusedArgs a, const int K, const int64_t G)
+template <int CH, int T, int CJ, int NG, int KQ, int NBUF, int MINB>
+__global__ void __launch_bounds__(T * CJ * NG, MINB) k_heads_comb(const __grid_constant__ HeadsFusedArgs a, const int K, const int64_t G)
 {
+    constexpr int CHC = CH / 8, BLK = T * CHC * 16, NTHR = T * CJ * NG;
     extern __shared__ __align__(128) uint8_t smem[];
     const int nblk = CJ + K - 1;                                        // staged v_L blocks per model
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
-    const uint32_t stage_bytes = (uint32_t)nblk * 1024;
-    const int tid = threadIdx.x, row = tid & 15, j = (tid >> 4) & (CJ - 1), kh = tid >> 8;
-    const int64_t G16 = G >> 4;
-    const int64_t c = blockIdx.x / G16, r = blockIdx.x % G16;
-    const int64_t t = (c * CJ + j) * G + 16 * r + row;                  // this thread's sample
+    const uint32_t stage_bytes = (uint32_t)nblk * BLK;
+    const int tid = threadIdx.x, row = tid % T, j = (tid / T) % CJ, kg = tid / (T * CJ);
+    const int64_t GT = G / T;
+    const int64_t c = blockIdx.x / GT, r = blockIdx.x % GT;
+    const int64_t t = (c * CJ + j) * G + T * r + row;                   // this thread's sample
     const bool live = t < a.n;
     const int64_t tc = live ? t : a.n - 1;
     const int64_t lo_row = -(int64_t)(K - 1) * G;                       // oldest ring row
     auto stage_load = [&](int m, int buf) {
-        const __half* vL = a.v[m] + a.lds * 32;
-        for (int e = tid; e < nblk * 64; e += COMB_THREADS) {           // (block i, row rr, chunk cc)
-            const int i = e >> 6, rr = (e >> 2) & 15, cc = e & 3;
-            int64_t s = (c * CJ + i - (K - 1)) * G + 16 * r + rr;
+        const __half* vL = a.v[m] + a.lds * CH;
+        for (int e = tid; e < nblk * T * CHC; e += NTHR) {              // (block i, row rr, chunk cc)
+            const int i = e / (T * CHC), rr = (e / CHC) % T, cc = e % CHC;
+            int64_t s = (c * CJ + i - (K - 1)) * G + T * r + rr;
             s = s < lo_row ? lo_row : (s > a.n - 1 ? a.n - 1 : s);
-            cp_async16(sbase + buf * stage_bytes + i * 1024 + cc * 256 + rr * 16, vL + s * 32 + cc * 8);
+            cp_async16(sbase + buf * stage_bytes + i * BLK + cc * (T * 16) + rr * 16, vL + s * CH + cc * 8);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    float sum[CKH];
-    uint32_t mk[(CKH + 3) / 4];
+    float sum[KQ];
+    uint32_t mk[(KQ + 3) / 4];
 #pragma unroll
-    for (int q = 0; q < CKH; q++) sum[q] = 0.f;
+    for (int q = 0; q < KQ; q++) sum[q] = 0.f;
 #pragma unroll
-    for (int q = 0; q < (CKH + 3) / 4; q++) mk[q] = 0u;
-    for (int e = tid; e < a.M * 16; e += COMB_THREADS) reinterpret_cast<uint32_t*>(smem + 2 * stage_bytes)[e] = a.w2[e >> 4][e & 15];
+    for (int q = 0; q < (KQ + 3) / 4; q++) mk[q] = 0u;
+    const uint32_t swb = sbase + NBUF * stage_bytes;                     // W2 of all models, CH / 2 words each
+    for (int e = tid; e < a.M * CHC * 4; e += NTHR) reinterpret_cast<uint32_t*>(smem + NBUF * stage_bytes)[e] = a.w2[e / (CHC * 4)][e % (CHC * 4)];
     stage_load(0, 0);
     for (int m = 0; m < a.M; m++) {
-        if (m + 1 < a.M) {
+        if (NBUF == 2 && m + 1 < a.M) {
             stage_load(m + 1, (m + 1) & 1);
             asm volatile("cp.async.wait_group 1;" ::: "memory");
         } else {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
         __syncthreads();
-        uint4 h[4];
+        uint4 h[CHC];
         {
-            const uint4* vH = reinterpret_cast<const uint4*>(a.v[m]) + tc * 4;
+            const uint4* vH = reinterpret_cast<const uint4*>(a.v[m]) + tc * CHC;
 #pragma unroll
-            for (int cc = 0; cc < 4; cc++) h[cc] = __ldg(vH + cc);
+            for (int cc = 0; cc < CHC; cc++) h[cc] = __ldg(vH + cc);
         }
-        // W2 of this model as broadcast shared-memory loads; the address of the thread's row in the block of lag k = 2 q + kh
-        // is sa0 - 2048 q (immediate offsets once the q loop is unrolled).  Lags past the list (k >= K, one of 34 at most)
-        // are evaluated on block 0 and dropped at the end: no branch in the loop.
-        const uint32_t sw = sbase + 2 * stage_bytes + m * 64;
-        const uint32_t sa0 = sbase + (m & 1) * stage_bytes + row * 16 + (uint32_t)(j - kh + K - 1) * 1024;
+        // W2 of this model as broadcast shared-memory loads; the address of the thread's row in the block of lag
+        // k = NG q + kg is sa0 - NG BLK q (immediate offsets once the q loop is unrolled).  Lags past the list (k >= K) are
+        // evaluated on block 0 and dropped at the end: no branch in the loop.
+        const uint32_t sw = swb + m * (CHC * 16);
+        const uint32_t st0 = sbase + (NBUF == 2 ? (m & 1) : 0) * stage_bytes + row * 16;
+        const uint32_t sa0 = st0 + (uint32_t)(j - kg + K - 1) * BLK;
         const float b2 = a.b2[m];
 #pragma unroll
-        for (int q = 0; q < CKH; q++) {
-            const uint32_t sa = (2 * q + kh < K) ? sa0 - 2048u * q : sbase + (m & 1) * stage_bytes + row * 16;
+        for (int q = 0; q < KQ; q++) {
+            const uint32_t sa = (NG * q + kg < K) ? sa0 - (uint32_t)(NG * BLK) * q : st0;
             float y = b2;
 #pragma unroll
-            for (int cc = 0; cc < 4; cc++) {
-                uint4 l, w;
-                asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(l.x), "=r"(l.y), "=r"(l.z), "=r"(l.w) : "r"(sa + cc * 256));
-                asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(sw + cc * 16));
-                uint32_t acc = mul2h(add_relu2(l.x, h[cc].x), w.x);
-                acc = fma2h(add_relu2(l.y, h[cc].y), w.y, acc);
-                acc = fma2h(add_relu2(l.z, h[cc].z), w.z, acc);
-                acc = fma2h(add_relu2(l.w, h[cc].w), w.w, acc);
-                const float2 f = h2f2(acc);
-                y += f.x + f.y;
-            }
+            for (int cc = 0; cc < CHC; cc++) y += chunk_y(h[cc], lds128(sa + cc * (T * 16)), lds128(sw + cc * 16));
             const float p = sigmoid_fast(y);
             sum[q] = __fadd_rn(sum[q], p);                               // 0 + p0 = p0 exactly: the T1 expression
             if (p > a.theta) mk[q >> 2] |= 1u << (8 * (q & 3) + m);
         }
-        __syncthreads();                                                // the stage is refilled two models later
+        __syncthreads();                                                // the stage is refilled by a later model
+        if (NBUF == 1 && m + 1 < a.M) stage_load(m + 1, 0);
     }
     const float fM = (float)a.M;
     const int lane = tid & 31;
-    const int64_t blk16 = t >> 4;                                        // 16-sample block of this thread (same for its 16 rows)
 #pragma unroll
-    for (int q = 0; q < CKH; q++) {
-        const int k = 2 * q + kh;
-        if (k < K) {                                                     // warp-uniform (kh is)
+    for (int q = 0; q < KQ; q++) {
+        const int k = NG * q + kg;
+        if (k < K) {                                                     // warp-uniform (kg is)
             const float pb = __fdiv_rn(sum[q], fM);
             const uint32_t w = __ballot_sync(0xffffffffu, live && pb > a.theta);
-            if ((lane & 15) == 0 && blk16 < 2 * a.bits_stride)
-                reinterpret_cast<uint16_t*>(a.bits + (size_t)k * a.bits_stride)[blk16] = (uint16_t)(w >> (lane & 16));
+            // the warp holds 32 / T blocks of T samples: each writes its T mask bits
+            if ((lane % T) == 0) {
+                if (T == 16) {
+                    if ((t >> 4) < 2 * a.bits_stride) reinterpret_cast<uint16_t*>(a.bits + (size_t)k * a.bits_stride)[t >> 4] = (uint16_t)(w >> (lane & 16));
+                } else {
+                    if ((t >> 3) < 4 * a.bits_stride) reinterpret_cast<uint8_t*>(a.bits + (size_t)k * a.bits_stride)[t >> 3] = (uint8_t)(w >> (lane & 24));
+                }
+            }
             if (live) {
                 a.pbar[(size_t)k * a.row_stride + t] = pb;
                 a.mm[(size_t)k * a.row_stride + t] = (uint8_t)(mk[q >> 2] >> (8 * (q & 3)));
@@ -232,20 +237,23 @@ __global__ void __launch_bounds__(COMB_THREADS, 2) k_heads_comb(const __grid_con
 
 } // namespace
 
-// packs W2 / b2 of the models and launches; d_v[m] = row 0 of the chunk inside model m's [2][lds][32] buffer
+// packs W2 / b2 of the models and launches; d_v[m] = row 0 of the chunk inside model m's [2][lds][CH] buffer, CH = Hh = 32
+// (narrow architecture) or 128 (paper scale)
 gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* const* d_v, int64_t lds, int n, const int64_t* d_lags,
                            int n_lags, const int64_t* h_lags, float theta, uint32_t* d_bits, int64_t bits_stride, float* d_pbar,
                            uint8_t* d_mm, int64_t row_stride, float* d_prob, cudaStream_t st)
 {
-    if (M < 1 || M > HF_MAX_M) {
-        gwi_set_error("gwi_heads_fused: 1..%d models", HF_MAX_M);
+    const int CH = models[0]->arch.Hh;
+    if (M < 1 || M > HF_MAX_M || (CH != 32 && CH != 128)) {
+        gwi_set_error("gwi_heads_fused: 1..%d models with 32 or 128 head channels", HF_MAX_M);
         return GWI_ERR_UNSUPPORTED;
     }
     HeadsFusedArgs a;
+    memset(a.w2, 0, sizeof(a.w2));
     for (int m = 0; m < M; m++) {
         a.v[m] = d_v[m];
         const float* W = models[m]->host_blob.data();
-        for (int c = 0; c < 16; c++) {
+        for (int c = 0; c < CH / 2; c++) {
             __half lo = __float2half_rn(W[models[m]->off.W2 + 2 * c]), hi = __float2half_rn(W[models[m]->off.W2 + 2 * c + 1]);
             uint16_t ul, uh;
             memcpy(&ul, &lo, 2), memcpy(&uh, &hi, 2);
@@ -255,26 +263,41 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
     }
     a.lds = lds, a.n = n, a.M = M, a.n_lags = n_lags, a.lags = d_lags, a.theta = theta;
     a.bits = d_bits, a.bits_stride = bits_stride, a.pbar = d_pbar, a.mm = d_mm, a.row_stride = row_stride, a.prob = d_prob;
-    // regular lag list k G (G a multiple of 16, at most CK_MAX slides, mean rule): the comb schedule
-    std::vector<int64_t> hl((size_t)n_lags);
-    bool comb = !d_prob && n_lags >= 2 && n_lags <= CK_MAX && h_lags != nullptr;
+    // regular lag list k G (G a multiple of 16, mean rule): the comb schedule (<= 34 slides of 32 channels, <= 64 of 128)
+    const int kmax = CH == 32 ? 34 : 64;
+    bool comb = !d_prob && n_lags >= 2 && n_lags <= kmax && h_lags != nullptr;
     int64_t G = 0;
     if (comb) {
         G = h_lags[1];
         comb = G > 0 && G % 16 == 0;
         for (int k = 0; k < n_lags && comb; k++) comb = h_lags[k] == (int64_t)k * G;
     }
-    if (comb) {
+    if (comb && CH == 32) {
+        constexpr int CJ = 16;
+        auto kern = k_heads_comb<32, 16, CJ, 2, 17, 2, 2>;
         const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
         const size_t smem = (size_t)2 * (CJ + n_lags - 1) * 1024 + HF_MAX_M * 64;
         static bool attr = false;
         if (!attr) {
-            GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_comb, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (CJ + CK_MAX - 1) * 1024 + HF_MAX_M * 64));
+            GWI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (CJ + 34 - 1) * 1024 + HF_MAX_M * 64));
             attr = true;
         }
-        k_heads_comb<<<(unsigned)(groups * (G / 16)), COMB_THREADS, smem, st>>>(a, n_lags, G);
+        kern<<<(unsigned)(groups * (G / 16)), 512, smem, st>>>(a, n_lags, G);
+    } else if (comb) {
+        constexpr int CJ = 8;
+        auto kern = k_heads_comb<128, 8, CJ, 4, 16, 1, 1>;
+        const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
+        const size_t smem = (size_t)(CJ + n_lags - 1) * 2048 + HF_MAX_M * 256;
+        static bool attr = false;
+        if (!attr) {
+            GWI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (CJ + 64 - 1) * 2048 + HF_MAX_M * 256));
+            attr = true;
+        }
+        kern<<<(unsigned)(groups * (G / 8)), 256, smem, st>>>(a, n_lags, G);
+    } else if (CH == 32) {
+        k_heads_fused<32><<<(n + 255) / 256, 256, 0, st>>>(a);
     } else {
-        k_heads_fused<<<(n + 255) / 256, 256, 0, st>>>(a);
+        k_heads_fused<128><<<(n + 255) / 256, 256, 0, st>>>(a);
     }
     gwi_count_launch(1);
     GWI_CUDA_CHECK(cudaGetLastError());
