@@ -11,12 +11,14 @@
 // compares with the threshold and writes, per slide, the bit mask the run clustering works on, pbar (the statistics of
 // the few triggers are taken from it) and one byte per sample saying which models exceeded the threshold on their own --
 // no per-model, per-slide probability array exists (it was 7.8 GB per hour of data at 33 slides and 4 models).
+#include <algorithm>
 #include <cstring>
 #include <vector>
 
 #include <cuda_fp16.h>
 
 #include "gwi_internal.h"
+#include "gwi_tc_ptx.h"
 
 namespace {
 
@@ -235,6 +237,166 @@ __global__ void __launch_bounds__(T * CJ * NG, MINB) k_heads_comb(const __grid_c
     }
 }
 
+// ---- the comb schedule for 128-channel rows (paper-scale models, up to 64 slides) ---------------------------------------
+// The work is cut along the diagonals: a staged v_L block i serves every item (j, k) with j - k = i - (K - 1), so a warp =
+// 8 rows x 4 channel quarters keeps the v_H quarter rows of JB = 4 neighbouring comb blocks in registers, walks the staged
+// blocks (i = slot, slot + 8, ...) and evaluates up to four items per 64 bytes read from shared memory.  The quarter sums
+// of the four items are reduced across the four lanes with a transposing butterfly (3 shuffles) that leaves item jj on
+// the lane of quarter jj, which adds its sigmoid to the running sum of the item in shared memory (each item belongs to
+// one lane for all models: the T1 expression in model order, no atomics).
+//
+// Persistent CTAs (one per SM) walk the work items (comb group c fastest, so that the CTAs running at the same time
+// share their v_L rows in L2; then the lag pass; then the row group r); one step = one model of one item.  The rows of a
+// step (v_L blocks and the CJ v_H blocks) are fetched with 16-byte cp.async copies into one of two stages while the
+// step before is evaluated (256-byte bulk copies, one per row, ran at a third of this: the copy engine's cost per
+// request); rows sit 272 bytes apart, which makes the quarter-warp's 16-byte reads of eight neighbouring rows
+// conflict-free.  Lag lists longer than 33 are evaluated in passes of at most 33 lags, so that
+// two stages always fit.
+constexpr int C128_THREADS = 512, C128_KS_MAX = 33;
+constexpr int C128_ROWB = 272, C128_BLKB = 8 * C128_ROWB;
+
+__host__ __device__ constexpr size_t c128_smem_bytes(int KS)
+{
+    return (size_t)2 * (8 + KS - 1 + 8) * C128_BLKB + (size_t)8 * KS * 8 * 5 + HF_MAX_M * 256 + 16;
+}
+
+__global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_constant__ HeadsFusedArgs a, const int K, const int KS,
+                                                                  const int npass, const int64_t G, const int64_t groups,
+                                                                  const int64_t nitems)
+{
+    using namespace tc;
+    constexpr int T = 8, CJ = 8, JB = 4, NS = 8, CH = 128, ROWB = C128_ROWB, BLKB = C128_BLKB;
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int nblk_max = CJ + KS - 1;
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t stage_bytes = (uint32_t)(nblk_max + CJ) * BLKB;
+    const int nsum = CJ * KS * T;
+    float* sums = reinterpret_cast<float*>(smem + 2 * (size_t)stage_bytes);             // [j][k'][row]
+    uint8_t* smm = reinterpret_cast<uint8_t*>(sums + nsum);                             // same order
+    const uint32_t w2off = 2 * stage_bytes + nsum * 5;                                  // W2 of all models, 256 B each
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int q = lane >> 3, row = lane & 7, j0 = (warp & 1) * JB, slot = warp >> 1;
+    const int64_t lo_row = -(int64_t)(K - 1) * G;
+    for (int e = tid; e < nsum; e += C128_THREADS) sums[e] = 0.f, smm[e] = 0;
+    for (int e = tid; e < a.M * 64; e += C128_THREADS) reinterpret_cast<uint32_t*>(smem + w2off)[e] = a.w2[e >> 6][e & 63];
+    __syncthreads();
+
+    auto decode = [&](int64_t wi, int64_t& c, int64_t& r, int& ka, int& Kp) {
+        c = wi % groups;
+        const int64_t x = wi / groups;
+        const int p = (int)(x % npass);
+        r = x / npass;
+        ka = p * KS, Kp = min(KS, K - ka);
+    };
+    // all warps: the rows of model m of item wi into stage buf, 16 bytes per cp.async (a block = 8 rows = 2 KB contiguous in
+    // global memory = four warp-wide copies); one commit group per step
+    auto stage_load = [&](int64_t wi, int m, int buf) {
+        int64_t c, r;
+        int ka, Kp;
+        decode(wi, c, r, ka, Kp);
+        const int nblk = CJ + Kp - 1;
+        const __half* vH = a.v[m];
+        const __half* vL = a.v[m] + a.lds * CH;
+        const int ch = lane & 15, r0 = lane >> 4;
+        for (int blk = warp; blk < nblk + CJ; blk += C128_THREADS / 32) {
+            const bool isL = blk < nblk;
+            const int64_t s0 = isL ? (c * CJ + blk - (Kp - 1) - ka) * G + T * r : (c * CJ + (blk - nblk)) * G + T * r;
+            const int64_t lo = isL ? lo_row : 0;
+            const __half* base = (isL ? vL : vH) + ch * 8;
+            const uint32_t dst = sbase + buf * stage_bytes + (isL ? blk : nblk_max + blk - nblk) * BLKB + ch * 16;
+#pragma unroll
+            for (int x = 0; x < 4; x++) {
+                const int rr = r0 + 2 * x;
+                int64_t sr = s0 + rr;
+                sr = sr < lo ? lo : (sr > a.n - 1 ? a.n - 1 : sr);
+                cp_async16(dst + rr * ROWB, base + sr * CH);
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    int64_t wi = blockIdx.x;
+    int m = 0;
+    uint32_t step = 0;
+    if (wi < nitems) stage_load(wi, 0, 0);
+    while (wi < nitems) {
+        int64_t wn = wi;
+        int mn = m + 1;
+        if (mn == a.M) mn = 0, wn = wi + gridDim.x;
+        const int buf = step & 1;
+        if (wn < nitems) {
+            stage_load(wn, mn, buf ^ 1);                                // stage buf ^ 1 was released by the barrier below
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        __syncthreads();
+        int64_t c, r;
+        int ka, Kp;
+        decode(wi, c, r, ka, Kp);
+        const int nblk = CJ + Kp - 1;
+        const uint32_t bb = sbase + buf * stage_bytes + row * ROWB + q * 64;
+        uint4 h[JB][4], w[4];
+#pragma unroll
+        for (int jj = 0; jj < JB; jj++)
+#pragma unroll
+            for (int cc = 0; cc < 4; cc++) h[jj][cc] = lds128(bb + (nblk_max + j0 + jj) * BLKB + cc * 16);
+#pragma unroll
+        for (int cc = 0; cc < 4; cc++) w[cc] = lds128(sbase + w2off + m * 256 + q * 64 + cc * 16);
+        const float b2 = a.b2[m];
+        for (int i = slot; i < nblk; i += NS) {
+            uint4 l[4];
+#pragma unroll
+            for (int cc = 0; cc < 4; cc++) l[cc] = lds128(bb + i * BLKB + cc * 16);
+            const int kb = j0 - i + Kp - 1;                             // lag (within the pass) of item jj = kb + jj
+            float y[JB];
+#pragma unroll
+            for (int jj = 0; jj < JB; jj++) {
+                y[jj] = 0.f;
+                if (kb + jj >= 0 && kb + jj < Kp) {                     // warp-uniform
+#pragma unroll
+                    for (int cc = 0; cc < 4; cc++) y[jj] += chunk_y(h[jj][cc], l[cc], w[cc]);
+                }
+            }
+            // transposing butterfly over the four quarters: the lane of quarter jj ends with the whole sum of item jj
+            const bool hi = q & 2, od = q & 1;
+            float k0 = hi ? y[2] : y[0], k1 = hi ? y[3] : y[1];
+            k0 += __shfl_xor_sync(0xffffffffu, hi ? y[0] : y[2], 16);
+            k1 += __shfl_xor_sync(0xffffffffu, hi ? y[1] : y[3], 16);
+            float yy = od ? k1 : k0;
+            yy += __shfl_xor_sync(0xffffffffu, od ? k0 : k1, 8);
+            const int k = kb + q;
+            if (k >= 0 && k < Kp) {
+                const float p = sigmoid_fast(yy + b2);
+                const int idx = ((j0 + q) * KS + k) * T + row;
+                sums[idx] = __fadd_rn(sums[idx], p);                    // 0 + p0 = p0 exactly: the T1 expression
+                if (p > a.theta) smm[idx] |= (uint8_t)(1u << m);
+            }
+        }
+        __syncthreads();                                                // stage buf is free; the sums of this model are in
+        if (mn == 0) {
+            const float fM = (float)a.M;
+            for (int e = tid; e < CJ * Kp * T; e += C128_THREADS) {      // a multiple of 64: whole warps
+                const int rr = e & 7, jk = e >> 3, j = jk / Kp, kk = jk - j * Kp, idx = (j * KS + kk) * T + rr;
+                const int k = ka + kk;
+                const int64_t t = (c * CJ + j) * G + T * r + rr;
+                const bool live = t < a.n;
+                const float pb = __fdiv_rn(sums[idx], fM);
+                const uint32_t wd = __ballot_sync(0xffffffffu, live && pb > a.theta);
+                if (rr == 0 && (t >> 3) < 4 * a.bits_stride)
+                    reinterpret_cast<uint8_t*>(a.bits + (size_t)k * a.bits_stride)[t >> 3] = (uint8_t)(wd >> (lane & 24));
+                if (live) {
+                    a.pbar[(size_t)k * a.row_stride + t] = pb;
+                    a.mm[(size_t)k * a.row_stride + t] = smm[idx];
+                }
+                sums[idx] = 0.f, smm[idx] = 0;
+            }
+            __syncthreads();
+        }
+        wi = wn, m = mn, step++;
+    }
+}
+
 } // namespace
 
 // packs W2 / b2 of the models and launches; d_v[m] = row 0 of the chunk inside model m's [2][lds][CH] buffer, CH = Hh = 32
@@ -285,15 +447,17 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
         kern<<<(unsigned)(groups * (G / 16)), 512, smem, st>>>(a, n_lags, G);
     } else if (comb) {
         constexpr int CJ = 8;
-        auto kern = k_heads_comb<128, 8, CJ, 4, 16, 1, 1>;
         const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
-        const size_t smem = (size_t)(CJ + n_lags - 1) * 2048 + HF_MAX_M * 256;
-        static bool attr = false;
-        if (!attr) {
-            GWI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (CJ + 64 - 1) * 2048 + HF_MAX_M * 256));
-            attr = true;
+        const int npass = (n_lags + C128_KS_MAX - 1) / C128_KS_MAX, KS = (n_lags + npass - 1) / npass;
+        const int64_t nitems = groups * npass * (G / 8);
+        static int sms = 0;
+        if (!sms) {
+            int dev = 0;
+            GWI_CUDA_CHECK(cudaGetDevice(&dev));
+            GWI_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_comb128, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c128_smem_bytes(C128_KS_MAX)));
         }
-        kern<<<(unsigned)(groups * (G / 8)), 256, smem, st>>>(a, n_lags, G);
+        k_heads_comb128<<<(unsigned)std::min<int64_t>(nitems, sms), C128_THREADS, c128_smem_bytes(KS), st>>>(a, n_lags, KS, npass, G, groups, nitems);
     } else if (CH == 32) {
         k_heads_fused<32><<<(n + 255) / 256, 256, 0, st>>>(a);
     } else {

@@ -88,6 +88,8 @@ int64_t gwi_tc_max_windows(const gwi_model* m, int32_t T);
 int gwi_tc_num_sms(const gwi_model* m);
 gwi_status gwi_tc_stack(const gwi_model* m, const __half* d_strain, int64_t B, int32_t T, void* d_ws, size_t ws_bytes,
                         cudaStream_t st, const uint8_t** u_out);
+gwi_status gwi_tc_vhalf(const gwi_model* m, const uint8_t* u, int64_t B, int ntiles, int seg_tiles, int warm_tiles, int stream_start,
+                        int n_valid, __half* d_v, int64_t lds, cudaStream_t st);
 gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, const uint8_t* hist, int R, int64_t nq,
                               const int64_t* d_lags, int n_lags, int seg_tiles, int warm_tiles, int stream_start, int n_valid,
                               float* d_prob, int64_t stride_k, cudaStream_t st);

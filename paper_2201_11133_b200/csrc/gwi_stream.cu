@@ -18,6 +18,7 @@
 // mode.  In all of them each output sample is an independent fixed-order computation, which is what makes
 // chunked == unchunked exact.  Time-shard mode (gwi_stream_set_shard) runs one rank's span of a longer stream.
 #include <algorithm>
+#include <cstdlib>
 #include <new>
 #include <vector>
 
@@ -77,6 +78,7 @@ struct gwi_stream {
     // tensor-core back end (paper-scale models, FP16 mode, zero lag only)
     bool tcb = false;
     int seg = 0, segT = 0, segH = 0;        // outputs per segment, window length H + seg, warm-up H = R_f - 1 (seg, segT: of the
+    int64_t segx_cap = 0;                   // samples d_segx and the stack workspace hold (time-slide back end)
     int segT0 = 0;                          // current block, chosen by pick_seg; segT0 = the shortest window length)
     __half2* d_segx = nullptr;              // [B][segT][2] channels-last batch
     float* d_segp = nullptr;                // [B][segT] probabilities of the batch
@@ -85,6 +87,8 @@ struct gwi_stream {
     // ... with time slides (lags, n_total multiples of 128): incoming chunks are re-blocked into whole segments, the L1
     // feature tiles of the last max-lag samples are kept as history, one head launch per lag on the u tiles
     bool tcs = false;
+    bool tcv = false;                       // ... with the element-wise heads on the half-head rows v (gwi_tc_vhalf + gwi_heads_fused)
+                                            // instead of one tcgen05 GEMM per lag (GWI_TCS_GEMM_HEADS=1 keeps the latter)
     int Rt = 0;                             // history tiles = maxlag / 128
     __half* d_acc = nullptr;                // [2][acc_cap] samples received but not yet processed (+ the new chunk)
     int64_t acc_cap = 0, pend = 0, t_recv = 0;
@@ -156,14 +160,17 @@ constexpr int SEGT_MAX = 131072;   // longest segment window (samples)
 // ties go to the shorter one.  An hour of 4096 Hz data gives 148 segments of 101 760 samples (one round, 2 % warm-up)
 // instead of 1029 of 16 384 (seven rounds, 12.5 % warm-up).  Results do not depend on the segmentation: every output
 // sees its whole receptive field either way.
-void pick_seg(gwi_stream* s, int64_t n)
+void pick_seg(gwi_stream* s, int64_t n, int min_segT = 0)
 {
     const int sms = gwi_tc_num_sms(s->models[0]);
-    int best = s->segT0;
+    if (min_segT <= 0) min_segT = s->segT0;
+    int best = min_segT;
     int64_t best_cost = INT64_MAX;
-    for (int segT = s->segT0; segT <= SEGT_MAX; segT += 128) {
+    for (int segT = min_segT; segT <= SEGT_MAX; segT += 128) {
         const int64_t seg = segT - s->segH;
+        if (seg < 128) continue;
         const int64_t B = (n + seg - 1) / seg, jobs = ((B + 1) / 2) * 2, rounds = (jobs + sms - 1) / sms;
+        if (s->segx_cap > 0 && B * segT > s->segx_cap) continue;
         if (rounds * segT < best_cost) best_cost = rounds * segT, best = segT;
     }
     s->segT = best, s->seg = best - s->segH;
@@ -343,13 +350,35 @@ gwi_status tcs_block(gwi_stream* s, int n, bool last, cudaStream_t st)
         const uint8_t* u = nullptr;
         rc = gwi_tc_stack(s->models[m], (const __half*)s->d_segx, B, s->segT, s->d_tcws, s->tcws_bytes, st, &u);
         if (rc != GWI_OK) return rc;
+        if (s->tcv) {
+            rc = gwi_tc_vhalf(s->models[m], u, B, ntiles, seg_tiles, warm_tiles, start, n, s->d_u16[m] + (size_t)s->maxlag * 128, s->lds, st);
+            if (rc != GWI_OK) return rc;
+            continue;
+        }
         rc = gwi_tc_head_stream(s->models[m], u, ntiles, s->d_hist_t[s->hist_t_cur][m], s->Rt, nq, s->d_lags, nslides, seg_tiles,
                                 warm_tiles, start, n, s->d_prob + (size_t)m * s->sub, (int64_t)s->M * s->sub, st);
         if (rc != GWI_OK) return rc;
-        if (s->Rt > 0) {
+        if (s->Rt > 0 && !s->tcv) {
             k_hist_tiles<<<s->Rt, 256, 0, st>>>(u, ntiles, nq, s->Rt, seg_tiles, warm_tiles, start, s->d_hist_t[s->hist_t_cur][m],
                                                s->d_hist_t[s->hist_t_cur ^ 1][m]);
             gwi_count_launch(1);
+        }
+    }
+    if (s->tcv) {
+        // every lag, every model, mean and threshold element-wise on the half-head rows; then the L1 rings shift
+        const int64_t skip = (s->rule == GWI_RULE_PER_MODEL) ? 0 : (s->t_done < s->warm ? std::min<int64_t>(n, s->warm - s->t_done) : 0);
+        if (skip < n) {
+            const __half* vp[GWI_MAX_MODELS];
+            for (int m = 0; m < s->M; m++) vp[m] = s->d_u16[m] + (size_t)(s->maxlag + skip) * 128;
+            rc = gwi_heads_fused(s->models.data(), s->M, vp, s->lds, (int)(n - skip), s->d_lags, nslides, s->lags.data(), s->theta,
+                                 s->d_fbits, s->fbits_stride, s->d_fpbar, s->d_fmm, s->sub,
+                                 s->rule == GWI_RULE_PER_MODEL ? s->d_prob : nullptr, st);
+            if (rc != GWI_OK) return rc;
+        }
+        for (int m = 0; m < s->M; m++) {
+            __half* base = s->d_u16[m] + (size_t)s->lds * 128;
+            GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_tmp, base + (size_t)n * 128, (size_t)s->maxlag * 256, cudaMemcpyDeviceToDevice, st));
+            GWI_CUDA_CHECK(cudaMemcpyAsync(base, s->d_tmp, (size_t)s->maxlag * 256, cudaMemcpyDeviceToDevice, st));
         }
     }
     s->hist_t_cur ^= 1;
@@ -367,7 +396,9 @@ gwi_status tcs_append_and_run(gwi_stream* s, int xb, int64_t x0, int64_t n, cuda
     s->pend += n, s->t_recv += n;
     const bool final = s->t_recv == s->N_total;
     const int seg0 = s->segT0 - s->segH;
-    while (s->pend >= seg0 || (final && s->pend > 0)) {
+    // whole blocks only (a short block leaves most of the 148 SMs idle for a full segment time); what is left waits for
+    // the next push, or for the end of the stream
+    while (s->pend >= s->sub || (final && s->pend > 0)) {
         const int64_t avail = std::min<int64_t>(s->pend, s->sub);
         pick_seg(s, avail);
         int64_t proc = (final && avail == s->pend) ? avail : (avail / s->seg) * s->seg;
@@ -509,8 +540,11 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     if (s->tcb) sub = 1 << 24;
     if (s->tcs) {
         int64_t maxw = gwi_tc_max_windows(m0, s->segT);
-        sub = std::min<int64_t>(1 << 24, maxw * s->seg) / s->seg * s->seg;
-        if (sub < s->maxlag) s->tcs = false;               // the priming pass runs the tail as one block
+        const char* env = getenv("GWI_TCS_GEMM_HEADS");
+        s->tcv = n_models <= 8 && !(env && env[0] == '1');
+        // v rows cost 512 B per sample and model: blocks of at most 2^23 samples
+        sub = std::min<int64_t>(s->tcv ? 1 << 23 : 1 << 24, maxw * s->seg) / s->seg * s->seg;
+        if (sub < s->maxlag) s->tcs = s->tcv = false;      // the priming pass runs the tail as one block
     }
     sub = std::min<int64_t>(sub, 1 << 24);
     if (!s->tcs) sub = std::min<int64_t>(sub, s->xcap);
@@ -544,7 +578,9 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
         if ((e = cudaMalloc(&s->d_lags, (size_t)nslides * 8)) != cudaSuccess) return fail(e);
         if ((e = cudaMemcpy(s->d_lags, s->lags.data(), (size_t)nslides * 8, cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
         const int64_t Bmax = ((int64_t)((double)s->sub * s->segT0 / s->seg) + 2 * SEGT_MAX) / s->segT0 + 1;
-        s->acc_cap = (int64_t)s->sub + SEGT_MAX + std::min<int64_t>(s->xcap, s->sub);
+        // pending samples stay below one block (sub) and a piece of a push is at most one block
+        s->acc_cap = (int64_t)2 * s->sub + SEGT_MAX;
+        s->segx_cap = Bmax * s->segT;
         if ((e = cudaMalloc(&s->d_segx, (size_t)Bmax * s->segT * 4)) != cudaSuccess) return fail(e);
         s->tcws_bytes = gwi_tc_workspace_bytes(m0, Bmax, s->segT);
         if ((e = cudaMalloc(&s->d_tcws, s->tcws_bytes)) != cudaSuccess) return fail(e);
@@ -554,7 +590,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
             if ((e = cudaMalloc(&s->d_xh[b], (size_t)2 * s->segH * 2)) != cudaSuccess) return fail(e);
             if ((e = cudaMemset(s->d_xh[b], 0, (size_t)2 * s->segH * 2)) != cudaSuccess) return fail(e);
             s->d_hist_t[b].assign(s->M, nullptr);
-            for (int m = 0; m < s->M; m++) {
+            for (int m = 0; m < s->M && !s->tcv; m++) {
                 if ((e = cudaMalloc(&s->d_hist_t[b][m], (size_t)s->Rt * 32768)) != cudaSuccess) return fail(e);
                 if ((e = cudaMemset(s->d_hist_t[b][m], 0, (size_t)s->Rt * 32768)) != cudaSuccess) return fail(e);
             }
@@ -578,6 +614,17 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     }
     s->fused = s->tiny && nslides > 1 && s->M <= 8;
     for (int i = 0; i < n_models; i++) s->fused = s->fused && gwi_tiny_writes_v(models[i]);
+    if (s->tcv) {
+        // half-head rows of every model: [2 branches][maxlag ring + sub][128] fp16
+        s->fused = true;
+        s->d_u16.assign(s->M, nullptr);
+        for (int m = 0; m < s->M; m++) {
+            size_t ub = (size_t)2 * s->lds * 128 * 2;
+            if ((e = cudaMalloc(&s->d_u16[m], ub)) != cudaSuccess) return fail(e);
+            if ((e = cudaMemset(s->d_u16[m], 0, ub)) != cudaSuccess) return fail(e);
+        }
+        if ((e = cudaMalloc(&s->d_tmp, (size_t)s->maxlag * 256)) != cudaSuccess) return fail(e);
+    }
     if (s->fused) {
         s->fbits_stride = (s->sub + 31) / 32 + 8;
         if ((e = cudaMalloc(&s->d_fbits, (size_t)nslides * s->fbits_stride * 4)) != cudaSuccess) return fail(e);
@@ -694,7 +741,7 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
         GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_xh[0] + H + (H - pre), l1_tail, (size_t)pre * 2, cudaMemcpyDefault, st));
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_acc, 0, (size_t)n * 2, st));
         GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_acc + s->acc_cap, (const __half*)l1_tail + pre, (size_t)n * 2, cudaMemcpyDefault, st));
-        pick_seg(s, n);
+        pick_seg(s, n, std::max(4096, H + 128));             // short segments: the tail is one small block
         const int B = (int)((n + s->seg - 1) / s->seg);
         const int64_t total = (int64_t)B * s->segT;
         k_seg_gather<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(s->d_acc, s->acc_cap, s->d_xh[0], (int)n, s->seg, H, s->segT, 0,
@@ -704,6 +751,17 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
             const uint8_t* u = nullptr;
             gwi_status rc = gwi_tc_stack(s->models[m], (const __half*)s->d_segx, B, s->segT, s->d_tcws, s->tcws_bytes, st, &u);
             if (rc != GWI_OK) return rc;
+            if (s->tcv) {
+                // half-head rows of the tail (the H1 rows it produces are garbage and are overwritten by the first block),
+                // then the same ring shift as after a block: the tail's maxlag rows land in front of row 0
+                rc = gwi_tc_vhalf(s->models[m], u, B, s->segT / 128, s->seg / 128, H / 128, 0, (int)n, s->d_u16[m] + (size_t)s->maxlag * 128,
+                                  s->lds, st);
+                if (rc != GWI_OK) return rc;
+                __half* base = s->d_u16[m] + (size_t)s->lds * 128;
+                GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_tmp, base + (size_t)n * 128, (size_t)s->maxlag * 256, cudaMemcpyDeviceToDevice, st));
+                GWI_CUDA_CHECK(cudaMemcpyAsync(base, s->d_tmp, (size_t)s->maxlag * 256, cudaMemcpyDeviceToDevice, st));
+                continue;
+            }
             k_hist_tiles<<<s->Rt, 256, 0, st>>>(u, s->segT / 128, s->Rt, s->Rt, s->seg / 128, H / 128, 0, s->d_hist_t[1][m],
                                                s->d_hist_t[0][m]);
             gwi_count_launch(1);

@@ -572,6 +572,10 @@ struct HeadArgs {
     const int64_t* lags;      // device, samples, multiples of 128
     int64_t nq, stride_k;
     int n_lags, R, seg_tiles, warm_tiles, stream_start, n_valid;
+    // k_vhalf_tc: the two halves of the head's first layer per sample, fp16 rows of 128: v_H = W1[:, :128] u_H + b1 and
+    // v_L = W1[:, 128:] u_L, at vout + (branch * vlds + row) * 128, row = sample index inside the block (warm-up tiles skipped)
+    __half* vout;
+    int64_t vlds;
 };
 constexpr int HEAD_SMEM_EXTRA = 2048;   // barriers, TMEM slot, b1 | W2 | b2
 constexpr int HEAD_SMEM = 7 * U_TILE_BYTES + HEAD_SMEM_EXTRA;   // W1 (2 tiles) + 5 feature-tile buffers
@@ -768,6 +772,119 @@ __global__ void __launch_bounds__(HEAD_THREADS, 1) k_head_tc(const HeadArgs a)
     if (warp == 8) tmem_dealloc(tmem, 512);
 }
 
+// ---- half-heads for the element-wise time-slide evaluation (gwi_heads.cu) ---------------------------------------------
+// Same roles as k_head_tc (warps 0-7 epilogue in two sets, warp 8 bulk-copy producer, warp 9 MMA issuer), items = (window,
+// tile) of a block of segments; per item two accumulators: u_H . W1[:, :128]^T and u_L . W1[:, 128:]^T (8 K steps each),
+// written as fp16 rows.  Warm-up tiles of a segment are skipped by all three roles alike.
+__global__ void __launch_bounds__(HEAD_THREADS, 1) k_vhalf_tc(const HeadArgs a)
+{
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const uint32_t sbase = smem_u32(smem);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int W1B = 2 * U_TILE_BYTES, OFF_U = W1B, OFF_BAR = 7 * U_TILE_BYTES;
+    auto bar = [&](int i) { return sbase + OFF_BAR + 8 * i; };   // 0 w1_full, 1-2 u_full, 3-4 u_free, 5-6 acc_full, 7-8 acc_free
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * 20);
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 9; i++) mbar_init(bar(i), (i == 7 || i == 8) ? 128u : 1u);
+        mbar_fence_init();
+    }
+    if (warp == 8) tmem_alloc(smem_u32(tmem_slot), 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const int64_t nitems = a.nwin * a.ntiles;
+    auto skip = [&](int64_t it) { return (int)(it % a.ntiles) < (((it / a.ntiles) == 0 && a.stream_start) ? 0 : a.warm_tiles); };
+    if (warp == 8) {
+        if (lane == 0) {
+            mbar_arrive_expect_tx(bar(0), W1B);
+            bulk_g2s(sbase, a.w1, W1B, bar(0));
+            uint32_t n = 0;
+            for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x) {
+                if (skip(it)) continue;
+                const int st = n & 1;
+                const int64_t wl = it / a.ntiles, j = it % a.ntiles;
+                mbar_wait(bar(3 + st), ((n >> 1) & 1) ^ 1);
+                mbar_arrive_expect_tx(bar(1 + st), W1B);
+                for (int b = 0; b < 2; b++)
+                    bulk_g2s(sbase + OFF_U + st * W1B + b * U_TILE_BYTES, a.u + (((size_t)wl * 2 + b) * a.ntiles + j) * U_TILE_BYTES,
+                             U_TILE_BYTES, bar(1 + st));
+                n++;
+            }
+        }
+        __syncwarp();
+    } else if (warp == 9) {
+        if (elect_one()) {
+            const uint32_t idesc = make_idesc_f16(128, 128);
+            const uint64_t dW = make_sdesc(sbase, 2048, 128);
+            const uint64_t dU = make_sdesc(sbase + OFF_U, 2048, 128);
+            mbar_wait(bar(0), 0);
+            uint32_t n = 0;
+            for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x) {
+                if (skip(it)) continue;
+                const int st = n & 1;
+                const uint32_t ph = (n >> 1) & 1;
+                mbar_wait(bar(1 + st), ph);
+                mbar_wait(bar(7 + st), ph ^ 1);
+                tc_fence_after();
+                const uint64_t du = dU + st * (W1B >> 4);
+                const uint32_t dt = tmem + 256 * st;
+#pragma unroll
+                for (int kk = 0; kk < 8; kk++) tc_mma_f16(dt, du + kk * 256, dW + kk * 256, idesc, kk > 0 ? 1u : 0u);
+#pragma unroll
+                for (int kk = 8; kk < 16; kk++) tc_mma_f16(dt + 128, du + kk * 256, dW + kk * 256, idesc, kk > 8 ? 1u : 0u);
+                tc_commit(bar(5 + st));
+                tc_commit(bar(3 + st));
+                n++;
+            }
+        }
+        __syncwarp();
+    } else {
+        const int set = warp >> 2, r = (warp & 3) * 32 + lane;
+        const uint32_t lane_t = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+        uint32_t n = 0;
+        for (int64_t it = blockIdx.x; it < nitems; it += gridDim.x) {
+            if (skip(it)) continue;
+            const uint32_t my = n++;
+            if ((int)(my & 1) != set) continue;
+            const int64_t wl = it / a.ntiles, j = it % a.ntiles;
+            const int warm = (wl == 0 && a.stream_start) ? 0 : a.warm_tiles;
+            const int64_t row = (wl * a.seg_tiles + (j - warm)) * TM + r;
+            mbar_wait(bar(5 + set), (my >> 1) & 1);
+            tc_fence_after();
+#pragma unroll
+            for (int b = 0; b < 2; b++) {
+                uint4* dst = reinterpret_cast<uint4*>(a.vout + ((size_t)b * a.vlds + row) * 128);
+#pragma unroll
+                for (int cc = 0; cc < 4; cc++) {
+                    uint32_t v[32];
+                    tmem_ld32(lane_t + 256 * set + 128 * b + 32 * cc, v);
+                    tc_wait_ld();
+                    if (row < a.n_valid) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) {
+                            uint32_t q[4];
+#pragma unroll
+                            for (int e = 0; e < 4; e++) {
+                                const int col = 8 * c + 2 * e;
+                                float x0 = __uint_as_float(v[col]), x1 = __uint_as_float(v[col + 1]);
+                                if (b == 0) x0 += a.b1[32 * cc + col], x1 += a.b1[32 * cc + col + 1];
+                                q[e] = pack_half2(x0, x1);
+                            }
+                            dst[4 * cc + c] = make_uint4(q[0], q[1], q[2], q[3]);
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(bar(7 + set));
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 8) tmem_dealloc(tmem, 512);
+}
+
 } // namespace
 
 // ---- host side: packing and launch -----------------------------------------------------------------------------------
@@ -878,6 +995,7 @@ gwi_status gwi_tc_pack(gwi_model* m)
     p->num_sms = prop.multiProcessorCount;
     GWI_CUDA_CHECK(cudaFuncSetAttribute(k_stack, cudaFuncAttributeMaxDynamicSharedMemorySize, SM_TOTAL));
     GWI_CUDA_CHECK(cudaFuncSetAttribute(k_head_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, HEAD_SMEM));
+    GWI_CUDA_CHECK(cudaFuncSetAttribute(k_vhalf_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, HEAD_SMEM));
     return GWI_OK;
 }
 
@@ -938,7 +1056,7 @@ gwi_status gwi_tc_infer(const gwi_model* m, const __half* d_strain, int64_t B, i
         memcpy(ha.b1, p->h_hc, 128 * 4), memcpy(ha.w2, p->h_hc + 128, 128 * 4), ha.b2 = p->h_hc[256];
         ha.w1 = p->d_w1, ha.u = u, ha.prob = d_prob, ha.w0 = w0, ha.nwin = nwin, ha.T = T, ha.ntiles = ntiles,
         ha.n_branch = nb, ha.mode = 0, ha.hist = nullptr, ha.lags = nullptr, ha.nq = 0, ha.stride_k = 0, ha.n_lags = 0, ha.R = 0,
-        ha.seg_tiles = 0, ha.warm_tiles = 0, ha.stream_start = 0, ha.n_valid = 0;
+        ha.seg_tiles = 0, ha.warm_tiles = 0, ha.stream_start = 0, ha.n_valid = 0, ha.vout = nullptr, ha.vlds = 0;
         int64_t nitems = nwin * ntiles;
         int hgrid = (int)(nitems < p->num_sms ? nitems : p->num_sms);
         k_head_tc<<<hgrid, HEAD_THREADS, HEAD_SMEM, st>>>(ha);
@@ -1000,6 +1118,26 @@ gwi_status gwi_tc_stack(const gwi_model* m, const __half* d_strain, int64_t B, i
     return GWI_OK;
 }
 
+// Half-heads v_H, v_L of every output sample of a block of B windows whose u tiles gwi_tc_stack has just written (same
+// segment layout): fp16 rows at d_v + (branch * lds + row) * 128, row = sample index inside the block.
+gwi_status gwi_tc_vhalf(const gwi_model* m, const uint8_t* u, int64_t B, int ntiles, int seg_tiles, int warm_tiles, int stream_start,
+                        int n_valid, __half* d_v, int64_t lds, cudaStream_t st)
+{
+    const GwiTcPack* p = m->tc;
+    HeadArgs ha;
+    memcpy(ha.b1, p->h_hc, 128 * 4), memcpy(ha.w2, p->h_hc + 128, 128 * 4), ha.b2 = p->h_hc[256];
+    ha.w1 = p->d_w1, ha.u = u, ha.prob = nullptr, ha.w0 = 0, ha.nwin = B, ha.T = 0, ha.ntiles = ntiles;
+    ha.n_branch = 2, ha.mode = 0, ha.hist = nullptr, ha.lags = nullptr, ha.nq = 0, ha.stride_k = 0, ha.n_lags = 0, ha.R = 0;
+    ha.seg_tiles = seg_tiles, ha.warm_tiles = warm_tiles, ha.stream_start = stream_start, ha.n_valid = n_valid;
+    ha.vout = d_v, ha.vlds = lds;
+    const int64_t nitems = B * ntiles;
+    int grid = (int)(nitems < p->num_sms ? nitems : p->num_sms);
+    k_vhalf_tc<<<grid, HEAD_THREADS, HEAD_SMEM, st>>>(ha);
+    gwi_count_launch(1);
+    GWI_CUDA_CHECK(cudaGetLastError());
+    return GWI_OK;
+}
+
 // Heads of all lags over the nq output tiles of a block (see HeadArgs, stream mode); d_lags: device array of n_lags lags
 // in samples (multiples of 128); probabilities of lag k at d_prob + k * stride_k.
 gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, const uint8_t* hist, int R, int64_t nq,
@@ -1016,6 +1154,7 @@ gwi_status gwi_tc_head_stream(const gwi_model* m, const uint8_t* u, int ntiles, 
     ha.w1 = p->d_w1, ha.u = u, ha.prob = d_prob, ha.w0 = 0, ha.nwin = 0, ha.T = 0, ha.ntiles = ntiles;
     ha.n_branch = 2, ha.mode = 1, ha.hist = hist, ha.lags = d_lags, ha.nq = nq, ha.stride_k = stride_k, ha.n_lags = n_lags, ha.R = R;
     ha.seg_tiles = seg_tiles, ha.warm_tiles = warm_tiles, ha.stream_start = stream_start, ha.n_valid = n_valid;
+    ha.vout = nullptr, ha.vlds = 0;
     int hgrid = (int)(nq < p->num_sms ? nq : p->num_sms);
     k_head_tc<<<hgrid, HEAD_THREADS, HEAD_SMEM, st>>>(ha);
     gwi_count_launch(1);

@@ -331,6 +331,27 @@ def test_stream_paper_scale_slides_tensor_core_back_end(tmpdir_s):
     assert trig_tuples(r0) == _oracle_triggers(p0.astype(np.float64), float(np.float32(0.5)), 16)
 
 
+@pytest.mark.parametrize("seeds,G,K,check", [([0, 1], 2048, 7, None), ([0], 1024, 36, [0, 1, 2, 17, 18, 19, 34, 35])])
+def test_stream_paper_scale_regular_lags_comb_heads(tmpdir_s, seeds, G, K, check):
+    """Paper-scale models with a regular lag list k x G: the half-head rows v from the tensor cores, then the comb-scheduled
+    element-wise heads fused with the ensemble mean and the threshold (one pass for 7 slides, two passes of 18 for 36).
+    Parity of pbar with the oracle on every slide (on a spread of slides for the long list), triggers from pbar."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, seeds, gwi.FP16, arch=gs.PAPER_ARCH)
+    N = 128 * 320
+    x = gs.stream_noise(35, 0, N, dtype=np.float16)
+    lags = [k * G for k in range(1, K)]
+    n, recs, pbar = _run_stream(gms, x, _ragged(N, 4, 3000, 16000), lags, 0.5, 16, max_chunk=16000)
+    ks = list(range(K)) if check is None else check
+    want = _oracle_slides(oms, x, [lags[k - 1] for k in ks if k > 0])
+    assert ks[0] == 0 and np.max(np.abs(pbar[ks] - want)) <= 2e-3
+    got = trig_tuples(recs)
+    assert got == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 16)
+    # the same stream in one push: bit-identical
+    n1, r1, p1 = _run_stream(gms, x, [N], lags, 0.5, 16)
+    assert np.array_equal(pbar, p1) and trig_tuples(r1) == got
+
+
 @pytest.mark.parametrize("lags", [[], [4096, 12800]])
 def test_paper_scale_long_block_segment_choice(tmpdir_s, lags):
     """A block long enough that the tensor-core back ends pick segments longer than the minimum (pick_seg: > 296
