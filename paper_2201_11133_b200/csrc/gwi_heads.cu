@@ -1,17 +1,20 @@
-// gwi_heads.cu -- time-slide heads of the narrow-architecture ensemble, fused with the ensemble mean and the threshold
+// gwi_heads.cu -- time-slide heads of the ensemble (narrow architecture: 32 head channels; paper scale: 128), fused with
+// the ensemble mean and the threshold
 // (the per-timestep outputs of every slide are what
 // did not scale in the paper's post-processing).
 //
 //   p_{m,k}[t] = sigmoid(b2 + W2 . ReLU(W1 [u_H[t]; u_L[t - lag_k]] + b1))              (reading A24, C.1 step 5)
 //
-// W1 [u_H; u_L] + b1 = v_H[t] + v_L[t - lag_k] with v_H = W1[:, :32] u_H + b1 and v_L = W1[:, 32:] u_L, which the branch
-// kernel (gwi_tiny_tc.cu, time-slide mode) has already written per sample, in fp16.  What is left per (sample, lag,
-// model) is element-wise: 16 fused add-ReLU on half2 pairs, 16 half2 multiply-adds with W2, one sigmoid.  The kernel
+// W1 [u_H; u_L] + b1 = v_H[t] + v_L[t - lag_k] with v_H = W1[:, :Hh] u_H + b1 and v_L = W1[:, Hh:] u_L, which the branch
+// kernel (gwi_tiny_tc.cu in time-slide mode; gwi_tc.cu k_vhalf_tc for paper-scale models) has already written per
+// sample, in fp16.  What is left per (sample, lag, model) is element-wise: Hh / 2 fused add-ReLU on half2 pairs, Hh / 2
+// half2 multiply-adds with W2, one sigmoid.  The kernel
 // loops over the models in order and forms pbar = (((p0 + p1) + p2) + ...) / M in the fixed fp32 expression of tier T1,
 // compares with the threshold and writes, per slide, the bit mask the run clustering works on, pbar (the statistics of
 // the few triggers are taken from it) and one byte per sample saying which models exceeded the threshold on their own --
 // no per-model, per-slide probability array exists (it was 7.8 GB per hour of data at 33 slides and 4 models).
 #include <algorithm>
+#include <cstdint>
 #include <cstring>
 #include <vector>
 
@@ -136,8 +139,8 @@ __global__ void __launch_bounds__(256) k_heads_fused(const __grid_constant__ Hea
 // apart, t = (c CJ + j) G + T r + [0, T), j < CJ: for all K lags it needs only the CJ + K - 1 blocks of v_L rows at
 // (c CJ + i) G + T r, -K < i < CJ, which it stages in shared memory once per model: with T = 16 rows of 32 channels, 48 KB
 // feed 8448 evaluations, 8 x fewer bytes from L2 than one row per evaluation (double-buffered over the models: the next
-// model's blocks arrive by cp.async while this one is evaluated); with T = 8 rows of 128 channels (paper-scale models,
-// up to 64 slides) CJ = 8 and one 136 KB stage.  Threads = T rows x CJ blocks x NG interleaved groups of the lag list; a thread
+// model's blocks arrive by cp.async while this one is evaluated).  (128-channel rows: k_heads_comb128 below.)
+// Threads = T rows x CJ blocks x NG interleaved groups of the lag list; a thread
 // keeps the running sums of its <= KQ lags in registers across the models (fixed order m = 0, 1, ...: the T1 expression).
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src)
@@ -260,9 +263,34 @@ __host__ __device__ constexpr size_t c128_smem_bytes(int KS)
     return (size_t)2 * (8 + KS - 1 + 8) * C128_BLKB + (size_t)8 * KS * 8 * 5 + HF_MAX_M * 256 + 16;
 }
 
+struct C128Item {
+    int c, r, ka, Kp;      // comb group, row group, first lag and number of lags of the pass
+};
+
+// lo + hi of a half2 accumulator added to y in fp32: two mixed-precision multiply-adds by one (FHFMA)
+__device__ __forceinline__ float acc_to_y(uint32_t acc, float y)
+{
+    asm("{ .reg .f16 lo, hi, one;\n\t"
+        "mov.b32 {lo, hi}, %1;\n\t"
+        "mov.b16 one, 0x3C00;\n\t"
+        "fma.rn.f32.f16 %0, lo, one, %0;\n\t"
+        "fma.rn.f32.f16 %0, hi, one, %0; }"
+        : "+f"(y)
+        : "r"(acc));
+    return y;
+}
+// y + the contribution of 8 channels (one 16-byte chunk of v_H, v_L and W2): a half2 accumulator of four products
+__device__ __forceinline__ float chunk_acc(float y, uint4 h, uint4 l, uint4 w)
+{
+    uint32_t acc = mul2h(add_relu2(l.x, h.x), w.x);
+    acc = fma2h(add_relu2(l.y, h.y), w.y, acc);
+    acc = fma2h(add_relu2(l.z, h.z), w.z, acc);
+    acc = fma2h(add_relu2(l.w, h.w), w.w, acc);
+    return acc_to_y(acc, y);
+}
+
 __global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_constant__ HeadsFusedArgs a, const int K, const int KS,
-                                                                  const int npass, const int64_t G, const int64_t groups,
-                                                                  const int64_t nitems)
+                                                                  const int npass, const int G, const int groups, const int nitems)
 {
     using namespace tc;
     constexpr int T = 8, CJ = 8, JB = 4, NS = 8, CH = 128, ROWB = C128_ROWB, BLKB = C128_BLKB;
@@ -281,60 +309,39 @@ __global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_
     for (int e = tid; e < a.M * 64; e += C128_THREADS) reinterpret_cast<uint32_t*>(smem + w2off)[e] = a.w2[e >> 6][e & 63];
     __syncthreads();
 
-    auto decode = [&](int64_t wi, int64_t& c, int64_t& r, int& ka, int& Kp) {
-        c = wi % groups;
-        const int64_t x = wi / groups;
-        const int p = (int)(x % npass);
-        r = x / npass;
-        ka = p * KS, Kp = min(KS, K - ka);
+    auto decode = [&](int wi) {
+        C128Item it;
+        it.c = wi % groups;
+        const int x = wi / groups, p = x % npass;
+        it.r = x / npass;
+        it.ka = p * KS, it.Kp = min(KS, K - it.ka);
+        return it;
     };
-    // all warps: the rows of model m of item wi into stage buf, 16 bytes per cp.async (a block = 8 rows = 2 KB contiguous in
-    // global memory = four warp-wide copies); one commit group per step
-    auto stage_load = [&](int64_t wi, int m, int buf) {
-        int64_t c, r;
-        int ka, Kp;
-        decode(wi, c, r, ka, Kp);
-        const int nblk = CJ + Kp - 1;
-        const __half* vH = a.v[m];
-        const __half* vL = a.v[m] + a.lds * CH;
-        const int ch = lane & 15, r0 = lane >> 4;
+    // all warps: the rows of model m of an item into stage buf, 16 bytes per cp.async.  A block = 8 consecutive rows = 2 KB
+    // contiguous in global memory = four warp-wide copies; blocks start at multiples of 8 and n is one, so a block is
+    // inside the rows or outside (then any block will do: its items are dropped).  One commit group per step.
+    auto stage_load = [&](const C128Item& it, int m, int buf) {
+        const int nblk = CJ + it.Kp - 1;
+        const __half* vH = a.v[m] + (lane >> 4) * CH + (lane & 15) * 8;
+        const __half* vL = vH + a.lds * CH;
+        const uint32_t dst0 = sbase + buf * stage_bytes + (lane >> 4) * ROWB + (lane & 15) * 16;
+        const int gL = it.c * CJ - (it.Kp - 1) - it.ka, gH = it.c * CJ - nblk;
         for (int blk = warp; blk < nblk + CJ; blk += C128_THREADS / 32) {
             const bool isL = blk < nblk;
-            const int64_t s0 = isL ? (c * CJ + blk - (Kp - 1) - ka) * G + T * r : (c * CJ + (blk - nblk)) * G + T * r;
+            int64_t s0 = (int64_t)((isL ? gL : gH) + blk) * G + T * it.r;
             const int64_t lo = isL ? lo_row : 0;
-            const __half* base = (isL ? vL : vH) + ch * 8;
-            const uint32_t dst = sbase + buf * stage_bytes + (isL ? blk : nblk_max + blk - nblk) * BLKB + ch * 16;
+            s0 = s0 < lo ? lo : (s0 > a.n - T ? a.n - T : s0);
+            const __half* src = (isL ? vL : vH) + s0 * CH;
+            const uint32_t dst = dst0 + (isL ? blk : nblk_max + blk - nblk) * BLKB;
 #pragma unroll
-            for (int x = 0; x < 4; x++) {
-                const int rr = r0 + 2 * x;
-                int64_t sr = s0 + rr;
-                sr = sr < lo ? lo : (sr > a.n - 1 ? a.n - 1 : sr);
-                cp_async16(dst + rr * ROWB, base + sr * CH);
-            }
+            for (int x = 0; x < 4; x++) cp_async16(dst + 2 * x * ROWB, src + 2 * x * CH);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    int64_t wi = blockIdx.x;
-    int m = 0;
-    uint32_t step = 0;
-    if (wi < nitems) stage_load(wi, 0, 0);
-    while (wi < nitems) {
-        int64_t wn = wi;
-        int mn = m + 1;
-        if (mn == a.M) mn = 0, wn = wi + gridDim.x;
-        const int buf = step & 1;
-        if (wn < nitems) {
-            stage_load(wn, mn, buf ^ 1);                                // stage buf ^ 1 was released by the barrier below
-            asm volatile("cp.async.wait_group 1;" ::: "memory");
-        } else {
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
-        }
-        __syncthreads();
-        int64_t c, r;
-        int ka, Kp;
-        decode(wi, c, r, ka, Kp);
-        const int nblk = CJ + Kp - 1;
+    // one model of an item on the rows of stage buf
+    auto compute = [&](const C128Item& it, int m, int buf) {
+        const int Kp = it.Kp, nblk = CJ + Kp - 1;
         const uint32_t bb = sbase + buf * stage_bytes + row * ROWB + q * 64;
         uint4 h[JB][4], w[4];
 #pragma unroll
@@ -344,22 +351,31 @@ __global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_
 #pragma unroll
         for (int cc = 0; cc < 4; cc++) w[cc] = lds128(sbase + w2off + m * 256 + q * 64 + cc * 16);
         const float b2 = a.b2[m];
+        const bool hi = q & 2, od = q & 1;
         for (int i = slot; i < nblk; i += NS) {
             uint4 l[4];
 #pragma unroll
             for (int cc = 0; cc < 4; cc++) l[cc] = lds128(bb + i * BLKB + cc * 16);
             const int kb = j0 - i + Kp - 1;                             // lag (within the pass) of item jj = kb + jj
             float y[JB];
+            if (kb >= 0 && kb + JB <= Kp) {                             // warp-uniform: the whole diagonal piece is inside
 #pragma unroll
-            for (int jj = 0; jj < JB; jj++) {
-                y[jj] = 0.f;
-                if (kb + jj >= 0 && kb + jj < Kp) {                     // warp-uniform
+                for (int jj = 0; jj < JB; jj++) {
+                    y[jj] = 0.f;
 #pragma unroll
-                    for (int cc = 0; cc < 4; cc++) y[jj] += chunk_y(h[jj][cc], l[cc], w[cc]);
+                    for (int cc = 0; cc < 4; cc++) y[jj] = chunk_acc(y[jj], h[jj][cc], l[cc], w[cc]);
+                }
+            } else {
+#pragma unroll
+                for (int jj = 0; jj < JB; jj++) {
+                    y[jj] = 0.f;
+                    if (kb + jj >= 0 && kb + jj < Kp) {
+#pragma unroll
+                        for (int cc = 0; cc < 4; cc++) y[jj] = chunk_acc(y[jj], h[jj][cc], l[cc], w[cc]);
+                    }
                 }
             }
             // transposing butterfly over the four quarters: the lane of quarter jj ends with the whole sum of item jj
-            const bool hi = q & 2, od = q & 1;
             float k0 = hi ? y[2] : y[0], k1 = hi ? y[3] : y[1];
             k0 += __shfl_xor_sync(0xffffffffu, hi ? y[0] : y[2], 16);
             k1 += __shfl_xor_sync(0xffffffffu, hi ? y[1] : y[3], 16);
@@ -373,27 +389,52 @@ __global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_
                 if (p > a.theta) smm[idx] |= (uint8_t)(1u << m);
             }
         }
-        __syncthreads();                                                // stage buf is free; the sums of this model are in
-        if (mn == 0) {
-            const float fM = (float)a.M;
-            for (int e = tid; e < CJ * Kp * T; e += C128_THREADS) {      // a multiple of 64: whole warps
-                const int rr = e & 7, jk = e >> 3, j = jk / Kp, kk = jk - j * Kp, idx = (j * KS + kk) * T + rr;
-                const int k = ka + kk;
-                const int64_t t = (c * CJ + j) * G + T * r + rr;
-                const bool live = t < a.n;
-                const float pb = __fdiv_rn(sums[idx], fM);
-                const uint32_t wd = __ballot_sync(0xffffffffu, live && pb > a.theta);
-                if (rr == 0 && (t >> 3) < 4 * a.bits_stride)
-                    reinterpret_cast<uint8_t*>(a.bits + (size_t)k * a.bits_stride)[t >> 3] = (uint8_t)(wd >> (lane & 24));
-                if (live) {
-                    a.pbar[(size_t)k * a.row_stride + t] = pb;
-                    a.mm[(size_t)k * a.row_stride + t] = smm[idx];
-                }
-                sums[idx] = 0.f, smm[idx] = 0;
+    };
+    // mean, threshold, outputs of the item; the sums go back to zero.  Thread = (row, comb block j, lag slot)
+    auto finalize = [&](const C128Item& it) {
+        const float fM = (float)a.M;
+        const int rr = tid & 7, j = (tid >> 3) & 7;
+        const int64_t t = (int64_t)(it.c * CJ + j) * G + T * it.r + rr;
+        const bool live = t < a.n;
+        for (int kk = tid >> 6; kk < it.Kp; kk += C128_THREADS / 64) {  // warp-uniform
+            const int idx = (j * KS + kk) * T + rr, k = it.ka + kk;
+            const float pb = __fdiv_rn(sums[idx], fM);
+            const uint32_t wd = __ballot_sync(0xffffffffu, live && pb > a.theta);
+            if (rr == 0 && (t >> 3) < 4 * a.bits_stride)
+                reinterpret_cast<uint8_t*>(a.bits + (size_t)k * a.bits_stride)[t >> 3] = (uint8_t)(wd >> (lane & 24));
+            if (live) {
+                a.pbar[(size_t)k * a.row_stride + t] = pb;
+                a.mm[(size_t)k * a.row_stride + t] = smm[idx];
+            }
+            sums[idx] = 0.f, smm[idx] = 0;
+        }
+    };
+
+    int wi = blockIdx.x;
+    if (wi >= nitems) return;
+    C128Item cur = decode(wi), nxt = cur;
+    uint32_t step = 0;
+    stage_load(cur, 0, 0);
+    for (; wi < nitems; wi += gridDim.x) {
+        const bool more = wi + (int)gridDim.x < nitems;
+        if (more) nxt = decode(wi + gridDim.x);
+        for (int m = 0; m < a.M; m++, step++) {
+            const int buf = step & 1;
+            // the next step's rows go to the other stage (released by the barrier that ended the step before this one)
+            if (m + 1 < a.M || more) {
+                if (m + 1 < a.M) stage_load(cur, m + 1, buf ^ 1);
+                else stage_load(nxt, 0, buf ^ 1);
+                asm volatile("cp.async.wait_group 1;" ::: "memory");
+            } else {
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
             }
             __syncthreads();
+            compute(cur, m, buf);
+            __syncthreads();
         }
-        wi = wn, m = mn, step++;
+        finalize(cur);
+        __syncthreads();
+        cur = nxt;
     }
 }
 
@@ -450,6 +491,12 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
         const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
         const int npass = (n_lags + C128_KS_MAX - 1) / C128_KS_MAX, KS = (n_lags + npass - 1) / npass;
         const int64_t nitems = groups * npass * (G / 8);
+        if (n % 8 != 0 || nitems > INT32_MAX || G > INT32_MAX) {           // (whole 8-row blocks; 32-bit item arithmetic)
+            k_heads_fused<128><<<(n + 255) / 256, 256, 0, st>>>(a);
+            gwi_count_launch(1);
+            GWI_CUDA_CHECK(cudaGetLastError());
+            return GWI_OK;
+        }
         static int sms = 0;
         if (!sms) {
             int dev = 0;
@@ -457,7 +504,8 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
             GWI_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
             GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_comb128, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c128_smem_bytes(C128_KS_MAX)));
         }
-        k_heads_comb128<<<(unsigned)std::min<int64_t>(nitems, sms), C128_THREADS, c128_smem_bytes(KS), st>>>(a, n_lags, KS, npass, G, groups, nitems);
+        k_heads_comb128<<<(unsigned)std::min<int64_t>(nitems, sms), C128_THREADS, c128_smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups,
+                                                                                                       (int)nitems);
     } else if (CH == 32) {
         k_heads_fused<32><<<(n + 255) / 256, 256, 0, st>>>(a);
     } else {
