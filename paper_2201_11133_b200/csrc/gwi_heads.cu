@@ -15,6 +15,7 @@
 // no per-model, per-slide probability array exists (it was 7.8 GB per hour of data at 33 slides and 4 models).
 #include <algorithm>
 #include <cstdint>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -69,27 +70,32 @@ __device__ __forceinline__ float sigmoid_fast(float y)
     asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(0.5f * y));
     return fmaf(0.5f, t, 0.5f);
 }
-__device__ __forceinline__ float2 h2f2(uint32_t a)
-{
-    __half2 h = *reinterpret_cast<__half2*>(&a);
-    return __half22float2(h);
-}
-
 __device__ __forceinline__ uint4 lds128(uint32_t addr)
 {
     uint4 v;
     asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
 }
-// contribution of 8 channels (one 16-byte chunk of v_H, v_L and W2) to y: one half2 accumulator of four products, to fp32
-__device__ __forceinline__ float chunk_y(uint4 h, uint4 l, uint4 w)
+// lo + hi of a half2 accumulator added to y in fp32: two mixed-precision multiply-adds by one (FHFMA)
+__device__ __forceinline__ float acc_to_y(uint32_t acc, float y)
+{
+    asm("{ .reg .f16 lo, hi, one;\n\t"
+        "mov.b32 {lo, hi}, %1;\n\t"
+        "mov.b16 one, 0x3C00;\n\t"
+        "fma.rn.f32.f16 %0, lo, one, %0;\n\t"
+        "fma.rn.f32.f16 %0, hi, one, %0; }"
+        : "+f"(y)
+        : "r"(acc));
+    return y;
+}
+// y + the contribution of 8 channels (one 16-byte chunk of v_H, v_L and W2): a half2 accumulator of four products
+__device__ __forceinline__ float chunk_acc(float y, uint4 h, uint4 l, uint4 w)
 {
     uint32_t acc = mul2h(add_relu2(l.x, h.x), w.x);
     acc = fma2h(add_relu2(l.y, h.y), w.y, acc);
     acc = fma2h(add_relu2(l.z, h.z), w.z, acc);
     acc = fma2h(add_relu2(l.w, h.w), w.w, acc);
-    const float2 f = h2f2(acc);
-    return f.x + f.y;
+    return acc_to_y(acc, y);
 }
 
 // ---- any lag list: one thread per sample, the lagged row of every evaluation comes from global memory / L2 ---------------
@@ -114,7 +120,7 @@ __global__ void __launch_bounds__(256) k_heads_fused(const __grid_constant__ Hea
             const uint4* vL = reinterpret_cast<const uint4*>(a.v[m] + a.lds * CH) + (tc - lag) * CHC;
             float y = a.b2[m];
 #pragma unroll 4
-            for (int c = 0; c < CHC; c++) y += chunk_y(__ldg(vH + c), __ldg(vL + c), sw[m * CHC + c]);
+            for (int c = 0; c < CHC; c++) y = chunk_acc(y, __ldg(vH + c), __ldg(vL + c), sw[m * CHC + c]);
             const float p = sigmoid_fast(y);
             if (a.prob) {
                 if (live) a.prob[((size_t)k * a.M + m) * a.row_stride + t] = p;
@@ -208,7 +214,7 @@ __global__ void __launch_bounds__(T * CJ * NG, MINB) k_heads_comb(const __grid_c
             const uint32_t sa = (NG * q + kg < K) ? sa0 - (uint32_t)(NG * BLK) * q : st0;
             float y = b2;
 #pragma unroll
-            for (int cc = 0; cc < CHC; cc++) y += chunk_y(h[cc], lds128(sa + cc * (T * 16)), lds128(sw + cc * 16));
+            for (int cc = 0; cc < CHC; cc++) y = chunk_acc(y, h[cc], lds128(sa + cc * (T * 16)), lds128(sw + cc * 16));
             const float p = sigmoid_fast(y);
             sum[q] = __fadd_rn(sum[q], p);                               // 0 + p0 = p0 exactly: the T1 expression
             if (p > a.theta) mk[q >> 2] |= 1u << (8 * (q & 3) + m);
@@ -255,45 +261,35 @@ __global__ void __launch_bounds__(T * CJ * NG, MINB) k_heads_comb(const __grid_c
 // request); rows sit 272 bytes apart, which makes the quarter-warp's 16-byte reads of eight neighbouring rows
 // conflict-free.  Lag lists longer than 33 are evaluated in passes of at most 33 lags, so that
 // two stages always fit.
-constexpr int C128_THREADS = 512, C128_KS_MAX = 33;
-constexpr int C128_ROWB = 272, C128_BLKB = 8 * C128_ROWB;
+//
+// The same kernel serves the 32-channel rows of the narrow architecture: there a lane holds whole rows (no quarters, no
+// butterfly), a warp = 16 rows x 2 groups of four comb blocks, blocks are 16 rows, CJ = 16 and rows sit 80 bytes apart.
+constexpr int DG_THREADS = 512, DG_KS_MAX = 33;
 
-__host__ __device__ constexpr size_t c128_smem_bytes(int KS)
-{
-    return (size_t)2 * (8 + KS - 1 + 8) * C128_BLKB + (size_t)8 * KS * 8 * 5 + HF_MAX_M * 256 + 16;
-}
+template <int CH>
+struct DiagGeom {
+    static constexpr int QN = CH / 32;                  // lanes per row (channel quarters)
+    static constexpr int T = CH == 128 ? 8 : 16;        // rows per block
+    static constexpr int CJ = CH == 128 ? 8 : 16;       // comb blocks per item
+    static constexpr int ROWB = CH * 2 + 16;            // row pitch in shared memory
+    static constexpr int BLKB = T * ROWB;
+    static constexpr size_t smem_bytes(int KS)
+    {
+        return (size_t)2 * (CJ + KS - 1 + CJ) * BLKB + (size_t)CJ * KS * T * 5 + HF_MAX_M * CH * 2 + 16;
+    }
+};
 
-struct C128Item {
+struct DiagItem {
     int c, r, ka, Kp;      // comb group, row group, first lag and number of lags of the pass
 };
 
-// lo + hi of a half2 accumulator added to y in fp32: two mixed-precision multiply-adds by one (FHFMA)
-__device__ __forceinline__ float acc_to_y(uint32_t acc, float y)
-{
-    asm("{ .reg .f16 lo, hi, one;\n\t"
-        "mov.b32 {lo, hi}, %1;\n\t"
-        "mov.b16 one, 0x3C00;\n\t"
-        "fma.rn.f32.f16 %0, lo, one, %0;\n\t"
-        "fma.rn.f32.f16 %0, hi, one, %0; }"
-        : "+f"(y)
-        : "r"(acc));
-    return y;
-}
-// y + the contribution of 8 channels (one 16-byte chunk of v_H, v_L and W2): a half2 accumulator of four products
-__device__ __forceinline__ float chunk_acc(float y, uint4 h, uint4 l, uint4 w)
-{
-    uint32_t acc = mul2h(add_relu2(l.x, h.x), w.x);
-    acc = fma2h(add_relu2(l.y, h.y), w.y, acc);
-    acc = fma2h(add_relu2(l.z, h.z), w.z, acc);
-    acc = fma2h(add_relu2(l.w, h.w), w.w, acc);
-    return acc_to_y(acc, y);
-}
-
-__global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_constant__ HeadsFusedArgs a, const int K, const int KS,
-                                                                  const int npass, const int G, const int groups, const int nitems)
+template <int CH>
+__global__ void __launch_bounds__(DG_THREADS, 1) k_heads_diag(const __grid_constant__ HeadsFusedArgs a, const int K, const int KS,
+                                                             const int npass, const int G, const int groups, const int nitems)
 {
     using namespace tc;
-    constexpr int T = 8, CJ = 8, JB = 4, NS = 8, CH = 128, ROWB = C128_ROWB, BLKB = C128_BLKB;
+    using GEO = DiagGeom<CH>;
+    constexpr int T = GEO::T, CJ = GEO::CJ, JB = 4, NS = 8, QN = GEO::QN, ROWB = GEO::ROWB, BLKB = GEO::BLKB, CHC = CH / 8;
     extern __shared__ __align__(128) uint8_t smem[];
     const int nblk_max = CJ + KS - 1;
     const uint32_t sbase = smem_u32(smem);
@@ -303,44 +299,59 @@ __global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_
     uint8_t* smm = reinterpret_cast<uint8_t*>(sums + nsum);                             // same order
     const uint32_t w2off = 2 * stage_bytes + nsum * 5;                                  // W2 of all models, 256 B each
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int q = lane >> 3, row = lane & 7, j0 = (warp & 1) * JB, slot = warp >> 1;
+    // CH = 128: lane = (quarter, row), the warp serves one group of JB comb blocks; CH = 32: lane = (group, row)
+    const int q = QN == 4 ? lane >> 3 : 0, row = lane & (T - 1);
+    const int j0 = (QN == 4 ? (warp & 1) : (warp & 1) * 2 + (lane >> 4)) * JB, slot = warp >> 1;
     const int64_t lo_row = -(int64_t)(K - 1) * G;
-    for (int e = tid; e < nsum; e += C128_THREADS) sums[e] = 0.f, smm[e] = 0;
-    for (int e = tid; e < a.M * 64; e += C128_THREADS) reinterpret_cast<uint32_t*>(smem + w2off)[e] = a.w2[e >> 6][e & 63];
+    for (int e = tid; e < nsum; e += DG_THREADS) sums[e] = 0.f, smm[e] = 0;
+    for (int e = tid; e < a.M * (CH / 2); e += DG_THREADS) reinterpret_cast<uint32_t*>(smem + w2off)[e] = a.w2[e / (CH / 2)][e % (CH / 2)];
     __syncthreads();
 
     auto decode = [&](int wi) {
-        C128Item it;
+        DiagItem it;
         it.c = wi % groups;
         const int x = wi / groups, p = x % npass;
         it.r = x / npass;
         it.ka = p * KS, it.Kp = min(KS, K - it.ka);
         return it;
     };
-    // all warps: the rows of model m of an item into stage buf, 16 bytes per cp.async.  A block = 8 consecutive rows = 2 KB
-    // contiguous in global memory = four warp-wide copies; blocks start at multiples of 8 and n is one, so a block is
-    // inside the rows or outside (then any block will do: its items are dropped).  One commit group per step.
-    auto stage_load = [&](const C128Item& it, int m, int buf) {
+    // all warps: the rows of model m of an item into stage buf, 16 bytes per cp.async.  A block = T consecutive rows,
+    // contiguous in global memory (2 KB or 1 KB): a warp-wide copy moves 512 bytes of it.  128-channel rows: blocks
+    // start at multiples of 8 and n is one, so a block is inside the rows or outside (then any block will do: its items
+    // are dropped); 32-channel rows (any n): every row is clamped.  One commit group per step.
+    auto stage_load = [&](const DiagItem& it, int m, int buf) {
+        constexpr int RW = 32 / CHC, NX = T / RW;                       // rows per warp-wide copy, copies per block
         const int nblk = CJ + it.Kp - 1;
-        const __half* vH = a.v[m] + (lane >> 4) * CH + (lane & 15) * 8;
+        const int cr = lane / CHC, ch = lane % CHC;
+        const __half* vH = a.v[m] + ch * 8;
         const __half* vL = vH + a.lds * CH;
-        const uint32_t dst0 = sbase + buf * stage_bytes + (lane >> 4) * ROWB + (lane & 15) * 16;
+        const uint32_t dst0 = sbase + buf * stage_bytes + cr * ROWB + ch * 16;
         const int gL = it.c * CJ - (it.Kp - 1) - it.ka, gH = it.c * CJ - nblk;
-        for (int blk = warp; blk < nblk + CJ; blk += C128_THREADS / 32) {
+        for (int blk = warp; blk < nblk + CJ; blk += DG_THREADS / 32) {
             const bool isL = blk < nblk;
             int64_t s0 = (int64_t)((isL ? gL : gH) + blk) * G + T * it.r;
             const int64_t lo = isL ? lo_row : 0;
-            s0 = s0 < lo ? lo : (s0 > a.n - T ? a.n - T : s0);
-            const __half* src = (isL ? vL : vH) + s0 * CH;
             const uint32_t dst = dst0 + (isL ? blk : nblk_max + blk - nblk) * BLKB;
+            const __half* base = isL ? vL : vH;
+            if (CH == 128) {
+                s0 = s0 < lo ? lo : (s0 > a.n - T ? a.n - T : s0);
+                const __half* src = base + (s0 + cr) * CH;
 #pragma unroll
-            for (int x = 0; x < 4; x++) cp_async16(dst + 2 * x * ROWB, src + 2 * x * CH);
+                for (int x = 0; x < NX; x++) cp_async16(dst + x * RW * ROWB, src + x * RW * CH);
+            } else {
+#pragma unroll
+                for (int x = 0; x < NX; x++) {
+                    int64_t sr = s0 + cr + x * RW;
+                    sr = sr < lo ? lo : (sr > a.n - 1 ? a.n - 1 : sr);
+                    cp_async16(dst + x * RW * ROWB, base + sr * CH);
+                }
+            }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
     // one model of an item on the rows of stage buf
-    auto compute = [&](const C128Item& it, int m, int buf) {
+    auto compute = [&](const DiagItem& it, int m, int buf) {
         const int Kp = it.Kp, nblk = CJ + Kp - 1;
         const uint32_t bb = sbase + buf * stage_bytes + row * ROWB + q * 64;
         uint4 h[JB][4], w[4];
@@ -349,7 +360,7 @@ __global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_
 #pragma unroll
             for (int cc = 0; cc < 4; cc++) h[jj][cc] = lds128(bb + (nblk_max + j0 + jj) * BLKB + cc * 16);
 #pragma unroll
-        for (int cc = 0; cc < 4; cc++) w[cc] = lds128(sbase + w2off + m * 256 + q * 64 + cc * 16);
+        for (int cc = 0; cc < 4; cc++) w[cc] = lds128(sbase + w2off + m * (CH * 2) + q * 64 + cc * 16);
         const float b2 = a.b2[m];
         const bool hi = q & 2, od = q & 1;
         for (int i = slot; i < nblk; i += NS) {
@@ -375,33 +386,52 @@ __global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_
                     }
                 }
             }
-            // transposing butterfly over the four quarters: the lane of quarter jj ends with the whole sum of item jj
-            float k0 = hi ? y[2] : y[0], k1 = hi ? y[3] : y[1];
-            k0 += __shfl_xor_sync(0xffffffffu, hi ? y[0] : y[2], 16);
-            k1 += __shfl_xor_sync(0xffffffffu, hi ? y[1] : y[3], 16);
-            float yy = od ? k1 : k0;
-            yy += __shfl_xor_sync(0xffffffffu, od ? k0 : k1, 8);
-            const int k = kb + q;
-            if (k >= 0 && k < Kp) {
-                const float p = sigmoid_fast(yy + b2);
-                const int idx = ((j0 + q) * KS + k) * T + row;
-                sums[idx] = __fadd_rn(sums[idx], p);                    // 0 + p0 = p0 exactly: the T1 expression
-                if (p > a.theta) smm[idx] |= (uint8_t)(1u << m);
+            if (QN == 4) {
+                // transposing butterfly over the four quarters: the lane of quarter jj ends with the whole sum of item jj
+                float k0 = hi ? y[2] : y[0], k1 = hi ? y[3] : y[1];
+                k0 += __shfl_xor_sync(0xffffffffu, hi ? y[0] : y[2], 16);
+                k1 += __shfl_xor_sync(0xffffffffu, hi ? y[1] : y[3], 16);
+                float yy = od ? k1 : k0;
+                yy += __shfl_xor_sync(0xffffffffu, od ? k0 : k1, 8);
+                const int k = kb + q;
+                if (k >= 0 && k < Kp) {
+                    const float p = sigmoid_fast(yy + b2);
+                    const int idx = ((j0 + q) * KS + k) * T + row;
+                    sums[idx] = __fadd_rn(sums[idx], p);                // 0 + p0 = p0 exactly: the T1 expression
+                    if (p > a.theta) smm[idx] |= (uint8_t)(1u << m);
+                }
+            } else {
+#pragma unroll
+                for (int jj = 0; jj < JB; jj++) {
+                    const int k = kb + jj;
+                    if (k >= 0 && k < Kp) {
+                        const float p = sigmoid_fast(y[jj] + b2);
+                        const int idx = ((j0 + jj) * KS + k) * T + row;
+                        sums[idx] = __fadd_rn(sums[idx], p);
+                        if (p > a.theta) smm[idx] |= (uint8_t)(1u << m);
+                    }
+                }
             }
         }
     };
     // mean, threshold, outputs of the item; the sums go back to zero.  Thread = (row, comb block j, lag slot)
-    auto finalize = [&](const C128Item& it) {
+    auto finalize = [&](const DiagItem& it) {
         const float fM = (float)a.M;
-        const int rr = tid & 7, j = (tid >> 3) & 7;
+        const int rr = tid % T, j = (tid / T) % CJ;
         const int64_t t = (int64_t)(it.c * CJ + j) * G + T * it.r + rr;
         const bool live = t < a.n;
-        for (int kk = tid >> 6; kk < it.Kp; kk += C128_THREADS / 64) {  // warp-uniform
+        for (int kk = tid / (T * CJ); kk < it.Kp; kk += DG_THREADS / (T * CJ)) {   // warp-uniform
             const int idx = (j * KS + kk) * T + rr, k = it.ka + kk;
             const float pb = __fdiv_rn(sums[idx], fM);
             const uint32_t wd = __ballot_sync(0xffffffffu, live && pb > a.theta);
-            if (rr == 0 && (t >> 3) < 4 * a.bits_stride)
-                reinterpret_cast<uint8_t*>(a.bits + (size_t)k * a.bits_stride)[t >> 3] = (uint8_t)(wd >> (lane & 24));
+            // the warp holds 32 / T blocks of T samples: each writes its T mask bits
+            if (rr == 0) {
+                if (T == 16) {
+                    if ((t >> 4) < 2 * a.bits_stride) reinterpret_cast<uint16_t*>(a.bits + (size_t)k * a.bits_stride)[t >> 4] = (uint16_t)(wd >> (lane & 16));
+                } else {
+                    if ((t >> 3) < 4 * a.bits_stride) reinterpret_cast<uint8_t*>(a.bits + (size_t)k * a.bits_stride)[t >> 3] = (uint8_t)(wd >> (lane & 24));
+                }
+            }
             if (live) {
                 a.pbar[(size_t)k * a.row_stride + t] = pb;
                 a.mm[(size_t)k * a.row_stride + t] = smm[idx];
@@ -412,7 +442,7 @@ __global__ void __launch_bounds__(C128_THREADS, 1) k_heads_comb128(const __grid_
 
     int wi = blockIdx.x;
     if (wi >= nitems) return;
-    C128Item cur = decode(wi), nxt = cur;
+    DiagItem cur = decode(wi), nxt = cur;
     uint32_t step = 0;
     stage_load(cur, 0, 0);
     for (; wi < nitems; wi += gridDim.x) {
@@ -466,16 +496,45 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
     }
     a.lds = lds, a.n = n, a.M = M, a.n_lags = n_lags, a.lags = d_lags, a.theta = theta;
     a.bits = d_bits, a.bits_stride = bits_stride, a.pbar = d_pbar, a.mm = d_mm, a.row_stride = row_stride, a.prob = d_prob;
-    // regular lag list k G (G a multiple of 16, mean rule): the comb schedule (<= 34 slides of 32 channels, <= 64 of 128)
-    const int kmax = CH == 32 ? 34 : 64;
-    bool comb = !d_prob && n_lags >= 2 && n_lags <= kmax && h_lags != nullptr;
+    // regular lag list k G (G a multiple of 16, mean rule): the comb schedule, in passes of at most DG_KS_MAX lags
+    bool comb = !d_prob && n_lags >= 2 && h_lags != nullptr;
     int64_t G = 0;
     if (comb) {
         G = h_lags[1];
         comb = G > 0 && G % 16 == 0;
         for (int k = 0; k < n_lags && comb; k++) comb = h_lags[k] == (int64_t)k * G;
     }
-    if (comb && CH == 32) {
+    // 32-channel rows, up to 34 slides: the thread-per-item comb kernel below (measured 9 % faster per hour than the
+    // diagonal kernel there: 18.9 against 20.7 ms with 33 lags, the per-item work is too small to pay for the running sums
+    // in shared memory); longer lists and 128-channel rows: the diagonal kernel
+    if (comb && (CH == 32 ? n_lags > 34 : n % 8 == 0)) {
+        const int T = CH == 32 ? DiagGeom<32>::T : DiagGeom<128>::T, CJ = CH == 32 ? DiagGeom<32>::CJ : DiagGeom<128>::CJ;
+        const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
+        const int npass = (n_lags + DG_KS_MAX - 1) / DG_KS_MAX, KS = (n_lags + npass - 1) / npass;
+        const int64_t nitems = groups * npass * (G / T);
+        comb = nitems <= INT32_MAX && G <= INT32_MAX;                    // 32-bit item arithmetic in the kernel
+        if (comb) {
+            static int sms = 0;
+            if (!sms) {
+                int dev = 0;
+                GWI_CUDA_CHECK(cudaGetDevice(&dev));
+                GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                    (int)DiagGeom<32>::smem_bytes(DG_KS_MAX)));
+                GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                    (int)DiagGeom<128>::smem_bytes(DG_KS_MAX)));
+                GWI_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            }
+            const unsigned grid = (unsigned)std::min<int64_t>(nitems, sms);
+            if (CH == 32)
+                k_heads_diag<32><<<grid, DG_THREADS, DiagGeom<32>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
+            else
+                k_heads_diag<128><<<grid, DG_THREADS, DiagGeom<128>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
+            gwi_count_launch(1);
+            GWI_CUDA_CHECK(cudaGetLastError());
+            return GWI_OK;
+        }
+    }
+    if (comb && CH == 32 && n_lags <= 34) {
         constexpr int CJ = 16;
         auto kern = k_heads_comb<32, 16, CJ, 2, 17, 2, 2>;
         const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
@@ -486,26 +545,6 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
             attr = true;
         }
         kern<<<(unsigned)(groups * (G / 16)), 512, smem, st>>>(a, n_lags, G);
-    } else if (comb) {
-        constexpr int CJ = 8;
-        const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
-        const int npass = (n_lags + C128_KS_MAX - 1) / C128_KS_MAX, KS = (n_lags + npass - 1) / npass;
-        const int64_t nitems = groups * npass * (G / 8);
-        if (n % 8 != 0 || nitems > INT32_MAX || G > INT32_MAX) {           // (whole 8-row blocks; 32-bit item arithmetic)
-            k_heads_fused<128><<<(n + 255) / 256, 256, 0, st>>>(a);
-            gwi_count_launch(1);
-            GWI_CUDA_CHECK(cudaGetLastError());
-            return GWI_OK;
-        }
-        static int sms = 0;
-        if (!sms) {
-            int dev = 0;
-            GWI_CUDA_CHECK(cudaGetDevice(&dev));
-            GWI_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-            GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_comb128, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c128_smem_bytes(C128_KS_MAX)));
-        }
-        k_heads_comb128<<<(unsigned)std::min<int64_t>(nitems, sms), C128_THREADS, c128_smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups,
-                                                                                                       (int)nitems);
     } else if (CH == 32) {
         k_heads_fused<32><<<(n + 255) / 256, 256, 0, st>>>(a);
     } else {

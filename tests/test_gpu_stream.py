@@ -314,6 +314,20 @@ def test_config3_recipe_32_slides(tmpdir_s):
     assert got == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 64) and got == sorted(got)
 
 
+def test_stream_narrow_arch_40_regular_lags_two_passes(tmpdir_s):
+    """More regular lags than one pass of the comb heads holds (34): the diagonal kernel in two passes of 21 and 20 lags,
+    on chunk lengths that are not multiples of its 16-row blocks."""
+    import paper_2201_11133_b200 as gwi
+    oms, gms = _models(tmpdir_s, [0, 1, 2], gwi.FP16)
+    N = 41 * 256 + 3000 + 7
+    x = gs.stream_noise(36, 0, N, dtype=np.float16)
+    lags = [k * 256 for k in range(1, 41)]
+    want = _oracle_slides(oms, x, lags)
+    n, recs, pbar = _run_stream(gms, x, _ragged(N, 4, 1000, 5000), lags, 0.5, 40, max_chunk=5000)
+    assert np.max(np.abs(pbar - want)) <= 2e-3
+    assert trig_tuples(recs) == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 40)
+
+
 def test_stream_paper_scale_slides_tensor_core_back_end(tmpdir_s):
     """FP16 stream of paper-scale models WITH time slides: chunks re-blocked into whole segments, L1 feature tiles kept
     as history, one tcgen05 head launch per lag.  Parity with the oracle; chunked == unchunked bit for bit."""
