@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(256) k_heads_fused(const __grid_constant__ Hea
 // apart, t = (c CJ + j) G + T r + [0, T), j < CJ: for all K lags it needs only the CJ + K - 1 blocks of v_L rows at
 // (c CJ + i) G + T r, -K < i < CJ, which it stages in shared memory once per model: with T = 16 rows of 32 channels, 48 KB
 // feed 8448 evaluations, 8 x fewer bytes from L2 than one row per evaluation (double-buffered over the models: the next
-// model's blocks arrive by cp.async while this one is evaluated).  (128-channel rows: k_heads_comb128 below.)
+// model's blocks arrive by cp.async while this one is evaluated).  (128-channel rows and longer lists: k_heads_diag below.)
 // Threads = T rows x CJ blocks x NG interleaved groups of the lag list; a thread
 // keeps the running sums of its <= KQ lags in registers across the models (fixed order m = 0, 1, ...: the T1 expression).
 
