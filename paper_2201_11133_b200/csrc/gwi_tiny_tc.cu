@@ -58,10 +58,6 @@ constexpr int W1_B = 32 * 80 * 2;               // N = 32 x K = 80 ([u_H | u_L] 
 constexpr int ONES_B = 2 * 128 * 16;            // A operand of the bias steps: 128 rows x K = 16, element (r, 0) = 1
 constexpr int SR = 16;                          // stashed operand rows per (branch, block)
 constexpr int STASH_SLOT = 2 * TT_MAX_L * 2 * SR * 16;   // [branch][block][chunk][SR rows] x 16 B = 8 KB
-// k_tiny_tc2 (deferred residual, L <= 4): GEMM1 of block i >= 1 also contracts z' of block i - 1 with pre-multiplied weights
-constexpr int TT2_MAX_L = 4;
-constexpr int WFG2_L = 32 * 80 * 2;             // N = 32 x K = 80 (X past | X current | Z past | Z current | bias step)
-constexpr int STASH2_SLOT = 2 * (2 * TT2_MAX_L * 2 * SR * 16);   // X rows and Z rows: [branch][block][chunk][SR rows] x 16 B each = 8 KB
 constexpr int TCOLS = 80;                       // TMEM columns per slot: f 0-15, g 16-31 (z' over 16-23), h 32-47, skip 48-79
 
 struct TtArgs {
@@ -78,7 +74,6 @@ struct TtArgs {
     // constant-bank operands
     float lift[2][32];            // W_in[16], b_in[16]
     float head[33];               // W2[32], b2
-    float br[2][4][16];           // k_tiny_tc2: residual-conv biases (the operand of block i + 1 is fp16(h_i + br_i))
 };
 
 __device__ __forceinline__ void named_bar(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
@@ -272,9 +267,7 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
                     const uint64_t bw = dWfg + (uint64_t)(((b * L + i) * WFG_L) >> 4);
                     tc_mma_f16(tcol, dX - d, bw, idesc32, 0u);
                     tc_mma_f16(tcol, dX, bw + ((2 * 32 * 16) >> 4), idesc32, 1u);
-#ifndef GWI_TT_NOBIAS
                     tc_mma_f16(tcol, dOnes, bw + ((4 * 32 * 16) >> 4), idesc32, 1u);       // + bf | bg/2
-#endif
                 });
                 // ---- gate: z' = tanh(f) (1 + tanh(g/2)) (biases already in the accumulators), fp16, over the g columns = A operand of GEMM2
                 {
@@ -305,9 +298,7 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
                 mma_round([&] {
                     const uint64_t bw = dWrs + (uint64_t)(((b * L + i) * WRS_L) >> 4);
                     tc_mma_f16_ts(tcol + 32, tcol + 16, bw, idesc48, 1u);
-#ifndef GWI_TT_NOBIAS
                     tc_mma_f16(tcol + 32, dOnes, bw + ((2 * 48 * 16) >> 4), idesc48, 1u);   // + br | bs
-#endif
                 });
                 if (i < L - 1) {
                     // ---- operand of the next block: fp16(h)
@@ -395,281 +386,6 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
     if (warp == 0) tmem_dealloc(tmem, 512);
 }
 
-// ---- k_tiny_tc2: the same path with the residual update off the critical chain ("deferred residual") --------------------
-// In k_tiny_tc a block costs two MMA round trips (GEMM1 -> gate, GEMM2 -> operand of the next block), and the ~500 clocks
-// of each (barrier, issue, completion, mbarrier, wake) are what the six slots cannot hide.  By linearity the input of
-// block i + 1 is h_i + br_i + (Wr_i / 2) z'_i, so
-//
-//   f|g of block i + 1 = [X(t-d) | X(t)] . Wfg^T + [Z(t-d) | Z(t)] . (Wfg (Wr_i / 2))^T + b,    X = fp16(h_i + br_i), Z = z'_i
-//
-// with the products Wfg_{i+1} Wr_i folded on the host (fp16 of the product of the fp16 weights): GEMM1 of block i + 1
-// no longer waits for GEMM2 of block i.  Both go out in ONE round after the gate of block i: GEMM2_i (fp32 master of h
-// and the skip sum in tensor memory, as before) and GEMM1_{i+1}; the master h_i that X needs was completed by the
-// round before.  A branch is L + 1 rounds instead of 2 L.  z' is an operand in shared memory now (the dilated tap needs
-// row offsets), with its own stash of the last 16 rows per (branch, block).  Rows before the stream start are zero in X
-// and in Z (reading A4).  Used for L <= 4 blocks with all dilations <= 16 (BASELINE.json configs 3-5).
-template <int LT>
-__global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc2(const __grid_constant__ TtArgs a)
-{
-    extern __shared__ __align__(1024) uint8_t smem[];
-    const int L = LT ? LT : a.L;
-    const int OFF_WRS = 2 * L * WFG2_L, OFF_W1 = OFF_WRS + 2 * L * WRS_L, OFF_ONES = OFF_W1 + W1_B,
-              OFF_X = (OFF_ONES + ONES_B + 1023) & ~1023;
-    const int OFF_STASH = OFF_X + NSLOT * 2 * X_SLOT;             // per slot: X buffer, Z buffer
-    const int OFF_BAR = OFF_STASH + NSLOT * STASH2_SLOT;
-    const uint32_t sbase = smem_u32(smem);
-    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
-    const int slot = warp >> 2, q = warp & 3;
-    const int r = q * 32 + lane;                                  // row of the tile = TMEM lane
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + OFF_BAR + 8 * NSLOT);
-    {
-        const uint4* src = reinterpret_cast<const uint4*>(a.w);
-        uint4* dst = reinterpret_cast<uint4*>(smem);
-        for (int i = threadIdx.x; i < (OFF_W1 + W1_B) / 16; i += TT_THREADS) dst[i] = __ldg(src + i);
-        uint4* on = reinterpret_cast<uint4*>(smem + OFF_ONES);
-        for (int i = threadIdx.x; i < ONES_B / 16; i += TT_THREADS) on[i] = make_uint4(i < 128 ? 0x3C00u : 0u, 0, 0, 0);   // half(1.0) at k = 0
-        uint4* zx = reinterpret_cast<uint4*>(smem + OFF_X);
-        for (int i = threadIdx.x; i < NSLOT * (2 * X_SLOT + STASH2_SLOT) / 16; i += TT_THREADS) zx[i] = make_uint4(0, 0, 0, 0);
-        if (threadIdx.x == 0) {
-            for (int i = 0; i < NSLOT; i++) mbar_init(sbase + OFF_BAR + 8 * i, 1);
-            mbar_fence_init();
-        }
-    }
-    if (warp == 0) tmem_alloc(smem_u32(tmem_slot), 512);
-    fence_proxy_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);
-    const uint32_t tcol = tmem + TCOLS * slot;                    // the slot's columns (lane field 0: MMA operands)
-    const uint32_t tlane = tcol + ((uint32_t)(q * 32) << 16);     // this warp's lane quadrant (tcgen05.ld / st)
-    const uint32_t mbar = sbase + OFF_BAR + 8 * slot;
-    const uint32_t xs = sbase + OFF_X + slot * 2 * X_SLOT, zs = xs + X_SLOT;   // operand buffers; row 0 of the tile at + PADR * 16
-    const bool leader = q == 0;
-    uint32_t ph = 0;
-    const uint32_t idesc32 = make_idesc_f16(128, 32), idesc48 = make_idesc_f16(128, 48);
-    const uint64_t dX = make_sdesc(xs + PADR * 16, X_CH, 128), dZ = make_sdesc(zs + PADR * 16, X_CH, 128);
-    const uint64_t dWfg = make_sdesc(sbase, 32 * 16, 128), dWrs = make_sdesc(sbase + OFF_WRS, 48 * 16, 128),
-                   dW1 = make_sdesc(sbase + OFF_W1, 32 * 16, 128), dOnes = make_sdesc(sbase + OFF_ONES, 128 * 16, 128);
-    // rows 128 - SR .. 127 exchange their operand row with the stash of (buffer, branch, block): the row kept from the
-    // previous tile goes in front of the tile (rows -SR .. -1 of the buffer), the new one is kept for the next tile
-    const bool tail = r >= 128 - SR;
-    const uint32_t stash0 = sbase + OFF_STASH + slot * STASH2_SLOT + (r - (128 - SR)) * 16;
-    // which = 0: X (block input), 1: Z (gate output); bi = branch * TT2_MAX_L + block
-    auto put_operand = [&](int which, int bi, const uint32_t (&pk)[8]) {
-        const uint32_t row = xs + which * X_SLOT + (PADR + r) * 16;
-        st_shared_v4(row, pk[0], pk[1], pk[2], pk[3]);
-        st_shared_v4(row + X_CH, pk[4], pk[5], pk[6], pk[7]);
-        if (tail) {
-            const uint32_t sa = stash0 + (which * 2 * TT2_MAX_L + bi) * (2 * SR * 16);
-            const uint32_t pre = row - 128 * 16;                  // row r - 128 of the buffer = PADR - SR + (r - (128 - SR))
-            const uint4 o0 = ld_shared_v4(sa), o1 = ld_shared_v4(sa + SR * 16);
-            st_shared_v4(pre, o0.x, o0.y, o0.z, o0.w);
-            st_shared_v4(pre + X_CH, o1.x, o1.y, o1.z, o1.w);
-            st_shared_v4(sa, pk[0], pk[1], pk[2], pk[3]);
-            st_shared_v4(sa + SR * 16, pk[4], pk[5], pk[6], pk[7]);
-        }
-    };
-#ifdef GWI_TT_TRACE
-    int tt_k = 0;
-#endif
-    auto mma_round = [&](auto&& f) {
-        TT_TRACE(1);
-        if (leader) named_bar(1 + slot, 128);
-        else asm volatile("bar.arrive %0, %1;" ::"r"(1 + slot), "r"(128) : "memory");
-        TT_TRACE(2);
-        if (leader) {
-            if (elect_one()) {
-                tc_fence_after();
-                f();
-                tc_commit(mbar);
-            }
-            __syncwarp();
-        }
-        TT_TRACE(3);
-        mbar_wait_sleep(mbar, ph, GWI_TT_SLEEP_NS);
-        ph ^= 1;
-        tc_fence_after();
-        TT_TRACE(4);
-    };
-
-    // the slot's span [k0, k1) of the tiles, preceded by the warm-up tile k0 - 1 (nothing stored, fills the stashes)
-    const int64_t gs = (int64_t)blockIdx.x * NSLOT + slot, ns = (int64_t)gridDim.x * NSLOT;
-    const int k0 = (int)(gs * a.ntiles / ns), k1 = (int)((gs + 1) * a.ntiles / ns);
-    for (int tile = k0 < k1 ? k0 - 1 : k0; tile < k1; tile++) {
-        const int64_t tl = (int64_t)tile * 128 + r;              // chunk-local time of this thread's row
-        const bool dead = a.t0 + tl < 0;                          // before the stream start: zero at every layer input (A4)
-        const bool store = tile >= k0 && tl >= 0 && tl < a.n;
-        uint32_t uH[16];                                          // u of branch 0 (fp16 pairs), parked while branch 1 runs
-#pragma unroll 1
-        for (int b = 0; b < 2; b++) {
-            // ---- lift (C.1 step 1): h0 = W_in x + b_in -> fp32 master in TMEM; X = fp16(h0); skip sum starts at 0
-            {
-                float x = 0.f;
-                if (tl >= 0) {
-                    if (tl < a.n) x = __half2float(a.x[(int64_t)b * a.ldx + tl]);
-                } else if (tl >= -a.halo) {
-                    x = __half2float(a.xh[b * a.halo + a.halo + tl]);
-                }
-                uint32_t hv[16], pk[8];
-#pragma unroll
-                for (int c = 0; c < 16; c++) hv[c] = __float_as_uint(dead ? 0.f : fmaf(a.lift[b][c], x, a.lift[b][16 + c]));
-#pragma unroll
-                for (int c = 0; c < 8; c++) pk[c] = pack_half2(__uint_as_float(hv[2 * c]), __uint_as_float(hv[2 * c + 1]));
-                tmem_st16(tlane + 32, hv);
-                uint32_t sv[16];
-#pragma unroll
-                for (int c = 0; c < 16; c++) sv[c] = 0u;
-                tmem_st16(tlane + 48, sv);                        // the bs_i arrive with GEMM2's bias step
-                tmem_st16(tlane + 64, sv);
-                put_operand(0, b * TT2_MAX_L, pk);
-                tc_wait_st();
-                fence_proxy_async_smem();
-                tc_fence_before();
-            }
-            // ---- round 0: GEMM1 of block 0 on X alone                                          (C.1 step 2)
-            mma_round([&] {
-                const uint64_t bw = dWfg + (uint64_t)(((b * L) * WFG2_L) >> 4);
-                tc_mma_f16(tcol, dX - a.dil[0], bw, idesc32, 0u);
-                tc_mma_f16(tcol, dX, bw + 64, idesc32, 1u);
-#ifndef GWI_TT_NOBIAS
-                tc_mma_f16(tcol, dOnes, bw + 4 * 64, idesc32, 1u);                           // + bf | bg/2
-#endif
-            });
-#pragma unroll
-            for (int i = 0; i < (LT ? LT : L); i++) {
-                // ---- after GEMM1 of block i (and GEMM2 of block i - 1: the master h_i is complete):
-                // gate z' = tanh(f) (1 + tanh(g/2)) -> Z rows; X rows of block i + 1 = fp16(h_i + br_i)
-                {
-                    uint32_t f[16], g[16], hv[16], pk[8];
-                    tmem_ld16(tlane, f);
-                    tmem_ld16(tlane + 16, g);
-                    if (i < L - 1) tmem_ld16(tlane + 32, hv);
-                    tc_wait_ld();
-                    TT_TRACE(5);
-#pragma unroll
-                    for (int c = 0; c < 8; c++) {
-#ifdef GWI_TT_NOMUFU   // diagnostic only: the chain without the MUFU work
-                        const float t0 = __uint_as_float(f[2 * c]) * 0.5f, t1 = __uint_as_float(f[2 * c + 1]) * 0.5f;
-                        const float s0 = __uint_as_float(g[2 * c]) * 0.5f, s1 = __uint_as_float(g[2 * c + 1]) * 0.5f;
-#else
-                        const float t0 = tanh_approx(__uint_as_float(f[2 * c])), t1 = tanh_approx(__uint_as_float(f[2 * c + 1]));
-                        const float s0 = tanh_approx(__uint_as_float(g[2 * c])), s1 = tanh_approx(__uint_as_float(g[2 * c + 1]));
-#endif
-                        pk[c] = dead ? 0u : pack_half2(fmaf(t0, s0, t0), fmaf(t1, s1, t1));
-                    }
-                    TT_TRACE(6);
-                    put_operand(1, b * TT2_MAX_L + i, pk);
-                    TT_TRACE(7);
-                    if (i < L - 1) {
-#pragma unroll
-                        for (int c = 0; c < 8; c++)
-                            pk[c] = dead ? 0u : pack_half2(__uint_as_float(hv[2 * c]) + a.br[b][i][2 * c], __uint_as_float(hv[2 * c + 1]) + a.br[b][i][2 * c + 1]);
-                        put_operand(0, b * TT2_MAX_L + i + 1, pk);
-                    }
-                    TT_TRACE(9);
-                    fence_proxy_async_smem();
-                    tc_fence_before();
-                    TT_TRACE(10);
-                }
-                // ---- one round: GEMM2 of block i ([h | skip] += z' . [Wr/2 | Ws/2]^T + br | bs; the last block's residual
-                // conv is dead, reading A8) and GEMM1 of block i + 1
-                mma_round([&] {
-                    const uint64_t bw2 = dWrs + (uint64_t)(((b * L + i) * WRS_L) >> 4);
-                    if (i < L - 1) {
-                        const uint64_t bw = dWfg + (uint64_t)(((b * L + i + 1) * WFG2_L) >> 4);
-                        const int d = a.dil[i + 1];
-#ifdef GWI_TT2_NOSHIFT
-                        tc_mma_f16(tcol, dX, bw, idesc32, 0u);
-#else
-                        tc_mma_f16(tcol, dX - d, bw, idesc32, 0u);
-#endif
-                        tc_mma_f16(tcol, dX, bw + 64, idesc32, 1u);
-#ifndef GWI_TT2_NOZ
-                        tc_mma_f16(tcol, dZ - d, bw + 2 * 64, idesc32, 1u);
-                        tc_mma_f16(tcol, dZ, bw + 3 * 64, idesc32, 1u);
-#endif
-#ifndef GWI_TT_NOBIAS
-                        tc_mma_f16(tcol, dOnes, bw + 4 * 64, idesc32, 1u);
-#endif
-                    }
-                    tc_mma_f16(tcol + 32, dZ, bw2, idesc48, 1u);
-#ifndef GWI_TT_NOBIAS
-                    tc_mma_f16(tcol + 32, dOnes, bw2 + ((2 * 48 * 16) >> 4), idesc48, 1u);
-#endif
-                });
-            }
-            // ---- u_b = ReLU(skip sum)                                                         (C.1 step 3)
-            uint32_t u[16];
-            {
-                uint32_t sv[32];
-                tmem_ld32(tlane + 48, sv);
-                tc_wait_ld();
-#pragma unroll
-                for (int c = 0; c < 16; c++)
-                    u[c] = pack_half2(fmaxf(__uint_as_float(sv[2 * c]), 0.f), fmaxf(__uint_as_float(sv[2 * c + 1]), 0.f));
-            }
-            if (a.u16) {
-                // ---- time-slide mode: the branch's half of the head's first layer, v_b = W1[:, 32 b : 32 b + 32] u_b (+ b1 for
-                // b = 0).  W1 [u_H; u_L] + b1 = v_H[t] + v_L[t - lag] by linearity, so the per-lag work that follows
-                // (gwi_heads.cu) is element-wise: no contraction per (sample, lag).
-                tmem_st16(tlane + 32, u);
-                tc_wait_st();
-                tc_fence_before();
-                mma_round([&] {
-                    tc_mma_f16_ts(tcol, tcol + 32, dW1 + (uint64_t)(2 * b * 64), idesc32, 0u);
-                    tc_mma_f16_ts(tcol, tcol + 40, dW1 + (uint64_t)((2 * b + 1) * 64), idesc32, 1u);
-                    if (b == 0) tc_mma_f16(tcol, dOnes, dW1 + (uint64_t)(4 * 64), idesc32, 1u);
-                });
-                uint32_t v[32];
-                tmem_ld32(tlane, v);
-                tc_wait_ld();
-                if (store) {
-                    uint4* up = reinterpret_cast<uint4*>(a.u16 + ((size_t)b * a.lds + tl) * 32);
-#pragma unroll
-                    for (int c = 0; c < 4; c++)
-                        up[c] = make_uint4(pack_half2(__uint_as_float(v[8 * c]), __uint_as_float(v[8 * c + 1])),
-                                           pack_half2(__uint_as_float(v[8 * c + 2]), __uint_as_float(v[8 * c + 3])),
-                                           pack_half2(__uint_as_float(v[8 * c + 4]), __uint_as_float(v[8 * c + 5])),
-                                           pack_half2(__uint_as_float(v[8 * c + 6]), __uint_as_float(v[8 * c + 7])));
-                }
-                tc_fence_before();
-            } else if (b == 0) {
-#pragma unroll
-                for (int c = 0; c < 16; c++) uH[c] = u[c];
-            } else {
-                // ---- head (C.1 steps 4, 5): [u_H | u_L] as the A operand in TMEM (h and skip columns), D over the f|g columns
-                tmem_st16(tlane + 32, uH);
-                tmem_st16(tlane + 48, u);
-                tc_wait_st();
-                tc_fence_before();
-                mma_round([&] {
-#pragma unroll
-                    for (int kk = 0; kk < 4; kk++) tc_mma_f16_ts(tcol, tcol + 32 + 8 * kk, dW1 + (uint64_t)((kk * 2 * 32 * 16) >> 4), idesc32, kk > 0 ? 1u : 0u);
-                    tc_mma_f16(tcol, dOnes, dW1 + (uint64_t)((8 * 32 * 16) >> 4), idesc32, 1u);   // + b1
-                });
-                uint32_t v[32];
-                tmem_ld32(tlane, v);
-                tc_wait_ld();
-                float y0 = 0.f, y1 = 0.f, y2 = 0.f, y3 = 0.f;
-#pragma unroll
-                for (int c = 0; c < 32; c += 4) {
-                    y0 = fmaf(a.head[c], fmaxf(__uint_as_float(v[c]), 0.f), y0);
-                    y1 = fmaf(a.head[c + 1], fmaxf(__uint_as_float(v[c + 1]), 0.f), y1);
-                    y2 = fmaf(a.head[c + 2], fmaxf(__uint_as_float(v[c + 2]), 0.f), y2);
-                    y3 = fmaf(a.head[c + 3], fmaxf(__uint_as_float(v[c + 3]), 0.f), y3);
-                }
-                const float y = ((y0 + y1) + (y2 + y3)) + a.head[32];
-                if (store) a.prob[tl] = 1.0f / (1.0f + __expf(-y));
-                tc_fence_before();
-            }
-        }
-    }
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 0) tmem_dealloc(tmem, 512);
-}
-
 inline uint16_t h16(float v)
 {
     __half h = __float2half_rn(v);
@@ -685,10 +401,6 @@ struct GwiTinyTcPack {
     size_t w_bytes = 0;
     int smem = 0, num_sms = 148, halo = 16, stash = 0;
     float lift[2][32], head[33];
-    // k_tiny_tc2 (deferred residual): its own weight blob [2][L][WFG2_L] | [2][L][WRS_L] | W1_B, residual biases
-    uint8_t* d_w2 = nullptr;
-    int smem2 = 0;
-    float br[2][4][16];
 };
 
 bool gwi_tiny_tc_supported(const GwiArch& a)
@@ -756,45 +468,6 @@ gwi_status gwi_tiny_tc_pack(gwi_model* m)
     GWI_CUDA_CHECK(cudaMalloc((void**)&p->d_w, p->w_bytes));
     GWI_CUDA_CHECK(cudaMemcpy(p->d_w, w.data(), p->w_bytes, cudaMemcpyHostToDevice));
     p->smem = (int)(((off_w1 + W1_B + ONES_B + 1023) & ~(size_t)1023) + NSLOT * (X_SLOT + STASH_SLOT) + 8 * NSLOT + 16);
-    memset(p->br, 0, sizeof(p->br));
-    if (p->stash && L <= TT2_MAX_L) {
-        // deferred-residual kernel: GEMM1 of block i >= 1 gets two more K steps, (Wfg_i (Wr_{i-1} / 2)) per tap, folded from
-        // the fp16 weights the MMAs of k_tiny_tc see and rounded to fp16 once more
-        const size_t off_wrs2 = (size_t)2 * L * WFG2_L, off_w12 = off_wrs2 + (size_t)2 * L * WRS_L;
-        std::vector<uint16_t> w2(( off_w12 + W1_B) / 2, 0);
-        auto f16 = [&](float v) { return __half2float(__float2half_rn(v)); };
-        for (int b = 0; b < 2; b++) {
-            for (int i = 0; i < L; i++) {
-                const GwiLayerOff& lo = m->off.layer[b][i];
-                uint16_t* fg = w2.data() + ((size_t)(b * L + i) * WFG2_L) / 2;
-                auto wfg = [&](int n, int tap, int c) {
-                    return n < 16 ? W[lo.Wf + ((int64_t)n * 16 + c) * 2 + tap] : 0.5f * W[lo.Wg + ((int64_t)(n - 16) * 16 + c) * 2 + tap];
-                };
-                for (int n = 0; n < 32; n++) {
-                    for (int tap = 0; tap < 2; tap++) {
-                        for (int k = 0; k < 16; k++) {
-                            fg[tap * 512 + (k / 8) * 256 + n * 8 + k % 8] = h16(wfg(n, tap, k));
-                            if (i > 0) {
-                                const GwiLayerOff& lp = m->off.layer[b][i - 1];
-                                double acc = 0.0;
-                                for (int c = 0; c < 16; c++) acc += (double)f16(wfg(n, tap, c)) * (double)f16(0.5f * W[lp.Wr + (int64_t)c * 16 + k]);
-                                fg[(2 + tap) * 512 + (k / 8) * 256 + n * 8 + k % 8] = h16((float)acc);
-                            }
-                        }
-                    }
-                    fg[4 * 512 + n * 8] = h16(n < 16 ? W[lo.bf + n] : 0.5f * W[lo.bg + n - 16]);       // the bias step
-                }
-                for (int c = 0; c < 16; c++) p->br[b][i][c] = W[lo.br + c];
-                memcpy(w2.data() + (off_wrs2 + (size_t)(b * L + i) * WRS_L) / 2, w.data() + (off_wrs + (size_t)(b * L + i) * WRS_L) / 2, WRS_L);
-            }
-        }
-        memcpy(w2.data() + off_w12 / 2, w.data() + off_w1 / 2, W1_B);
-        GWI_CUDA_CHECK(cudaMalloc((void**)&p->d_w2, w2.size() * 2));
-        GWI_CUDA_CHECK(cudaMemcpy(p->d_w2, w2.data(), w2.size() * 2, cudaMemcpyHostToDevice));
-        p->smem2 = (int)(((off_w12 + W1_B + ONES_B + 1023) & ~(size_t)1023) + NSLOT * (2 * X_SLOT + STASH2_SLOT) + 8 * NSLOT + 16);
-        GWI_CUDA_CHECK(cudaFuncSetAttribute(k_tiny_tc2<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem2));
-        GWI_CUDA_CHECK(cudaFuncSetAttribute(k_tiny_tc2<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem2));
-    }
     cudaDeviceProp prop;
     GWI_CUDA_CHECK(cudaGetDeviceProperties(&prop, m->device));
     p->num_sms = prop.multiProcessorCount;
@@ -808,7 +481,6 @@ void gwi_tiny_tc_free(gwi_model* m)
     GwiTinyTcPack* p = m->tinytc;
     if (!p) return;
     cudaFree(p->d_w);
-    if (p->d_w2) cudaFree(p->d_w2);
     delete p;
     m->tinytc = nullptr;
 }
@@ -830,14 +502,7 @@ gwi_status gwi_tiny_tc_stream(const gwi_model* m, const __half* d_x, int64_t ldx
     memcpy(a.lift, p->lift, sizeof(a.lift)), memcpy(a.head, p->head, sizeof(a.head));
     const int slots = (a.ntiles + NSLOT - 1) / NSLOT;
     const int grid = slots < p->num_sms ? slots : p->num_sms;
-    // measured slower than k_tiny_tc (6.2 against 5.7 ms per 4-model hour): off unless asked for
-    static const bool v2 = [] { const char* e = getenv("GWI_TINY_V2"); return e && e[0] == '1'; }();
-    if (p->d_w2 && v2) {
-        a.w = p->d_w2;
-        memcpy(a.br, p->br, sizeof(a.br));
-        if (a.L == 4) k_tiny_tc2<4><<<grid, TT_THREADS, p->smem2, st>>>(a);
-        else k_tiny_tc2<0><<<grid, TT_THREADS, p->smem2, st>>>(a);
-    } else if (a.L == 4) k_tiny_tc<4><<<grid, TT_THREADS, p->smem, st>>>(a);
+    if (a.L == 4) k_tiny_tc<4><<<grid, TT_THREADS, p->smem, st>>>(a);
     else k_tiny_tc<0><<<grid, TT_THREADS, p->smem, st>>>(a);
     gwi_count_launch(1);
     GWI_CUDA_CHECK(cudaGetLastError());
