@@ -44,7 +44,10 @@ using namespace tc;
 
 namespace {
 
-constexpr int NSLOT = 6;
+#ifndef GWI_TT_NSLOT
+#define GWI_TT_NSLOT 6
+#endif
+constexpr int NSLOT = GWI_TT_NSLOT;
 constexpr int TT_THREADS = NSLOT * 128;
 constexpr int TT_MAX_L = 8;
 constexpr int PADR = 64;                        // zero rows in front of a tile (past-tap reads of its first rows)
@@ -233,7 +236,7 @@ __global__ void __launch_bounds__(TT_THREADS, 1) k_tiny_tc(const __grid_constant
         const bool dead = a.t0 + tl < 0;                          // before the stream start: zero at every layer input (A4)
         const bool store = (a.stash ? tile >= k0 : r >= a.halo) && tl >= 0 && tl < a.n;
         uint32_t uH[16];                                          // u of branch 0 (fp16 pairs), parked while branch 1 runs
-#pragma unroll 1
+#pragma unroll
         for (int b = 0; b < 2; b++) {
             // ---- lift (C.1 step 1): h0 = W_in x + b_in -> fp32 master in TMEM; skip sum starts at sum_i bs_i
             {
