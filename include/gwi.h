@@ -136,7 +136,10 @@ gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t n_models, i
  * per-sample halves, and every (sample, lag, model) is evaluated element-wise, fused with the mean and the threshold -- no
  * per-lag probability array exists unless d_pbar or the per-model rule asks for one); FP16-mode paper-scale models run on
  * the tcgen05 kernel over segments with recomputed warm-up (with slides when the lags and n_total are multiples of 128
- * samples and n_total >= max lag + R_f - 1); everything else (FP32 mode, other architectures) runs on the generic kernels.
+ * samples and n_total >= max lag + R_f - 1: the same split of the head, its halves contracted per sample on the tensor
+ * cores; this back end works in whole blocks of up to 2^23 samples, so the outputs of the last pushed samples may be
+ * produced by a later push, or by the push that completes n_total -- gwi_stream_samples_done tells how far it is);
+ * everything else (FP32 mode, other architectures) runs on the generic kernels.
  *
  * gwi_stream_create   models: HOST array of n_models loaded models sharing device, precision and architecture
  *                     (1..16).  lags: HOST array of n_lags lags in SAMPLES, each >= 1; a lag >= n_total wraps (lag mod n_total: the slides are
@@ -170,6 +173,7 @@ gwi_status gwi_stream_push(gwi_stream* s, const void* d_h1, const void* d_l1, in
 gwi_status gwi_stream_push_host(gwi_stream* s, const void* h_h1, const void* h_l1, int64_t n, void* cuda_stream);
 gwi_status gwi_stream_finish(gwi_stream* s, gwi_trigger* h_triggers, int32_t capacity, int32_t* h_count,
                              void* cuda_stream);
+/* samples whose outputs have been produced (enqueued) so far; n_total once the last push has been made */
 int64_t gwi_stream_samples_done(const gwi_stream* s);
 /* ---- time shards (one rank per GPU, the data sharded across ranks) -------------------------
  * A rank that owns the global samples [t_first, t_first + n) of a longer stream creates its handle with
