@@ -121,6 +121,21 @@ gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t n_models, i
                                  void* d_carry, gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count,
                                  float* d_pbar, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* The same call for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no workspace argument, the scratch is a file-scope device array inside the library,
+ * sized for N <= GWI_TRIGGERS_STATIC_MAX_N samples (2^24 = 68 min at 4096 Hz: 2.1 MB, held by every GPU that loads the
+ * library until the process exits).  The call allocates nothing: no cudaMalloc / cudaFree, no allocating library
+ * routine; inputs and outputs are the caller's, exactly as above, and so are the results (same kernels).
+ * The device that holds the buffers must be the CURRENT device (the scratch address is looked up per device, once).
+ * Every call on a device shares the one array: calls that overlap on the GPU (different streams, or graph branches
+ * without a dependency) race; serialise them.  Nothing is kept between calls (the scratch header is cleared by each call).
+ * Errors: as above, plus GWI_ERR_CAPACITY when N > GWI_TRIGGERS_STATIC_MAX_N (the message says so). */
+#define GWI_TRIGGERS_STATIC_MAX_N (1 << 24)
+gwi_status gwi_ensemble_triggers_static(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0,
+                                        float threshold, int64_t min_len, int32_t slide_id, int last_chunk,
+                                        void* d_carry, gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count,
+                                        float* d_pbar, void* cuda_stream);
+
 /* ---- streaming ensemble: one causal pass over a long two-detector stream ---
  *
  * What it computes (DESIGN.md C.1 "Stream", "Ensemble", "Slide k", "Triggers"):

@@ -11,7 +11,7 @@ STATUS_NAMES = {0: "GWI_OK", 1: "GWI_ERR_ARG", 2: "GWI_ERR_IO", 3: "GWI_ERR_FORM
                 5: "GWI_ERR_CUDA", 6: "GWI_ERR_NOMEM", 7: "GWI_ERR_CAPACITY"}
 EXPORTED_SYMBOLS = ["gwi_load_model", "gwi_free_model", "gwi_model_info", "gwi_model_uses_tensor_cores",
                     "gwi_infer_workspace_bytes", "gwi_infer", "gwi_carry_bytes", "gwi_triggers_workspace_bytes",
-                    "gwi_ensemble_triggers", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
+                    "gwi_ensemble_triggers", "gwi_ensemble_triggers_static", "gwi_last_error", "gwi_version", "gwi_launch_count", "gwi_stream_create",
                     "gwi_stream_tail_samples", "gwi_stream_prime", "gwi_stream_push", "gwi_stream_push_host",
                     "gwi_stream_finish", "gwi_stream_samples_done", "gwi_stream_backend", "gwi_stream_set_shard", "gwi_stream_destroy", "gwi_stream_set_rule",
                     "gwi_coincidence", "gwi_find_peaks_workspace_bytes", "gwi_find_peaks", "gwi_sweep_workspace_bytes", "gwi_threshold_sweep", "gwi_whiten_workspace_bytes",
@@ -63,6 +63,9 @@ def lib():
     L.gwi_ensemble_triggers.restype = C.c_int
     L.gwi_ensemble_triggers.argtypes = [C.POINTER(vp), C.c_int32, C.c_int64, C.c_int64, C.c_float, C.c_int64, C.c_int32,
                                         C.c_int, vp, vp, C.c_int32, vp, vp, vp, C.c_size_t, vp]
+    L.gwi_ensemble_triggers_static.restype = C.c_int
+    L.gwi_ensemble_triggers_static.argtypes = [C.POINTER(vp), C.c_int32, C.c_int64, C.c_int64, C.c_float, C.c_int64, C.c_int32,
+                                               C.c_int, vp, vp, C.c_int32, vp, vp, vp]
     L.gwi_stream_create.restype = C.c_int
     L.gwi_stream_create.argtypes = [C.POINTER(vp), C.c_int32, C.POINTER(C.c_int64), C.c_int32, C.c_int64, C.c_int64,
                                     C.c_float, C.c_int64, C.c_int32, vp, C.POINTER(vp)]
@@ -214,6 +217,26 @@ def ensemble_triggers(probs, threshold, min_len, t0=0, slide_id=0, last_chunk=Tr
         e.count, e.records = n, recs
         raise e
     return n, recs, pbar
+
+
+TRIGGERS_STATIC_MAX_N = 1 << 24
+
+
+def ensemble_triggers_static(probs, threshold, min_len, trig, cnt, t0=0, slide_id=0, last_chunk=True, carry=None, pbar=None):
+    """gwi_ensemble_triggers_static: the call that allocates nothing.  Every buffer is the caller's: probs = list of [N]
+    float32 device tensors (contiguous), trig = uint8 device tensor of capacity * sizeof(Trigger) bytes, cnt = int32[1],
+    pbar = optional float32 [N].  Asynchronous on the current stream; N <= TRIGGERS_STATIC_MAX_N."""
+    dev = probs[0].device
+    if not probs[0].is_cuda:
+        raise GwiError(1, "probabilities must be CUDA tensors (no CPU fallback)")
+    N = probs[0].numel()
+    ptrs = (C.c_void_p * len(probs))(*[p.data_ptr() for p in probs])
+    with torch.cuda.device(dev):
+        _check(lib().gwi_ensemble_triggers_static(ptrs, len(probs), N, int(t0), float(threshold), int(min_len), int(slide_id),
+                                                  int(bool(last_chunk)), C.c_void_p(carry.data_ptr()) if carry is not None else None,
+                                                  C.c_void_p(trig.data_ptr()), trig.numel() // C.sizeof(Trigger),
+                                                  C.c_void_p(cnt.data_ptr()),
+                                                  C.c_void_p(pbar.data_ptr()) if pbar is not None else None, _stream_ptr(dev)))
 
 
 def threshold_sweep(probs, thresholds, min_len):

@@ -356,6 +356,59 @@ extern "C" gwi_status gwi_ensemble_triggers(const float* const* d_prob, int32_t 
                         d_count, 0, d_pbar, d_workspace, workspace_bytes, (cudaStream_t)cuda_stream, -1, -1);
 }
 
+// ---- gwi_ensemble_triggers_static: the same call on a file-scope scratch array (no allocation anywhere in the call) ------
+namespace {
+constexpr size_t r256(size_t b) { return (b + 255) & ~(size_t)255; }
+// layout(N).total, as a constant expression
+constexpr size_t layout_total(int64_t N)
+{
+    return r256(sizeof(Header)) + r256((size_t)((N + 31) / 32 + 4) * 4) + r256((size_t)(((N + 31) / 32 + WB - 1) / WB)) +
+           2 * r256((size_t)(((N + 31) / 32 + RT - 1) / RT) * 4);
+}
+constexpr size_t STATIC_SCRATCH_BYTES = layout_total(GWI_TRIGGERS_STATIC_MAX_N);
+constexpr int STATIC_MAX_DEVICES = 64;
+}
+// In host code this name is a host-side stand-in, not a device address: the address comes from cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned char g_triggers_scratch[STATIC_SCRATCH_BYTES];
+
+extern "C" gwi_status gwi_ensemble_triggers_static(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0,
+                                                   float threshold, int64_t min_len, int32_t slide_id, int last_chunk,
+                                                   void* d_carry, gwi_trigger* d_triggers, int32_t capacity,
+                                                   int32_t* d_count, float* d_pbar, void* cuda_stream)
+{
+    if (N > (int64_t)GWI_TRIGGERS_STATIC_MAX_N) {
+        gwi_set_error("gwi_ensemble_triggers_static: N = %lld exceeds GWI_TRIGGERS_STATIC_MAX_N = %d (use gwi_ensemble_triggers "
+                      "with a caller-owned workspace)", (long long)N, (int)GWI_TRIGGERS_STATIC_MAX_N);
+        return GWI_ERR_CAPACITY;
+    }
+    if (N >= 1 && layout(N).total > STATIC_SCRATCH_BYTES) {   // cannot happen: layout_total restates layout()
+        gwi_set_error("gwi_ensemble_triggers_static: internal scratch too small");
+        return GWI_ERR_NOMEM;
+    }
+    // the array's device address, looked up once per device with that device current
+    static void* scratch_of[STATIC_MAX_DEVICES] = {};
+    int dev = -1;
+    GWI_CUDA_CHECK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) {
+        gwi_set_error("gwi_ensemble_triggers_static: device %d out of range", dev);
+        return GWI_ERR_UNSUPPORTED;
+    }
+    if (!scratch_of[dev]) {
+        void* ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_triggers_scratch);
+        if (e != cudaSuccess || !ptr) {
+            gwi_set_error("gwi_ensemble_triggers_static: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            return GWI_ERR_CUDA;
+        }
+        scratch_of[dev] = ptr;
+    }
+    void* ws = scratch_of[dev];
+    // the array keeps the previous call's contents: the header starts from zero (the rest is fully rewritten before it is read)
+    GWI_CUDA_CHECK(cudaMemsetAsync(ws, 0, r256(sizeof(Header)), (cudaStream_t)cuda_stream));
+    return gwi_post_run(d_prob, n_models, N, t0, threshold, min_len, slide_id, last_chunk, d_carry, d_triggers, capacity,
+                        d_count, 0, d_pbar, ws, STATIC_SCRATCH_BYTES, (cudaStream_t)cuda_stream, -1, -1);
+}
+
 // append != 0: *d_count holds the number of records already in d_triggers; the new ones go behind them.
 static gwi_status post_from_bits(const Ptrs& P, int n_models, const uint8_t* d_mm, const uint32_t* bits, int64_t N, int64_t t0,
                                  float threshold, int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry,
