@@ -271,6 +271,51 @@ def stream_bench(dev, work, rank, n_chunks=744, paper_month=False):
         del probs
     except Exception as ex:
         out["post"] = {"error": repr(ex)}
+    # ---- NEXT-1 legs: the paper's peak rule on one model's probabilities, and the one-pass threshold sweep (both HBM-bound)
+    try:
+        Nf = 1 << 26
+        g = torch.Generator(device=dev)
+        g.manual_seed(8)
+        xs = [torch.rand(Nf, generator=g, device=dev, dtype=torch.float32) * 0.45 for _ in range(4)]
+        for k in range(16):                                    # 16 plateaus of 1 s: flat-top peaks of width 4096
+            for x_ in xs:
+                x_[(k + 1) * 3_500_003:(k + 1) * 3_500_003 + gs.FS] = 0.9
+        hbm = peaks()[0].get("hbm_gbs", 6650.0)
+        times = []
+        for rep in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            npk, _ = gwi.find_peaks(xs[0], THETA, float(LMIN), capacity=4096, sync=False)
+            e1.record()
+            torch.cuda.synchronize()
+            times.append(e0.elapsed_time(e1))
+            npk = int(npk.item())
+        ms = float(np.median(times[1:]))
+        gbs = Nf * 4 / (ms * 1e-3) / 1e9
+        out["find_peaks"] = {"workload": "gwi_find_peaks (SciPy find_peaks(height, width) rule) on 2^26 float32 probabilities of one model "
+                                         "(268 MB > L2), height 0.5, width >= 2048",
+                             "ms": ms, "peaks": npk, "bound": "hbm", "algorithmic_bytes": Nf * 4, "achieved_gb_per_s": gbs,
+                             "peak_gb_per_s": hbm, "frac": gbs / hbm,
+                             "note": "algorithmic bytes = one read of the array (level 1 of the pyramids and the candidate mask come from "
+                                     "the same pass); the rest is 3-6 small launches on 3 % of the data"}
+        ths = [0.30 + 0.01 * k for k in range(64)]
+        gwi.threshold_sweep(xs, ths, LMIN)
+        times = []
+        for rep in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            cnts = gwi.threshold_sweep(xs, ths, LMIN)
+            e1.record()
+            torch.cuda.synchronize()
+            times.append(e0.elapsed_time(e1))
+        ms = float(np.median(times[1:]))
+        gbs = 4 * Nf * 4 / (ms * 1e-3) / 1e9
+        out["sweep"] = {"workload": "gwi_threshold_sweep: trigger counts at 64 thresholds in one pass over 4 x 2^26 float32 probabilities "
+                                    "(1.07 GB > L2), L_min 2048", "ms": ms, "counts_at_0.5": int(cnts[20].item()), "bound": "hbm",
+                        "algorithmic_bytes": 4 * Nf * 4, "achieved_gb_per_s": gbs, "peak_gb_per_s": hbm, "frac": gbs / hbm}
+        del xs
+    except Exception as ex:
+        out["find_peaks"] = {"error": repr(ex)}
     # ---- whitening front end (NEXT-4): one 4096 s segment (2^24 samples) of one detector, raw fp32 -> fp16
     try:
         nw, nper = 1 << 24, 2 * gs.FS

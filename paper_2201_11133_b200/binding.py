@@ -259,9 +259,9 @@ class Peak(C.Structure):
                 ("left_ip", C.c_double), ("right_ip", C.c_double)]
 
 
-def find_peaks(x, height, min_width, capacity=65536):
+def find_peaks(x, height, min_width, capacity=65536, sync=True):
     """gwi_find_peaks on a [N] float32 device tensor -> (count, [Peak...]) sorted by index; raises GwiError(GWI_ERR_CAPACITY)
-    when count > capacity."""
+    when count > capacity.  sync=False: nothing is read back, returns the device tensors (count int32[1], records as bytes)."""
     if not x.is_cuda or x.dtype != torch.float32:
         raise GwiError(1, "x must be a float32 CUDA tensor (no CPU fallback)")
     x = x.contiguous()
@@ -271,6 +271,8 @@ def find_peaks(x, height, min_width, capacity=65536):
     ws = torch.empty(max(lib().gwi_find_peaks_workspace_bytes(N, int(capacity)), 256), dtype=torch.uint8, device=x.device)
     _check(lib().gwi_find_peaks(C.c_void_p(x.data_ptr()), N, float(height), float(min_width), C.c_void_p(out.data_ptr()),
                                 int(capacity), C.c_void_p(cnt.data_ptr()), C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(x.device)))
+    if not sync:
+        return cnt, out
     n = int(cnt.item())
     if n > capacity:
         raise GwiError(7, f"{n} peaks > capacity {capacity}")

@@ -21,6 +21,7 @@ namespace {
 
 constexpr int WB = 256;    // words per all-ones block
 constexpr int RT = 1024;   // threads (= words) per CTA in k_runs
+constexpr int ST_THREADS = 1024;   // threads per CTA in k_stats
 
 struct Ptrs {
     const float* p[GWI_MAX_MODELS];
@@ -107,12 +108,24 @@ __device__ int64_t find_end(const uint32_t* __restrict__ bits, const uint8_t* __
     int64_t i = pos >> 5;
     uint32_t w = ~bits[i] & (0xffffffffu << (pos & 31));
     if (w) return min((int64_t)(i * 32 + __ffs(w) - 1), N);
-    for (i++; i < NW; i++) {
-        if ((i % WB) == 0)
+    i++;
+    while (i < NW) {
+        if ((i % WB) == 0) {
             while (i + WB <= NW && flags[i / WB]) i += WB;
-        if (i >= NW) break;
-        w = ~bits[i];
-        if (w) return min((int64_t)(i * 32 + __ffs(w) - 1), N);
+            if (i >= NW) break;
+        }
+        // the words up to the next block boundary, eight independent loads at a time (a 1 s run is 128 words: walked one
+        // dependent load after the other it was the longest chain of the whole call)
+        const int64_t stop = min(NW, (i / WB + 1) * WB);
+        for (; i < stop; i += 8) {
+            uint32_t v[8];
+#pragma unroll
+            for (int u = 0; u < 8; u++) v[u] = (i + u < stop) ? ~bits[i + u] : 0u;
+#pragma unroll
+            for (int u = 0; u < 8; u++)
+                if (v[u]) return min((int64_t)((i + u) * 32 + __ffs(v[u]) - 1), N);
+        }
+        i = stop;
     }
     return N;
 }
@@ -253,18 +266,20 @@ __global__ void k_scan(const uint32_t* __restrict__ blkcnt, uint32_t* __restrict
     }
 }
 
-// statistics of pbar over local [a,b): peak, sum (double), per-model mask.  256 threads cooperate.
+// statistics of pbar over local [a,b): peak, sum (double), per-model mask.  The ST_THREADS threads of the CTA cooperate (a
+// 1 s run is four samples per thread: the loads of a record are all in flight at once).
 // mm (fused time-slide heads, gwi_heads.cu): one byte per sample with the models that exceeded the threshold on their own;
 // P then holds the mean itself (M = 1)
 __device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t b, float& peak, double& sum, int& mask,
                           const uint8_t* __restrict__ mm)
 {
-    __shared__ float s_peak[256];
-    __shared__ double s_sum[256];
-    __shared__ int s_mask[256];
+    __shared__ float s_peak[ST_THREADS];
+    __shared__ double s_sum[ST_THREADS];
+    __shared__ int s_mask[ST_THREADS];
     float pk = -1.f;
     double sm = 0.0;
     int mk = 0;
+#pragma unroll 4
     for (int64_t i = a + threadIdx.x; i < b; i += blockDim.x) {
         float v = ens_mean(P, M, i);
         pk = fmaxf(pk, v);
@@ -275,7 +290,7 @@ __device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t 
     }
     s_peak[threadIdx.x] = pk, s_sum[threadIdx.x] = sm, s_mask[threadIdx.x] = mk;
     __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
+    for (int o = ST_THREADS / 2; o > 0; o >>= 1) {
         if ((int)threadIdx.x < o) {
             s_peak[threadIdx.x] = fmaxf(s_peak[threadIdx.x], s_peak[threadIdx.x + o]);
             s_sum[threadIdx.x] += s_sum[threadIdx.x + o];
@@ -427,7 +442,7 @@ static gwi_status post_from_bits(const Ptrs& P, int n_models, const uint8_t* d_m
     k_runs<1><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
                                              d_triggers, capacity, shard_begin, shard_end);
     int sgrid = capacity < 128 ? capacity + 1 : 129;   // records are few: 128 CTAs loop over them, the last one writes the carry
-    k_stats<<<sgrid, 256, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry, shard_begin, shard_end, d_mm);
+    k_stats<<<sgrid, ST_THREADS, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry, shard_begin, shard_end, d_mm);
     gwi_count_launch(6);
     GWI_CUDA_CHECK(cudaGetLastError());
     return GWI_OK;

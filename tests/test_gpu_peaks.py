@@ -10,10 +10,18 @@ from oracle import gwo
 pytestmark = pytest.mark.gpu
 
 
-def _compare(x32, height, width, cap=1 << 17):
+def _compare(x32, height, width, cap=1 << 17, shift=0):
+    """shift > 0: the device array starts `shift` floats into an allocation, i.e. is not 16-byte aligned (the level-1 /
+    candidate pass then takes its scalar-load variant)"""
     import torch
     import paper_2201_11133_b200 as gwi
-    n, pk = gwi.find_peaks(torch.from_numpy(x32).cuda(), height, width, capacity=cap)
+    xd = torch.from_numpy(x32).cuda()
+    if shift:
+        buf = torch.empty(x32.size + shift, dtype=torch.float32, device="cuda")
+        buf[shift:] = xd
+        xd = buf[shift:]
+        assert xd.data_ptr() % 16 != 0 and xd.is_contiguous()
+    n, pk = gwi.find_peaks(xd, height, width, capacity=cap)
     on, opk = gwo.find_peaks(x32.astype(np.float64), float(np.float32(height)), width, cap=cap)
     assert n == on and [p.index for p in pk] == [p[0] for p in opk]
     for g, o in zip(pk, opk):
@@ -42,11 +50,12 @@ def _traces():
     yield np.concatenate([np.linspace(0, 1, 40_000), np.linspace(1, 0, 50_000)]).astype(np.float32)   # one peak, N-wide searches
 
 
-@pytest.mark.parametrize("height,width", [(0.0, 0.0), (0.5, 0.0), (0.5, 3.0), (0.45, 20.0), (0.5, 2048.0)])
-def test_find_peaks_matches_oracle(height, width):
+@pytest.mark.parametrize("height,width,shift", [(0.0, 0.0, 0), (0.5, 0.0, 0), (0.5, 3.0, 0), (0.45, 20.0, 0), (0.5, 2048.0, 0),
+                                                (0.0, 0.0, 1), (0.5, 3.0, 3), (0.5, 2048.0, 2)])
+def test_find_peaks_matches_oracle(height, width, shift):
     tot = 0
     for x in _traces():
-        tot += _compare(x, height, width)
+        tot += _compare(x, height, width, shift=shift)
     assert tot > 0
 
 
