@@ -113,7 +113,25 @@ __global__ void __launch_bounds__(SW_THREADS) k_sweep_vh(SwPtrs P, int M, int64_
     for (int i = threadIdx.x; i < K; i += SW_THREADS) th[i] = thr[i];
     if (vec) {
         // four samples per thread and load instruction (all pointers 16-byte aligned, TT % 4 == 0)
-        for (int i4 = threadIdx.x; 4 * i4 < len; i4 += SW_THREADS) {
+        int i4 = threadIdx.x;
+        if (base >= 0 && base + len + 3 < N && M == 4) {
+            // interior tile of a 4-model ensemble: no bounds, three iterations of loads (12 x 16 bytes per thread) in flight
+            const float inv = 0.25f;                              // s * 0.25f is the correctly rounded s / 4
+#pragma unroll 3
+            for (; 4 * i4 + 3 < len; i4 += SW_THREADS) {
+                const int64_t t = base + 4 * i4;
+                float4 s = __ldg(reinterpret_cast<const float4*>(P.p[0] + t));
+                const float4 q1 = __ldg(reinterpret_cast<const float4*>(P.p[1] + t));
+                const float4 q2 = __ldg(reinterpret_cast<const float4*>(P.p[2] + t));
+                const float4 q3 = __ldg(reinterpret_cast<const float4*>(P.p[3] + t));
+                s.x = __fadd_rn(__fadd_rn(__fadd_rn(s.x, q1.x), q2.x), q3.x), s.y = __fadd_rn(__fadd_rn(__fadd_rn(s.y, q1.y), q2.y), q3.y);
+                s.z = __fadd_rn(__fadd_rn(__fadd_rn(s.z, q1.z), q2.z), q3.z), s.w = __fadd_rn(__fadd_rn(__fadd_rn(s.w, q1.w), q2.w), q3.w);
+                const int p0 = padi(4 * i4);
+                G[p0] = H[p0] = __fmul_rn(s.x, inv), G[p0 + 1] = H[p0 + 1] = __fmul_rn(s.y, inv);
+                G[p0 + 2] = H[p0 + 2] = __fmul_rn(s.z, inv), G[p0 + 3] = H[p0 + 3] = __fmul_rn(s.w, inv);
+            }
+        }
+        for (; 4 * i4 < len; i4 += SW_THREADS) {
             const int64_t t = base + 4 * i4;
             float v[4] = {INFINITY, INFINITY, INFINITY, INFINITY};
             if (t >= 0 && t + 3 < N) {
@@ -151,7 +169,7 @@ __global__ void __launch_bounds__(SW_THREADS) k_sweep_vh(SwPtrs P, int M, int64_
     __syncthreads();
     {
         const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-        const int nbk = (len - OFF + L - 1) / L, C = (L + 31) / 32;
+        const int nbk = (len - OFF + L - 1) / L, C = ((L + 31) / 32) | 1;   // odd chunk length: the lanes' walks fall on different banks
         for (int task = warp; task < 2 * nbk; task += SW_THREADS / 32) {
             const int q = task >> 1, back = task & 1;
             const int b0 = OFF + q * L, b1 = min(b0 + L, len);         // block [b0, b1)
