@@ -24,6 +24,10 @@
 #include "gwi_internal.h"
 #include "gwi_tc_ptx.h"
 
+#ifndef GWI_COMB_MINB
+#define GWI_COMB_MINB 2
+#endif
+
 namespace {
 
 constexpr int HF_MAX_M = 8;
@@ -283,7 +287,26 @@ struct DiagItem {
     int c, r, ka, Kp;      // comb group, row group, first lag and number of lags of the pass
 };
 
-template <int CH>
+// warp-level tensor-core pieces of the MMA variant below
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t addr)
+{
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void mma16816(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+// MMA = true (32-channel rows): the element-wise work is bound by the fp16 pipe (HFMA2 issues every other clock per
+// scheduler; measured on B200: HFMA2 / HFMA2.RELU / HADD2 0.5 per clock and scheduler, FFMA / FHFMA / HMNMX2 1.0), and two
+// thirds of it is the dot product with W2.  That part moves to the (otherwise idle) warp-level tensor path: a tile = the 16
+// samples of a comb block x one lag; z = ReLU(v_H + v_L) is formed on ldmatrix fragments (A operand, 16 x CH) and
+// multiplied by a B operand that holds W2 in column n for the n-th tile of a group of eight lags, so that eight tiles
+// accumulate into ONE 16 x 8 fp32 accumulator whose lane (g, t) ends up with y of lags 2t, 2t + 1 for samples g, g + 8:
+// every lane owns four evaluations of the group for all models (T1's model order in registers, no shared-memory sums).
+template <int CH, bool MMA>
 __global__ void __launch_bounds__(DG_THREADS, 1) k_heads_diag(const __grid_constant__ HeadsFusedArgs a, const int K, const int KS,
                                                              const int npass, const int G, const int groups, const int nitems)
 {
@@ -335,6 +358,10 @@ __global__ void __launch_bounds__(DG_THREADS, 1) k_heads_diag(const __grid_const
             const __half* base = isL ? vL : vH;
             if (CH == 128) {
                 s0 = s0 < lo ? lo : (s0 > a.n - T ? a.n - T : s0);
+                const __half* src = base + (s0 + cr) * CH;
+#pragma unroll
+                for (int x = 0; x < NX; x++) cp_async16(dst + x * RW * ROWB, src + x * RW * CH);
+            } else if (s0 >= lo && s0 + T <= a.n) {                 // warp-uniform: the whole block is inside the rows
                 const __half* src = base + (s0 + cr) * CH;
 #pragma unroll
                 for (int x = 0; x < NX; x++) cp_async16(dst + x * RW * ROWB, src + x * RW * CH);
@@ -414,6 +441,109 @@ __global__ void __launch_bounds__(DG_THREADS, 1) k_heads_diag(const __grid_const
             }
         }
     };
+    // ---- MMA variant: warp = comb block j, lane (g, t) owns the evaluations (lag 8 gq + 2 t + (e & 1), row g + 8 (e >> 1))
+    constexpr int NGRP = (DG_KS_MAX + 7) / 8;
+    float rsum[NGRP][4];
+    uint32_t rmk[NGRP];
+#pragma unroll
+    for (int gq = 0; gq < NGRP; gq++) {
+        rmk[gq] = 0;
+#pragma unroll
+        for (int e = 0; e < 4; e++) rsum[gq][e] = 0.f;
+    }
+    const int fg = lane >> 2, ft = lane & 3;                        // fragment coordinates of the lane
+    const uint32_t frag_off = ((lane & 7) + ((lane >> 3) & 1) * 8) * ROWB + (lane >> 4) * 16;   // ldmatrix row address of the lane
+    auto mma_compute = [&](const DiagItem& it, int m, int buf) {
+        constexpr int KST = CH / 16;                                 // k-steps of a tile
+        const int Kp = it.Kp;
+        const uint32_t stage = sbase + buf * stage_bytes;
+        uint32_t hf[KST][4], wf[KST][2];
+#pragma unroll
+        for (int s = 0; s < KST; s++) {
+            ldmatrix_x4(hf[s], stage + (nblk_max + warp) * BLKB + frag_off + s * 32);
+            const uint32_t* w2s = reinterpret_cast<const uint32_t*>(smem + w2off) + m * (CH / 2) + s * 8 + ft;
+            wf[s][0] = w2s[0], wf[s][1] = w2s[4];
+        }
+        const float hb2 = 0.5f * a.b2[m];
+        // B operand of tile n of a group: W2 in column n, i.e. on the lanes with g == n
+        auto tile = [&](float (&c)[4], uint32_t lb, int n) {
+            const bool mine = fg == n;
+#pragma unroll
+            for (int s = 0; s < KST; s++) {
+                uint32_t z[4];
+                ldmatrix_x4(z, lb + s * 32);
+#pragma unroll
+                for (int x = 0; x < 4; x++) z[x] = add_relu2(z[x], hf[s][x]);
+                mma16816(c, z, mine ? wf[s][0] : 0u, mine ? wf[s][1] : 0u);
+            }
+        };
+        auto epilogue = [&](int gq, int e, float y) {              // sigmoid(y + b2) = 0.5 + 0.5 tanh((y + b2) / 2)
+            float th;
+            asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(fmaf(0.5f, y, hb2)));
+            const float p = fmaf(0.5f, th, 0.5f);
+            rsum[gq][e] = __fadd_rn(rsum[gq][e], p);               // 0 + p0 = p0 exactly: the T1 expression
+            if (p > a.theta) rmk[gq] |= 1u << (8 * e + m);
+        };
+#pragma unroll
+        for (int gq = 0; gq < NGRP; gq++) {
+            if (8 * gq >= Kp) break;                                 // warp-uniform
+            // two accumulators (even / odd tiles: they fill different columns): half the chain of dependent HMMAs
+            float c[4] = {0.f, 0.f, 0.f, 0.f}, d[4] = {0.f, 0.f, 0.f, 0.f};
+            const uint32_t lb0 = stage + (warp - 8 * gq + Kp - 1) * BLKB + frag_off;   // staged block of the group's first lag
+            if (8 * gq + 8 <= Kp) {                                  // a whole group: no checks inside
+#pragma unroll
+                for (int n = 0; n < 8; n += 2) tile(c, lb0 - n * BLKB, n), tile(d, lb0 - (n + 1) * BLKB, n + 1);
+#pragma unroll
+                for (int e = 0; e < 4; e++) epilogue(gq, e, c[e] + d[e]);
+            } else {
+#pragma unroll
+                for (int n = 0; n < 8; n++)
+                    if (8 * gq + n < Kp) tile(c, lb0 - n * BLKB, n);
+#pragma unroll
+                for (int e = 0; e < 4; e++)
+                    if (8 * gq + 2 * ft + (e & 1) < Kp) epilogue(gq, e, c[e]);
+            }
+        }
+    };
+    auto mma_finalize = [&](const DiagItem& it) {
+        const float fM = (float)a.M;
+        const int64_t tb = (int64_t)(it.c * CJ + warp) * G + T * it.r;   // first sample of the comb block (a multiple of 16)
+#pragma unroll
+        for (int gq = 0; gq < NGRP; gq++) {
+            if (8 * gq >= it.Kp) break;
+            bool pr[4];
+#pragma unroll
+            for (int e = 0; e < 4; e++) {
+                const int kk = 8 * gq + 2 * ft + (e & 1);
+                const int64_t t = tb + fg + 8 * (e >> 1);
+                const bool live = kk < it.Kp && t < a.n;
+                const float pb = __fdiv_rn(rsum[gq][e], fM);
+                pr[e] = live && pb > a.theta;
+                if (live) {
+                    a.pbar[(size_t)(it.ka + kk) * a.row_stride + t] = pb;
+                    a.mm[(size_t)(it.ka + kk) * a.row_stride + t] = (uint8_t)(rmk[gq] >> (8 * e));
+                }
+                rsum[gq][e] = 0.f;
+            }
+            rmk[gq] = 0;
+            // mask bits: the 16 samples of (lag 2 t + par) sit on the lanes with this t, rows g (e = par) and g + 8 (e = par + 2)
+#pragma unroll
+            for (int par = 0; par < 2; par++) {
+                const uint32_t lo = __ballot_sync(0xffffffffu, pr[par]), hi = __ballot_sync(0xffffffffu, pr[par + 2]);
+                const int kk = 8 * gq + 2 * ft + par;
+                if (fg == 0 && kk < it.Kp && (tb >> 4) < 2 * a.bits_stride) {
+                    // bits 4 g + t of the ballots -> bits g: three shift-or steps
+                    auto gather = [&](uint32_t x) {
+                        x = (x >> ft) & 0x11111111u;
+                        x = (x | (x >> 3)) & 0x03030303u;
+                        x = (x | (x >> 6)) & 0x000f000fu;
+                        return (x | (x >> 12)) & 0xffu;
+                    };
+                    reinterpret_cast<uint16_t*>(a.bits + (size_t)(it.ka + kk) * a.bits_stride)[tb >> 4] = (uint16_t)(gather(lo) | (gather(hi) << 8));
+                }
+            }
+        }
+    };
     // mean, threshold, outputs of the item; the sums go back to zero.  Thread = (row, comb block j, lag slot)
     auto finalize = [&](const DiagItem& it) {
         const float fM = (float)a.M;
@@ -459,10 +589,12 @@ __global__ void __launch_bounds__(DG_THREADS, 1) k_heads_diag(const __grid_const
                 asm volatile("cp.async.wait_group 0;" ::: "memory");
             }
             __syncthreads();
-            compute(cur, m, buf);
+            if (MMA) mma_compute(cur, m, buf);
+            else compute(cur, m, buf);
             __syncthreads();
         }
-        finalize(cur);
+        if (MMA) mma_finalize(cur);
+        else finalize(cur);
         __syncthreads();
         cur = nxt;
     }
@@ -507,7 +639,10 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
     // 32-channel rows, up to 34 slides: the thread-per-item comb kernel below (measured 9 % faster per hour than the
     // diagonal kernel there: 18.9 against 20.7 ms with 33 lags, the per-item work is too small to pay for the running sums
     // in shared memory); longer lists and 128-channel rows: the diagonal kernel
-    if (comb && (CH == 32 ? n_lags > 34 : n % 8 == 0)) {
+    // GWI_HEADS_IMPL (A/B runs, 32-channel rows): 0 = the tensor-core variant of the diagonal kernel (default), 1 = the
+    // element-wise diagonal kernel, 2 = the thread-per-item comb kernel (up to 34 slides)
+    static const int impl = [] { const char* e = getenv("GWI_HEADS_IMPL"); return e ? atoi(e) : 0; }();
+    if (comb && (CH == 32 ? (impl != 2 || n_lags > 34) : n % 8 == 0)) {
         const int T = CH == 32 ? DiagGeom<32>::T : DiagGeom<128>::T, CJ = CH == 32 ? DiagGeom<32>::CJ : DiagGeom<128>::CJ;
         const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
         const int npass = (n_lags + DG_KS_MAX - 1) / DG_KS_MAX, KS = (n_lags + npass - 1) / npass;
@@ -518,17 +653,21 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
             if (!sms) {
                 int dev = 0;
                 GWI_CUDA_CHECK(cudaGetDevice(&dev));
-                GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                     (int)DiagGeom<32>::smem_bytes(DG_KS_MAX)));
-                GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                    (int)DiagGeom<32>::smem_bytes(DG_KS_MAX)));
+                GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                     (int)DiagGeom<128>::smem_bytes(DG_KS_MAX)));
                 GWI_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
             }
             const unsigned grid = (unsigned)std::min<int64_t>(nitems, sms);
-            if (CH == 32)
-                k_heads_diag<32><<<grid, DG_THREADS, DiagGeom<32>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
+            if (CH == 32 && impl == 1)
+                k_heads_diag<32, false><<<grid, DG_THREADS, DiagGeom<32>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
+            else if (CH == 32)
+                k_heads_diag<32, true><<<grid, DG_THREADS, DiagGeom<32>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
             else
-                k_heads_diag<128><<<grid, DG_THREADS, DiagGeom<128>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
+                k_heads_diag<128, false><<<grid, DG_THREADS, DiagGeom<128>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
             gwi_count_launch(1);
             GWI_CUDA_CHECK(cudaGetLastError());
             return GWI_OK;
@@ -536,7 +675,7 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
     }
     if (comb && CH == 32 && n_lags <= 34) {
         constexpr int CJ = 16;
-        auto kern = k_heads_comb<32, 16, CJ, 2, 17, 2, 2>;
+        auto kern = k_heads_comb<32, 16, CJ, 2, 17, 2, GWI_COMB_MINB>;
         const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
         const size_t smem = (size_t)2 * (CJ + n_lags - 1) * 1024 + HF_MAX_M * 64;
         static bool attr = false;
