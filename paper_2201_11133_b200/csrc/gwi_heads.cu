@@ -544,6 +544,106 @@ __global__ void __launch_bounds__(DG_THREADS, 1) k_heads_diag(const __grid_const
             }
         }
     };
+    // ---- MMA variant for 8-row blocks (128-channel rows): a 16-row tile = the 8 samples of comb block j at TWO consecutive
+    // lags (rows 0-7: lag 2 tau from staged block i, rows 8-15: lag 2 tau + 1 from block i - 1; ldmatrix takes any row
+    // addresses), v_H of the 8 samples serves both halves.  Two warps per comb block j = warp & 7 take the tiles of even /
+    // odd tau; a warp accumulates eight of its tiles (local index n -> column n) per accumulator pair, so lane (g, t) owns
+    // the evaluations (tile n = 2 t + (e & 1), lag 2 tau + (e >> 1), sample g) of the group, tau = 16 lg + 2 n + (warp >> 3).
+    constexpr int NGRP8 = 2;                                        // <= 9 tiles per warp and pass of <= 33 lags
+    const int jw8 = warp & 7, hh8 = warp >> 3;
+    const uint32_t frag8 = (lane & 7) * ROWB + (lane >> 4) * 16;    // (the second-lag lanes 8-15, 24-31 go one block back)
+    const bool second8 = (lane >> 3) & 1;
+    auto mma_compute8 = [&](const DiagItem& it, int m, int buf) {
+        constexpr int KST = CH / 16;
+        const int Kp = it.Kp, ntile = (Kp + 1) >> 1;
+        const uint32_t stage = sbase + buf * stage_bytes;
+        uint32_t hf[KST][2], wf[KST][2];
+#pragma unroll
+        for (int s2 = 0; s2 < KST / 2; s2++) {                       // v_H: one ldmatrix.x4 = the (a0, a2) pairs of two k-steps
+            uint32_t r4[4];
+            ldmatrix_x4(r4, stage + (nblk_max + jw8) * BLKB + (lane & 7) * ROWB + (lane >> 3) * 16 + s2 * 64);
+            hf[2 * s2][0] = r4[0], hf[2 * s2][1] = r4[1], hf[2 * s2 + 1][0] = r4[2], hf[2 * s2 + 1][1] = r4[3];
+        }
+#pragma unroll
+        for (int s = 0; s < KST; s++) {
+            const uint32_t* w2s = reinterpret_cast<const uint32_t*>(smem + w2off) + m * (CH / 2) + s * 8 + ft;
+            wf[s][0] = w2s[0], wf[s][1] = w2s[4];
+        }
+        const float hb2 = 0.5f * a.b2[m];
+        auto tile = [&](float (&c)[4], uint32_t lb, int n) {
+            const bool mine = fg == n;
+#pragma unroll
+            for (int s = 0; s < KST; s++) {
+                uint32_t z[4];
+                ldmatrix_x4(z, lb + s * 32);
+                z[0] = add_relu2(z[0], hf[s][0]), z[1] = add_relu2(z[1], hf[s][0]);
+                z[2] = add_relu2(z[2], hf[s][1]), z[3] = add_relu2(z[3], hf[s][1]);
+                mma16816(c, z, mine ? wf[s][0] : 0u, mine ? wf[s][1] : 0u);
+            }
+        };
+        auto epilogue = [&](int lg, int e, float y) {
+            float th;
+            asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(fmaf(0.5f, y, hb2)));
+            const float p = fmaf(0.5f, th, 0.5f);
+            rsum[lg][e] = __fadd_rn(rsum[lg][e], p);               // 0 + p0 = p0 exactly: the T1 expression
+            if (p > a.theta) rmk[lg] |= 1u << (8 * e + m);
+        };
+#pragma unroll
+        for (int lg = 0; lg < NGRP8; lg++) {
+            const int tau0 = 16 * lg + hh8;                          // first tile of the group
+            if (tau0 >= ntile) break;                                // warp-uniform
+            float c[4] = {0.f, 0.f, 0.f, 0.f}, d[4] = {0.f, 0.f, 0.f, 0.f};
+            // staged block of the first lag of tile n: i = j - 2 tau + Kp - 1, tau = tau0 + 2 n
+            const uint32_t lb0 = stage + (jw8 - 2 * tau0 + Kp - 1) * BLKB + frag8;
+            if (2 * (tau0 + 14) + 1 < Kp) {                          // a whole group, every second lag inside: no checks
+                const uint32_t lbs = lb0 - (second8 ? BLKB : 0);
+#pragma unroll
+                for (int n = 0; n < 8; n += 2) tile(c, lbs - 4 * n * BLKB, n), tile(d, lbs - 4 * (n + 1) * BLKB, n + 1);
+#pragma unroll
+                for (int e = 0; e < 4; e++) epilogue(lg, e, c[e] + d[e]);
+            } else {
+#pragma unroll
+                for (int n = 0; n < 8; n++) {
+                    const int k0 = 2 * (tau0 + 2 * n);
+                    if (k0 < Kp) tile(c, lb0 - 4 * n * BLKB - ((second8 && k0 + 1 < Kp) ? BLKB : 0), n);   // (a missing second lag re-reads the first)
+                }
+#pragma unroll
+                for (int e = 0; e < 4; e++)
+                    if (2 * (tau0 + 2 * (2 * ft + (e & 1))) + (e >> 1) < Kp) epilogue(lg, e, c[e]);
+            }
+        }
+    };
+    auto mma_finalize8 = [&](const DiagItem& it) {
+        const float fM = (float)a.M;
+        const int64_t tb = (int64_t)(it.c * CJ + jw8) * G + T * it.r;    // first sample of the comb block (a multiple of 8)
+        const int64_t t = tb + fg;
+        auto gather = [&](uint32_t x) {                              // bits 4 g + t of a ballot -> bits g
+            x = (x >> ft) & 0x11111111u;
+            x = (x | (x >> 3)) & 0x03030303u;
+            x = (x | (x >> 6)) & 0x000f000fu;
+            return (x | (x >> 12)) & 0xffu;
+        };
+#pragma unroll
+        for (int lg = 0; lg < NGRP8; lg++) {
+            const int tau0 = 16 * lg + hh8;
+            if (2 * tau0 >= it.Kp) break;
+#pragma unroll
+            for (int e = 0; e < 4; e++) {
+                const int kk = 2 * (tau0 + 2 * (2 * ft + (e & 1))) + (e >> 1);
+                const bool live = kk < it.Kp && t < a.n;
+                const float pb = __fdiv_rn(rsum[lg][e], fM);
+                if (live) {
+                    a.pbar[(size_t)(it.ka + kk) * a.row_stride + t] = pb;
+                    a.mm[(size_t)(it.ka + kk) * a.row_stride + t] = (uint8_t)(rmk[lg] >> (8 * e));
+                }
+                rsum[lg][e] = 0.f;
+                const uint32_t bal = __ballot_sync(0xffffffffu, live && pb > a.theta);
+                if (fg == 0 && kk < it.Kp && (tb >> 3) < 4 * a.bits_stride)
+                    reinterpret_cast<uint8_t*>(a.bits + (size_t)(it.ka + kk) * a.bits_stride)[tb >> 3] = (uint8_t)gather(bal);
+            }
+            rmk[lg] = 0;
+        }
+    };
     // mean, threshold, outputs of the item; the sums go back to zero.  Thread = (row, comb block j, lag slot)
     auto finalize = [&](const DiagItem& it) {
         const float fM = (float)a.M;
@@ -589,11 +689,13 @@ __global__ void __launch_bounds__(DG_THREADS, 1) k_heads_diag(const __grid_const
                 asm volatile("cp.async.wait_group 0;" ::: "memory");
             }
             __syncthreads();
-            if (MMA) mma_compute(cur, m, buf);
+            if (MMA && T == 16) mma_compute(cur, m, buf);
+            else if (MMA) mma_compute8(cur, m, buf);
             else compute(cur, m, buf);
             __syncthreads();
         }
-        if (MMA) mma_finalize(cur);
+        if (MMA && T == 16) mma_finalize(cur);
+        else if (MMA) mma_finalize8(cur);
         else finalize(cur);
         __syncthreads();
         cur = nxt;
@@ -657,6 +759,8 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
                                                     (int)DiagGeom<32>::smem_bytes(DG_KS_MAX)));
                 GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                     (int)DiagGeom<32>::smem_bytes(DG_KS_MAX)));
+                GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                    (int)DiagGeom<128>::smem_bytes(DG_KS_MAX)));
                 GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                     (int)DiagGeom<128>::smem_bytes(DG_KS_MAX)));
                 GWI_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -666,8 +770,10 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
                 k_heads_diag<32, false><<<grid, DG_THREADS, DiagGeom<32>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
             else if (CH == 32)
                 k_heads_diag<32, true><<<grid, DG_THREADS, DiagGeom<32>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
-            else
+            else if (impl == 1)
                 k_heads_diag<128, false><<<grid, DG_THREADS, DiagGeom<128>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
+            else
+                k_heads_diag<128, true><<<grid, DG_THREADS, DiagGeom<128>::smem_bytes(KS), st>>>(a, n_lags, KS, npass, (int)G, (int)groups, (int)nitems);
             gwi_count_launch(1);
             GWI_CUDA_CHECK(cudaGetLastError());
             return GWI_OK;
