@@ -314,6 +314,20 @@ def test_config3_recipe_32_slides(tmpdir_s):
     assert got == _oracle_triggers(pbar.astype(np.float64), float(np.float32(0.5)), 64) and got == sorted(got)
 
 
+@pytest.mark.parametrize("impl", ["1", "2"])
+def test_config3_recipe_with_the_other_head_kernels(impl):
+    """The slide heads have three implementations for regular lag lists (csrc/gwi_heads.cu: the tensor-path diagonal kernel
+    is the default, GWI_HEADS_IMPL=1 the element-wise diagonal kernel, 2 the thread-per-item comb kernel).  The switch is read
+    once per process, so the configs[3] parity test runs again in a child process under each of the other two."""
+    import subprocess
+    import sys
+    env = dict(os.environ, GWI_HEADS_IMPL=impl)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_gpu_stream.py", "-m", "gpu", "-x", "-q", "-k",
+                        "test_config3_recipe_32_slides"], cwd=root, env=env, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0 and "1 passed" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
+
+
 def test_stream_narrow_arch_40_regular_lags_two_passes(tmpdir_s):
     """More regular lags than one pass of the comb heads holds (34): the diagonal kernel in two passes of 21 and 20 lags,
     on chunk lengths that are not multiples of its 16-row blocks."""
