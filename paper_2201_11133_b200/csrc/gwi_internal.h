@@ -100,6 +100,11 @@ gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N,
                         int32_t capacity, int32_t* d_count, int append, float* d_pbar, void* d_workspace,
                         size_t workspace_bytes, cudaStream_t st, int64_t shard_begin = -1, int64_t shard_end = -1);
 
+size_t gwi_post_batch_workspace_bytes(int64_t N, int nslides);
+gwi_status gwi_post_run_bits_batch(const uint32_t* d_bits, int64_t bits_stride, const float* d_pbar, const uint8_t* d_mm, int64_t row_stride,
+                                   int nslides, int64_t N, int64_t t0, float threshold, int64_t min_len, int32_t slide0, int last_chunk,
+                                   void* d_carry, gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count, int append,
+                                   void* d_workspace, size_t workspace_bytes, cudaStream_t st, int64_t shard_begin, int64_t shard_end);
 gwi_status gwi_post_run_bits(const uint32_t* d_bits, const float* d_pbar, const uint8_t* d_mm, int64_t N, int64_t t0, float threshold,
                              int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry, gwi_trigger* d_triggers,
                              int32_t capacity, int32_t* d_count, int append, void* d_workspace, size_t workspace_bytes,

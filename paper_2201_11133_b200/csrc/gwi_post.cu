@@ -15,6 +15,8 @@
 //   k_scan      exclusive scan of the per-CTA counts -> output offsets, total -> *d_count
 //   k_runs<1>   same walk, writes {slide,start,end} at its slot (records come out sorted by start)
 //   k_stats     one CTA per record: peak / mean / model_mask over the run; last CTA updates the carry block
+#include <type_traits>
+
 #include "gwi_internal.h"
 
 namespace {
@@ -93,8 +95,19 @@ __global__ void k_mask(Ptrs P, int M, int64_t N, float theta, uint32_t* __restri
     }
 }
 
-__global__ void k_blkflags(const uint32_t* __restrict__ bits, int64_t NW, uint8_t* __restrict__ flags)
+// Several slides in one launch (the fused slide heads leave one mask per slide, gwi_post_run_bits_batch): slide y works on
+// the mask at bits + y * bits_stride, the mean / model bytes at + y * row_stride, its own scratch block (header, flags,
+// counts, offsets: ws_stride bytes apart) and its own carry.  A single slide has all strides 0.
+struct Batch {
+    int64_t bits_stride, row_stride;
+    size_t ws_stride;
+};
+template <class T>
+__device__ __forceinline__ T* ws_of(T* p, const Batch& b, int y) { return reinterpret_cast<T*>(reinterpret_cast<char*>(const_cast<typename std::remove_const<T>::type*>(p)) + (size_t)y * b.ws_stride); }
+
+__global__ void k_blkflags(const uint32_t* __restrict__ bits, int64_t NW, uint8_t* __restrict__ flags, Batch bt)
 {
+    bits += blockIdx.y * bt.bits_stride, flags = ws_of(flags, bt, blockIdx.y);
     int64_t i = (int64_t)blockIdx.x * WB + threadIdx.x;
     int ok = (i < NW) ? (bits[i] == 0xffffffffu) : 0;
     int all = __syncthreads_and(ok);
@@ -135,9 +148,11 @@ __device__ int64_t find_end(const uint32_t* __restrict__ bits, const uint8_t* __
 // neighbouring shard; the host merges and applies L_min afterwards) and is flagged in model_mask by k_stats.
 __global__ void k_head_run(const uint32_t* __restrict__ bits, const uint8_t* __restrict__ flags, int64_t NW, int64_t N,
                            int64_t t0, int64_t Lmin, int last_chunk, const Carry* __restrict__ carry, Header* hd,
-                           int64_t shard_begin, int64_t shard_end)
+                           int64_t shard_begin, int64_t shard_end, Batch bt)
 {
     if (threadIdx.x != 0) return;
+    bits += blockIdx.x * bt.bits_stride, flags = ws_of(flags, bt, blockIdx.x), hd = ws_of(hd, bt, blockIdx.x);
+    if (carry) carry += blockIdx.x;
     Carry c;
     if (carry) c = *carry;
     else { c.open = 0, c.mask = 0, c.start = 0, c.sum = 0.0, c.peak = 0.f, c.pad = 0; }
@@ -161,9 +176,11 @@ template <int MODE>
 __global__ void k_runs(const uint32_t* __restrict__ bits, const uint8_t* __restrict__ flags, int64_t NW, int64_t N,
                        int64_t t0, int64_t Lmin, int last_chunk, int slide, Header* hd, uint32_t* __restrict__ blkcnt,
                        const uint32_t* __restrict__ blkoff, gwi_trigger* __restrict__ out, int capacity,
-                       int64_t shard_begin, int64_t shard_end)
+                       int64_t shard_begin, int64_t shard_end, Batch bt)
 {
     __shared__ uint32_t wsum[RT / 32];
+    bits += blockIdx.y * bt.bits_stride, flags = ws_of(flags, bt, blockIdx.y), hd = ws_of(hd, bt, blockIdx.y);
+    blkcnt = ws_of(blkcnt, bt, blockIdx.y), blkoff = ws_of(blkoff, bt, blockIdx.y), slide += blockIdx.y;
     if (MODE == 1 && blkcnt[blockIdx.x] == 0) return;   // the counting pass found no qualifying run in this CTA's words
     const int64_t i = (int64_t)blockIdx.x * RT + threadIdx.x;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -219,13 +236,19 @@ __global__ void k_runs(const uint32_t* __restrict__ bits, const uint8_t* __restr
     }
 }
 
-__global__ void k_scan(const uint32_t* __restrict__ blkcnt, uint32_t* __restrict__ blkoff, int64_t nblk, int64_t t0,
-                       int slide, Header* hd, gwi_trigger* __restrict__ out, int capacity, int32_t* __restrict__ d_count,
-                       int append)
+__global__ void k_scan(const uint32_t* __restrict__ blkcnt0, uint32_t* __restrict__ blkoff0, int64_t nblk, int64_t t0,
+                       int slide0, Header* hd0, gwi_trigger* __restrict__ out, int capacity, int32_t* __restrict__ d_count,
+                       int append0, Batch bt, int nslides)
 {
     __shared__ uint32_t wsum[32];
     __shared__ uint32_t running;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  // the slides of a batch one after the other: the records of slide y + 1 go behind those of slide y (append)
+  for (int y = 0; y < nslides; y++) {
+    const uint32_t* blkcnt = ws_of(blkcnt0, bt, y);
+    uint32_t* blkoff = ws_of(blkoff0, bt, y);
+    Header* hd = ws_of(hd0, bt, y);
+    const int slide = slide0 + y, append = y > 0 ? 1 : append0;
     if (threadIdx.x == 0) {
         hd->base = append ? *d_count : 0;
         running = (uint32_t)hd->base + (uint32_t)hd->head_emit;   // the carried run, if emitted, is the first new record
@@ -264,6 +287,8 @@ __global__ void k_scan(const uint32_t* __restrict__ blkcnt, uint32_t* __restrict
             out[hd->base] = r;
         }
     }
+    __syncthreads();
+  }
 }
 
 // statistics of pbar over local [a,b): peak, sum (double), per-model mask.  The ST_THREADS threads of the CTA cooperate (a
@@ -304,8 +329,14 @@ __device__ void run_stats(const Ptrs& P, int M, float theta, int64_t a, int64_t 
 
 __global__ void k_stats(Ptrs P, int M, float theta, int64_t N, int64_t t0, const Header* __restrict__ hd,
                         gwi_trigger* __restrict__ out, int capacity, Carry* carry, int64_t shard_begin, int64_t shard_end,
-                        const uint8_t* __restrict__ mm)
+                        const uint8_t* __restrict__ mm, Batch bt)
 {
+    hd = ws_of(hd, bt, blockIdx.y);
+    if (bt.row_stride) {                                   // (batches come from the fused heads: P holds the mean itself)
+        P.p[0] += blockIdx.y * bt.row_stride;
+        if (mm) mm += blockIdx.y * bt.row_stride;
+    }
+    if (carry) carry += blockIdx.y;
     const int nrec = min(hd->total, capacity);
     if ((int)blockIdx.x == (int)gridDim.x - 1) {   // last CTA: write the outgoing carry
         if (!carry) return;
@@ -340,7 +371,7 @@ struct Layout {
     size_t hdr, bits, flags, cnt, off, total;
     int64_t NW, NB, NR;
 };
-Layout layout(int64_t N)
+Layout layout(int64_t N, bool with_bits = true)
 {
     Layout L;
     L.NW = (N + 31) / 32;
@@ -349,7 +380,7 @@ Layout layout(int64_t N)
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 255) & ~(size_t)255; return at; };
     L.hdr = take(sizeof(Header));
-    L.bits = take((size_t)(L.NW + 4) * 4);
+    L.bits = with_bits ? take((size_t)(L.NW + 4) * 4) : 0;   // (a batch works on masks that the caller holds)
     L.flags = take((size_t)L.NB);
     L.cnt = take((size_t)L.NR * 4);
     L.off = take((size_t)L.NR * 4);
@@ -428,21 +459,24 @@ extern "C" gwi_status gwi_ensemble_triggers_static(const float* const* d_prob, i
 static gwi_status post_from_bits(const Ptrs& P, int n_models, const uint8_t* d_mm, const uint32_t* bits, int64_t N, int64_t t0,
                                  float threshold, int64_t min_len, int32_t slide_id, int last_chunk, void* d_carry,
                                  gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count, int append, char* ws, const Layout& L,
-                                 cudaStream_t st, int64_t shard_begin, int64_t shard_end)
+                                 cudaStream_t st, int64_t shard_begin, int64_t shard_end, int K = 1, Batch bt = Batch{0, 0, 0})
 {
+    // K > 1: the slides slide_id .. slide_id + K - 1 in the same six launches (bt: their strides)
     Header* hd = (Header*)(ws + L.hdr);
     uint8_t* flags = (uint8_t*)(ws + L.flags);
     uint32_t* cnt = (uint32_t*)(ws + L.cnt);
     uint32_t* off = (uint32_t*)(ws + L.off);
-    k_blkflags<<<(unsigned)L.NB, WB, 0, st>>>(bits, L.NW, flags);
-    k_head_run<<<1, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd, shard_begin, shard_end);
-    k_runs<0><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
-                                             d_triggers, capacity, shard_begin, shard_end);
-    k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append);
-    k_runs<1><<<(unsigned)L.NR, RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
-                                             d_triggers, capacity, shard_begin, shard_end);
-    int sgrid = capacity < 128 ? capacity + 1 : 129;   // records are few: 128 CTAs loop over them, the last one writes the carry
-    k_stats<<<sgrid, ST_THREADS, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry, shard_begin, shard_end, d_mm);
+    k_blkflags<<<dim3((unsigned)L.NB, K), WB, 0, st>>>(bits, L.NW, flags, bt);
+    k_head_run<<<K, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd, shard_begin, shard_end, bt);
+    k_runs<0><<<dim3((unsigned)L.NR, K), RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
+                                                      d_triggers, capacity, shard_begin, shard_end, bt);
+    k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append, bt, K);
+    k_runs<1><<<dim3((unsigned)L.NR, K), RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
+                                                      d_triggers, capacity, shard_begin, shard_end, bt);
+    // records are few: up to 128 CTAs per slide loop over them (32 per slide in a batch), the last one writes the carry
+    int sgrid = K > 1 ? (capacity < 32 ? capacity + 1 : 33) : (capacity < 128 ? capacity + 1 : 129);
+    k_stats<<<dim3(sgrid, K), ST_THREADS, 0, st>>>(P, n_models, threshold, N, t0, hd, d_triggers, capacity, (Carry*)d_carry, shard_begin,
+                                                   shard_end, d_mm, bt);
     gwi_count_launch(6);
     GWI_CUDA_CHECK(cudaGetLastError());
     return GWI_OK;
@@ -467,6 +501,28 @@ gwi_status gwi_post_run_bits(const uint32_t* d_bits, const float* d_pbar, const 
     if (!d_carry) last_chunk = 1;
     return post_from_bits(P, 1, d_mm, d_bits, N, t0, threshold, min_len, slide_id, last_chunk, d_carry, d_triggers, capacity, d_count,
                           append, (char*)d_workspace, L, st, shard_begin, shard_end);
+}
+
+// The same for `nslides` slides at once: masks bits_stride words apart, means / model bytes row_stride apart, consecutive
+// carry blocks; slide ids slide0 .. slide0 + nslides - 1; the records are appended slide after slide exactly as nslides
+// calls of gwi_post_run_bits with append = 1 would leave them.
+size_t gwi_post_batch_workspace_bytes(int64_t N, int nslides) { return N < 1 ? 0 : layout(N, false).total * (size_t)nslides; }
+
+gwi_status gwi_post_run_bits_batch(const uint32_t* d_bits, int64_t bits_stride, const float* d_pbar, const uint8_t* d_mm, int64_t row_stride,
+                                   int nslides, int64_t N, int64_t t0, float threshold, int64_t min_len, int32_t slide0, int last_chunk,
+                                   void* d_carry, gwi_trigger* d_triggers, int32_t capacity, int32_t* d_count, int append,
+                                   void* d_workspace, size_t workspace_bytes, cudaStream_t st, int64_t shard_begin, int64_t shard_end)
+{
+    Layout L = layout(N, false);
+    if (workspace_bytes < L.total * (size_t)nslides || !d_bits || !d_pbar || !d_carry || nslides < 1 || nslides > 65535) {
+        gwi_set_error("gwi_post_run_bits_batch: bad argument / workspace");
+        return GWI_ERR_ARG;
+    }
+    Ptrs P;
+    P.p[0] = d_pbar;
+    for (int j = 1; j < GWI_MAX_MODELS; j++) P.p[j] = nullptr;
+    return post_from_bits(P, 1, d_mm, d_bits, N, t0, threshold, min_len, slide0, last_chunk, d_carry, d_triggers, capacity, d_count,
+                          append, (char*)d_workspace, L, st, shard_begin, shard_end, nslides, Batch{bits_stride, row_stride, L.total});
 }
 
 gwi_status gwi_post_run(const float* const* d_prob, int32_t n_models, int64_t N, int64_t t0, float threshold,

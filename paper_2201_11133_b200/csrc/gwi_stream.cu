@@ -295,16 +295,14 @@ gwi_status post_block(gwi_stream* s, int n, bool last, cudaStream_t st)
     }
     if (s->fused) {
         // the fused heads kernel has written mask, mean and model bytes of the kept samples, starting at index 0
-        for (int k = 0; k < nslides; k++) {
-            gwi_status rc = gwi_post_run_bits(s->d_fbits + (size_t)k * s->fbits_stride, s->d_fpbar + (size_t)k * s->sub,
-                                              s->d_fmm + (size_t)k * s->sub, nn, t0, s->theta, s->min_len, k, last ? 1 : 0,
-                                              (char*)s->d_carry + (size_t)k * gwi_carry_bytes(), s->d_trig, s->cap, s->d_count, 1,
-                                              s->d_post_ws, s->post_ws_bytes, st, sb, se);
-            if (rc != GWI_OK) return rc;
-            if (s->d_pbar)
-                GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_pbar + (size_t)k * Nk + kept, s->d_fpbar + (size_t)k * s->sub, (size_t)nn * 4,
-                                               cudaMemcpyDeviceToDevice, st));
-        }
+        // ... of every slide: one batch of six launches clusters all of them (198 launches per block at 33 slides before)
+        gwi_status rc = gwi_post_run_bits_batch(s->d_fbits, s->fbits_stride, s->d_fpbar, s->d_fmm, s->sub, nslides, nn, t0, s->theta,
+                                                s->min_len, 0, last ? 1 : 0, s->d_carry, s->d_trig, s->cap, s->d_count, 1,
+                                                s->d_post_ws, s->post_ws_bytes, st, sb, se);
+        if (rc != GWI_OK) return rc;
+        if (s->d_pbar)
+            GWI_CUDA_CHECK(cudaMemcpy2DAsync(s->d_pbar + kept, (size_t)Nk * 4, s->d_fpbar, (size_t)s->sub * 4, (size_t)nn * 4, nslides,
+                                             cudaMemcpyDeviceToDevice, st));
         s->t_done += n;
         return GWI_OK;
     }
@@ -639,7 +637,7 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     if ((e = cudaMemset(s->d_carry, 0, (size_t)nslides * gwi_carry_bytes())) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_carry_pm, (size_t)nslides * s->M * gwi_carry_bytes())) != cudaSuccess) return fail(e);
     if ((e = cudaMemset(s->d_carry_pm, 0, (size_t)nslides * s->M * gwi_carry_bytes())) != cudaSuccess) return fail(e);
-    s->post_ws_bytes = gwi_triggers_workspace_bytes(s->sub);
+    s->post_ws_bytes = std::max(gwi_triggers_workspace_bytes(s->sub), gwi_post_batch_workspace_bytes(s->sub, nslides));
     if ((e = cudaMalloc(&s->d_post_ws, s->post_ws_bytes)) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_trig, (size_t)capacity * sizeof(gwi_trigger))) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc(&s->d_count, 4)) != cudaSuccess) return fail(e);
