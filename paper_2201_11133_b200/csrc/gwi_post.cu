@@ -190,6 +190,16 @@ __global__ void k_runs(const uint32_t* __restrict__ bits, const uint8_t* __restr
         uint32_t w = bits[i];
         uint32_t prev = (i > 0) ? (bits[i - 1] >> 31) : (uint32_t)(hd->in.open != 0);
         uint32_t starts = w & ~((w << 1) | prev);
+        if (Lmin > 32 && starts) {
+            // a run that starts below another start of the same word ends inside the word: shorter than L_min.  Only the
+            // topmost start can qualify (or reach the chunk end), and the start that sits on the shard's first sample is
+            // emitted whatever its length.  (Dense masks -- probabilities that hover around the threshold -- otherwise cost
+            // up to 16 walks per word.)
+            uint32_t keep = 0x80000000u >> __clz(starts);
+            const int64_t gb = shard_begin - t0 - i * 32;
+            if (shard_begin >= 0 && gb >= 0 && gb < 32) keep |= 1u << gb;
+            starts &= keep;
+        }
         while (starts) {
             int s = __ffs(starts) - 1;
             starts &= starts - 1;
