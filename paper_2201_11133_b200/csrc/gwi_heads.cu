@@ -487,6 +487,21 @@ __global__ void __launch_bounds__(DG_THREADS, 1) k_heads_diag(const __grid_const
 #pragma unroll
         for (int gq = 0; gq < NGRP; gq++) {
             if (8 * gq >= Kp) break;                                 // warp-uniform
+            if ((gq & 1) == 0 && gq + 1 < NGRP && 8 * gq + 16 <= Kp) {
+                // two whole groups at once: four independent accumulator chains and twice the ldmatrix loads in flight (the
+                // kernel runs four warps per scheduler and waits on those latencies)
+                float c0[4] = {0.f, 0.f, 0.f, 0.f}, d0[4] = {0.f, 0.f, 0.f, 0.f}, c1[4] = {0.f, 0.f, 0.f, 0.f}, d1[4] = {0.f, 0.f, 0.f, 0.f};
+                const uint32_t la = stage + (warp - 8 * gq + Kp - 1) * BLKB + frag_off, lb = la - 8 * BLKB;
+#pragma unroll
+                for (int n = 0; n < 8; n += 2) {
+                    tile(c0, la - n * BLKB, n), tile(c1, lb - n * BLKB, n);
+                    tile(d0, la - (n + 1) * BLKB, n + 1), tile(d1, lb - (n + 1) * BLKB, n + 1);
+                }
+#pragma unroll
+                for (int e = 0; e < 4; e++) epilogue(gq, e, c0[e] + d0[e]), epilogue(gq + 1 < NGRP ? gq + 1 : gq, e, c1[e] + d1[e]);
+                continue;
+            }
+            if ((gq & 1) == 1 && 8 * gq + 8 <= Kp) continue;         // done with the group before
             // two accumulators (even / odd tiles: they fill different columns): half the chain of dependent HMMAs
             float c[4] = {0.f, 0.f, 0.f, 0.f}, d[4] = {0.f, 0.f, 0.f, 0.f};
             const uint32_t lb0 = stage + (warp - 8 * gq + Kp - 1) * BLKB + frag_off;   // staged block of the group's first lag
