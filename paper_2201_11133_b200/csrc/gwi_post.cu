@@ -301,6 +301,62 @@ __global__ void k_scan(const uint32_t* __restrict__ blkcnt0, uint32_t* __restric
   }
 }
 
+// The scan of a batch of slides with the slides in parallel: per-slide totals (a warp per slide), their exclusive scan in
+// slide order (one thread: the append order of the records is the slides' order), then the offsets inside every slide.
+// Same results as k_scan walking the slides one after the other (57 us for 33 slides), in a tenth of the time.
+__global__ void k_scan_batch(const uint32_t* __restrict__ blkcnt0, uint32_t* __restrict__ blkoff0, int64_t nblk, int64_t t0,
+                             int slide0, Header* hd0, gwi_trigger* __restrict__ out, int capacity, int32_t* __restrict__ d_count,
+                             int append0, Batch bt, int nslides)
+{
+    extern __shared__ uint32_t sbase[];                     // [nslides]: totals, then first record index of the slide
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int y = wid; y < nslides; y += nw) {
+        const uint32_t* c = ws_of(blkcnt0, bt, y);
+        uint32_t sum = 0;
+        for (int64_t i = lane; i < nblk; i += 32) sum += c[i];
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        if (lane == 0) sbase[y] = sum + (uint32_t)ws_of(hd0, bt, y)->head_emit;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t run = append0 ? (uint32_t)*d_count : 0u;
+        for (int y = 0; y < nslides; y++) {
+            const uint32_t t = sbase[y];
+            sbase[y] = run;
+            run += t;
+        }
+        *d_count = (int32_t)run;
+    }
+    __syncthreads();
+    for (int y = wid; y < nslides; y += nw) {
+        const uint32_t* c = ws_of(blkcnt0, bt, y);
+        uint32_t* off = ws_of(blkoff0, bt, y);
+        Header* hd = ws_of(hd0, bt, y);
+        const uint32_t base = sbase[y];
+        uint32_t running = base + (uint32_t)hd->head_emit;     // the carried run, if emitted, is the slide's first new record
+        for (int64_t i0 = 0; i0 < nblk; i0 += 32) {
+            const int64_t i = i0 + lane;
+            const uint32_t v = i < nblk ? c[i] : 0u;
+            uint32_t incl = v;
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += u;
+            }
+            if (i < nblk) off[i] = running + incl - v;
+            running += __shfl_sync(0xffffffffu, incl, 31);
+        }
+        if (lane == 0) {
+            hd->base = (int32_t)base;
+            hd->total = (int32_t)running;
+            if (hd->head_emit && (int)base < capacity && out) {
+                gwi_trigger r;
+                r.slide = slide0 + y, r.model_mask = 0, r.start = hd->in.start, r.end = t0 + hd->head_end, r.peak_p = 0.f, r.mean_p = 0.f;
+                out[base] = r;
+            }
+        }
+    }
+}
+
 // statistics of pbar over local [a,b): peak, sum (double), per-model mask.  The ST_THREADS threads of the CTA cooperate (a
 // 1 s run is four samples per thread: the loads of a record are all in flight at once).
 // mm (fused time-slide heads, gwi_heads.cu): one byte per sample with the models that exceeded the threshold on their own;
@@ -480,7 +536,8 @@ static gwi_status post_from_bits(const Ptrs& P, int n_models, const uint8_t* d_m
     k_head_run<<<K, 32, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, (const Carry*)d_carry, hd, shard_begin, shard_end, bt);
     k_runs<0><<<dim3((unsigned)L.NR, K), RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
                                                       d_triggers, capacity, shard_begin, shard_end, bt);
-    k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append, bt, K);
+    if (K > 1 && K <= 8192) k_scan_batch<<<1, 1024, (size_t)K * 4, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append, bt, K);
+    else k_scan<<<1, 1024, 0, st>>>(cnt, off, L.NR, t0, slide_id, hd, d_triggers, capacity, d_count, append, bt, K);
     k_runs<1><<<dim3((unsigned)L.NR, K), RT, 0, st>>>(bits, flags, L.NW, N, t0, min_len, last_chunk, slide_id, hd, cnt, off,
                                                       d_triggers, capacity, shard_begin, shard_end, bt);
     // records are few: up to 128 CTAs per slide loop over them (32 per slide in a batch), the last one writes the carry
