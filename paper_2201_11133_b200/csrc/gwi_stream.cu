@@ -739,7 +739,7 @@ extern "C" gwi_status gwi_stream_prime(gwi_stream* s, const void* l1_tail, int64
         GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_xh[0] + H + (H - pre), l1_tail, (size_t)pre * 2, cudaMemcpyDefault, st));
         GWI_CUDA_CHECK(cudaMemsetAsync(s->d_acc, 0, (size_t)n * 2, st));
         GWI_CUDA_CHECK(cudaMemcpyAsync(s->d_acc + s->acc_cap, (const __half*)l1_tail + pre, (size_t)n * 2, cudaMemcpyDefault, st));
-        pick_seg(s, n, std::max(4096, H + 128));             // short segments: the tail is one small block
+        pick_seg(s, n, H + 128);                             // any segment length: the tail is one small block, one round of the grid
         const int B = (int)((n + s->seg - 1) / s->seg);
         const int64_t total = (int64_t)B * s->segT;
         k_seg_gather<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(s->d_acc, s->acc_cap, s->d_xh[0], (int)n, s->seg, H, s->segT, 0,
