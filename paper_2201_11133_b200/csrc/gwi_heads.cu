@@ -766,10 +766,12 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
         const int64_t nitems = groups * npass * (G / T);
         comb = nitems <= INT32_MAX && G <= INT32_MAX;                    // 32-bit item arithmetic in the kernel
         if (comb) {
-            static int sms = 0;
+            // once per device (the attribute belongs to the device's copy of the kernel)
+            static int sms_of[64] = {};
+            int dev = 0;
+            GWI_CUDA_CHECK(cudaGetDevice(&dev));
+            int& sms = sms_of[dev & 63];
             if (!sms) {
-                int dev = 0;
-                GWI_CUDA_CHECK(cudaGetDevice(&dev));
                 GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                     (int)DiagGeom<32>::smem_bytes(DG_KS_MAX)));
                 GWI_CUDA_CHECK(cudaFuncSetAttribute(k_heads_diag<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -799,10 +801,12 @@ gwi_status gwi_heads_fused(const gwi_model* const* models, int M, const __half* 
         auto kern = k_heads_comb<32, 16, CJ, 2, 17, 2, GWI_COMB_MINB>;
         const int64_t nG = (n + G - 1) / G, groups = (nG + CJ - 1) / CJ;
         const size_t smem = (size_t)2 * (CJ + n_lags - 1) * 1024 + HF_MAX_M * 64;
-        static bool attr = false;
-        if (!attr) {
+        static bool attr_of[64] = {};
+        int dev = 0;
+        GWI_CUDA_CHECK(cudaGetDevice(&dev));
+        if (!attr_of[dev & 63]) {
             GWI_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (CJ + 34 - 1) * 1024 + HF_MAX_M * 64));
-            attr = true;
+            attr_of[dev & 63] = true;
         }
         kern<<<(unsigned)(groups * (G / 16)), 512, smem, st>>>(a, n_lags, G);
     } else if (CH == 32) {
