@@ -535,6 +535,13 @@ extern "C" gwi_status gwi_stream_create(const gwi_model* const* models, int32_t 
     int64_t per = (int64_t)s->nb * 2 * s->R * 4;
     int64_t sub = std::max<int64_t>(4096, (2LL << 30) / per);
     if (s->tiny) sub = std::max<int64_t>(4096, (4LL << 30) / ((int64_t)(1 + n_lags) * n_models * 4));   // <= 4 GiB of probabilities
+    {
+        // the fused slide path keeps no per-lag, per-model probabilities (mean, model bytes and mask per slide, half-head
+        // rows per model: ~0.7 KB per sample at 33 slides x 4 models): whole 2^24-sample blocks, half the launches per hour
+        bool fused_ok = s->tiny && n_lags > 0 && n_models <= 8;
+        for (int i = 0; i < n_models; i++) fused_ok = fused_ok && gwi_tiny_writes_v(models[i]);
+        if (fused_ok && (int64_t)(1 + n_lags) * n_models <= 512) sub = 1 << 24;
+    }
     if (s->tcb) sub = 1 << 24;
     if (s->tcs) {
         int64_t maxw = gwi_tc_max_windows(m0, s->segT);
