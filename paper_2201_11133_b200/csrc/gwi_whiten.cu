@@ -62,15 +62,34 @@ __device__ __forceinline__ float raw_scale(const double* stats, int64_t n)
     return ms > 0.0 ? (float)(1.0 / sqrt(ms)) : 1.0f;
 }
 
-// frames[k][i] = scale * x[k * step + i] * hann(i)
-__global__ void k_frames(const float* __restrict__ x, int nper, int K, float* __restrict__ frames, const double* __restrict__ rs,
-                         int64_t n)
+// win[i] = hann(i), once per call (the frames repeat it K times)
+__global__ void k_window(int nper, float* __restrict__ win)
 {
-    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (int64_t)K * nper) return;
-    const int k = (int)(idx / nper), i = (int)(idx % nper);
-    const float w = 0.5f - 0.5f * cospif(2.0f * (float)i / (float)(nper - 1));
-    frames[idx] = x[(int64_t)k * (nper / 2) + i] * raw_scale(rs, n) * w;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < nper) win[i] = 0.5f - 0.5f * cospif(2.0f * (float)i / (float)(nper - 1));
+}
+
+// frames[k][i] = scale * x[k * step + i] * hann(i); a block = 1024 samples of one frame, four per thread (the first
+// version took a 64-bit division, the window's cosine and the fp64 scale per sample and was instruction-bound at 5 x its
+// HBM time)
+__global__ void k_frames(const float* __restrict__ x, int nper, int K, float* __restrict__ frames, const double* __restrict__ rs,
+                         int64_t n, const float* __restrict__ win)
+{
+    __shared__ float s_scale;
+    if (threadIdx.x == 0) s_scale = raw_scale(rs, n);
+    __syncthreads();
+    const float sc = s_scale;
+    const unsigned bpf = (unsigned)(nper + 1023) / 1024;   // blocks per frame
+    const int k = (int)(blockIdx.x / bpf), i0 = (int)((blockIdx.x % bpf) * blockDim.x + threadIdx.x) * 4;
+    if (i0 >= nper) return;
+    const float* xs = x + (int64_t)k * (nper / 2) + i0;
+    float* fr = frames + (int64_t)k * nper + i0;
+    if ((nper & 7) == 0 && (reinterpret_cast<uintptr_t>(x) & 15) == 0) {   // every frame starts on a 16-byte boundary
+        const float4 v = *reinterpret_cast<const float4*>(xs), w = *reinterpret_cast<const float4*>(win + i0);
+        *reinterpret_cast<float4*>(fr) = make_float4(v.x * sc * w.x, v.y * sc * w.y, v.z * sc * w.z, v.w * sc * w.w);
+    } else {
+        for (int e = 0; e < 4 && i0 + e < nper; e++) fr[e] = xs[e] * sc * win[i0 + e];
+    }
 }
 
 // P[j] = mean over frames of |F[k][j]|^2, in two steps with a fixed summation order (a thread per bin walking all K frames
@@ -97,20 +116,36 @@ __global__ void k_periodogram_sum(const double* __restrict__ part, int nf, int K
     P[j] = (float)(acc / K);
 }
 
-// X[i] /= sqrt(P interpolated at i * nper / n)
+// X[i] /= sqrt(P interpolated at i * nper / n); four consecutive bins per thread, the fp64 ratio nper / n once per thread
+// (one fp64 division per bin made the pass instruction-bound)
 __global__ void k_divide(float2* __restrict__ X, int64_t nx, int64_t n, int nper, const float* __restrict__ P,
                          const double* __restrict__ rs)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nx) return;
-    const double pos = (double)i * nper / (double)n;
-    int j = (int)pos;
-    if (j > nper / 2 - 1) j = nper / 2 - 1;
-    const float frac = (float)(pos - j);
-    const float p = P[j] * (1.0f - frac) + P[j + 1] * frac;
-    const float s = rsqrtf(fmaxf(p, 1e-30f)) * raw_scale(rs, n);
-    float2 v = X[i];
-    X[i] = make_float2(v.x * s, v.y * s);
+    const int64_t i0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (i0 >= nx) return;
+    const double ratio = (double)nper / (double)n;
+    const float sc = raw_scale(rs, n);
+    auto factor = [&](int64_t i) {
+        const double pos = (double)i * ratio;
+        int j = (int)pos;
+        if (j > nper / 2 - 1) j = nper / 2 - 1;
+        const float frac = (float)(pos - j);
+        const float p = P[j] * (1.0f - frac) + P[j + 1] * frac;
+        return rsqrtf(fmaxf(p, 1e-30f)) * sc;
+    };
+    if (i0 + 3 < nx) {   // X is 256-byte aligned (workspace layout), i0 a multiple of 4
+        float4* X4 = reinterpret_cast<float4*>(X + i0);
+        float4 a = X4[0], b = X4[1];
+        const float s0 = factor(i0), s1 = factor(i0 + 1), s2 = factor(i0 + 2), s3 = factor(i0 + 3);
+        X4[0] = make_float4(a.x * s0, a.y * s0, a.z * s1, a.w * s1);
+        X4[1] = make_float4(b.x * s2, b.y * s2, b.z * s3, b.w * s3);
+    } else {
+        for (int64_t i = i0; i < nx; i++) {
+            const float s = factor(i);
+            float2 v = X[i];
+            X[i] = make_float2(v.x * s, v.y * s);
+        }
+    }
 }
 
 // stats[0] += sum y, stats[1] += sum y^2 (double)
@@ -118,7 +153,19 @@ __global__ void k_stats_y(const float* __restrict__ y, int64_t n, double* __rest
 {
     __shared__ double s0[256], s1[256];
     double a = 0.0, b = 0.0;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (int64_t)gridDim.x * blockDim.x;
+    int64_t done = 0;
+    if ((reinterpret_cast<uintptr_t>(y) & 15) == 0) {   // 16-byte loads over the whole groups of four, the tail below
+        const int64_t n4 = n >> 2;
+#pragma unroll 4
+        for (int64_t i = tid; i < n4; i += nth) {
+            const float4 q = reinterpret_cast<const float4*>(y)[i];
+            const double v0 = q.x, v1 = q.y, v2 = q.z, v3 = q.w;
+            a += (v0 + v1) + (v2 + v3), b += (v0 * v0 + v1 * v1) + (v2 * v2 + v3 * v3);
+        }
+        done = n4 << 2;
+    }
+    for (int64_t i = done + tid; i < n; i += nth) {
         double v = y[i];
         a += v, b += v * v;
     }
@@ -134,6 +181,28 @@ __global__ void k_stats_y(const float* __restrict__ y, int64_t n, double* __rest
     }
 }
 
+// eight consecutive outputs (i0 a multiple of 8) with vector stores where the caller's pointer allows it
+__device__ __forceinline__ void store8(float* o, float a, float b, float c, float d, float e, float f, float g, float h)
+{
+    if ((reinterpret_cast<uintptr_t>(o) & 15) == 0) {
+        *reinterpret_cast<float4*>(o) = make_float4(a, b, c, d), *reinterpret_cast<float4*>(o + 4) = make_float4(e, f, g, h);
+    } else {
+        o[0] = a, o[1] = b, o[2] = c, o[3] = d, o[4] = e, o[5] = f, o[6] = g, o[7] = h;
+    }
+}
+__device__ __forceinline__ void store8(__half* o, float a, float b, float c, float d, float e, float f, float g, float h)
+{
+    if ((reinterpret_cast<uintptr_t>(o) & 15) == 0) {
+        union { __half2 h2[4]; uint4 u; } pk;
+        pk.h2[0] = __halves2half2((__half)a, (__half)b), pk.h2[1] = __halves2half2((__half)c, (__half)d);
+        pk.h2[2] = __halves2half2((__half)e, (__half)f), pk.h2[3] = __halves2half2((__half)g, (__half)h);
+        *reinterpret_cast<uint4*>(o) = pk.u;
+    } else {
+        o[0] = (__half)a, o[1] = (__half)b, o[2] = (__half)c, o[3] = (__half)d;
+        o[4] = (__half)e, o[5] = (__half)f, o[6] = (__half)g, o[7] = (__half)h;
+    }
+}
+
 template <typename OT>
 __global__ void k_scale_out(const float* __restrict__ y, int64_t n, const double* __restrict__ stats, OT* __restrict__ out)
 {
@@ -144,15 +213,14 @@ __global__ void k_scale_out(const float* __restrict__ y, int64_t n, const double
     const int64_t i0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 8;
     if (i0 + 7 < n) {
         const float4 a = *reinterpret_cast<const float4*>(y + i0), b = *reinterpret_cast<const float4*>(y + i0 + 4);
-        out[i0] = (OT)(a.x * inv), out[i0 + 1] = (OT)(a.y * inv), out[i0 + 2] = (OT)(a.z * inv), out[i0 + 3] = (OT)(a.w * inv);
-        out[i0 + 4] = (OT)(b.x * inv), out[i0 + 5] = (OT)(b.y * inv), out[i0 + 6] = (OT)(b.z * inv), out[i0 + 7] = (OT)(b.w * inv);
+        store8(out + i0, a.x * inv, a.y * inv, a.z * inv, a.w * inv, b.x * inv, b.y * inv, b.z * inv, b.w * inv);
     } else {
         for (int64_t i = i0; i < n; i++) out[i] = (OT)(y[i] * inv);
     }
 }
 
 struct WsLayout {
-    size_t frames, spec, P, X, y, stats, total;
+    size_t frames, spec, P, X, y, stats, win, total;
     int K;
 };
 WsLayout ws_layout(int64_t n, int nper)
@@ -167,6 +235,7 @@ WsLayout ws_layout(int64_t n, int nper)
     L.X = take((size_t)(n / 2 + 1) * 8);
     L.y = take((size_t)n * 4);
     L.stats = take(32);
+    L.win = take((size_t)nper * 4);
     L.total = o;
     return L;
 }
@@ -205,6 +274,7 @@ extern "C" gwi_status gwi_whiten(const float* d_raw, int64_t n, int32_t nper, vo
     float2* X = (float2*)(ws + L.X);
     float* y = (float*)(ws + L.y);
     double* stats = (double*)(ws + L.stats);
+    float* win = (float*)(ws + L.win);
     const int K = L.K, nf = nper / 2 + 1;
     // The three plans (and the work areas they own) are cached per (device, n, nper, stream) for the life of the process,
     // so the call only enqueues work and returns: segment after segment of the same length re-uses them.
@@ -238,22 +308,28 @@ extern "C" gwi_status gwi_whiten(const float* d_raw, int64_t n, int32_t nper, vo
         gwi_set_error("gwi_whiten: cuFFT %s failed", what);
         return GWI_ERR_CUDA;
     };
-    const int64_t nfr = (int64_t)K * nper;
     cudaMemsetAsync(stats, 0, 32, st);
     k_stats_y<<<592, 256, 0, st>>>(d_raw, n, stats + 2);          // stats[2..3]: sum and sum of squares of the raw input
-    k_frames<<<(unsigned)((nfr + 255) / 256), 256, 0, st>>>(d_raw, nper, K, frames, stats + 2, n);
+    k_window<<<(nper + 255) / 256, 256, 0, st>>>(nper, win);
+    k_frames<<<(unsigned)((int64_t)K * ((nper + 1023) / 1024)), 256, 0, st>>>(d_raw, nper, K, frames, stats + 2, n, win);
     if (fft.ExecR2C(pf, frames, (cufftComplex*)spec) != CUFFT_SUCCESS) return fail("exec (frames)");
     // (the time-domain frames are dead once transformed: their buffer holds the partial sums, PG_Y x nf doubles)
     k_periodogram_part<<<dim3((nf + 127) / 128, PG_Y), 128, 0, st>>>(spec, nf, K, (double*)frames);
     k_periodogram_sum<<<(nf + 127) / 128, 128, 0, st>>>((const double*)frames, nf, K, P);
     // cuFFT R2C is out of place here: the raw input stays untouched
-    if (fft.ExecR2C(pr, const_cast<float*>(d_raw), (cufftComplex*)X) != CUFFT_SUCCESS) return fail("exec (forward)");
-    k_divide<<<(unsigned)((n / 2 + 1 + 255) / 256), 256, 0, st>>>(X, n / 2 + 1, n, nper, P, stats + 2);
+    // (an input off a 16-byte boundary goes through y first: the transform wants its vector alignment)
+    const float* fwd_in = d_raw;
+    if ((uintptr_t)d_raw & 15) {
+        GWI_CUDA_CHECK(cudaMemcpyAsync(y, d_raw, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
+        fwd_in = y;
+    }
+    if (fft.ExecR2C(pr, const_cast<float*>(fwd_in), (cufftComplex*)X) != CUFFT_SUCCESS) return fail("exec (forward)");
+    k_divide<<<(unsigned)((n / 2 + 1 + 1023) / 1024), 256, 0, st>>>(X, n / 2 + 1, n, nper, P, stats + 2);
     if (fft.ExecC2R(pi, (cufftComplex*)X, y) != CUFFT_SUCCESS) return fail("exec (inverse)");
     k_stats_y<<<592, 256, 0, st>>>(y, n, stats);
     if (out_is_half) k_scale_out<__half><<<(unsigned)((n + 2047) / 2048), 256, 0, st>>>(y, n, stats, (__half*)d_out);
     else k_scale_out<float><<<(unsigned)((n + 2047) / 2048), 256, 0, st>>>(y, n, stats, (float*)d_out);
-    gwi_count_launch(6);
+    gwi_count_launch(8);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
         gwi_set_error("gwi_whiten: %s", cudaGetErrorString(e));

@@ -32,6 +32,21 @@ def test_whiten_matches_oracle(n, nper):
     assert np.array_equal(xd.cpu().numpy(), x)                  # the input is not modified
 
 
+@pytest.mark.parametrize("n,nper,off", [(10002, 500, 0), (20000, 1004, 0), (1 << 16, 4096, 1), (30000, 500, 3)])
+def test_whiten_scalar_and_unaligned_paths(n, nper, off):
+    """Frame lengths that are no multiple of 8 (no 16-byte frame starts) and input pointers off a 16-byte boundary take
+    the scalar loads of the framing / statistics kernels; same bar as above."""
+    import torch
+    import paper_2201_11133_b200 as gwi
+    x = (1e-19 * _coloured(7 + off, n + off)).astype(np.float32)
+    want = ow.whiten(x[off:].astype(np.float64), nper)
+    xd = torch.from_numpy(x).cuda()[off:]
+    got32 = gwi.whiten(xd, nper, half=False).cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(got32 - want)) <= 1e-3
+    got16 = gwi.whiten(xd, nper, half=True).cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(got16 - want)) <= 1e-3 + np.max(np.abs(want)) * 2.0 ** -11
+
+
 def test_whiten_argument_errors():
     import torch
     import paper_2201_11133_b200 as gwi
