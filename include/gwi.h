@@ -279,8 +279,8 @@ gwi_status gwi_find_peaks(const float* d_x, int64_t N, float height, double min_
  * take as input): Welch estimate of the segment's own PSD (frames of nper samples every nper/2, symmetric Hann window,
  * mean of the squared magnitudes), linear interpolation of it to the segment's frequencies, division of the spectrum
  * by its square root, inverse transform, division by the population standard deviation.
- * d_raw: DEVICE [n] float (not modified).  d_out: DEVICE [n], float, or __half when out_is_half != 0 (may not alias
- * d_raw).  n, nper even, 4 <= nper <= n <= 2^30.  d_workspace: DEVICE, >= gwi_whiten_workspace_bytes(n, nper), 256 B
+ * d_raw: DEVICE [n] float (not modified; any 4-byte alignment is accepted, 16 bytes is the fast path -- other pointers
+ * cost one staging copy).  d_out: DEVICE [n], float, or __half when out_is_half != 0 (may not alias d_raw).  n, nper even, 4 <= nper <= n <= 2^30.  d_workspace: DEVICE, >= gwi_whiten_workspace_bytes(n, nper), 256 B
  * aligned.  The FFTs are cuFFT transforms; the library is loaded on first use (GWI_ERR_UNSUPPORTED if it cannot be).
  * The call enqueues on cuda_stream and returns; the FFT plans are cached per (device, n, nper, stream) for the life of the
  * process, so successive segments of one length re-use them.

@@ -366,7 +366,9 @@ def test_stream_paper_scale_regular_lags_comb_heads(tmpdir_s, seeds, G, K, check
     Parity of pbar with the oracle on every slide (on a spread of slides for the long list), triggers from pbar."""
     import paper_2201_11133_b200 as gwi
     oms, gms = _models(tmpdir_s, seeds, gwi.FP16, arch=gs.PAPER_ARCH)
-    N = 128 * 320
+    # long enough for the largest lag plus several ragged chunks; the oracle costs about a minute per model per 40 000
+    # samples on the GPU box's host cores, so the two-model case takes the shorter stream
+    N = 128 * 320 if (K - 1) * G > 128 * 150 else 128 * 200
     x = gs.stream_noise(35, 0, N, dtype=np.float16)
     lags = [k * G for k in range(1, K)]
     n, recs, pbar = _run_stream(gms, x, _ragged(N, 4, 3000, 16000), lags, 0.5, 16, max_chunk=16000)
